@@ -1,0 +1,323 @@
+"""fp64 CPU oracle for the periodic Coulomb path of arxiv 2503.21176.
+
+TEST INFRASTRUCTURE -- NOT PART OF THE PRODUCT PATH.  Only tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package.  It shares no code with paper_2503_21176_b200/ and
+neither imports the other.
+
+The arithmetic lives in sqeq_oracle.c (plain C, fp64, OpenMP over independent
+outer iterations); this module only marshals numpy arrays into it and writes
+out, in numpy, the few dense linear-algebra definitions (QEq KKT system,
+Eq. 18; the shadow-MD closed form, Eq. 22).  Inputs may be fp32 arrays (the
+very arrays the GPU receives); they are promoted to fp64 exactly and
+everything after that is fp64.
+
+Citations: PAPER.md:N = line N of /root/reference/PAPER.md.
+Pins (tests/test_oracle_*.py): rock-salt / CsCl / zincblende Madelung
+constants, the cubic self-image constant xi, alpha-independence, finite
+differences, PME grid-shift invariance and operator symmetry, numpy.fft,
+scipy B-splines, scipy periodic cKDTree, brute-force multi-image sums.
+Functions whose parity is unpinned: shadow_md_step (integrator constants are
+not given by the paper -- DESIGN.md R-MD).
+"""
+import ctypes
+import math
+import os
+
+import numpy as np
+
+from . import build as _build
+
+KE_EV_A = 14.3996454784255  # e^2/(4 pi eps0) in eV*Angstrom (DESIGN.md R-units)
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        c_dp = ctypes.POINTER(ctypes.c_double)
+        c_ip = ctypes.POINTER(ctypes.c_int)
+        i64 = ctypes.c_int64
+        L.orc_num_threads.restype = ctypes.c_int
+        L.orc_nl_row_counts.argtypes = [i64, c_dp, c_dp, ctypes.c_double, ctypes.c_void_p]
+        L.orc_nl_fill.argtypes = [i64, c_dp, c_dp, ctypes.c_double, ctypes.c_void_p,
+                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        L.orc_nl_row.argtypes = [i64, c_dp, c_dp, ctypes.c_double, i64, i64,
+                                 ctypes.c_void_p, ctypes.c_void_p]
+        L.orc_nl_row.restype = i64
+        L.orc_realspace.argtypes = [i64, c_dp, c_dp, c_dp, ctypes.c_double,
+                                    ctypes.c_double, c_dp, c_dp]
+        L.orc_realspace_rows.argtypes = [i64, c_dp, c_dp, c_dp, ctypes.c_double,
+                                         ctypes.c_double, i64, ctypes.c_void_p, c_dp, c_dp]
+        L.orc_ewald_direct.argtypes = [i64, c_dp, c_dp, c_dp, ctypes.c_double,
+                                       ctypes.c_double, c_ip, c_ip, ctypes.c_int,
+                                       c_dp, c_dp, c_dp]
+        L.orc_bspline.argtypes = [ctypes.c_int, ctypes.c_double]
+        L.orc_bspline.restype = ctypes.c_double
+        L.orc_bspline_deriv.argtypes = [ctypes.c_int, ctypes.c_double]
+        L.orc_bspline_deriv.restype = ctypes.c_double
+        L.orc_pme_spread.argtypes = [i64, c_dp, c_dp, c_dp, c_ip, ctypes.c_int, c_dp]
+        L.orc_dft3.argtypes = [c_dp, c_ip, ctypes.c_int]
+        L.orc_pme_influence_table.argtypes = [c_dp, c_ip, ctypes.c_int, ctypes.c_double, c_dp]
+        L.orc_pme_gather.argtypes = [i64, c_dp, c_dp, c_dp, c_ip, ctypes.c_int, c_dp, c_dp, c_dp]
+        L.orc_pme_recip.argtypes = [i64, c_dp, c_dp, c_dp, c_ip, ctypes.c_int,
+                                    ctypes.c_double, c_dp, c_dp, c_dp, c_dp, c_dp]
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _ip(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+
+
+def _f64(a, shape=None):
+    a = np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def _box(box):
+    b = _f64(box).reshape(-1)
+    if b.size == 1:
+        b = np.repeat(b, 3)
+    assert b.size == 3
+    return np.ascontiguousarray(b)
+
+
+# --------------------------------------------------------------------------
+# c-NL  neighbour list = the plain O(N^2) definition (Alg. 1)
+# --------------------------------------------------------------------------
+def neighbour_list(pos, box, rlist):
+    """Unique pairs i<j sorted by (i,j) with int8 shift s.t. r_j + s*L - r_i is in range."""
+    pos = _f64(pos, (-1, 3))
+    box = _box(box)
+    n = pos.shape[0]
+    counts = np.zeros(n, dtype=np.int64)
+    lib().orc_nl_row_counts(n, _dp(pos), _dp(box), float(rlist), counts.ctypes.data)
+    offsets = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(counts, out=offsets[1:])
+    tot = int(offsets[-1])
+    pi = np.empty(tot, dtype=np.int32)
+    pj = np.empty(tot, dtype=np.int32)
+    sh = np.empty((tot, 3), dtype=np.int8)
+    lib().orc_nl_fill(n, _dp(pos), _dp(box), float(rlist), offsets.ctypes.data,
+                      pi.ctypes.data, pj.ctypes.data, sh.ctypes.data)
+    return pi, pj, sh
+
+
+def neighbour_row(pos, box, rlist, i, cap=4096):
+    """All neighbours j != i of atom i (ascending j) and the shift of the ordered pair (i,j)."""
+    pos = _f64(pos, (-1, 3))
+    box = _box(box)
+    n = pos.shape[0]
+    while True:
+        oj = np.empty(cap, dtype=np.int32)
+        os_ = np.empty((cap, 3), dtype=np.int8)
+        c = int(lib().orc_nl_row(n, _dp(pos), _dp(box), float(rlist), int(i), cap,
+                                 oj.ctypes.data, os_.ctypes.data))
+        if c <= cap:
+            return oj[:c].copy(), os_[:c].copy()
+        cap = c
+
+
+# --------------------------------------------------------------------------
+# c-RS  real-space erfc sum, Eq. 3, r < rc, minimum image
+# --------------------------------------------------------------------------
+def realspace(pos, q, box, rc, alpha):
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box)
+    n = pos.shape[0]
+    phi = np.zeros(n); F = np.zeros((n, 3))
+    lib().orc_realspace(n, _dp(pos), _dp(q), _dp(box), float(rc), float(alpha), _dp(phi), _dp(F))
+    return phi, F
+
+
+def realspace_rows(pos, q, box, rc, alpha, rows):
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box)
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    n = pos.shape[0]
+    phi = np.zeros(rows.size); F = np.zeros((rows.size, 3))
+    lib().orc_realspace_rows(n, _dp(pos), _dp(q), _dp(box), float(rc), float(alpha),
+                             rows.size, rows.ctypes.data, _dp(phi), _dp(F))
+    return phi, F
+
+
+# --------------------------------------------------------------------------
+# c-EW  direct Ewald, Eqs. 2-5 -- pins PME, not a parity target
+# --------------------------------------------------------------------------
+def ewald_direct(pos, q, box, alpha, tol=1e-16, background=False):
+    """Converged regular Ewald sum: phi, F (= -dE/dr), E = 1/2 sum q phi.
+
+    The real-space sum runs over all images with erfc(alpha r) above `tol`, the
+    reciprocal sum over all k with exp(-k^2/4 alpha^2) above `tol`.
+    """
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box)
+    n = pos.shape[0]
+    x = math.sqrt(-math.log(tol))          # erfc(x) < exp(-x^2) = tol
+    rcut = x / alpha
+    kmax = 2.0 * alpha * x                 # exp(-k^2/4a^2) = tol
+    nimg = np.array([int(math.ceil(rcut / L)) for L in box], dtype=np.intc)
+    mmax = np.array([int(math.ceil(kmax * L / (2 * math.pi))) for L in box], dtype=np.intc)
+    phi = np.zeros(n); F = np.zeros((n, 3)); E = np.zeros(1)
+    lib().orc_ewald_direct(n, _dp(pos), _dp(q), _dp(box), float(alpha), float(rcut),
+                           _ip(nimg), _ip(mmax), int(bool(background)), _dp(phi), _dp(F), _dp(E))
+    return phi, F, float(E[0])
+
+
+# --------------------------------------------------------------------------
+# c-PME  smooth PME, Alg. 2
+# --------------------------------------------------------------------------
+def bspline(n, u):
+    return float(lib().orc_bspline(int(n), float(u)))
+
+
+def bspline_deriv(n, u):
+    return float(lib().orc_bspline_deriv(int(n), float(u)))
+
+
+def _grid(grid):
+    g = np.asarray(grid, dtype=np.intc).reshape(-1)
+    if g.size == 1:
+        g = np.repeat(g, 3)
+    return np.ascontiguousarray(g, dtype=np.intc)
+
+
+def pme_spread(pos, q, box, grid, order):
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box); K = _grid(grid)
+    Q = np.zeros(tuple(int(k) for k in K))
+    lib().orc_pme_spread(pos.shape[0], _dp(pos), _dp(q), _dp(box), _ip(K), int(order), _dp(Q))
+    return Q
+
+
+def dft3(z, sign):
+    """Unnormalised 3-D DFT, out[m] = sum_k z[k] exp(sign 2 pi i m.k/K), naive line DFTs."""
+    z = np.ascontiguousarray(z, dtype=np.complex128).copy()
+    K = np.array(z.shape, dtype=np.intc)
+    lib().orc_dft3(z.view(np.float64).ctypes.data_as(ctypes.POINTER(ctypes.c_double)), _ip(K), int(sign))
+    return z
+
+
+def pme_influence(box, grid, order, alpha):
+    box = _box(box); K = _grid(grid)
+    G = np.zeros(tuple(int(k) for k in K))
+    lib().orc_pme_influence_table(_dp(box), _ip(K), int(order), float(alpha), _dp(G))
+    return G
+
+
+def pme_recip(pos, q, box, grid, order, alpha, return_grids=False):
+    """Alg. 2 steps 1-5: phi_rec, F_rec, E_rec (and optionally the Q and Phi grids)."""
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box); K = _grid(grid)
+    n = pos.shape[0]
+    phi = np.zeros(n); F = np.zeros((n, 3)); E = np.zeros(1)
+    shape = tuple(int(k) for k in K)
+    if return_grids:
+        Qg = np.zeros(shape); Pg = np.zeros(shape)
+        lib().orc_pme_recip(n, _dp(pos), _dp(q), _dp(box), _ip(K), int(order), float(alpha),
+                            _dp(phi), _dp(F), _dp(E), _dp(Qg), _dp(Pg))
+        return phi, F, float(E[0]), Qg, Pg
+    lib().orc_pme_recip(n, _dp(pos), _dp(q), _dp(box), _ip(K), int(order), float(alpha),
+                        _dp(phi), _dp(F), _dp(E), None, None)
+    return phi, F, float(E[0])
+
+
+def self_potential(q, alpha):
+    """phi_i^self = -(2 alpha/sqrt(pi)) q_i, from E_self of Eq. 5."""
+    return -(2.0 * alpha / math.sqrt(math.pi)) * _f64(q)
+
+
+def coulomb_pme(pos, q, box, rc, alpha, grid, order, rows=None):
+    """Total PME Coulomb evaluation (Eq. 2): real(r<rc) + reciprocal + self.
+
+    Returns phi (dE/dq), F (-dE/dr), E = 1/2 sum q phi, and a dict of the parts.
+    With `rows` given, the O(N^2) real-space part is evaluated only for those
+    atoms and phi, F are returned for those rows only (E is then None).
+    """
+    q64 = _f64(q)
+    p_rec, F_rec, E_rec = pme_recip(pos, q, box, grid, order, alpha)
+    p_self = self_potential(q, alpha)
+    if rows is None:
+        p_real, F_real = realspace(pos, q, box, rc, alpha)
+        phi = p_real + p_rec + p_self
+        F = F_real + F_rec
+        E = 0.5 * float(np.dot(q64, phi))
+        parts = dict(phi_real=p_real, F_real=F_real, phi_rec=p_rec, F_rec=F_rec,
+                     phi_self=p_self, E_rec=E_rec,
+                     E_real=0.5 * float(np.dot(q64, p_real)),
+                     E_self=0.5 * float(np.dot(q64, p_self)))
+        return phi, F, E, parts
+    rows = np.asarray(rows, dtype=np.int64)
+    p_real, F_real = realspace_rows(pos, q, box, rc, alpha, rows)
+    phi = p_real + p_rec[rows] + p_self[rows]
+    F = F_real + F_rec[rows]
+    parts = dict(phi_real=p_real, F_real=F_real, phi_rec=p_rec[rows], F_rec=F_rec[rows],
+                 E_rec=E_rec)
+    return phi, F, None, parts
+
+
+# --------------------------------------------------------------------------
+# c-QEq  Eq. 18: [[C,1],[1^T,0]] [q;lambda] = [-chi; Qtot],
+#        C v = J o v + ke * phi[v]   (sign reading G3)
+# --------------------------------------------------------------------------
+def coulomb_matrix_pme(pos, box, rc, alpha, grid, order):
+    """Dense A with phi[v] = A v, column by column: A[:,j] = phi[e_j] (small N only)."""
+    pos = _f64(pos, (-1, 3))
+    n = pos.shape[0]
+    A = np.zeros((n, n))
+    e = np.zeros(n)
+    for j in range(n):
+        e[:] = 0.0
+        e[j] = 1.0
+        A[:, j] = coulomb_pme(pos, e, box, rc, alpha, grid, order)[0]
+    return A
+
+
+def qeq_kkt(A, chi, J, ke, qtot):
+    """Assemble Eq. 18's (N+1)x(N+1) matrix and right-hand side."""
+    n = A.shape[0]
+    M = np.zeros((n + 1, n + 1))
+    M[:n, :n] = ke * A + np.diag(_f64(J))
+    M[:n, n] = 1.0
+    M[n, :n] = 1.0
+    b = np.concatenate([-_f64(chi), [float(qtot)]])
+    return M, b
+
+
+def qeq_dense_solve(A, chi, J, ke, qtot):
+    """Solve Eq. 18 densely (LU with partial pivoting): returns q, lambda."""
+    M, b = qeq_kkt(A, chi, J, ke, qtot)
+    x = np.linalg.solve(M, b)
+    return x[:-1], float(x[-1])
+
+
+def qeq_residual(pos, box, rc, alpha, grid, order, chi, J, ke, qtot, q, lam):
+    """True relative residual ||b - A x||/||b|| of Eq. 18 with the fp64 oracle mat-vec
+    (the paper's convergence measure)."""
+    q = _f64(q)
+    phi = coulomb_pme(pos, q, box, rc, alpha, grid, order)[0]
+    r_top = -_f64(chi) - (_f64(J) * q + ke * phi + lam)
+    r_bot = float(qtot) - q.sum()
+    bnorm = math.sqrt(float(np.dot(_f64(chi), _f64(chi))) + float(qtot) ** 2)
+    return math.sqrt(float(np.dot(r_top, r_top)) + r_bot ** 2) / bnorm
+
+
+# --------------------------------------------------------------------------
+# c-MD  shadow-energy closed form, Eq. 22 (reading G4)
+# --------------------------------------------------------------------------
+def shadow_charges(chi, u, v, qtot):
+    """q[n], lambda from the quasi-diagonal system Eq. 22 given v = ke*phi[n]:
+         u_i q_i + lambda = -chi_i - v_i ,  sum q = Qtot."""
+    chi = _f64(chi); u = _f64(u); v = _f64(v)
+    lam = -(float(qtot) + np.sum((chi + v) / u)) / np.sum(1.0 / u)
+    q = -(chi + v + lam) / u
+    return q, float(lam)

@@ -1,0 +1,396 @@
+"""Pins of the fp64 oracle against things other than itself (CPU only).
+
+Each test is chosen so that a plausible mistake in oracle/sqeq_oracle.c (a dropped term,
+a wrong sign or index, a transposed operand, a wrong normalisation) fails it:
+literature lattice constants, closed forms, independent libraries (numpy.fft,
+scipy.interpolate.BSpline, scipy.spatial.cKDTree), finite differences, exact invariants,
+brute-force image sums written out in numpy inside the test.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.interpolate import BSpline
+from scipy.spatial import cKDTree
+from scipy.special import erfc
+
+import oracle
+from paper_2503_21176_b200 import workloads as W
+
+GOLD = {}
+with open(os.path.join(os.path.dirname(__file__), "golden", "constants.txt")) as fh:
+    for line in fh:
+        if line.strip() and not line.startswith("#"):
+            k, *v = line.split()
+            GOLD[k] = v
+
+
+def g(name):
+    return float(GOLD[name][0])
+
+
+def relrms(a, b):
+    return math.sqrt(((np.asarray(a) - np.asarray(b)) ** 2).sum() / (np.asarray(b) ** 2).sum())
+
+
+def random_neutral(n, L, seed, dmin=0.8):
+    rng = np.random.default_rng(seed)
+    pos = []
+    while len(pos) < n:
+        p = rng.uniform(0, L, 3)
+        if all(np.linalg.norm((p - o + L / 2) % L - L / 2) > dmin for o in pos):
+            pos.append(p)
+    q = rng.uniform(-1, 1, n)
+    q -= q.mean()
+    return np.array(pos), q
+
+
+# ---------------------------------------------------------------- Madelung constants
+def _nacl_cell(a=5.64):
+    idx = np.array([[i, j, k] for i in range(2) for j in range(2) for k in range(2)])
+    return idx * (a / 2), np.where(idx.sum(1) % 2 == 0, 1.0, -1.0)
+
+
+@pytest.mark.parametrize("alpha", [0.45, 0.8])
+def test_madelung_rocksalt_direct_ewald(alpha):
+    pos, q = _nacl_cell()
+    phi, F, E = oracle.ewald_direct(pos, q, [5.64] * 3, alpha)
+    M = g("madelung_nacl")
+    r0 = 2.82
+    assert np.allclose(phi, -q * M / r0, rtol=0, atol=2e-10)
+    assert abs(E - (-4 * M / r0)) < 1e-9
+    assert np.abs(F).max() < 1e-12
+
+
+def test_madelung_cscl_and_zincblende_direct_ewald():
+    a = 4.0
+    pos = np.array([[0, 0, 0], [0.5, 0.5, 0.5]]) * a
+    q = np.array([1.0, -1.0])
+    phi, F, E = oracle.ewald_direct(pos, q, [a] * 3, 1.0)
+    r0 = a * math.sqrt(3) / 2
+    assert np.allclose(phi, -q * g("madelung_cscl") / r0, atol=2e-10)
+    fcc = np.array([[0, 0, 0], [0, .5, .5], [.5, 0, .5], [.5, .5, 0]])
+    pos = np.concatenate([fcc, fcc + 0.25]) * a
+    q = np.array([1.0] * 4 + [-1.0] * 4)
+    phi, F, E = oracle.ewald_direct(pos, q, [a] * 3, 1.0)
+    r0 = a * math.sqrt(3) / 4
+    assert np.allclose(phi, -q * g("madelung_zns") / r0, atol=2e-10)
+    assert np.abs(F).max() < 1e-12
+
+
+@pytest.mark.parametrize("alpha", [0.6, 0.9])
+def test_single_charge_self_image_constant(alpha):
+    L = 7.3
+    phi, F, E = oracle.ewald_direct([[1.1, 2.2, 3.3]], [1.0], [L] * 3, alpha, background=True)
+    assert abs(phi[0] * L - g("xi_cubic")) < 1e-9
+    assert np.abs(F).max() < 1e-12
+
+
+def test_madelung_config1_pme_and_direct():
+    """cfg 1 with sigma=0 (BASELINE.json configs[1]): phi_i = -+M/r0, E = -4000 M/r0, F = 0."""
+    c = W.CONFIGS[1]
+    pos, q = W.make(1, sigma=0.0)
+    phi, F, E, parts = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order)
+    M, r0 = g("madelung_nacl"), 2.82
+    # PME is an approximation: discretisation error at h = 0.88 A, order 6 is ~1e-5 relative
+    assert np.abs(phi + q * M / r0).max() < 3e-5 * M / r0
+    assert abs(E / (-4000 * M / r0) - 1) < 3e-5
+    assert np.abs(F).max() < 1e-4 / r0 ** 2
+
+
+# ---------------------------------------------------------------- Ewald invariances
+def test_alpha_independence_and_energy_identity():
+    pos, q = random_neutral(24, 9.0, 1)
+    box = [9.0, 10.0, 11.0]
+    a = oracle.ewald_direct(pos, q, box, 0.5)
+    b = oracle.ewald_direct(pos, q, box, 0.75)
+    assert np.allclose(a[0], b[0], atol=1e-12)
+    assert np.allclose(a[1], b[1], atol=1e-12)
+    assert abs(a[2] - b[2]) < 1e-12
+    assert abs(a[2] - 0.5 * np.dot(q, a[0])) < 1e-13
+    # translation and permutation invariance
+    perm = np.random.default_rng(0).permutation(len(q))
+    c = oracle.ewald_direct(pos[perm] + [1.3, -2.2, 40.0], q[perm], box, 0.5)
+    assert np.allclose(c[0], a[0][perm], atol=1e-11)
+    assert np.allclose(c[1], a[1][perm], atol=1e-11)
+
+
+def test_alpha_independence_non_neutral_needs_background():
+    pos, q = random_neutral(12, 8.0, 2)
+    q = q + 0.3
+    a = oracle.ewald_direct(pos, q, [8.0] * 3, 0.5, background=True)
+    b = oracle.ewald_direct(pos, q, [8.0] * 3, 0.7, background=True)
+    assert np.allclose(a[0], b[0], atol=1e-12)
+    c = oracle.ewald_direct(pos, q, [8.0] * 3, 0.5)
+    d = oracle.ewald_direct(pos, q, [8.0] * 3, 0.7)
+    V = 512.0
+    shift = -math.pi * q.sum() / V * (1 / 0.5 ** 2 - 1 / 0.7 ** 2)
+    assert np.allclose((a[0] - c[0]) - (b[0] - d[0]), shift, atol=1e-12)
+
+
+def test_two_charges_ewald_vs_explicit_image_sum():
+    """Brute force on a tiny input: a +1/-1 pair in a cubic box.  Bare 1/r summed over whole
+    neutral cells inside a sphere of 60 cells converges to the Ewald (tin-foil) energy plus the
+    dipole surface term 2 pi |D|^2/(3V) -- this pins the reciprocal and self terms' prefactors."""
+    L = 6.0
+    pos = np.array([[1.0, 1.5, 2.0], [3.2, 2.5, 2.9]])
+    q = np.array([1.0, -1.0])
+    phi, F, E = oracle.ewald_direct(pos, q, [L] * 3, 0.6)
+    # explicit sum over neutral cells inside a sphere + dipole surface term 2 pi |D|^2 /(3V)
+    R = 60
+    rng = np.arange(-R, R + 1)
+    nx, ny, nz = np.meshgrid(rng, rng, rng, indexing="ij")
+    n = np.stack([nx, ny, nz], -1).reshape(-1, 3).astype(float)
+    n = n[(n ** 2).sum(1) <= R * R]
+    d12 = pos[0] - pos[1]
+    e = 0.0
+    nn = n[(n ** 2).sum(1) > 0] * L
+    # E = 1/2 sum_{i,j,n}' q_i q_j /|r_ij + nL|
+    e += 0.5 * 2 * (q[0] * q[1] / np.linalg.norm(d12 + n * L, axis=1)).sum()
+    e += 0.5 * (q[0] ** 2 + q[1] ** 2) * (1.0 / np.linalg.norm(nn, axis=1)).sum()
+    D = (q[:, None] * pos).sum(0)
+    e_ewald_vacuum = E + 2 * math.pi * np.dot(D, D) / (3 * L ** 3)
+    assert abs(e - e_ewald_vacuum) < 2e-4 * abs(e)
+
+
+# ---------------------------------------------------------------- finite differences
+def _fd(fun, pos, i, k, h=1e-5):
+    p = pos.copy(); p[i, k] += h
+    m = pos.copy(); m[i, k] -= h
+    return -(fun(p) - fun(m)) / (2 * h)
+
+
+def test_forces_are_minus_gradient_direct_real_and_pme():
+    pos, q = random_neutral(20, 20.0, 3)
+    box = [20.0, 21.0, 22.0]
+    phi, F, E = oracle.ewald_direct(pos, q, box, 0.4)
+    assert abs(_fd(lambda p: oracle.ewald_direct(p, q, box, 0.4)[2], pos, 3, 1) - F[3, 1]) < 1e-8
+    # real-space part alone (min image, rc = 9 < L/2)
+    pr, Fr = oracle.realspace(pos, q, box, 9.0, 0.35)
+    er = lambda p: 0.5 * np.dot(q, oracle.realspace(p, q, box, 9.0, 0.35)[0])
+    # the truncated sum jumps when a pair crosses rc; random geometry keeps pairs away from it
+    assert abs(_fd(er, pos, 5, 0, 1e-6) - Fr[5, 0]) < 1e-7
+    # PME: analytic forces are the exact derivative of the PME energy
+    pp, Fp, Ep = oracle.pme_recip(pos, q, box, [24, 24, 28], 6, 0.35)
+    ep = lambda p: oracle.pme_recip(p, q, box, [24, 24, 28], 6, 0.35)[2]
+    for (i, k) in [(0, 0), (7, 1), (11, 2)]:
+        assert abs(_fd(ep, pos, i, k) - Fp[i, k]) < 1e-8
+    assert abs(Ep - 0.5 * np.dot(q, pp)) < 1e-13
+
+
+def test_realspace_matches_numpy_image_sum_and_newton3():
+    pos, q = random_neutral(30, 12.0, 4)
+    L = 12.0; rc = 5.5; al = 0.4
+    phi, F = oracle.realspace(pos, q, [L] * 3, rc, al)
+    ref = np.zeros(30); Fref = np.zeros((30, 3))
+    for i in range(30):
+        for j in range(30):
+            for n in np.ndindex(3, 3, 3):
+                if i == j:
+                    continue
+                d = pos[i] - pos[j] - (np.array(n) - 1) * L
+                r = np.linalg.norm(d)
+                if r < rc:
+                    ref[i] += q[j] * erfc(al * r) / r
+                    Fref[i] += q[i] * q[j] * (erfc(al * r) / r ** 2 + 2 * al / math.sqrt(math.pi)
+                                              * math.exp(-al * al * r * r) / r) * d / r
+    assert np.allclose(phi, ref, atol=1e-13)
+    assert np.allclose(F, Fref, atol=1e-13)
+    assert np.abs(F.sum(0)).max() < 1e-13
+    rows = np.array([3, 17, 29])
+    p2, F2 = oracle.realspace_rows(pos, q, [L] * 3, rc, al, rows)
+    assert np.array_equal(p2, phi[rows]) and np.array_equal(F2, F[rows])
+
+
+# ---------------------------------------------------------------- neighbour list
+def test_neighbour_list_vs_periodic_kdtree():
+    rng = np.random.default_rng(5)
+    box = np.array([11.0, 12.5, 14.0])
+    pos = rng.uniform(0, 1, (400, 3)) * box
+    shifted = pos + rng.integers(-2, 3, (400, 3)) * box      # unwrapped input
+    rl = 4.9
+    i, j, s = oracle.neighbour_list(shifted, box, rl)
+    tree = cKDTree(pos % box, boxsize=box)
+    ref = tree.query_pairs(rl, output_type="ndarray")
+    ref = np.sort(ref, axis=1)
+    ref = ref[np.lexsort((ref[:, 1], ref[:, 0]))]
+    assert np.array_equal(np.stack([i, j], 1), ref)
+    # shift reproduces the in-range vector from the RAW positions
+    d = shifted[j] + s * box - shifted[i]
+    r = np.linalg.norm(d, axis=1)
+    assert (r < rl).all()
+    # sorted by (i,j), unique
+    key = i.astype(np.int64) * 400 + j
+    assert (np.diff(key) > 0).all() and (i < j).all()
+
+
+def test_neighbour_list_hand_case_strict_cutoff_and_face_crossing():
+    box = [10.0, 10.0, 10.0]
+    pos = np.array([[0.5, 5.0, 5.0], [9.5, 5.0, 5.0], [4.5, 5.0, 5.0]])
+    # 0-1 are 1.0 apart across the x face; 0-2 are exactly 4.0 apart
+    i, j, s = oracle.neighbour_list(pos, box, 4.0)
+    assert list(zip(i, j)) == [(0, 1)]              # strict '<': r = 4.0 is excluded
+    assert s.tolist() == [[-1, 0, 0]]
+    i, j, s = oracle.neighbour_list(pos, box, 4.0 + 1e-12)
+    assert list(zip(i, j)) == [(0, 1), (0, 2)]
+    jr, sr = oracle.neighbour_row(pos, box, 4.0, 1)
+    assert jr.tolist() == [0] and sr.tolist() == [[1, 0, 0]]
+
+
+def test_neighbour_rows_are_the_symmetric_closure():
+    pos, q = W.make(0)
+    box = W.CONFIGS[0].box
+    i, j, s = oracle.neighbour_list(pos, box, 9.0)
+    for a in (0, 101, 647):
+        jr, sr = oracle.neighbour_row(pos, box, 9.0, a)
+        up = j[i == a]; dn = i[j == a]
+        assert np.array_equal(np.sort(np.concatenate([up, dn])), jr)
+        assert np.array_equal(sr[jr > a], s[i == a])
+        assert np.array_equal(sr[jr < a], -s[j == a])
+
+
+# ---------------------------------------------------------------- PME pieces
+def test_bspline_vs_scipy_and_knot_values():
+    for p in (4, 5, 6, 8):
+        b = BSpline.basis_element(np.arange(p + 1), extrapolate=False)
+        for u in np.linspace(0.01, p - 0.01, 57):
+            assert abs(oracle.bspline(p, u) - float(b(u))) < 1e-14
+            assert abs(oracle.bspline_deriv(p, u) - float(b.derivative()(u))) < 1e-13
+    knots = [float(v) for v in GOLD["m6_knots_x120"]]
+    assert np.allclose([oracle.bspline(6, k) * 120 for k in range(1, 6)], knots, atol=1e-13)
+    for w in (0.0, 0.3, 0.999):
+        assert abs(sum(oracle.bspline(6, w + j) for j in range(6)) - 1) < 1e-14
+        assert abs(sum(oracle.bspline_deriv(6, w + j) for j in range(6))) < 1e-14
+
+
+def test_dft3_vs_numpy_fft():
+    rng = np.random.default_rng(6)
+    z = rng.normal(size=(6, 10, 9)) + 1j * rng.normal(size=(6, 10, 9))
+    assert np.allclose(oracle.dft3(z, -1), np.fft.fftn(z), atol=1e-11)
+    assert np.allclose(oracle.dft3(z, +1), np.fft.ifftn(z) * z.size, atol=1e-11)
+
+
+def test_spread_conserves_charge_and_matches_definition():
+    pos, q = random_neutral(15, 10.0, 7)
+    q = q + 0.2
+    box = np.array([10.0, 10.0, 10.0]); K = np.array([12, 14, 16])
+    Q = oracle.pme_spread(pos - 30.0, q, box, K, 6)       # also exercises wrapping
+    assert abs(Q.sum() - q.sum()) < 1e-13
+    # definition: Q(k) = sum_i q_i prod_d sum_n M_6(u_d - k_d - n K_d)
+    b = BSpline.basis_element(np.arange(7), extrapolate=False)
+    M = lambda x: np.nan_to_num(b(x))
+    u = ((pos - 30.0) / box % 1.0) * K
+    ref = np.zeros(K)
+    for a in range(len(q)):
+        w = []
+        for d in range(3):
+            k = np.arange(K[d])
+            w.append(sum(M(u[a, d] - k - n * K[d]) for n in (-1, 0, 1)))
+        ref += q[a] * np.einsum("i,j,k->ijk", *w)
+    assert np.allclose(Q, ref, atol=1e-14)
+
+
+def test_influence_function_is_eq4_times_bspline_deconvolution():
+    box = np.array([9.0, 10.0, 11.0]); K = [10, 12, 14]; al = 0.4
+    G = oracle.pme_influence(box, K, 6, al)
+    assert G[0, 0, 0] == 0.0
+    V = box.prod()
+    for m in [(1, 0, 0), (2, 3, 1), (9, 11, 13), (5, 6, 7)]:
+        mp = [mi if mi <= Ki // 2 else mi - Ki for mi, Ki in zip(m, K)]
+        k = 2 * math.pi * np.array(mp) / box
+        k2 = np.dot(k, k)
+        eq4 = 4 * math.pi / k2 * math.exp(-k2 / (4 * al * al)) / V      # (1/2V)(4 pi/k^2)e^.. x2
+        B = 1.0
+        for d in range(3):
+            s = sum(oracle.bspline(6, kk + 1) * np.exp(2j * math.pi * m[d] * kk / K[d]) for kk in range(5))
+            B /= abs(s) ** 2
+        assert abs(G[m] / (eq4 * B) - 1) < 1e-12
+    # Hermitian symmetry G(m) = G(-m)
+    assert np.allclose(G[1:, 1:, 1:], G[1:, 1:, 1:][::-1, ::-1, ::-1], rtol=1e-13)
+
+
+def test_pme_exact_invariants():
+    pos, q = random_neutral(25, 12.0, 8)
+    box = np.array([12.0, 13.0, 14.0]); K = np.array([16, 18, 20])
+    p1, F1, E1, Q1, P1 = oracle.pme_recip(pos, q, box, K, 6, 0.4, return_grids=True)
+    # shifting all atoms by whole grid spacings changes nothing
+    h = box / K
+    p2, F2, E2 = oracle.pme_recip(pos + h * [3, -5, 40], q, box, K, 6, 0.4)
+    assert np.allclose(p1, p2, atol=1e-13) and np.allclose(F1, F2, atol=1e-13)
+    assert abs(E1 - E2) < 1e-13
+    # operator symmetry x^T phi[y] = y^T phi[x]
+    x = np.random.default_rng(1).normal(size=25); y = np.random.default_rng(2).normal(size=25)
+    px = oracle.pme_recip(pos, x, box, K, 6, 0.4)[0]
+    py = oracle.pme_recip(pos, y, box, K, 6, 0.4)[0]
+    assert abs(np.dot(x, py) - np.dot(y, px)) < 1e-13
+    # Phi is dE/dQ: E = 1/2 sum Q Phi
+    assert abs(E1 - 0.5 * (Q1 * P1).sum()) < 1e-13
+
+
+def test_pme_converges_to_direct_ewald_with_grid_refinement():
+    pos, q = random_neutral(40, 12.0, 9)
+    box = [12.0] * 3
+    # alpha = 0.9: erfc(0.9 * 5.99) = 2e-14, so the rc < L/2 real-space sum is converged and
+    # the whole difference to direct Ewald is PME's discretisation error
+    pd, Fd, Ed = oracle.ewald_direct(pos, q, box, 0.9)
+    errs = []
+    for K in (24, 36, 48):
+        pp, Fp, Ep, _ = oracle.coulomb_pme(pos, q, box, 5.99, 0.9, K, 6)
+        errs.append((relrms(pp, pd), relrms(Fp, Fd)))
+    assert errs[0][0] > 5 * errs[1][0] > 25 * errs[2][0]      # ~h^6 convergence
+    assert errs[0][1] > 4 * errs[1][1] > 16 * errs[2][1]
+    assert errs[2][0] < 1e-5 and errs[2][1] < 1e-4
+
+
+def test_pme_vs_direct_ewald_config0():
+    c = W.CONFIGS[0]
+    pos, q = W.make(0)
+    pd, Fd, Ed = oracle.ewald_direct(pos, q, c.box, c.alpha)
+    pp, Fp, Ep, _ = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order)
+    assert relrms(pp, pd) < 2e-5          # method error at h = 0.776 A, order 6
+    assert relrms(Fp, Fd) < 5e-5
+    assert abs(Ep / Ed - 1) < 2e-5
+
+
+def test_config0_generator_regression_pins():
+    pos, q = W.make(0)
+    c = W.CONFIGS[0]
+    assert pos.dtype == np.float32 and pos.shape == (648, 3)
+    assert abs(q.sum()) < 1e-4
+    i, j, s = oracle.neighbour_list(pos, c.box, 9.0)
+    assert abs(2 * len(i) / 648 - g("cfg0_neighbours_per_atom_9A")) < 0.01
+    d = pos[j].astype(float) + s * c.box - pos[i].astype(float)
+    assert abs(np.linalg.norm(d, axis=1).min() - g("cfg0_min_distance")) < 1e-3
+    E = oracle.ewald_direct(pos, q, c.box, 0.5)[2]
+    assert abs(E - g("cfg0_E_coul")) < 2e-3
+
+
+# ---------------------------------------------------------------- QEq
+def test_qeq_operator_symmetric_and_dense_solution_equalises():
+    pos, q0 = random_neutral(18, 14.0, 10, dmin=1.2)
+    box = [14.0] * 3
+    A = oracle.coulomb_matrix_pme(pos, box, 6.5, 0.4, 16, 6)
+    assert np.abs(A - A.T).max() < 1e-13                     # symmetry of C
+    # A reproduces phi[q] for an arbitrary vector
+    assert np.allclose(A @ q0, oracle.coulomb_pme(pos, q0, box, 6.5, 0.4, 16, 6)[0], atol=1e-13)
+    rng = np.random.default_rng(3)
+    chi = rng.uniform(-1, 1, 18); J = rng.uniform(20, 30, 18)
+    q, lam = oracle.qeq_dense_solve(A, chi, J, oracle.KE_EV_A, 0.5)
+    assert abs(q.sum() - 0.5) < 1e-12                        # Eq. 17
+    mu = chi + J * q + oracle.KE_EV_A * (A @ q)              # dE/dq_i, Eq. 16
+    assert np.abs(mu + lam).max() < 1e-11                    # electronegativity equalisation
+    assert oracle.qeq_residual(pos, box, 6.5, 0.4, 16, 6, chi, J, oracle.KE_EV_A, 0.5, q, lam) < 1e-12
+    # q minimises E(q) = q.chi + 1/2 q.J q + 1/2 ke q.A q on the constraint surface
+    Efun = lambda v: v @ chi + 0.5 * v @ (J * v) + 0.5 * oracle.KE_EV_A * v @ A @ v
+    dq = rng.normal(size=18); dq -= dq.mean()
+    assert Efun(q + 1e-3 * dq) > Efun(q) and Efun(q - 1e-3 * dq) > Efun(q)
+
+
+def test_shadow_closed_form_eq22():
+    rng = np.random.default_rng(4)
+    n = rng.normal(size=12); chi = rng.uniform(-1, 1, 12); u = rng.uniform(5, 10, 12)
+    v = rng.normal(size=12)
+    q, lam = oracle.shadow_charges(chi, u, v, 0.25)
+    assert abs(q.sum() - 0.25) < 1e-13
+    assert np.abs(u * q + lam + chi + v).max() < 1e-13       # rows of Eq. 22
