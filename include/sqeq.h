@@ -1,0 +1,190 @@
+/* sqeq.h -- C ABI of libsqeq: B200-native periodic Coulomb evaluation for the shadow
+ * charge-equilibration MD of arxiv 2503.21176 (cell-list neighbour build, erfc-screened
+ * real-space pair sum, smooth Particle Mesh Ewald, and the QEq / shadow-MD drivers built on
+ * them).  Citations "PAPER.md:N" are lines of the paper text; "DESIGN.md R-x" are the readings
+ * adopted where the paper is silent or garbled.
+ *
+ * General conventions
+ *  - Every call returns SQEQ_OK (0) or a negative SQEQ_E* code; the message is available from
+ *    sqeq_last_error(ctx).  No exceptions, no abort().
+ *  - "device" pointers are CUDA device memory owned by the caller (e.g. torch tensor
+ *    data_ptr()); "host" pointers are ordinary host memory.  The library owns the context, the
+ *    neighbour lists, all workspaces and the cuFFT plans.
+ *  - All work is enqueued on the context's stream.  A call synchronises that stream only where
+ *    it returns a host scalar (documented per call).
+ *  - Orthorhombic periodic boxes: box = host double[3] edge lengths (Angstrom).  Positions are
+ *    device fp32 [n][3] row-major, any finite values (wrapped internally), |x| < 127 box edges.
+ *  - Units: k_e = 1 in sqeq_coulomb (e, Angstrom, e/Angstrom, e^2/Angstrom); the QEq and MD
+ *    drivers take ke explicitly (14.3996454784255 eV*Angstrom/e^2 for eV parameters).
+ *  - One context per host thread; a context is bound to one device.
+ *  - There is no CPU fallback: every entry point fails with SQEQ_ECUDA if no device is usable.
+ */
+#ifndef SQEQ_H
+#define SQEQ_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SQEQ_OK          0
+#define SQEQ_EINVAL     -1   /* bad argument (n<=0, box<=0 or non-finite, cutoff>=min(box)/2, rc>list cutoff,
+                                grid<order, unsupported order, NULL where not allowed, |x| too large) */
+#define SQEQ_ECAPACITY  -2   /* an internal fixed-capacity buffer overflowed (message says which) */
+#define SQEQ_ECUDA      -3   /* CUDA runtime error */
+#define SQEQ_ECUFFT     -4   /* cuFFT error */
+#define SQEQ_ENOTCONV   -5   /* sqeq_qeq_solve: max_iter reached; last iterate and residual still written */
+#define SQEQ_ENOMEM     -6   /* device or host allocation failed */
+
+typedef struct sqeq_ctx   sqeq_ctx;    /* opaque: stream, workspaces, cuFFT plans */
+typedef struct sqeq_nlist sqeq_nlist;  /* opaque: device neighbour list + cell-major permutation */
+
+/* ---- context ------------------------------------------------------------------------------- */
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (may be NULL = legacy default stream); the
+ * caller keeps ownership of the stream. */
+int  sqeq_create (sqeq_ctx** out, int device, void* cuda_stream);
+int  sqeq_destroy(sqeq_ctx* ctx);
+/* Context-owned NUL-terminated message of the last failing call; never freed by the caller.
+ * ctx may be NULL (returns the message of the last failing sqeq_create in this thread). */
+const char* sqeq_last_error(const sqeq_ctx* ctx);
+/* Library version string and the compute capability it was built for ("sm_100a"). */
+const char* sqeq_version(void);
+
+/* ---- neighbour list: PAPER.md:43-71 (section 3.1, Alg. 1) ------------------------------------
+ * Builds the list of all pairs with minimum-image distance STRICTLY below `cutoff`
+ * (= r_c + skin), defined as the fp64 predicate of DESIGN.md R-NL evaluated on the fp32 input
+ * values, so the set is unique and bit-reproducible.
+ *   n       number of atoms, 1 <= n < 2^27
+ *   pos     device fp32 [n][3]
+ *   box     host double[3]
+ *   cutoff  list cutoff; must satisfy 0 < cutoff < min(box)/2 (one image per pair)
+ *   out     receives a new list handle (free with sqeq_nl_free)
+ * Internally: atoms are wrapped, binned into cells of edge >= cutoff, reordered cell-major; the
+ * list is a directed CSR over the reordered atoms with the 27-valued image code packed into each
+ * 32-bit entry.  Synchronises the stream (the pair count sizes the list allocation). */
+int  sqeq_nl_build (sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3],
+                    double cutoff, sqeq_nlist** out);
+/* Number of unique (i<j) pairs in the list.  host int64 out. */
+int  sqeq_nl_count (const sqeq_nlist* nl, int64_t* n_pairs_unique);
+/* Canonical export for parity: unique pairs i<j in the CALLER's atom numbering, sorted by (i,j);
+ * shift3[k] = int8[3] s such that pos[j] + s*box - pos[i] (raw, unwrapped caller positions at
+ * build time) is the in-range vector.  i, j: device int32 [n_pairs_unique]; shift3: device int8
+ * [n_pairs_unique][3]; caller-owned.  Synchronises the stream. */
+int  sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
+/* List introspection (host outputs, any may be NULL): cells per axis, directed entries, max row. */
+int  sqeq_nl_info  (const sqeq_nlist* nl, int ncell[3], int64_t* n_directed, int* max_row);
+int  sqeq_nl_free  (sqeq_nlist* nl);
+
+/* ---- Coulomb evaluation: Eq. 2 = Eq. 3 (real space, r < rc) + Alg. 2 (smooth PME,
+ * PAPER.md:140-151) + Eq. 5 (self term) ------------------------------------------------------
+ *   nl      list built from (an earlier state of) these atoms; positions may have moved by less
+ *           than (list cutoff - rc)/2 since the build.  Pairs are re-tested against rc in-kernel.
+ *   pos     device fp32 [n][3], current positions, caller order
+ *   q       device fp32 [n], charges (any vector: Krylov vectors need not be neutral; the uniform
+ *           background term is omitted, DESIGN.md R-G11)
+ *   rc      real-space cutoff, 0 < rc <= list cutoff
+ *   alpha   Ewald splitting parameter (1/Angstrom), > 0
+ *   grid    host int[3] PME grid points per axis, each >= order and even; order in {4, 6, 8}
+ *   phi     device fp32 [n]    out: phi_i = dE/dq_i (may be NULL)
+ *   force   device fp32 [n][3] out: F_i = -dE/dr_i; NULL selects the cheaper potential-only mode
+ *   energy  host double* out: E = 1/2 sum q_i phi_i (may be NULL; non-NULL synchronises the stream)
+ */
+int  sqeq_coulomb  (sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                    const float* q, const double box[3], double rc, double alpha,
+                    const int grid[3], int order, float* phi, float* force, double* energy);
+
+/* The same evaluation with HOST buffers (pos, q, phi, force are host fp32 arrays, ideally pinned):
+ * host->device copies of pos and q, the evaluation, and device->host copies of phi / force all
+ * happen inside the call on the context's stream; always synchronises.  This is the end-to-end
+ * entry bench.py times (copies inside the timed region). */
+int  sqeq_coulomb_host(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos_host,
+                       const float* q_host, const double box[3], double rc, double alpha,
+                       const int grid[3], int order, float* phi_host, float* force_host,
+                       double* energy);
+
+/* Parts of the last sqeq_coulomb call on this context, for diagnostics and stage-wise parity
+ * (caller order; device fp32 outputs, any may be NULL): phi_real[n], F_real[n][3], phi_rec[n],
+ * F_rec[n][3]; host double E_rec = 1/2 sum_m G|Qhat|^2 (Alg. 2 step 3).  Synchronises. */
+int  sqeq_coulomb_parts(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* phi_real,
+                        float* F_real, float* phi_rec, float* F_rec, double* E_rec);
+/* Copies the PME real-space grids of the last call: charge grid Q after step 1 (if which = 0) or
+ * potential grid Phi after step 4 (which = 1) into device fp32 out[K0][K1][K2]. */
+int  sqeq_pme_grid (sqeq_ctx* ctx, int which, float* out);
+
+/* ---- QEq solve: Eq. 18, matrix-free GMRES with C v = J o v + ke*phi[v]
+ * (PAPER.md:186-194); zero initial guess, fp64 Krylov basis, CGS2 orthogonalisation --------------
+ *   chi, J      device fp32 [n] electronegativity and hardness
+ *   tol         stop when the GMRES residual estimate ||b-Ax||/||b|| <= tol
+ *   max_iter    maximum number of Coulomb evaluations; restart: Krylov dimension (0 = unrestarted,
+ *               i.e. up to max_iter vectors)
+ *   q_out       device fp32 [n]; lambda_out, iters_out, relres_out: host scalars (may be NULL)
+ * Returns SQEQ_ENOTCONV if tol was not reached (outputs are still written).  Synchronises. */
+int  sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                    const double box[3], double rc, double alpha, const int grid[3], int order,
+                    double ke, const float* chi, const float* J, double total_charge,
+                    double tol, int max_iter, int restart,
+                    float* q_out, double* lambda_out, int* iters_out, double* relres_out);
+
+/* ---- shadow XL-BOMD step: PAPER.md:206-246 (Eqs. 20-27); DESIGN.md R-MD ------------------------
+ * State arrays are caller-owned device memory, updated in place:
+ *   pos [n][3], vel [n][3] fp32 (Angstrom, Angstrom/fs); mass [n] fp32 (amu);
+ *   nhist fp64 [nhist_len][n]: n(t), n(t-dt), ... most recent first (nhist_len = 7);
+ *   chi, u [n] fp32 (eV/e, eV/e^2);
+ *   molecule stand-in potential: atoms 3m, 3m+1, 3m+2 form O,H,H with harmonic O-H and H-H terms
+ *   (k_oh, r_oh, k_hh, r_hh; eV/Angstrom^2, Angstrom); pass k_oh = k_hh = 0 to disable.
+ * One call advances one velocity-Verlet step of length dt (fs) with `krylov_rank` Krylov updates
+ * of the kernel equation J ndd = -omega^2 (q[n] - n) (Eq. 27).  force [n][3] fp32 holds F(t) on
+ * entry (from the previous step, or from sqeq_shadow_md_init) and F(t+dt) on exit.
+ * energies: host double[4] out = {shadow potential energy (Eq. 21 incl. stand-in), kinetic energy,
+ * ||q[n]-n||_2, Coulomb evaluations done}; may be NULL (then the call does not synchronise). */
+typedef struct sqeq_md_params {
+    double dt;            /* fs */
+    double ke;            /* eV*Angstrom/e^2 */
+    double total_charge;
+    double rc, alpha;
+    int    grid[3];
+    int    order;
+    int    krylov_rank;   /* m Krylov updates per step (cfg 4: 4) */
+    double k_oh, r_oh, k_hh, r_hh;
+    double kappa;         /* dt^2 omega^2 */
+    double alpha_diss;    /* dissipation strength */
+    double c[7];          /* dissipation coefficients c_0..c_6 */
+} sqeq_md_params;
+
+int  sqeq_shadow_md_init(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                         const double box[3], const sqeq_md_params* p, const float* chi,
+                         const float* u, double tol, int max_iter,
+                         double* nhist, float* force, double* energies);
+int  sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* pos, float* vel,
+                         const float* mass, const double box[3], const sqeq_md_params* p,
+                         const float* chi, const float* u, double* nhist, float* force,
+                         double* energies);
+
+/* ---- per-stage device timing (CUDA events on the context's stream) ----------------------------
+ * Stages: see SQEQ_T_*.  Enable, run, then read: total milliseconds and number of launches per
+ * stage since the last reset.  sqeq_profile_read synchronises the stream. */
+enum {
+    SQEQ_T_NL_BIN = 0,   /* bin + sort + reorder                      (a-1) */
+    SQEQ_T_NL_PAIRS,     /* pair enumeration, count + fill            (a-2) */
+    SQEQ_T_PREP,         /* per-evaluation re-gather / fractional coordinates */
+    SQEQ_T_REAL,         /* real-space erfc pair sum                  (a-3) */
+    SQEQ_T_SPREAD,       /* B-spline spreading incl. grid clear       (a-4) */
+    SQEQ_T_FFT_FWD,      /* cuFFT R2C                                 (a-5) */
+    SQEQ_T_INFLUENCE,    /* influence multiply + energy               (a-6) */
+    SQEQ_T_FFT_INV,      /* cuFFT C2R                                 (a-7) */
+    SQEQ_T_GATHER,       /* gather                                    (a-8) */
+    SQEQ_T_ASSEMBLE,     /* self term, sum, un-permute, energy        (a-9) */
+    SQEQ_T_KRYLOV,       /* GMRES / MD vector algebra                 (a-10, a-11) */
+    SQEQ_T_COUNT
+};
+int  sqeq_profile_enable(sqeq_ctx* ctx, int on);
+int  sqeq_profile_reset (sqeq_ctx* ctx);
+int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* launches);
+/* Number of the library's own kernel launches (cuFFT's excluded) since sqeq_create / last reset. */
+int  sqeq_launch_count  (sqeq_ctx* ctx, int64_t* launches, int reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SQEQ_H */

@@ -1,0 +1,304 @@
+"""Thin ctypes binding of libsqeq (include/sqeq.h): argument marshalling only.
+
+Every step of the path runs in the CUDA library; PyTorch supplies device memory and streams.
+There is no fallback: `load()` raises if the library is missing, and every call raises
+`SqeqError` with the library's message on a non-zero return code.
+"""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsqeq.so")
+
+OK, EINVAL, ECAPACITY, ECUDA, ECUFFT, ENOTCONV, ENOMEM = 0, -1, -2, -3, -4, -5, -6
+STAGES = ["nl_bin", "nl_pairs", "prep", "real", "spread", "fft_fwd", "influence", "fft_inv",
+          "gather", "assemble", "krylov"]
+
+_lib = None
+
+
+class SqeqError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libsqeq error {code}: {msg}")
+        self.code = code
+
+
+class MdParams(ctypes.Structure):
+    _fields_ = [("dt", ctypes.c_double), ("ke", ctypes.c_double), ("total_charge", ctypes.c_double),
+                ("rc", ctypes.c_double), ("alpha", ctypes.c_double), ("grid", ctypes.c_int * 3),
+                ("order", ctypes.c_int), ("krylov_rank", ctypes.c_int),
+                ("k_oh", ctypes.c_double), ("r_oh", ctypes.c_double),
+                ("k_hh", ctypes.c_double), ("r_hh", ctypes.c_double),
+                ("kappa", ctypes.c_double), ("alpha_diss", ctypes.c_double),
+                ("c", ctypes.c_double * 7)]
+
+
+def load():
+    """Load libsqeq.so (built in-tree by `python -m paper_2503_21176_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2503_21176_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, dbl, cint = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+    dp = ctypes.POINTER(ctypes.c_double)
+    ip = ctypes.POINTER(ctypes.c_int)
+    L.sqeq_version.restype = ctypes.c_char_p
+    L.sqeq_last_error.restype = ctypes.c_char_p
+    L.sqeq_last_error.argtypes = [vp]
+    L.sqeq_create.argtypes = [ctypes.POINTER(vp), cint, vp]
+    L.sqeq_destroy.argtypes = [vp]
+    L.sqeq_nl_build.argtypes = [vp, i64, vp, dp, dbl, ctypes.POINTER(vp)]
+    L.sqeq_nl_count.argtypes = [vp, ctypes.POINTER(i64)]
+    L.sqeq_nl_export.argtypes = [vp, vp, vp, vp, vp]
+    L.sqeq_nl_info.argtypes = [vp, ip, ctypes.POINTER(i64), ip]
+    L.sqeq_nl_free.argtypes = [vp]
+    L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
+    L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
+    L.sqeq_coulomb_parts.argtypes = [vp, vp, i64, vp, vp, vp, vp, dp]
+    L.sqeq_pme_grid.argtypes = [vp, cint, vp]
+    L.sqeq_qeq_solve.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint, dbl, vp, vp, dbl, dbl, cint,
+                                 cint, vp, dp, ip, dp]
+    L.sqeq_shadow_md_init.argtypes = [vp, vp, i64, vp, dp, ctypes.POINTER(MdParams), vp, vp, dbl, cint,
+                                      vp, vp, dp]
+    L.sqeq_shadow_md_step.argtypes = [vp, vp, i64, vp, vp, vp, dp, ctypes.POINTER(MdParams), vp, vp,
+                                      vp, vp, dp]
+    L.sqeq_profile_enable.argtypes = [vp, cint]
+    L.sqeq_profile_reset.argtypes = [vp]
+    L.sqeq_profile_read.argtypes = [vp, cint, dp, ctypes.POINTER(i64)]
+    L.sqeq_launch_count.argtypes = [vp, ctypes.POINTER(i64), cint]
+    _lib = L
+    return L
+
+
+def _box(box):
+    b = np.ascontiguousarray(np.asarray(box, dtype=np.float64).reshape(-1))
+    if b.size == 1:
+        b = np.repeat(b, 3)
+    return (ctypes.c_double * 3)(*b.tolist())
+
+
+def _grid(grid):
+    g = np.asarray(grid, dtype=np.int64).reshape(-1)
+    if g.size == 1:
+        g = np.repeat(g, 3)
+    return (ctypes.c_int * 3)(*[int(v) for v in g])
+
+
+def _ptr(t, dtype, numel=None):
+    if t is None:
+        return None
+    assert isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype, \
+        f"expected a contiguous CUDA tensor of {dtype}"
+    if numel is not None:
+        assert t.numel() == numel, f"expected {numel} elements, got {t.numel()}"
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class NeighbourList:
+    """Handle of a device neighbour list (sqeq_nlist*)."""
+
+    def __init__(self, ctx, handle, n, box, cutoff):
+        self.ctx, self.handle, self.n, self.box, self.cutoff = ctx, handle, n, box, cutoff
+
+    def count(self):
+        c = ctypes.c_int64()
+        self.ctx._check(load().sqeq_nl_count(self.handle, ctypes.byref(c)))
+        return c.value
+
+    def info(self):
+        nc = (ctypes.c_int * 3)()
+        nd = ctypes.c_int64()
+        mr = ctypes.c_int()
+        self.ctx._check(load().sqeq_nl_info(self.handle, nc, ctypes.byref(nd), ctypes.byref(mr)))
+        return dict(ncell=list(nc), n_directed=nd.value, max_row=mr.value)
+
+    def export(self):
+        """Canonical (i, j, shift) arrays on the device: unique pairs i<j sorted by (i,j)."""
+        m = self.count()
+        dev = self.ctx.device
+        i = torch.empty(m, dtype=torch.int32, device=dev)
+        j = torch.empty(m, dtype=torch.int32, device=dev)
+        s = torch.empty((m, 3), dtype=torch.int8, device=dev)
+        self.ctx._check(load().sqeq_nl_export(self.ctx.handle, self.handle,
+                                              ctypes.c_void_p(i.data_ptr()), ctypes.c_void_p(j.data_ptr()),
+                                              ctypes.c_void_p(s.data_ptr())))
+        return i, j, s
+
+    def free(self):
+        if self.handle:
+            load().sqeq_nl_free(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Context:
+    """sqeq_ctx*: bound to one device and one stream (default: torch's current stream)."""
+
+    def __init__(self, device=0, stream=None):
+        L = load()
+        if not torch.cuda.is_available():
+            raise SqeqError(ECUDA, "no CUDA device: libsqeq has no CPU fallback")
+        self.device = torch.device("cuda", device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        h = ctypes.c_void_p()
+        rc = L.sqeq_create(ctypes.byref(h), device, ctypes.c_void_p(stream.cuda_stream))
+        if rc != OK:
+            raise SqeqError(rc, L.sqeq_last_error(None).decode())
+        self.handle = h
+
+    def _check(self, rc, allow=()):
+        if rc != OK and rc not in allow:
+            raise SqeqError(rc, load().sqeq_last_error(self.handle).decode())
+        return rc
+
+    def close(self):
+        if self.handle:
+            load().sqeq_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- nl_build(pos, box, cutoff) -> pair list
+    def nl_build(self, pos, box, cutoff):
+        n = pos.shape[0]
+        h = ctypes.c_void_p()
+        self._check(load().sqeq_nl_build(self.handle, n, _ptr(pos, torch.float32, 3 * n), _box(box),
+                                         float(cutoff), ctypes.byref(h)))
+        return NeighbourList(self, h, n, box, cutoff)
+
+    # ---- coulomb(pos, q, box, alpha, grid, order) -> per-atom potential, forces, energy
+    def coulomb(self, nl, pos, q, box, rc, alpha, grid, order=6, want_force=True, want_energy=True,
+                phi=None, force=None):
+        n = pos.shape[0]
+        if phi is None:
+            phi = torch.empty(n, dtype=torch.float32, device=self.device)
+        if want_force and force is None:
+            force = torch.empty((n, 3), dtype=torch.float32, device=self.device)
+        e = ctypes.c_double()
+        self._check(load().sqeq_coulomb(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                        _ptr(q, torch.float32, n), _box(box), float(rc), float(alpha),
+                                        _grid(grid), int(order), _ptr(phi, torch.float32, n),
+                                        _ptr(force, torch.float32, 3 * n) if want_force else None,
+                                        ctypes.byref(e) if want_energy else None))
+        return phi, (force if want_force else None), (e.value if want_energy else None)
+
+    def coulomb_host(self, nl, pos, q, box, rc, alpha, grid, order, phi, force, want_energy=True):
+        """Same evaluation with HOST buffers (pinned CPU tensors): H2D and D2H copies inside the call."""
+        n = pos.shape[0]
+        for t in (pos, q, phi) + ((force,) if force is not None else ()):
+            assert not t.is_cuda and t.is_contiguous() and t.dtype == torch.float32
+        e = ctypes.c_double()
+        self._check(load().sqeq_coulomb_host(self.handle, nl.handle, n, ctypes.c_void_p(pos.data_ptr()),
+                                             ctypes.c_void_p(q.data_ptr()), _box(box), float(rc), float(alpha),
+                                             _grid(grid), int(order), ctypes.c_void_p(phi.data_ptr()),
+                                             ctypes.c_void_p(force.data_ptr()) if force is not None else None,
+                                             ctypes.byref(e) if want_energy else None))
+        return e.value if want_energy else None
+
+    def coulomb_parts(self, nl, want_force=True):
+        n = nl.n
+        mk = lambda *s: torch.empty(s, dtype=torch.float32, device=self.device)
+        pr, prc = mk(n), mk(n)
+        fr, frc = (mk(n, 3), mk(n, 3)) if want_force else (None, None)
+        e = ctypes.c_double()
+        self._check(load().sqeq_coulomb_parts(self.handle, nl.handle, n, _ptr(pr, torch.float32),
+                                              _ptr(fr, torch.float32), _ptr(prc, torch.float32),
+                                              _ptr(frc, torch.float32), ctypes.byref(e)))
+        return dict(phi_real=pr, F_real=fr, phi_rec=prc, F_rec=frc, E_rec=e.value)
+
+    def pme_grid(self, which, grid):
+        g = _grid(grid)
+        out = torch.empty(tuple(g), dtype=torch.float32, device=self.device)
+        rc = load().sqeq_pme_grid(self.handle, int(which), ctypes.c_void_p(out.data_ptr()))
+        return out if rc == OK else None
+
+    # ---- qeq_solve(chi, J, total_charge)
+    def qeq_solve(self, nl, pos, box, rc, alpha, grid, order, ke, chi, J, total_charge, tol=1e-6,
+                  max_iter=100, restart=0, raise_on_notconv=False):
+        n = pos.shape[0]
+        q = torch.empty(n, dtype=torch.float32, device=self.device)
+        lam, rel = ctypes.c_double(), ctypes.c_double()
+        it = ctypes.c_int()
+        r = self._check(load().sqeq_qeq_solve(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                              _box(box), float(rc), float(alpha), _grid(grid), int(order),
+                                              float(ke), _ptr(chi, torch.float32, n), _ptr(J, torch.float32, n),
+                                              float(total_charge), float(tol), int(max_iter), int(restart),
+                                              _ptr(q, torch.float32, n), ctypes.byref(lam), ctypes.byref(it),
+                                              ctypes.byref(rel)),
+                        allow=() if raise_on_notconv else (ENOTCONV,))
+        return q, lam.value, it.value, rel.value, r == OK
+
+    # ---- shadow XL-BOMD
+    def shadow_md_init(self, nl, pos, box, params, chi, u, tol=1e-8, max_iter=200):
+        n = pos.shape[0]
+        nhist = torch.zeros((7, n), dtype=torch.float64, device=self.device)
+        force = torch.empty((n, 3), dtype=torch.float32, device=self.device)
+        en = (ctypes.c_double * 4)()
+        self._check(load().sqeq_shadow_md_init(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                               _box(box), ctypes.byref(params), _ptr(chi, torch.float32, n),
+                                               _ptr(u, torch.float32, n), float(tol), int(max_iter),
+                                               ctypes.c_void_p(nhist.data_ptr()), _ptr(force, torch.float32),
+                                               en))
+        return nhist, force, list(en)
+
+    def shadow_md_step(self, nl, pos, vel, mass, box, params, chi, u, nhist, force, want_energies=True):
+        n = pos.shape[0]
+        en = (ctypes.c_double * 4)()
+        self._check(load().sqeq_shadow_md_step(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                               _ptr(vel, torch.float32, 3 * n), _ptr(mass, torch.float32, n),
+                                               _box(box), ctypes.byref(params), _ptr(chi, torch.float32, n),
+                                               _ptr(u, torch.float32, n), ctypes.c_void_p(nhist.data_ptr()),
+                                               _ptr(force, torch.float32, 3 * n),
+                                               en if want_energies else None))
+        return list(en) if want_energies else None
+
+    # ---- timing
+    def profile_enable(self, on=True):
+        self._check(load().sqeq_profile_enable(self.handle, int(on)))
+
+    def profile_reset(self):
+        self._check(load().sqeq_profile_reset(self.handle))
+
+    def profile_read(self):
+        out = {}
+        for k, name in enumerate(STAGES):
+            ms, cnt = ctypes.c_double(), ctypes.c_int64()
+            self._check(load().sqeq_profile_read(self.handle, k, ctypes.byref(ms), ctypes.byref(cnt)))
+            out[name] = (ms.value, cnt.value)
+        return out
+
+    def launch_count(self, reset=False):
+        c = ctypes.c_int64()
+        self._check(load().sqeq_launch_count(self.handle, ctypes.byref(c), int(reset)))
+        return c.value
+
+
+def md_params(cfg, dt=0.5, ke=14.3996454784255, total_charge=0.0, krylov_rank=4,
+              k_oh=48.0, r_oh=0.9572, k_hh=10.0, r_hh=1.5139):
+    """sqeq_md_params for a workloads.Config with the XL-BOMD constants of DESIGN.md R-MD."""
+    p = MdParams()
+    p.dt, p.ke, p.total_charge = dt, ke, total_charge
+    p.rc, p.alpha = cfg.rc, cfg.alpha
+    p.grid[:] = [cfg.grid] * 3
+    p.order, p.krylov_rank = cfg.order, krylov_rank
+    p.k_oh, p.r_oh, p.k_hh, p.r_hh = k_oh, r_oh, k_hh, r_hh
+    p.kappa, p.alpha_diss = 1.82, 0.018
+    p.c[:] = [-6.0, 14.0, -8.0, -3.0, 4.0, -1.0, 0.0]
+    return p

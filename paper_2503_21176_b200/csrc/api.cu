@@ -1,0 +1,356 @@
+// api.cu -- C-ABI entry points of libsqeq: context, error reporting, argument validation,
+// per-stage event timing, and the sqeq_coulomb orchestration (include/sqeq.h).
+#include <math.h>
+#include <stdarg.h>
+
+#include "common.cuh"
+
+static thread_local char g_create_err[512] = "";
+
+int sqeq_fail(sqeq_ctx* ctx, int code, const char* fmt, ...)
+{
+    char* dst = ctx ? ctx->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int sqeq_reserve(sqeq_ctx* ctx, DevBuf& b, size_t bytes)
+{
+    if (bytes <= b.cap) return SQEQ_OK;
+    if (b.p) {
+        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        if (ctx->stream2) CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream2));
+        cudaFree(b.p);
+        b.p = nullptr;
+        b.cap = 0;
+    }
+    size_t want = bytes + bytes / 8 + 256;
+    cudaError_t e = cudaMalloc(&b.p, want);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return sqeq_fail(ctx, SQEQ_ENOMEM, "cudaMalloc(%zu bytes) failed: %s", want,
+                         cudaGetErrorString(e));
+    }
+    b.cap = want;
+    return SQEQ_OK;
+}
+
+StageTimer::StageTimer(sqeq_ctx* c, int stage, cudaStream_t s) : ctx(c), st(s ? s : c->stream)
+{
+    if (!ctx->profiling) return;
+    TimerRec r;
+    r.stage = stage;
+    for (cudaEvent_t* e : {&r.a, &r.b}) {
+        if (!ctx->free_events.empty()) {
+            *e = ctx->free_events.back();
+            ctx->free_events.pop_back();
+        } else {
+            cudaEventCreate(e);
+        }
+    }
+    cudaEventRecord(r.a, st);
+    idx = (int)ctx->pending.size();
+    ctx->pending.push_back(r);
+}
+
+StageTimer::~StageTimer()
+{
+    if (idx >= 0) cudaEventRecord(ctx->pending[idx].b, st);
+}
+
+extern "C" {
+
+const char* sqeq_version(void) { return "sqeq-b200 0.1 (sm_100a)"; }
+
+const char* sqeq_last_error(const sqeq_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
+{
+    if (!out) return sqeq_fail(nullptr, SQEQ_EINVAL, "sqeq_create: out is NULL");
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return sqeq_fail(nullptr, SQEQ_ECUDA,
+                         "sqeq_create: no CUDA device available (%s); libsqeq has no CPU fallback",
+                         e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    if (device < 0 || device >= ndev)
+        return sqeq_fail(nullptr, SQEQ_EINVAL, "sqeq_create: device %d out of range [0,%d)", device, ndev);
+    e = cudaSetDevice(device);
+    if (e != cudaSuccess)
+        return sqeq_fail(nullptr, SQEQ_ECUDA, "cudaSetDevice(%d): %s", device, cudaGetErrorString(e));
+    sqeq_ctx* ctx = new sqeq_ctx();
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
+    e = cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_scal, 16 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->scal.p, 16 * sizeof(double));
+    if (e != cudaSuccess) {
+        sqeq_fail(nullptr, SQEQ_ECUDA, "sqeq_create: %s", cudaGetErrorString(e));
+        delete ctx;
+        return SQEQ_ECUDA;
+    }
+    ctx->scal.cap = 16 * sizeof(double);
+    *out = ctx;
+    return SQEQ_OK;
+}
+
+int sqeq_destroy(sqeq_ctx* ctx)
+{
+    if (!ctx) return SQEQ_OK;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->stream2) cudaStreamSynchronize(ctx->stream2);
+    if (ctx->plans_ok) {
+        cufftDestroy(ctx->plan_r2c);
+        cufftDestroy(ctx->plan_c2r);
+    }
+    DevBuf* bufs[] = {&ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
+                      &ctx->base, &ctx->real_out, &ctx->rec_out, &ctx->scal, &ctx->kry_V,
+                      &ctx->kry_w, &ctx->kry_h};
+    for (DevBuf* b : bufs)
+        if (b->p) cudaFree(b->p);
+    for (auto& b : ctx->vec_f) if (b.p) cudaFree(b.p);
+    for (auto& b : ctx->vec_d) if (b.p) cudaFree(b.p);
+    for (auto& b : ctx->vec_f3) if (b.p) cudaFree(b.p);
+    for (auto& b : ctx->stage) if (b.p) cudaFree(b.p);
+    if (ctx->h_scal) cudaFreeHost(ctx->h_scal);
+    for (auto& r : ctx->pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto& e : ctx->free_events) cudaEventDestroy(e);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+    if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
+    delete ctx;
+    return SQEQ_OK;
+}
+
+// ---------------------------------------------------------------------------- profiling
+static int drain_timers(sqeq_ctx* ctx)
+{
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream2));
+    for (auto& r : ctx->pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) {
+            ctx->t_total[r.stage] += ms;
+            ctx->t_count[r.stage] += 1;
+        } else {
+            cudaGetLastError();
+        }
+        ctx->free_events.push_back(r.a);
+        ctx->free_events.push_back(r.b);
+    }
+    ctx->pending.clear();
+    return SQEQ_OK;
+}
+
+int sqeq_profile_enable(sqeq_ctx* ctx, int on)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(drain_timers(ctx));
+    ctx->profiling = on != 0;
+    return SQEQ_OK;
+}
+
+int sqeq_profile_reset(sqeq_ctx* ctx)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(drain_timers(ctx));
+    for (int s = 0; s < SQEQ_T_COUNT; ++s) { ctx->t_total[s] = 0; ctx->t_count[s] = 0; }
+    return SQEQ_OK;
+}
+
+int sqeq_profile_read(sqeq_ctx* ctx, int stage, double* total_ms, int64_t* launches)
+{
+    if (!ctx || stage < 0 || stage >= SQEQ_T_COUNT)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_profile_read: bad stage %d", stage);
+    SQEQ_TRY(drain_timers(ctx));
+    if (total_ms) *total_ms = ctx->t_total[stage];
+    if (launches) *launches = ctx->t_count[stage];
+    return SQEQ_OK;
+}
+
+int sqeq_launch_count(sqeq_ctx* ctx, int64_t* launches, int reset)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (launches) *launches = ctx->launches;
+    if (reset) ctx->launches = 0;
+    return SQEQ_OK;
+}
+
+// ---------------------------------------------------------------------------- neighbour list
+static int check_box(sqeq_ctx* ctx, const double box[3], const char* who)
+{
+    if (!box) return sqeq_fail(ctx, SQEQ_EINVAL, "%s: box is NULL", who);
+    for (int d = 0; d < 3; ++d)
+        if (!(box[d] > 0.0) || !isfinite(box[d]))
+            return sqeq_fail(ctx, SQEQ_EINVAL, "%s: box[%d] = %g must be finite and > 0", who, d, box[d]);
+    return SQEQ_OK;
+}
+
+int sqeq_nl_build(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
+                  sqeq_nlist** out)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!out) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_build: out is NULL");
+    *out = nullptr;
+    if (n <= 0 || n >= (1LL << 27))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_build: n = %lld must be in [1, 2^27)", (long long)n);
+    if (!pos) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_build: pos is NULL");
+    SQEQ_TRY(check_box(ctx, box, "sqeq_nl_build"));
+    double lmin = fmin(box[0], fmin(box[1], box[2]));
+    if (!(cutoff > 0.0) || !isfinite(cutoff) || !(cutoff < 0.5 * lmin))
+        return sqeq_fail(ctx, SQEQ_EINVAL,
+                         "sqeq_nl_build: cutoff %g must satisfy 0 < cutoff < min(box)/2 = %g "
+                         "(minimum image needs box > 2*cutoff)", cutoff, 0.5 * lmin);
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return nl_build_impl(ctx, n, pos, box, cutoff, out);
+}
+
+int sqeq_nl_count(const sqeq_nlist* nl, int64_t* n_pairs_unique)
+{
+    if (!nl || !n_pairs_unique) return SQEQ_EINVAL;
+    *n_pairs_unique = nl->n_directed / 2;
+    return SQEQ_OK;
+}
+
+int sqeq_nl_info(const sqeq_nlist* nl, int ncell[3], int64_t* n_directed, int* max_row)
+{
+    if (!nl) return SQEQ_EINVAL;
+    if (ncell) for (int d = 0; d < 3; ++d) ncell[d] = nl->ncell[d];
+    if (n_directed) *n_directed = nl->n_directed;
+    if (max_row) *max_row = nl->max_row;
+    return SQEQ_OK;
+}
+
+int sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!nl || nl->ctx != ctx) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_export: list does not belong to this context");
+    if (nl->n_directed > 0 && (!i || !j || !shift3))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_export: NULL output");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return nl_export_impl(ctx, nl, i, j, shift3);
+}
+
+int sqeq_nl_free(sqeq_nlist* nl)
+{
+    if (!nl) return SQEQ_OK;
+    if (nl->ctx) {
+        cudaSetDevice(nl->ctx->device);
+        cudaStreamSynchronize(nl->ctx->stream);
+        cudaStreamSynchronize(nl->ctx->stream2);
+    }
+    cudaFree(nl->perm);
+    cudaFree(nl->cell_of);
+    cudaFree(nl->cell_start);
+    cudaFree(nl->wrapc);
+    cudaFree(nl->row_start);
+    cudaFree(nl->nbr);
+    delete nl;
+    return SQEQ_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------- coulomb
+int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3],
+                          double rc, double alpha, const int grid[3], int order, const char* who)
+{
+    if (!nl || nl->ctx != ctx)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: neighbour list missing or from another context", who);
+    if (n != nl->n)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: n = %lld but the list was built for %lld atoms", who,
+                         (long long)n, (long long)nl->n);
+    SQEQ_TRY(check_box(ctx, box, who));
+    for (int d = 0; d < 3; ++d)
+        if (box[d] != nl->box[d])
+            return sqeq_fail(ctx, SQEQ_EINVAL, "%s: box differs from the box the list was built with", who);
+    if (!(rc > 0.0) || !(rc <= nl->cutoff))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: rc = %g must satisfy 0 < rc <= list cutoff %g", who, rc, nl->cutoff);
+    if (!(alpha > 0.0) || !isfinite(alpha))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: alpha = %g must be > 0", who, alpha);
+    if (order != 4 && order != 6 && order != 8)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: spline order %d unsupported (4, 6 or 8)", who, order);
+    if (!grid) return sqeq_fail(ctx, SQEQ_EINVAL, "%s: grid is NULL", who);
+    for (int d = 0; d < 3; ++d)
+        if (grid[d] < order || grid[d] > 2048 || (grid[d] & 1))
+            return sqeq_fail(ctx, SQEQ_EINVAL, "%s: grid[%d] = %d must be even and in [order, 2048]", who, d, grid[d]);
+    return SQEQ_OK;
+}
+
+int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc,
+                 double alpha, float* phi, float* force, bool want_energy)
+{
+    const bool want_force = force != nullptr;
+    // fork: PME on the side stream, real space on the main stream
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream2, ctx->ev_fork, 0));
+    SQEQ_TRY(pme_run(ctx, n, box, want_force, false, ctx->stream2));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_join, ctx->stream2));
+    SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+    SQEQ_TRY(assemble_run(ctx, nl, alpha, phi, force, want_energy, ctx->stream));
+    ctx->last_had_force = want_force;
+    ctx->last_n = n;
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_coulomb(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const float* q,
+                 const double box[3], double rc, double alpha, const int grid[3], int order,
+                 float* phi, float* force, double* energy)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_coulomb"));
+    if (!pos || !q) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb: pos or q is NULL");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    SQEQ_TRY(prep_atoms(ctx, nl, pos, q, ctx->K, ctx->stream));
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, phi, force, energy != nullptr));
+    if (energy) {
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal.p, 2 * sizeof(double),
+                                      cudaMemcpyDeviceToHost, ctx->stream));
+        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        *energy = ctx->h_scal[0];
+    }
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_coulomb_host(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos_host,
+                                 const float* q_host, const double box[3], double rc, double alpha,
+                                 const int grid[3], int order, float* phi_host, float* force_host,
+                                 double* energy)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_coulomb_host"));
+    if (!pos_host || !q_host) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_host: pos or q is NULL");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->stage[0], sizeof(float) * 3 * n));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->stage[1], sizeof(float) * n));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->stage[2], sizeof(float) * n));
+    if (force_host) SQEQ_TRY(sqeq_reserve(ctx, ctx->stage[3], sizeof(float) * 3 * n));
+    float* d_pos = (float*)ctx->stage[0].p;
+    float* d_q = (float*)ctx->stage[1].p;
+    float* d_phi = (float*)ctx->stage[2].p;
+    float* d_f = force_host ? (float*)ctx->stage[3].p : nullptr;
+    cudaStream_t st = ctx->stream;
+    CUDA_TRY(ctx, cudaMemcpyAsync(d_pos, pos_host, sizeof(float) * 3 * n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(ctx, cudaMemcpyAsync(d_q, q_host, sizeof(float) * n, cudaMemcpyHostToDevice, st));
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    SQEQ_TRY(prep_atoms(ctx, nl, d_pos, d_q, ctx->K, st));
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, d_phi, d_f, energy != nullptr));
+    if (phi_host) CUDA_TRY(ctx, cudaMemcpyAsync(phi_host, d_phi, sizeof(float) * n, cudaMemcpyDeviceToHost, st));
+    if (force_host) CUDA_TRY(ctx, cudaMemcpyAsync(force_host, d_f, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, st));
+    if (energy) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal.p, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    if (energy) *energy = ctx->h_scal[0];
+    return SQEQ_OK;
+}

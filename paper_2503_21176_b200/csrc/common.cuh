@@ -1,0 +1,150 @@
+// common.cuh -- internal declarations of libsqeq (context, list, error and timing helpers).
+// Not part of the public boundary (include/sqeq.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <vector>
+
+#include "../../include/sqeq.h"
+
+#define SQEQ_MAX_ORDER 8
+#define SQEQ_NHIST 7
+
+struct DevBuf {
+    void*  p = nullptr;
+    size_t cap = 0;
+};
+
+struct TimerRec {
+    int stage;
+    cudaEvent_t a, b;
+};
+
+struct sqeq_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    cudaStream_t stream2 = nullptr;       // side stream: PME runs beside the real-space kernel
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    char err[512] = {0};
+    int sm_count = 148;
+
+    // ---- PME state (cached by grid/order/box/alpha) ----
+    int K[3] = {0, 0, 0};
+    int order = 0;
+    double tab_box[3] = {0, 0, 0};
+    double tab_alpha = 0;
+    cufftHandle plan_r2c = 0, plan_c2r = 0;
+    bool plans_ok = false;
+    DevBuf grid;      // float  [K0][K1][K2]        charge grid Q, then potential grid Phi
+    DevBuf gridQ;     // float  copy of Q kept for sqeq_pme_grid (diagnostics only when enabled)
+    DevBuf spec;      // float2 [K0][K1][K2/2+1]
+    DevBuf tabs;      // float  per-axis tables: |b|^2, gaussian, mtilde^2  (3 x (K0+K1+K2))
+
+    // ---- per-evaluation atom workspaces (sorted = cell-major order of the list) ----
+    DevBuf xq;        // float4 [n]  wrapped x,y,z (build-time image) + charge
+    DevBuf frac;      // float4 [n]  fractional offsets w_x,w_y,w_z in [0,1), charge
+    DevBuf base;      // int4   [n]  floor grid index f_x,f_y,f_z
+    DevBuf real_out;  // float4 [n]  F_real xyz, phi_real   (sorted order)
+    DevBuf rec_out;   // float4 [n]  F_rec  xyz, phi_rec    (sorted order)
+    DevBuf scal;      // double [16] device scalars (energy sums, dots)
+    double* h_scal = nullptr;  // pinned host mirror
+    bool last_had_force = false;
+    int64_t last_n = 0;
+
+    // ---- Krylov / MD workspaces ----
+    DevBuf kry_V;     // double [m+1][n+1]
+    DevBuf kry_w;     // double [n+1]
+    DevBuf kry_h;     // double [m+2]
+    DevBuf vec_f[6];  // float  [n] scratch charge / potential vectors
+    DevBuf vec_d[6];  // double [n] scratch
+    DevBuf vec_f3[2]; // float  [n][3] scratch forces
+    DevBuf stage[4];  // device staging for sqeq_coulomb_host: pos, q, phi, force
+
+    // ---- timing ----
+    bool profiling = false;
+    std::vector<TimerRec> pending;
+    std::vector<cudaEvent_t> free_events;
+    double t_total[SQEQ_T_COUNT] = {0};
+    int64_t t_count[SQEQ_T_COUNT] = {0};
+    int64_t launches = 0;
+};
+
+struct sqeq_nlist {
+    sqeq_ctx* ctx = nullptr;
+    int64_t n = 0;
+    double box[3] = {0, 0, 0};
+    double cutoff = 0;
+    int ncell[3] = {1, 1, 1};
+    int64_t n_directed = 0;
+    int max_row = 0;
+    // device arrays
+    int*      perm = nullptr;        // [n]   sorted index -> caller index
+    int*      cell_of = nullptr;     // [n]   cell id of sorted atom
+    int*      cell_start = nullptr;  // [ncells+1]
+    char4*    wrapc = nullptr;       // [n]   floor(x/L) per axis at build time (sorted order)
+    int64_t*  row_start = nullptr;   // [n+1] CSR offsets (sorted order)
+    uint32_t* nbr = nullptr;         // [n_directed]  j (27 bits) | image code (5 bits) << 27
+};
+
+// ---------------------------------------------------------------------------------------------
+int sqeq_fail(sqeq_ctx* ctx, int code, const char* fmt, ...);
+int sqeq_reserve(sqeq_ctx* ctx, DevBuf& b, size_t bytes);
+
+#define CUDA_TRY(ctx, expr)                                                              \
+    do {                                                                                 \
+        cudaError_t _e = (expr);                                                         \
+        if (_e != cudaSuccess)                                                           \
+            return sqeq_fail((ctx), SQEQ_ECUDA, "%s failed: %s (%s:%d)", #expr,          \
+                             cudaGetErrorString(_e), __FILE__, __LINE__);                \
+    } while (0)
+
+#define SQEQ_TRY(expr)                  \
+    do {                                \
+        int _r = (expr);                \
+        if (_r != SQEQ_OK) return _r;   \
+    } while (0)
+
+#define KERNEL_CHECK(ctx)                                                                \
+    do {                                                                                 \
+        (ctx)->launches++;                                                               \
+        cudaError_t _e = cudaGetLastError();                                             \
+        if (_e != cudaSuccess)                                                           \
+            return sqeq_fail((ctx), SQEQ_ECUDA, "kernel launch failed: %s (%s:%d)",      \
+                             cudaGetErrorString(_e), __FILE__, __LINE__);                \
+    } while (0)
+
+// RAII stage timer: records a CUDA-event pair on the given stream when profiling is on.
+struct StageTimer {
+    sqeq_ctx* ctx;
+    cudaStream_t st;
+    int idx = -1;
+    StageTimer(sqeq_ctx* c, int stage, cudaStream_t s = nullptr);
+    ~StageTimer();
+};
+
+static inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ---- stage entry points (implemented in the .cu files) ----
+int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
+                  sqeq_nlist** out);
+int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
+
+// Re-gather positions/charges into the list's order (and PME fractional coordinates if K != null).
+int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* q,
+               const int* K, cudaStream_t st);
+// Only refresh the charge component (fixed geometry, new Krylov vector). q may be float or double.
+int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const double* q_d,
+                 cudaStream_t st);
+int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
+                  cudaStream_t st);
+int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3], int order);
+int pme_run(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_force, bool want_energy,
+            cudaStream_t st);
+int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, float* force,
+                 bool want_energy, cudaStream_t st);
+// Full evaluation on prepared geometry (used by coulomb, qeq and md drivers).
+int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc,
+                 double alpha, float* phi, float* force, bool want_energy);

@@ -1,0 +1,299 @@
+// qeq.cu -- a-10: matrix-free GMRES on the QEq KKT system, Eq. 18:
+//     [ C  1 ] [ q      ]   [ -chi ]
+//     [ 1' 0 ] [ lambda ] = [ Qtot ],     C v = J o v + ke * phi[v]
+// Each Krylov iteration is one potential-only Coulomb evaluation on fixed geometry ("Each
+// iteration involves calculating a Coulomb-like potential").  Krylov basis, dots and
+// updates are fp64 on the device; the (m+1) x m Hessenberg least-squares problem (Givens
+// rotations) is solved on the host.  Orthogonalisation: classical Gram-Schmidt applied twice
+// (CGS2), which needs two batched dot/update launches per iteration instead of j sequential ones.
+// Zero initial guess, no preconditioner (DESIGN.md R-G13).
+#include <math.h>
+
+#include <vector>
+
+#include "common.cuh"
+
+int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3],
+                          double rc, double alpha, const int grid[3], int order, const char* who);
+
+// b = [-chi ; Qtot]  -> V0 (unnormalised), also accumulates ||b||^2 into nrm2
+__global__ void k_qeq_rhs(int64_t n, const float* __restrict__ chi, double qtot, double* __restrict__ v0)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) v0[i] = -(double)chi[i];
+    else if (i == n) v0[n] = qtot;
+}
+
+// w = A v for v = [v_q ; mu]:  w_i = J_i v_i + ke phi_i + mu,  w_N = sum_i v_i (accumulated atomically)
+__global__ void k_qeq_matvec(int64_t n, const double* __restrict__ v, const float* __restrict__ J,
+                             const float* __restrict__ phi, double ke, double* __restrict__ w)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    double s = 0.0;
+    if (i < n) {
+        const double vi = v[i];
+        w[i] = (double)J[i] * vi + ke * (double)phi[i] + v[n];
+        s = vi;
+    }
+    __shared__ double red[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        s = red[threadIdx.x];
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) s += __shfl_xor_sync(0xffu, s, o);
+        if (threadIdx.x == 0) atomicAdd(w + n, s);
+    }
+}
+
+// h[k] += <V_k, w> for k < nv; grid = (chunks, nv); V has leading dimension ld
+#define DOT_CHUNK 8192
+__global__ void __launch_bounds__(256)
+k_dots(int64_t len, int64_t ld, const double* __restrict__ V, const double* __restrict__ w,
+       double* __restrict__ h)
+{
+    const double* vk = V + (int64_t)blockIdx.y * ld;
+    const int64_t beg = (int64_t)blockIdx.x * DOT_CHUNK;
+    const int64_t end = beg + DOT_CHUNK < len ? beg + DOT_CHUNK : len;
+    double s = 0.0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += 256) s += vk[i] * w[i];
+    __shared__ double red[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        s = red[threadIdx.x];
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) s += __shfl_xor_sync(0xffu, s, o);
+        if (threadIdx.x == 0) atomicAdd(h + blockIdx.y, s);
+    }
+}
+
+// w -= sum_k h[k] V_k
+__global__ void k_sub_combo(int64_t len, int64_t ld, int nv, const double* __restrict__ V,
+                            const double* __restrict__ h, double* __restrict__ w)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    double acc = w[i];
+    for (int k = 0; k < nv; ++k) acc -= h[k] * V[(int64_t)k * ld + i];
+    w[i] = acc;
+}
+
+// x += sum_k y[k] V_k
+__global__ void k_add_combo(int64_t len, int64_t ld, int nv, const double* __restrict__ V,
+                            const double* __restrict__ y, double* __restrict__ x)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    double acc = x[i];
+    for (int k = 0; k < nv; ++k) acc += y[k] * V[(int64_t)k * ld + i];
+    x[i] = acc;
+}
+
+// dst = src * (1/sqrt(*nrm2))
+__global__ void k_normalise(int64_t len, const double* __restrict__ src, const double* __restrict__ nrm2,
+                            double* __restrict__ dst)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    const double s = *nrm2 > 0.0 ? rsqrt(*nrm2) : 0.0;
+    dst[i] = src[i] * s;
+}
+
+__global__ void k_axpby(int64_t len, double a, const double* __restrict__ x, double b, double* __restrict__ y)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < len) y[i] = a * x[i] + b * y[i];
+}
+
+__global__ void k_d2f(int64_t n, const double* __restrict__ x, float* __restrict__ y)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) y[i] = (float)x[i];
+}
+
+struct QeqOp {
+    sqeq_ctx* ctx;
+    const sqeq_nlist* nl;
+    int64_t n;
+    const double* box;
+    double rc, alpha, ke;
+    const float* J;
+    float* phi;   // scratch [n]
+};
+
+// w = A v   (one potential-only Coulomb evaluation on the prepared geometry)
+static int qeq_apply(const QeqOp& op, const double* v, double* w)
+{
+    sqeq_ctx* ctx = op.ctx;
+    cudaStream_t st = ctx->stream;
+    const int64_t n = op.n;
+    SQEQ_TRY(prep_charges(ctx, op.nl, nullptr, v, st));
+    SQEQ_TRY(coulomb_eval(ctx, op.nl, n, op.box, op.rc, op.alpha, op.phi, nullptr, false));
+    StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+    CUDA_TRY(ctx, cudaMemsetAsync(w + n, 0, sizeof(double), st));
+    k_qeq_matvec<<<ceil_div(n, 256), 256, 0, st>>>(n, v, op.J, op.phi, op.ke, w);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                              const double box[3], double rc, double alpha, const int grid[3], int order,
+                              double ke, const float* chi, const float* J, double total_charge,
+                              double tol, int max_iter, int restart, float* q_out, double* lambda_out,
+                              int* iters_out, double* relres_out)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_qeq_solve"));
+    if (!pos || !chi || !J || !q_out) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: NULL argument");
+    if (max_iter < 1 || restart < 0 || !(tol >= 0.0))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: need max_iter >= 1, restart >= 0, tol >= 0");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int m = restart > 0 ? (restart < max_iter ? restart : max_iter) : max_iter;
+    const int64_t len = n + 1;
+    const int64_t ld = (len + 31) & ~(int64_t)31;
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_V, sizeof(double) * (size_t)ld * (m + 1)));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_w, sizeof(double) * (size_t)ld * 2));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_h, sizeof(double) * (size_t)(2 * (m + 2) + 2)));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_f[0], sizeof(float) * n));
+    double* V = (double*)ctx->kry_V.p;
+    double* w = (double*)ctx->kry_w.p;
+    double* x = w + ld;
+    double* h = (double*)ctx->kry_h.p;          // [m+2] first-pass coefficients (+ norm at [m+1])
+    double* h2 = h + (m + 2);                    // second pass
+    double* nrm2 = h2 + (m + 2);
+    std::vector<double> hh((size_t)2 * (m + 2) + 2);
+    QeqOp op{ctx, nl, n, box, rc, alpha, ke, J, (float*)ctx->vec_f[0].p};
+    // geometry once; the charge slot is refreshed per mat-vec (q = chi is only a placeholder here)
+    SQEQ_TRY(prep_atoms(ctx, nl, pos, chi, ctx->K, st));
+    const int nbl = ceil_div(len, 256);
+    const int nchunk = ceil_div(len, DOT_CHUNK);
+    CUDA_TRY(ctx, cudaMemsetAsync(x, 0, sizeof(double) * ld, st));
+
+    // |b|
+    double bnorm = 0.0;
+    {
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        k_qeq_rhs<<<nbl, 256, 0, st>>>(n, chi, total_charge, w);
+        KERNEL_CHECK(ctx);
+        CUDA_TRY(ctx, cudaMemsetAsync(nrm2, 0, sizeof(double), st));
+        k_dots<<<dim3(nchunk, 1), 256, 0, st>>>(len, ld, w, w, nrm2);
+        KERNEL_CHECK(ctx);
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 4, nrm2, sizeof(double), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        bnorm = sqrt(ctx->h_scal[4]);
+    }
+    int iters = 0;
+    double relres = 1.0;
+    bool converged = false;
+    if (bnorm == 0.0) { converged = true; relres = 0.0; }
+    bool first_cycle = true;
+    std::vector<double> H((size_t)(m + 1) * m), cs(m), sn(m), gvec(m + 1), y(m);
+    while (!converged && iters < max_iter) {
+        // r = b - A x  (x = 0 in the first cycle: r = b, already in w)
+        double beta = bnorm;
+        if (!first_cycle) {
+            double* r = V;  // reuse V_0 as scratch for A x
+            SQEQ_TRY(qeq_apply(op, x, r));
+            ++iters;
+            StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+            k_qeq_rhs<<<nbl, 256, 0, st>>>(n, chi, total_charge, w);
+            KERNEL_CHECK(ctx);
+            k_axpby<<<nbl, 256, 0, st>>>(len, -1.0, r, 1.0, w);
+            KERNEL_CHECK(ctx);
+            CUDA_TRY(ctx, cudaMemsetAsync(nrm2, 0, sizeof(double), st));
+            k_dots<<<dim3(nchunk, 1), 256, 0, st>>>(len, ld, w, w, nrm2);
+            KERNEL_CHECK(ctx);
+            CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 4, nrm2, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(ctx, cudaStreamSynchronize(st));
+            beta = sqrt(ctx->h_scal[4]);
+            relres = beta / bnorm;
+            if (relres <= tol) { converged = true; break; }
+        }
+        first_cycle = false;
+        {
+            StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+            k_normalise<<<nbl, 256, 0, st>>>(len, w, nrm2, V);
+            KERNEL_CHECK(ctx);
+        }
+        std::fill(gvec.begin(), gvec.end(), 0.0);
+        gvec[0] = beta;
+        int j = 0;
+        for (; j < m && iters < max_iter; ++j) {
+            SQEQ_TRY(qeq_apply(op, V + (int64_t)j * ld, w));
+            ++iters;
+            {
+                StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+                CUDA_TRY(ctx, cudaMemsetAsync(h, 0, sizeof(double) * (2 * (m + 2) + 1), st));
+                k_dots<<<dim3(nchunk, j + 1), 256, 0, st>>>(len, ld, V, w, h);
+                KERNEL_CHECK(ctx);
+                k_sub_combo<<<nbl, 256, 0, st>>>(len, ld, j + 1, V, h, w);
+                KERNEL_CHECK(ctx);
+                k_dots<<<dim3(nchunk, j + 1), 256, 0, st>>>(len, ld, V, w, h2);
+                KERNEL_CHECK(ctx);
+                k_sub_combo<<<nbl, 256, 0, st>>>(len, ld, j + 1, V, h2, w);
+                KERNEL_CHECK(ctx);
+                k_dots<<<dim3(nchunk, 1), 256, 0, st>>>(len, ld, w, w, nrm2);
+                KERNEL_CHECK(ctx);
+                k_normalise<<<nbl, 256, 0, st>>>(len, w, nrm2, V + (int64_t)(j + 1) * ld);
+                KERNEL_CHECK(ctx);
+                CUDA_TRY(ctx, cudaMemcpyAsync(hh.data(), h, sizeof(double) * (2 * (m + 2) + 1),
+                                              cudaMemcpyDeviceToHost, st));
+                CUDA_TRY(ctx, cudaStreamSynchronize(st));
+            }
+            // Hessenberg column j (column-major, leading dimension m+1)
+            double* Hj = H.data() + (size_t)j * (m + 1);
+            for (int k = 0; k <= j; ++k) Hj[k] = hh[k] + hh[(m + 2) + k];
+            Hj[j + 1] = sqrt(hh[2 * (m + 2)]);
+            for (int k = 0; k < j; ++k) {
+                double t = cs[k] * Hj[k] + sn[k] * Hj[k + 1];
+                Hj[k + 1] = -sn[k] * Hj[k] + cs[k] * Hj[k + 1];
+                Hj[k] = t;
+            }
+            double a = Hj[j], b = Hj[j + 1], rr = hypot(a, b);
+            cs[j] = rr > 0 ? a / rr : 1.0;
+            sn[j] = rr > 0 ? b / rr : 0.0;
+            Hj[j] = rr;
+            Hj[j + 1] = 0.0;
+            gvec[j + 1] = -sn[j] * gvec[j];
+            gvec[j] = cs[j] * gvec[j];
+            relres = fabs(gvec[j + 1]) / bnorm;
+            if (relres <= tol || b == 0.0) { ++j; converged = relres <= tol; break; }
+        }
+        // y = R^{-1} g ;  x += V y
+        const int k = j;
+        for (int i = k - 1; i >= 0; --i) {
+            double s = gvec[i];
+            for (int l = i + 1; l < k; ++l) s -= H[(size_t)l * (m + 1) + i] * y[l];
+            y[i] = s / H[(size_t)i * (m + 1) + i];
+        }
+        if (k > 0) {
+            StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+            CUDA_TRY(ctx, cudaMemcpyAsync(h, y.data(), sizeof(double) * k, cudaMemcpyHostToDevice, st));
+            k_add_combo<<<nbl, 256, 0, st>>>(len, ld, k, V, h, x);
+            KERNEL_CHECK(ctx);
+            CUDA_TRY(ctx, cudaStreamSynchronize(st));   // y is a host vector reused next cycle
+        }
+        if (converged || restart == 0) break;
+    }
+    {
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        k_d2f<<<ceil_div(n, 256), 256, 0, st>>>(n, x, q_out);
+        KERNEL_CHECK(ctx);
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 5, x + n, sizeof(double), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    }
+    if (lambda_out) *lambda_out = ctx->h_scal[5];
+    if (iters_out) *iters_out = iters;
+    if (relres_out) *relres_out = relres;
+    if (!converged)
+        return sqeq_fail(ctx, SQEQ_ENOTCONV, "sqeq_qeq_solve: relative residual %.3e > tol %.3e after %d Coulomb evaluations",
+                         relres, tol, iters);
+    return SQEQ_OK;
+}

@@ -1,0 +1,231 @@
+// realspace.cu -- per-evaluation atom re-gather (prep) and the erfc-screened real-space pair sum,
+// Eq. 3 restricted to r < rc over the neighbour list (step a-3), plus the final
+// assembly with the self term of Eq. 5 (step a-9).
+//
+// One warp per atom row: lanes stride over the row's packed entries (coalesced 128 B list loads),
+// gather the neighbour's float4 (x,y,z,q) from the cell-major array (L1/L2 resident), apply the
+// image shift from a 27-entry shared table, accumulate phi and F in registers, then a shuffle
+// reduction -- no atomics (the paper's ELLPACK row sum, without the padding).
+#include <math.h>
+
+#include "common.cuh"
+
+struct PrepGeom {
+    double L[3];
+    int    K[3];   // 0 => no PME coordinates wanted
+};
+
+__global__ void k_prep(int64_t n, const float* __restrict__ pos, const float* __restrict__ q,
+                       const int* __restrict__ perm, const char4* __restrict__ wrapc, PrepGeom g,
+                       float4* __restrict__ xq, float4* __restrict__ frac, int4* __restrict__ base)
+{
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int o = perm[s];
+    const char4 w = wrapc[s];
+    const int wd[3] = {w.x, w.y, w.z};
+    const float qi = q[o];
+    float xw[3], fw[3];
+    int f[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        // same periodic image as at build time, so the list's image codes stay valid
+        double x = (double)pos[3 * (int64_t)o + d] - (double)wd[d] * g.L[d];
+        xw[d] = (float)x;
+        if (g.K[0] > 0) {
+            // fractional grid coordinate in fp64 (an fp32 product x*K/L loses ~1e-5 of a cell at x~150)
+            double u = x / g.L[d];
+            u -= floor(u);
+            u *= (double)g.K[d];
+            int fi = (int)u;
+            if (fi >= g.K[d]) { fi -= g.K[d]; u -= (double)g.K[d]; }
+            double wv = u - (double)fi;
+            fw[d] = wv < 0.0 ? 0.f : (float)wv;
+            f[d] = fi;
+        }
+    }
+    xq[s] = make_float4(xw[0], xw[1], xw[2], qi);
+    if (g.K[0] > 0) {
+        frac[s] = make_float4(fw[0], fw[1], fw[2], qi);
+        base[s] = make_int4(f[0], f[1], f[2], 0);
+    }
+}
+
+__global__ void k_prep_charges(int64_t n, const float* __restrict__ qf, const double* __restrict__ qd,
+                               const int* __restrict__ perm, float4* __restrict__ xq,
+                               float4* __restrict__ frac)
+{
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int o = perm[s];
+    const float qi = qf ? qf[o] : (float)qd[o];
+    xq[s].w = qi;
+    frac[s].w = qi;
+}
+
+int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* q, const int* K,
+               cudaStream_t st)
+{
+    const int64_t n = nl->n;
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * n));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->frac, sizeof(float4) * n));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->base, sizeof(int4) * n));
+    PrepGeom g;
+    for (int d = 0; d < 3; ++d) { g.L[d] = nl->box[d]; g.K[d] = K ? K[d] : 0; }
+    StageTimer tm(ctx, SQEQ_T_PREP, st);
+    k_prep<<<ceil_div(n, 256), 256, 0, st>>>(n, pos, q, nl->perm, nl->wrapc, g, (float4*)ctx->xq.p,
+                                              (float4*)ctx->frac.p, (int4*)ctx->base.p);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
+int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const double* q_d,
+                 cudaStream_t st)
+{
+    const int64_t n = nl->n;
+    StageTimer tm(ctx, SQEQ_T_PREP, st);
+    k_prep_charges<<<ceil_div(n, 256), 256, 0, st>>>(n, q_f, q_d, nl->perm, (float4*)ctx->xq.p,
+                                                      (float4*)ctx->frac.p);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+struct RealParams {
+    float Lx, Ly, Lz;
+    float rc2;
+    float alpha;
+    float c2;        // 2 alpha / sqrt(pi)
+};
+
+template <bool FORCE>
+__global__ void __launch_bounds__(256)
+k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row_start,
+       const uint32_t* __restrict__ nbr, RealParams p, float4* __restrict__ out)
+{
+    __shared__ float4 sh[32];
+    if (threadIdx.x < 27) {
+        int img = threadIdx.x;
+        sh[img] = make_float4((img / 9 - 1) * p.Lx, ((img / 3) % 3 - 1) * p.Ly, (img % 3 - 1) * p.Lz, 0.f);
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (s >= n) return;
+    const float4 xi = xq[s];
+    const int64_t beg = row_start[s], end = row_start[s + 1];
+    float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+#pragma unroll 2
+    for (int64_t k = beg + lane; k < end; k += 32) {
+        const uint32_t e = __ldg(nbr + k);
+        const float4 xj = __ldg(xq + (e & 0x07ffffffu));
+        const float4 s4 = sh[e >> 27];
+        // d = r_i - (r_j + shift)
+        const float dx = (xi.x - xj.x) - s4.x;
+        const float dy = (xi.y - xj.y) - s4.y;
+        const float dz = (xi.z - xj.z) - s4.z;
+        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        if (r2 < p.rc2) {
+            const float rinv = rsqrtf(r2);
+            const float r = r2 * rinv;
+            const float ar = p.alpha * r;
+            const float t = erfcf(ar) * rinv;                 // erfc(alpha r)/r
+            phi = fmaf(xj.w, t, phi);
+            if (FORCE) {
+                const float ex = expf(-ar * ar);
+                const float gq = xj.w * fmaf(p.c2, ex, t) * (rinv * rinv);
+                fx = fmaf(gq, dx, fx);
+                fy = fmaf(gq, dy, fy);
+                fz = fmaf(gq, dz, fz);
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        phi += __shfl_xor_sync(0xffffffffu, phi, o);
+        if (FORCE) {
+            fx += __shfl_xor_sync(0xffffffffu, fx, o);
+            fy += __shfl_xor_sync(0xffffffffu, fy, o);
+            fz += __shfl_xor_sync(0xffffffffu, fz, o);
+        }
+    }
+    if (lane == 0) out[s] = make_float4(xi.w * fx, xi.w * fy, xi.w * fz, phi);
+}
+
+int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
+                  cudaStream_t st)
+{
+    const int64_t n = nl->n;
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->real_out, sizeof(float4) * n));
+    RealParams p;
+    p.Lx = (float)nl->box[0]; p.Ly = (float)nl->box[1]; p.Lz = (float)nl->box[2];
+    p.rc2 = (float)(rc * rc);
+    p.alpha = (float)alpha;
+    p.c2 = (float)(2.0 * alpha / sqrt(M_PI));
+    StageTimer tm(ctx, SQEQ_T_REAL, st);
+    const int nb = ceil_div(n * 32, 256);
+    if (want_force)
+        k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->nbr, p,
+                                          (float4*)ctx->real_out.p);
+    else
+        k_real<false><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->nbr, p,
+                                           (float4*)ctx->real_out.p);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a-9: phi_i = phi_real + phi_rec - (2 alpha/sqrt(pi)) q_i ; F = F_real + F_rec ; E = 1/2 sum q phi
+// written back in the caller's atom order.  scal[0] += E (fp64 accumulation).
+template <bool FORCE>
+__global__ void k_assemble(int64_t n, const float4* __restrict__ xq, const float4* __restrict__ real_out,
+                           const float4* __restrict__ rec_out, const int* __restrict__ perm, float cself,
+                           float* __restrict__ phi, float* __restrict__ force, double* __restrict__ scal)
+{
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (s < n) {
+        const float4 a = real_out[s], b = rec_out[s];
+        const float qi = xq[s].w;
+        const float ph = a.w + b.w - cself * qi;
+        const int64_t o = perm[s];
+        if (phi) phi[o] = ph;
+        if (FORCE) {
+            force[3 * o + 0] = a.x + b.x;
+            force[3 * o + 1] = a.y + b.y;
+            force[3 * o + 2] = a.z + b.z;
+        }
+        e = 0.5 * (double)qi * (double)ph;
+    }
+    if (scal) {
+        __shared__ double red[8];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = e;
+        __syncthreads();
+        if (threadIdx.x < 8) {
+            e = red[threadIdx.x];
+#pragma unroll
+            for (int o = 4; o > 0; o >>= 1) e += __shfl_xor_sync(0xffu, e, o);
+            if (threadIdx.x == 0) atomicAdd(scal, e);
+        }
+    }
+}
+
+int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, float* force,
+                 bool want_energy, cudaStream_t st)
+{
+    const int64_t n = nl->n;
+    const float cself = (float)(2.0 * alpha / sqrt(M_PI));
+    double* scal = want_energy ? (double*)ctx->scal.p : nullptr;
+    StageTimer tm(ctx, SQEQ_T_ASSEMBLE, st);
+    if (want_energy) CUDA_TRY(ctx, cudaMemsetAsync(ctx->scal.p, 0, sizeof(double), st));
+    if (force)
+        k_assemble<true><<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->xq.p,
+            (const float4*)ctx->real_out.p, (const float4*)ctx->rec_out.p, nl->perm, cself, phi, force, scal);
+    else
+        k_assemble<false><<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->xq.p,
+            (const float4*)ctx->real_out.p, (const float4*)ctx->rec_out.p, nl->perm, cself, phi, force, scal);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
