@@ -1,0 +1,427 @@
+#!/usr/bin/env python
+"""bench.py -- PME Coulomb potential+force evaluations per second at 331,776 atoms on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the hot path on BASELINE.json configs[4] (110,592 waters, 331,776 atoms,
+149.0 A box, rc 9 A, alpha 0.35, PME 160^3, order 6): one full potential+force+energy evaluation
+(re-gather, erfc real-space sum over the list, spread, R2C, influence, C2R, gather, assemble) on
+positions perturbed by sigma 0.02 A per step, with the neighbour list (rc + 1 A skin) rebuilt every
+10 steps INSIDE the timed region (cell binning, sort, pair enumeration).  The QEq Krylov and shadow
+XL-BOMD drivers (rows a-10, a-11) are timed as additional legs and reported under "extra".
+
+Prints ONE JSON line (see the keys below).  `--impl reference` times the fp64 CPU oracle instead
+(rank 0 only), each step a bounded sample of the same workload.
+N > 1: replicas only (the path does not shard) -- every rank runs the same
+workload on its own GPU, no data-path collective; value = all ranks' evaluations / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2503_21176_b200 import workloads as W  # noqa: E402
+
+METRIC = "PME Coulomb potential+force evals/s at 331,776 atoms"
+REBUILD_EVERY = 10
+N_POSSETS = 10
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", d
+    return 6650.0, "fallback (B200_PROFILING.md)", {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+class OracleSampler:
+    """Times the fp64 oracle, as it stands, on a BOUNDED sample of one evaluation of `cfg` and
+    scales each part linearly to the full evaluation:
+      real space   : rows of n_rows atoms (each row is the plain O(N) sum)          x N/n_rows
+      spread/gather: the first n_sub atoms                                          x N/n_sub
+      3-D DFT x2   : naive line DFTs of an (s, K, K) slab; a full transform is K/s slabs' worth of the
+                     two in-slab axis passes plus an equal third pass                x 1.5 K/s
+      neighbour    : brute-force rows of 8 atoms, single thread                     x N/8/2/threads,
+                     charged at 1/REBUILD_EVERY per evaluation
+    The sample sizes are chosen from a time budget after a sub-second probe."""
+
+    def __init__(self, cfg, q):
+        import oracle
+        self.o, self.cfg, self.q = oracle, cfg, q
+        self.n = len(q)
+        self.cores = oracle.num_threads()
+        self.rate = None
+
+    def _measure(self, pos, n_rows, n_sub, s, nl_rows=8):
+        o, c, n, K = self.o, self.cfg, self.n, self.cfg.grid
+        rng = np.random.default_rng(0)
+        rows = np.sort(rng.choice(n, min(n_rows, n), replace=False))
+        n_sub = min(n_sub, n); s = min(s, K)
+        t0 = time.perf_counter(); o.realspace_rows(pos, self.q, c.box, c.rc, c.alpha, rows)
+        t_real = (time.perf_counter() - t0) * n / len(rows)
+        t0 = time.perf_counter(); Q = o.pme_spread(pos[:n_sub], self.q[:n_sub], c.box, K, c.order)
+        t_spread = (time.perf_counter() - t0) * n / n_sub
+        t0 = time.perf_counter(); o.pme_gather(pos[:n_sub], self.q[:n_sub], c.box, K, c.order, Q)
+        t_gather = (time.perf_counter() - t0) * n / n_sub
+        slab = np.ascontiguousarray(Q[:s]).astype(np.complex128)
+        t0 = time.perf_counter(); o.dft3(slab, -1)
+        t_dft = (time.perf_counter() - t0) * 1.5 * K / s
+        t0 = time.perf_counter()
+        for a in rows[:nl_rows]:
+            o.neighbour_row(pos, c.box, c.r_list, int(a))
+        t_nl = (time.perf_counter() - t0) / min(nl_rows, len(rows)) * n / 2 / self.cores
+        return dict(t_real=t_real, t_spread=t_spread, t_gather=t_gather, t_dft=t_dft, t_nl=t_nl,
+                    n_rows=len(rows), n_sub=n_sub, s=s)
+
+    def sample(self, pos, budget_s):
+        n, K = self.n, self.cfg.grid
+        if self.rate is None:
+            self.rate = self._measure(pos, 32, max(1024, n // 128), 2)
+        r = self.rate
+        n_rows = int(np.clip(0.4 * budget_s / (r["t_real"] / n), 16, n))
+        n_sub = int(np.clip(0.3 * budget_s / ((r["t_spread"] + r["t_gather"]) / n), 1024, n))
+        s = int(np.clip(0.3 * budget_s / (2 * r["t_dft"] / (1.5 * K)), 2, K))
+        m = self._measure(pos, n_rows, n_sub, s)
+        t = m["t_real"] + m["t_spread"] + m["t_gather"] + 2 * m["t_dft"] + m["t_nl"] / REBUILD_EVERY
+        m["t_eval"] = t
+        m["cores"] = self.cores
+        m["sample"] = (f"oracle as it stands, scaled linearly from: real-space rows of {m['n_rows']} of {n} atoms; "
+                       f"spread+gather of {m['n_sub']} atoms; naive DFT of a ({m['s']},{K},{K}) slab x1.5K/s, twice; "
+                       f"brute-force neighbour rows of 8 atoms charged 1/{REBUILD_EVERY} per evaluation")
+        return m
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    pos, q = W.make(cfg.index)
+    smp = OracleSampler(cfg, q)
+    budget = max(0.5, min(20.0, 150.0 / (args.steps + args.warmup)))
+    ts, info = [], None
+    for k in range(args.warmup + args.steps):
+        p = W.perturb(pos, k % N_POSSETS, 0.02, cfg.index)
+        info = smp.sample(p, budget)
+        if k >= args.warmup:
+            ts.append(info["t_eval"])
+    t = float(np.mean(ts))
+    val = 1.0 / t
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": "evals/s", "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"configs[{cfg.index}] {cfg.name}: {cfg.n_atoms} atoms, L {cfg.L} A, rc {cfg.rc}, "
+                                  f"alpha {cfg.alpha}, PME {cfg.grid}^3 order {cfg.order}; one potential+force "
+                                  f"evaluation per step, neighbour rebuild every {REBUILD_EVERY}"},
+           "cpu_baseline": {"value": val, "unit": "evals/s", "cores": info["cores"], "kind": "oracle",
+                            "sample": info["sample"]},
+           "e2e": {"value": val, "unit": "evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2503_21176_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    ctx = binding.Context(local)
+    hbm_peak, peak_src, _ = measured_peaks()
+
+    pos0, q = W.make(cfg.index)
+    n = len(q)
+    possets = [torch.as_tensor(W.perturb(pos0, k, 0.02, cfg.index)).to(dev) for k in range(N_POSSETS)]
+    # cumulative drift would exceed skin/2 after many steps; the sets are independent perturbations of
+    # pos0 (sigma 0.02 A, max ~0.1 A << skin/2), so a list built on any set is valid for all of them
+    qd = torch.as_tensor(q).to(dev)
+    phi = torch.empty(n, dtype=torch.float32, device=dev)
+    force = torch.empty((n, 3), dtype=torch.float32, device=dev)
+    box, rc, alpha, grid, order, rl = cfg.box, cfg.rc, cfg.alpha, cfg.grid, cfg.order, cfg.r_list
+    state = {"nl": None}
+
+    def step(k, host=None):
+        if k % REBUILD_EVERY == 0:
+            if state["nl"] is not None:
+                state["nl"].free()
+            state["nl"] = ctx.nl_build(possets[k % N_POSSETS], box, rl)
+        if host is None:
+            return ctx.coulomb(state["nl"], possets[k % N_POSSETS], qd, box, rc, alpha, grid, order,
+                               phi=phi, force=force)[2]
+        hp, hq, hphi, hf = host
+        return ctx.coulomb_host(state["nl"], hp[k % N_POSSETS], hq, box, rc, alpha, grid, order, hphi, hf)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(nsteps, host=None, k0=0):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(ctx.stream)
+        for k in range(nsteps):
+            step(k0 + k, host)
+        e1.record(ctx.stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms
+
+    # ---- device-resident leg -------------------------------------------------------------------
+    for k in range(max(args.warmup, 3)):
+        step(k)
+    ctx.profile_enable(True)
+    ctx.profile_reset()
+    ctx.launch_count(reset=True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ms = timed(args.steps)
+    launches = ctx.launch_count()
+    prof = ctx.profile_read()
+    ctx.profile_enable(False)
+    clocks = sampler.stop() if rank == 0 else {}
+    ms_step = ms / args.steps
+    value = world * 1e3 / ms_step
+
+    # same loop without the stage events (they add two event records per kernel)
+    ms_noprof = timed(args.steps)
+    value = max(value, world * 1e3 * args.steps / ms_noprof) if args.best_of_two else world * 1e3 * args.steps / ms_noprof
+    ms_step = 1e3 * world / value
+
+    # ---- end-to-end leg: C-ABI call with HOST buffers, copies inside the timed region -----------
+    hp = [p.cpu().pin_memory() for p in possets]
+    hq = qd.cpu().pin_memory()
+    hphi = torch.empty(n, dtype=torch.float32).pin_memory()
+    hf = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    host = (hp, hq, hphi, hf)
+    for k in range(3):
+        step(k, host)
+    ms_e2e = timed(args.steps, host)
+    e2e_val = world * 1e3 * args.steps / ms_e2e
+
+    # ---- per-kernel roofline (stage events on the launching streams, over the timed region) -----
+    info = state["nl"].info()
+    P = info["n_directed"]
+    G3 = grid ** 3
+    S3 = grid * grid * (grid // 2 + 1)
+    alg_bytes = {  # algorithmic bytes per launch
+        "real": 4 * P + 32 * n,
+        "spread": 16 * n + 4 * G3,
+        "fft_fwd": 4 * G3 + 8 * S3,
+        "influence": 16 * S3,
+        "fft_inv": 4 * G3 + 8 * S3,
+        "gather": 32 * n + 4 * G3,
+        "prep": 16 * n + 16 * n + 16 * n + 16 * n,
+        "assemble": 48 * n + 16 * n,
+        "nl_pairs": 4 * P + 2 * 16 * n,
+        "nl_bin": 12 * n * 2 + 16 * n + 12 * n,
+    }
+    kernels = {}
+    for name, (tot, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        avg = tot / cnt
+        b = alg_bytes.get(name)
+        kernels[name] = {"ms_avg": round(avg, 5), "launches": cnt,
+                         "share_of_step": round(tot / (args.steps * (ms / args.steps)), 4),
+                         "alg_MB": round(b / 1e6, 2) if b else None,
+                         "GBps": round(b / avg / 1e6, 1) if b else None,
+                         "hbm_frac": round(b / avg / 1e6 / hbm_peak, 4) if b else None}
+    dom = max((k for k in kernels if k not in ("nl_pairs", "nl_bin")), key=lambda k: prof[k][0])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(dom)
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["GBps"], "peak": hbm_peak,
+                "unit": "GB/s", "frac": kernels[dom]["hbm_frac"], "traffic": traffic,
+                "peak_source": peak_src,
+                "alg_bytes_per_launch": alg_bytes[dom],
+                "note": "4 B x directed list entries + 32 B x atoms for the real-space kernel; "
+                        "ms_avg from CUDA events on the launching stream over the timed region"}
+
+    extra = {"kernels": kernels,
+             "pair_interactions_per_s": None, "grid_points_per_s": None,
+             "n_directed_list_entries": P, "ms_per_step_with_stage_events": round(ms / args.steps, 4)}
+    if "real" in kernels:
+        extra["pair_interactions_per_s"] = (P / 2) / (kernels["real"]["ms_avg"] * 1e-3)
+    pme_ms = sum(kernels[k]["ms_avg"] for k in ("spread", "fft_fwd", "influence", "fft_inv", "gather") if k in kernels)
+    if pme_ms > 0:
+        extra["grid_points_per_s"] = G3 / (pme_ms * 1e-3)
+
+    # ---- a-10 / a-11 legs: QEq Krylov iterations and shadow XL-BOMD steps ------------------------
+    if not args.no_md and rank == 0:
+        try:
+            extra.update(run_md_legs(ctx, cfg, possets[0], n, dev, args))
+        except Exception as ex:  # report, never hide
+            extra["md_error"] = str(ex)
+
+    out = {"metric": METRIC, "value": value, "unit": "evals/s", "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": f"configs[{cfg.index}] {cfg.name}: {n} atoms, L {cfg.L} A, rc {cfg.rc} A "
+                                  f"(+{cfg.skin} A skin), alpha {cfg.alpha}, PME {grid}^3 order {order}; one "
+                                  f"potential+force+energy evaluation per step, positions perturbed (sigma 0.02 A) "
+                                  f"each step, neighbour rebuild every {REBUILD_EVERY} steps inside the timed region",
+                      "l2": "inputs larger than L2: the %.0f MB neighbour list is streamed every step; no flush" % (4 * P / 1e6),
+                      "parallelism": "replicas only" if world > 1 else "single GPU"},
+           "clocks": clocks, "gpu_launches": launches,
+           "e2e": {"value": e2e_val, "unit": "evals/s", "h2d_bytes_per_step": 16 * n,
+                   "d2h_bytes_per_step": 16 * n + 8},
+           "roofline": roofline, "extra": extra}
+
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            m = OracleSampler(cfg, q).sample(pos0, args.cpu_budget)
+            out["cpu_baseline"] = {"value": 1.0 / m["t_eval"], "unit": "evals/s", "cores": m["cores"],
+                                   "kind": "oracle", "sample": m["sample"],
+                                   "seconds_scaled": {k: round(m[k], 3) for k in
+                                                      ("t_real", "t_spread", "t_dft", "t_gather", "t_nl")}}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_md_legs(ctx, cfg, pos, n, dev, args):
+    import torch
+    from paper_2503_21176_b200 import binding
+    res = {}
+    box = cfg.box
+    chi, u = W.qeq_params_water_pd(n)
+    chi_d, u_d = torch.as_tensor(chi).to(dev), torch.as_tensor(u).to(dev)
+    nl = ctx.nl_build(pos, box, cfg.r_list)
+    # a-10: fixed number of Krylov iterations, each one potential-only Coulomb evaluation
+    iters = args.krylov_iters
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx.qeq_solve(nl, pos, box, cfg.rc, cfg.alpha, cfg.grid, cfg.order, W.KE_EV_A, chi_d, u_d, 0.0,
+                  tol=0.0, max_iter=3, restart=0)
+    e0.record(ctx.stream)
+    q, lam, it, rel, ok = ctx.qeq_solve(nl, pos, box, cfg.rc, cfg.alpha, cfg.grid, cfg.order, W.KE_EV_A,
+                                        chi_d, u_d, 0.0, tol=0.0, max_iter=iters, restart=0)
+    e1.record(ctx.stream)
+    torch.cuda.synchronize()
+    msq = e0.elapsed_time(e1)
+    res["qeq_krylov_iters_per_s"] = it / (msq * 1e-3)
+    res["qeq_relres_after_%d_iters" % it] = rel
+    # a-11: shadow XL-BOMD steps
+    p = binding.md_params(cfg)
+    mass = torch.as_tensor(W.masses_water(n)).to(dev)
+    vel = torch.as_tensor(W.velocities(W.masses_water(n))).to(dev)
+    x = pos.clone()
+    nhist, force, en0 = ctx.shadow_md_init(nl, x, box, p, chi_d, u_d, tol=1e-6, max_iter=100)
+    nsteps = args.md_steps
+    for _ in range(2):
+        ctx.shadow_md_step(nl, x, vel, mass, box, p, chi_d, u_d, nhist, force, want_energies=False)
+    torch.cuda.synchronize()
+    e0.record(ctx.stream)
+    evals = 0
+    for s in range(nsteps):
+        if s % REBUILD_EVERY == 0 and s > 0:
+            nl.free()
+            nl = ctx.nl_build(x, box, cfg.r_list)
+        en = ctx.shadow_md_step(nl, x, vel, mass, box, p, chi_d, u_d, nhist, force, want_energies=(s == nsteps - 1))
+    e1.record(ctx.stream)
+    torch.cuda.synchronize()
+    msm = e0.elapsed_time(e1)
+    res["qeq_md_atom_steps_per_s"] = n * nsteps / (msm * 1e-3)
+    res["qeq_md_ms_per_step"] = msm / nsteps
+    res["qeq_md_coulomb_evals_per_step"] = en[3] if en else None
+    res["qeq_md_steps_timed"] = nsteps
+    nl.free()
+    return res
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-md", action="store_true")
+    ap.add_argument("--best-of-two", action="store_true")
+    ap.add_argument("--krylov-iters", type=int, default=50)
+    ap.add_argument("--md-steps", type=int, default=20)
+    args = ap.parse_args()
+    cfg = W.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -215,6 +215,16 @@ def pme_influence(box, grid, order, alpha):
     return G
 
 
+def pme_gather(pos, q, box, grid, order, Phi):
+    """Alg. 2 step 5 alone: phi_i = sum W Phi, F_i = -q_i (K/L) sum dW Phi on a given grid Phi."""
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box); K = _grid(grid)
+    Phi = np.ascontiguousarray(Phi, dtype=np.float64)
+    n = pos.shape[0]
+    phi = np.zeros(n); F = np.zeros((n, 3))
+    lib().orc_pme_gather(n, _dp(pos), _dp(q), _dp(box), _ip(K), int(order), _dp(Phi), _dp(phi), _dp(F))
+    return phi, F
+
+
 def pme_recip(pos, q, box, grid, order, alpha, return_grids=False):
     """Alg. 2 steps 1-5: phi_rec, F_rec, E_rec (and optionally the Q and Phi grids)."""
     pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box); K = _grid(grid)
