@@ -17,8 +17,9 @@ Pins (tests/test_oracle_*.py): rock-salt / CsCl / zincblende Madelung
 constants, the cubic self-image constant xi, alpha-independence, finite
 differences, PME grid-shift invariance and operator symmetry, numpy.fft,
 scipy B-splines, scipy periodic cKDTree, brute-force multi-image sums.
-Functions whose parity is unpinned: shadow_md_step (integrator constants are
-not given by the paper -- DESIGN.md R-MD).
+Functions whose parity is unpinned: shadow_md_step / shadow_md_init (the n(t)
+integrator's constants and history start are not given by the paper -- DESIGN.md
+R-MD); their ingredients (Eq. 22, shadow forces = -grad U, Eq. 24's J, GMRES) are pinned.
 """
 import ctypes
 import math
@@ -331,3 +332,133 @@ def shadow_charges(chi, u, v, qtot):
     lam = -(float(qtot) + np.sum((chi + v) / u)) / np.sum(1.0 / u)
     q = -(chi + v + lam) / u
     return q, float(lam)
+
+
+# --------------------------------------------------------------------------
+# c-MD  shadow XL-BOMD step (Eqs. 19-27; readings DESIGN.md R-MD)
+#       Integrator constants are not in the paper: PARITY UNPINNED for those.
+#       Pinned: Eq. 22 rows, sum q = Qtot, forces = -grad of the shadow potential
+#       (finite differences), residual 0 and BO forces when n = q_min.
+# --------------------------------------------------------------------------
+ACC_CONV = 0.00964853321  # (eV/Angstrom)/amu -> Angstrom/fs^2
+
+
+def harmonic_water(pos, k_oh, r_oh, k_hh, r_hh):
+    """Stand-in for V_short (Eq. 14): atoms 3m,3m+1,3m+2 = O,H,H with
+    1/2 k_oh (|r_OH|-r_oh)^2 on both O-H bonds and 1/2 k_hh (|r_HH|-r_hh)^2.  Returns V, F."""
+    pos = _f64(pos, (-1, 3))
+    F = np.zeros_like(pos)
+    V = 0.0
+    mol = pos.reshape(-1, 3, 3)
+    Fm = F.reshape(-1, 3, 3)
+    for a, b, k, r0 in ((0, 1, k_oh, r_oh), (0, 2, k_oh, r_oh), (1, 2, k_hh, r_hh)):
+        d = mol[:, b] - mol[:, a]
+        r = np.linalg.norm(d, axis=1)
+        V += 0.5 * k * float(np.sum((r - r0) ** 2))
+        f = (k * (r - r0) / r)[:, None] * d       # force on a (towards b when stretched)
+        Fm[:, a] += f
+        Fm[:, b] -= f
+    return V, F
+
+
+def shadow_eval(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin=None):
+    """Shadow potential, charges and forces at fixed n (Eqs. 20-22).
+
+    v = ke*phi[n] (one Coulomb potential); q[n], lambda from Eq. 22;
+    U = sum q chi + 1/2 sum q^2 u + sum_i (q_i - n_i/2) v_i  (+ stand-in V_short), which is
+    Eq. 20 with sum_{j!=i} phi_ij n_j read as the periodic Ewald potential of n;
+    F = -grad_R U at fixed q, n = F_Coul[q] - F_Coul[q-n]  (polarisation identity:
+    1/2 (2q-n)' Phi n = 1/2 q' Phi q - 1/2 (q-n)' Phi (q-n)), times ke, plus stand-in forces.
+    """
+    n = _f64(n); chi = _f64(chi); u = _f64(u)
+    phi_n = coulomb_pme(pos, n, box, rc, alpha, grid, order)[0]
+    v = ke * phi_n
+    q, lam = shadow_charges(chi, u, v, qtot)
+    U = float(np.dot(q, chi) + 0.5 * np.dot(q * q, u) + np.dot(q - 0.5 * n, v))
+    Fq = coulomb_pme(pos, q, box, rc, alpha, grid, order)[1]
+    Fd = coulomb_pme(pos, q - n, box, rc, alpha, grid, order)[1]
+    F = ke * (Fq - Fd)
+    if standin is not None:
+        Vs, Fs = harmonic_water(pos, *standin)
+        U += Vs
+        F = F + Fs
+    return dict(U=U, q=q, lam=lam, v=v, F=F, res=q - n)
+
+
+def kernel_jacobian_apply(pos, w, u, ke, box, rc, alpha, grid, order):
+    """J w with J = d(q[n]-n)/dn (Eq. 24).  From Eq. 22,
+    q[n] = -(chi + ke Phi n + lambda)/u with lambda fixing sum q, so
+    J w = -w - (ke Phi w + dlam)/u,  dlam = -sum_i (ke Phi w)_i/u_i / sum_i 1/u_i."""
+    w = _f64(w); u = _f64(u)
+    pw = ke * coulomb_pme(pos, w, box, rc, alpha, grid, order)[0]
+    dlam = -float(np.sum(pw / u)) / float(np.sum(1.0 / u))
+    return -w - (pw + dlam) / u
+
+
+def gmres_fixed(apply, b, m):
+    """m steps of GMRES from a zero initial guess: Arnoldi with modified Gram-Schmidt, then
+    the (m+1) x m least-squares problem by numpy.linalg.lstsq.  Returns x_m."""
+    b = _f64(b)
+    beta = float(np.linalg.norm(b))
+    if beta == 0.0:
+        return np.zeros_like(b)
+    V = [b / beta]
+    H = np.zeros((m + 1, m))
+    k = m
+    for j in range(m):
+        w = apply(V[j])
+        for i in range(j + 1):
+            H[i, j] = float(np.dot(V[i], w))
+            w = w - H[i, j] * V[i]
+        H[j + 1, j] = float(np.linalg.norm(w))
+        if H[j + 1, j] == 0.0:
+            k = j + 1
+            break
+        V.append(w / H[j + 1, j])
+    e1 = np.zeros(k + 1); e1[0] = beta
+    y = np.linalg.lstsq(H[:k + 1, :k], e1, rcond=None)[0]
+    return sum(y[i] * V[i] for i in range(k))
+
+
+def shadow_md_force_and_ndd(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin,
+                            kappa, krylov_rank):
+    """Everything the integrator needs at one time level: shadow forces (Eq. 25) and
+    dt^2 * ndd from Eq. 27, J (dt^2 ndd) = -kappa (q[n]-n), kappa = dt^2 omega^2, solved by
+    `krylov_rank` GMRES steps from zero (the paper's low-rank Krylov approximation of K = J^-1,
+    PAPER.md:244-246).  Coulomb evaluations: 1 (v) + 2 (forces) + krylov_rank."""
+    ev = shadow_eval(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin)
+    apply = lambda w: kernel_jacobian_apply(pos, w, u, ke, box, rc, alpha, grid, order)
+    ev["ndd_dt2"] = gmres_fixed(apply, -kappa * ev["res"], krylov_rank)
+    return ev
+
+
+def shadow_md_init(pos, n0, chi, u, ke, qtot, box, rc, alpha, grid, order, standin, kappa,
+                   krylov_rank):
+    """History rows 0..5 = n0 (PAPER.md is silent on the start: DESIGN.md R-MD), row 6 = dt^2 ndd."""
+    n0 = _f64(n0)
+    ev = shadow_md_force_and_ndd(pos, n0, chi, u, ke, qtot, box, rc, alpha, grid, order, standin,
+                                 kappa, krylov_rank)
+    nhist = np.vstack([np.tile(n0, (6, 1)), ev["ndd_dt2"][None, :]])
+    return dict(pos=_f64(pos, (-1, 3)).copy(), nhist=nhist, F=ev["F"], U=ev["U"], q=ev["q"],
+                res=ev["res"])
+
+
+def shadow_md_step(state, vel, mass, dt, chi, u, ke, qtot, box, rc, alpha, grid, order, standin,
+                   kappa, alpha_diss, c, krylov_rank):
+    """One velocity-Verlet step for R and one Verlet step with dissipation for n
+    (R-MD):  n(t+dt) = 2 n(t) - n(t-dt) + dt^2 ndd(t) + alpha_diss * sum_k c_k n(t - k dt).
+    Returns the new state, new velocities and the kinetic energy (eV)."""
+    pos = state["pos"]; nh = state["nhist"]
+    mass = _f64(mass); vel = _f64(vel, (-1, 3))
+    a = ACC_CONV * state["F"] / mass[:, None]
+    vel = vel + 0.5 * dt * a
+    pos = pos + dt * vel
+    n_new = 2.0 * nh[0] - nh[1] + nh[6] + alpha_diss * sum(c[k] * nh[k] for k in range(6))
+    ev = shadow_md_force_and_ndd(pos, n_new, chi, u, ke, qtot, box, rc, alpha, grid, order,
+                                 standin, kappa, krylov_rank)
+    nhist = np.vstack([n_new[None, :], nh[0:5], ev["ndd_dt2"][None, :]])
+    a = ACC_CONV * ev["F"] / mass[:, None]
+    vel = vel + 0.5 * dt * a
+    ekin = 0.5 * float(np.sum(mass[:, None] * vel * vel)) / ACC_CONV
+    new = dict(pos=pos, nhist=nhist, F=ev["F"], U=ev["U"], q=ev["q"], res=ev["res"])
+    return new, vel, ekin

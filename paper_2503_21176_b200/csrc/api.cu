@@ -288,7 +288,7 @@ int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const 
 }
 
 int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc,
-                 double alpha, float* phi, float* force, bool want_energy)
+                 double alpha, float* phi, float* force, bool want_energy, bool field_mode)
 {
     const bool want_force = force != nullptr;
     // fork: PME on the side stream, real space on the main stream
@@ -298,7 +298,7 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev_join, ctx->stream2));
     SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
     CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
-    SQEQ_TRY(assemble_run(ctx, nl, alpha, phi, force, want_energy, ctx->stream));
+    SQEQ_TRY(assemble_run(ctx, nl, alpha, phi, force, want_energy, field_mode, ctx->stream));
     ctx->last_had_force = want_force;
     ctx->last_n = n;
     return SQEQ_OK;

@@ -6,6 +6,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
+#include <functional>
 #include <vector>
 
 #include "../../include/sqeq.h"
@@ -144,7 +145,15 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
 int pme_run(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_force, bool want_energy,
             cudaStream_t st);
 int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, float* force,
-                 bool want_energy, cudaStream_t st);
+                 bool want_energy, bool field_mode, cudaStream_t st);
 // Full evaluation on prepared geometry (used by coulomb, qeq and md drivers).
+// field_mode: `force` receives the per-unit-charge field f_i (F_i = q_i f_i) instead of F_i.
 int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc,
-                 double alpha, float* phi, float* force, bool want_energy);
+                 double alpha, float* phi, float* force, bool want_energy, bool field_mode = false);
+
+// Generic restarted/unrestarted GMRES on device fp64 vectors (qeq.cu); x_out points into ctx->kry_w.
+int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double*, double*)>& apply,
+                const std::function<int(double*)>& load_rhs, double tol, int max_iter, int restart,
+                double** x_out, int* iters_out, double* relres_out, bool* converged_out);
+int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3],
+                          double rc, double alpha, const int grid[3], int order, const char* who);

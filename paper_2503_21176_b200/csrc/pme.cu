@@ -159,7 +159,7 @@ k_gather(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ ba
             gz_ += __shfl_xor_sync(0xffffffffu, gz_, o);
         }
     }
-    if (lane == 0) out[s] = make_float4(-fw.w * sx * gx_, -fw.w * sy * gy_, -fw.w * sz * gz_, ph);
+    if (lane == 0) out[s] = make_float4(-sx * gx_, -sy * gy_, -sz * gz_, ph);   // per unit charge; a-9 applies q_i
 }
 
 // -------------------------------------------------------------------------------------- host side
@@ -294,15 +294,16 @@ int pme_run(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_force, bool
 }
 
 // -------------------------------------------------------------------------------------- diagnostics
-__global__ void k_unpermute_parts(int64_t n, const float4* __restrict__ src, const int* __restrict__ perm,
-                                  float* __restrict__ phi, float* __restrict__ F)
+__global__ void k_unpermute_parts(int64_t n, const float4* __restrict__ src, const float4* __restrict__ xq,
+                                  const int* __restrict__ perm, float* __restrict__ phi, float* __restrict__ F)
 {
     int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (s >= n) return;
     const float4 v = src[s];
+    const float qi = xq[s].w;
     const int64_t o = perm[s];
     if (phi) phi[o] = v.w;
-    if (F) { F[3 * o] = v.x; F[3 * o + 1] = v.y; F[3 * o + 2] = v.z; }
+    if (F) { F[3 * o] = qi * v.x; F[3 * o + 1] = qi * v.y; F[3 * o + 2] = qi * v.z; }
 }
 
 extern "C" int sqeq_coulomb_parts(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* phi_real,
@@ -313,9 +314,9 @@ extern "C" int sqeq_coulomb_parts(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n
     if ((F_real || F_rec) && !ctx->last_had_force)
         return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_parts: the last evaluation was potential-only");
     cudaStream_t st = ctx->stream;
-    k_unpermute_parts<<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->real_out.p, nl->perm, phi_real, F_real);
+    k_unpermute_parts<<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->real_out.p, (const float4*)ctx->xq.p, nl->perm, phi_real, F_real);
     KERNEL_CHECK(ctx);
-    k_unpermute_parts<<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->rec_out.p, nl->perm, phi_rec, F_rec);
+    k_unpermute_parts<<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->rec_out.p, (const float4*)ctx->xq.p, nl->perm, phi_rec, F_rec);
     KERNEL_CHECK(ctx);
     CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 8, (double*)ctx->scal.p + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));

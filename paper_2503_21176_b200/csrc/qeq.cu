@@ -9,6 +9,7 @@
 // Zero initial guess, no preconditioner (DESIGN.md R-G13).
 #include <math.h>
 
+#include <functional>
 #include <vector>
 
 #include "common.cuh"
@@ -116,72 +117,37 @@ __global__ void k_d2f(int64_t n, const double* __restrict__ x, float* __restrict
     if (i < n) y[i] = (float)x[i];
 }
 
-struct QeqOp {
-    sqeq_ctx* ctx;
-    const sqeq_nlist* nl;
-    int64_t n;
-    const double* box;
-    double rc, alpha, ke;
-    const float* J;
-    float* phi;   // scratch [n]
-};
-
-// w = A v   (one potential-only Coulomb evaluation on the prepared geometry)
-static int qeq_apply(const QeqOp& op, const double* v, double* w)
+// ------------------------------------------------------------------------------------------------
+// Generic GMRES on device fp64 vectors of length `len` (leading dimension ld).  Zero initial guess.
+//   apply(v, w): w = A v        load_rhs(w): w = b
+// On return x (ctx->kry_w + ld) holds the iterate.  Host side: Givens-rotated Hessenberg.
+int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double*, double*)>& apply,
+                const std::function<int(double*)>& load_rhs, double tol, int max_iter, int restart,
+                double** x_out, int* iters_out, double* relres_out, bool* converged_out)
 {
-    sqeq_ctx* ctx = op.ctx;
-    cudaStream_t st = ctx->stream;
-    const int64_t n = op.n;
-    SQEQ_TRY(prep_charges(ctx, op.nl, nullptr, v, st));
-    SQEQ_TRY(coulomb_eval(ctx, op.nl, n, op.box, op.rc, op.alpha, op.phi, nullptr, false));
-    StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
-    CUDA_TRY(ctx, cudaMemsetAsync(w + n, 0, sizeof(double), st));
-    k_qeq_matvec<<<ceil_div(n, 256), 256, 0, st>>>(n, v, op.J, op.phi, op.ke, w);
-    KERNEL_CHECK(ctx);
-    return SQEQ_OK;
-}
-
-extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
-                              const double box[3], double rc, double alpha, const int grid[3], int order,
-                              double ke, const float* chi, const float* J, double total_charge,
-                              double tol, int max_iter, int restart, float* q_out, double* lambda_out,
-                              int* iters_out, double* relres_out)
-{
-    if (!ctx) return SQEQ_EINVAL;
-    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_qeq_solve"));
-    if (!pos || !chi || !J || !q_out) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: NULL argument");
-    if (max_iter < 1 || restart < 0 || !(tol >= 0.0))
-        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: need max_iter >= 1, restart >= 0, tol >= 0");
-    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const int m = restart > 0 ? (restart < max_iter ? restart : max_iter) : max_iter;
-    const int64_t len = n + 1;
     const int64_t ld = (len + 31) & ~(int64_t)31;
-    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_V, sizeof(double) * (size_t)ld * (m + 1)));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_w, sizeof(double) * (size_t)ld * 2));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_h, sizeof(double) * (size_t)(2 * (m + 2) + 2)));
-    SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_f[0], sizeof(float) * n));
     double* V = (double*)ctx->kry_V.p;
     double* w = (double*)ctx->kry_w.p;
     double* x = w + ld;
-    double* h = (double*)ctx->kry_h.p;          // [m+2] first-pass coefficients (+ norm at [m+1])
+    double* h = (double*)ctx->kry_h.p;          // [m+2] first-pass coefficients
     double* h2 = h + (m + 2);                    // second pass
     double* nrm2 = h2 + (m + 2);
     std::vector<double> hh((size_t)2 * (m + 2) + 2);
-    QeqOp op{ctx, nl, n, box, rc, alpha, ke, J, (float*)ctx->vec_f[0].p};
-    // geometry once; the charge slot is refreshed per mat-vec (q = chi is only a placeholder here)
-    SQEQ_TRY(prep_atoms(ctx, nl, pos, chi, ctx->K, st));
     const int nbl = ceil_div(len, 256);
     const int nchunk = ceil_div(len, DOT_CHUNK);
     CUDA_TRY(ctx, cudaMemsetAsync(x, 0, sizeof(double) * ld, st));
+    *x_out = x;
 
     // |b|
     double bnorm = 0.0;
     {
+        SQEQ_TRY(load_rhs(w));
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
-        k_qeq_rhs<<<nbl, 256, 0, st>>>(n, chi, total_charge, w);
-        KERNEL_CHECK(ctx);
         CUDA_TRY(ctx, cudaMemsetAsync(nrm2, 0, sizeof(double), st));
         k_dots<<<dim3(nchunk, 1), 256, 0, st>>>(len, ld, w, w, nrm2);
         KERNEL_CHECK(ctx);
@@ -200,11 +166,10 @@ extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, co
         double beta = bnorm;
         if (!first_cycle) {
             double* r = V;  // reuse V_0 as scratch for A x
-            SQEQ_TRY(qeq_apply(op, x, r));
+            SQEQ_TRY(apply(x, r));
             ++iters;
+            SQEQ_TRY(load_rhs(w));
             StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
-            k_qeq_rhs<<<nbl, 256, 0, st>>>(n, chi, total_charge, w);
-            KERNEL_CHECK(ctx);
             k_axpby<<<nbl, 256, 0, st>>>(len, -1.0, r, 1.0, w);
             KERNEL_CHECK(ctx);
             CUDA_TRY(ctx, cudaMemsetAsync(nrm2, 0, sizeof(double), st));
@@ -226,7 +191,7 @@ extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, co
         gvec[0] = beta;
         int j = 0;
         for (; j < m && iters < max_iter; ++j) {
-            SQEQ_TRY(qeq_apply(op, V + (int64_t)j * ld, w));
+            SQEQ_TRY(apply(V + (int64_t)j * ld, w));
             ++iters;
             {
                 StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
@@ -282,6 +247,69 @@ extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, co
         }
         if (converged || restart == 0) break;
     }
+    if (iters_out) *iters_out = iters;
+    if (relres_out) *relres_out = relres;
+    if (converged_out) *converged_out = converged;
+    return SQEQ_OK;
+}
+
+// w = A v for Eq. 18 (one potential-only Coulomb evaluation on the prepared geometry)
+struct QeqOp {
+    sqeq_ctx* ctx;
+    const sqeq_nlist* nl;
+    int64_t n;
+    const double* box;
+    double rc, alpha, ke;
+    const float* J;
+    float* phi;   // scratch [n]
+};
+
+static int qeq_apply(const QeqOp& op, const double* v, double* w)
+{
+    sqeq_ctx* ctx = op.ctx;
+    cudaStream_t st = ctx->stream;
+    const int64_t n = op.n;
+    SQEQ_TRY(prep_charges(ctx, op.nl, nullptr, v, st));
+    SQEQ_TRY(coulomb_eval(ctx, op.nl, n, op.box, op.rc, op.alpha, op.phi, nullptr, false));
+    StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+    CUDA_TRY(ctx, cudaMemsetAsync(w + n, 0, sizeof(double), st));
+    k_qeq_matvec<<<ceil_div(n, 256), 256, 0, st>>>(n, v, op.J, op.phi, op.ke, w);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                              const double box[3], double rc, double alpha, const int grid[3], int order,
+                              double ke, const float* chi, const float* J, double total_charge,
+                              double tol, int max_iter, int restart, float* q_out, double* lambda_out,
+                              int* iters_out, double* relres_out)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_qeq_solve"));
+    if (!pos || !chi || !J || !q_out) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: NULL argument");
+    if (max_iter < 1 || restart < 0 || !(tol >= 0.0))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: need max_iter >= 1, restart >= 0, tol >= 0");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int64_t len = n + 1;
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_f[0], sizeof(float) * n));
+    QeqOp op{ctx, nl, n, box, rc, alpha, ke, J, (float*)ctx->vec_f[0].p};
+    // geometry once; the charge slot is refreshed per mat-vec (q = chi is only a placeholder here)
+    SQEQ_TRY(prep_atoms(ctx, nl, pos, chi, ctx->K, st));
+    const int nbl = ceil_div(len, 256);
+    auto apply = [&](const double* v, double* w) { return qeq_apply(op, v, w); };
+    auto load_rhs = [&](double* w) {
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        k_qeq_rhs<<<nbl, 256, 0, st>>>(n, chi, total_charge, w);
+        KERNEL_CHECK(ctx);
+        return (int)SQEQ_OK;
+    };
+    double* x = nullptr;
+    int iters = 0;
+    double relres = 1.0;
+    bool converged = false;
+    SQEQ_TRY(gmres_solve(ctx, len, apply, load_rhs, tol, max_iter, restart, &x, &iters, &relres, &converged));
     {
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
         k_d2f<<<ceil_div(n, 256), 256, 0, st>>>(n, x, q_out);

@@ -149,7 +149,8 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
             fz += __shfl_xor_sync(0xffffffffu, fz, o);
         }
     }
-    if (lane == 0) out[s] = make_float4(xi.w * fx, xi.w * fy, xi.w * fz, phi);
+    // the field sum_j q_j g d (no q_i factor: a-9 applies it, or not in field mode)
+    if (lane == 0) out[s] = make_float4(fx, fy, fz, phi);
 }
 
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
@@ -175,12 +176,15 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// a-9: phi_i = phi_real + phi_rec - (2 alpha/sqrt(pi)) q_i ; F = F_real + F_rec ; E = 1/2 sum q phi
-// written back in the caller's atom order.  scal[0] += E (fp64 accumulation).
+// a-9: phi_i = phi_real + phi_rec - (2 alpha/sqrt(pi)) q_i ; F = q_i (f_real + f_rec) with f the
+// per-unit-charge fields the two kernels leave behind (field != 0: write f itself, used by the
+// shadow-MD force of Eq. 20); E = 1/2 sum q phi.  Written back in the caller's atom order.
+// scal[0] += E (fp64 accumulation).
 template <bool FORCE>
 __global__ void k_assemble(int64_t n, const float4* __restrict__ xq, const float4* __restrict__ real_out,
                            const float4* __restrict__ rec_out, const int* __restrict__ perm, float cself,
-                           float* __restrict__ phi, float* __restrict__ force, double* __restrict__ scal)
+                           int field, float* __restrict__ phi, float* __restrict__ force,
+                           double* __restrict__ scal)
 {
     int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     double e = 0.0;
@@ -191,9 +195,10 @@ __global__ void k_assemble(int64_t n, const float4* __restrict__ xq, const float
         const int64_t o = perm[s];
         if (phi) phi[o] = ph;
         if (FORCE) {
-            force[3 * o + 0] = a.x + b.x;
-            force[3 * o + 1] = a.y + b.y;
-            force[3 * o + 2] = a.z + b.z;
+            const float sc = field ? 1.f : qi;
+            force[3 * o + 0] = sc * (a.x + b.x);
+            force[3 * o + 1] = sc * (a.y + b.y);
+            force[3 * o + 2] = sc * (a.z + b.z);
         }
         e = 0.5 * (double)qi * (double)ph;
     }
@@ -213,7 +218,7 @@ __global__ void k_assemble(int64_t n, const float4* __restrict__ xq, const float
 }
 
 int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, float* force,
-                 bool want_energy, cudaStream_t st)
+                 bool want_energy, bool field_mode, cudaStream_t st)
 {
     const int64_t n = nl->n;
     const float cself = (float)(2.0 * alpha / sqrt(M_PI));
@@ -222,10 +227,10 @@ int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, 
     if (want_energy) CUDA_TRY(ctx, cudaMemsetAsync(ctx->scal.p, 0, sizeof(double), st));
     if (force)
         k_assemble<true><<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->xq.p,
-            (const float4*)ctx->real_out.p, (const float4*)ctx->rec_out.p, nl->perm, cself, phi, force, scal);
+            (const float4*)ctx->real_out.p, (const float4*)ctx->rec_out.p, nl->perm, cself, field_mode ? 1 : 0, phi, force, scal);
     else
         k_assemble<false><<<ceil_div(n, 256), 256, 0, st>>>(n, (const float4*)ctx->xq.p,
-            (const float4*)ctx->real_out.p, (const float4*)ctx->rec_out.p, nl->perm, cself, phi, force, scal);
+            (const float4*)ctx->real_out.p, (const float4*)ctx->rec_out.p, nl->perm, cself, field_mode ? 1 : 0, phi, force, scal);
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
 }

@@ -134,10 +134,12 @@ def qeq_params(n_atoms: int, seed: int = SEED0 + 100):
 
 
 def qeq_params_water_pd(n_atoms: int):
-    """cfg 4 per-element parameters making C positive definite:
-    chi_O = +8.2, chi_H = -8.2 eV/e, u = 30 eV/e^2."""
-    chi = np.tile(np.array([8.2, -8.2, -8.2], dtype=np.float32), n_atoms // 3)
-    u = np.full(n_atoms, 30.0, dtype=np.float32)
+    """cfg 4 per-element parameters: chi_O = +16.4, chi_H = -16.4 eV/e,
+    u = 60 eV/e^2.  C is positive definite (k_e*A has eigenvalues down to about -20 eV/e^2) and the
+    unshielded point-charge model stays bound with the harmonic stand-in (q_O ~ -0.51 e); with
+    u = 30 (q_O ~ -0.84 e) the intramolecular O-H Coulomb attraction wins within ~10 steps."""
+    chi = np.tile(np.array([16.4, -16.4, -16.4], dtype=np.float32), n_atoms // 3)
+    u = np.full(n_atoms, 60.0, dtype=np.float32)
     return chi, u
 
 
