@@ -126,18 +126,28 @@ int  sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float*
                     double tol, int max_iter, int restart,
                     float* q_out, double* lambda_out, int* iters_out, double* relres_out);
 
-/* ---- shadow XL-BOMD step: PAPER.md:206-246 (Eqs. 20-27); DESIGN.md R-MD ------------------------
+/* ---- shadow XL-BOMD step: PAPER.md:196-246 (Eqs. 19-27); DESIGN.md R-MD -------------------------
  * State arrays are caller-owned device memory, updated in place:
  *   pos [n][3], vel [n][3] fp32 (Angstrom, Angstrom/fs); mass [n] fp32 (amu);
- *   nhist fp64 [nhist_len][n]: n(t), n(t-dt), ... most recent first (nhist_len = 7);
+ *   nhist fp64 [7][n]: rows 0..5 = n(t), n(t-dt), ..., n(t-5dt) (most recent first),
+ *                      row 6 = dt^2 * ndd(t), the solution of Eq. 27 at the current time level;
  *   chi, u [n] fp32 (eV/e, eV/e^2);
- *   molecule stand-in potential: atoms 3m, 3m+1, 3m+2 form O,H,H with harmonic O-H and H-H terms
+ *   force [n][3] fp32: F(t) = -grad U(R, n) of Eq. 21/25 (eV/Angstrom), in and out.
+ *   V_short stand-in: atoms 3m, 3m+1, 3m+2 form O,H,H with harmonic O-H and H-H terms
  *   (k_oh, r_oh, k_hh, r_hh; eV/Angstrom^2, Angstrom); pass k_oh = k_hh = 0 to disable.
- * One call advances one velocity-Verlet step of length dt (fs) with `krylov_rank` Krylov updates
- * of the kernel equation J ndd = -omega^2 (q[n] - n) (Eq. 27).  force [n][3] fp32 holds F(t) on
- * entry (from the previous step, or from sqeq_shadow_md_init) and F(t+dt) on exit.
- * energies: host double[4] out = {shadow potential energy (Eq. 21 incl. stand-in), kinetic energy,
- * ||q[n]-n||_2, Coulomb evaluations done}; may be NULL (then the call does not synchronise). */
+ * sqeq_shadow_md_init: sets the history and evaluates force, row 6 and energies at t = 0.
+ *   max_iter > 0: n(0) = q_min from sqeq_qeq_solve(tol, max_iter, unrestarted), copied to rows 0..5
+ *                 (returns SQEQ_ENOTCONV if tol is not reached);
+ *   max_iter = 0: the caller supplies n(0) in row 0; it is copied to rows 1..5.
+ * sqeq_shadow_md_step: one velocity-Verlet step of length dt (fs) for R and one Verlet step with
+ *   dissipation for n,  n(t+dt) = 2n(t) - n(t-dt) + dt^2 ndd(t) + alpha_diss sum_k c_k n(t-k dt),
+ *   then, at t+dt: v = ke*phi[n], q[n] from Eq. 22, forces, and `krylov_rank` GMRES steps (zero
+ *   start) on Eq. 27, J x = -kappa (q[n]-n) with kappa = dt^2 omega^2 (krylov_rank = 0: J ~ -I).
+ *   Coulomb evaluations per step: 2 (potential+field of n, field of q-n) + krylov_rank.
+ *   The list may be stale by less than (list cutoff - rc)/2, as for sqeq_coulomb.
+ * energies: host double[4] out = {shadow potential energy U (Eq. 20/21 incl. stand-in), kinetic
+ * energy (0 from init), ||q[n]-n||_2, Coulomb evaluations done}; may be NULL (then the call does
+ * not synchronise, except inside the Krylov iterations). */
 typedef struct sqeq_md_params {
     double dt;            /* fs */
     double ke;            /* eV*Angstrom/e^2 */
@@ -149,7 +159,7 @@ typedef struct sqeq_md_params {
     double k_oh, r_oh, k_hh, r_hh;
     double kappa;         /* dt^2 omega^2 */
     double alpha_diss;    /* dissipation strength */
-    double c[7];          /* dissipation coefficients c_0..c_6 */
+    double c[7];          /* dissipation coefficients c_0..c_5 (c[6] unused) */
 } sqeq_md_params;
 
 int  sqeq_shadow_md_init(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,

@@ -246,9 +246,12 @@ class Context:
         return q, lam.value, it.value, rel.value, r == OK
 
     # ---- shadow XL-BOMD
-    def shadow_md_init(self, nl, pos, box, params, chi, u, tol=1e-8, max_iter=200):
+    def shadow_md_init(self, nl, pos, box, params, chi, u, tol=1e-8, max_iter=200, n0=None):
+        """n0 given (numpy/torch fp64 [n]) with max_iter=0: start the history from n0 instead of q_min."""
         n = pos.shape[0]
         nhist = torch.zeros((7, n), dtype=torch.float64, device=self.device)
+        if n0 is not None:
+            nhist[0] = torch.as_tensor(n0, dtype=torch.float64).to(self.device)
         force = torch.empty((n, 3), dtype=torch.float32, device=self.device)
         en = (ctypes.c_double * 4)()
         self._check(load().sqeq_shadow_md_init(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),

@@ -222,3 +222,48 @@ def test_full_size_sampled_rows(ctx, k):
         assert np.array_equal(allj[o], jr) and np.array_equal(alls[o], sr)
     check_coulomb(ctx, nl, pos, q, c, rows=rows)
     nl.free()
+
+
+def test_shadow_md_steps_against_oracle(ctx):
+    """a-11: three shadow XL-BOMD steps on 216 aligned waters vs the fp64 oracle step (same n(0),
+    deliberately off the ground state so that the residual and Eq. 27's solution are O(1e-2))."""
+    from paper_2503_21176_b200 import binding
+    rng = np.random.default_rng(5)
+    nlat = 4
+    L = 3.1066 * nlat
+    frame = W._water_frame()
+    o = (np.stack(np.meshgrid(*[np.arange(nlat)] * 3, indexing="ij"), -1).reshape(-1, 3) + 0.5) * (L / nlat)
+    pos = ((o[:, None, :] + frame[None, :, :]).reshape(-1, 3) + rng.normal(0, 0.03, (3 * nlat ** 3, 3))).astype(np.float32)
+    n = len(pos)
+    chi, u = W.qeq_params_water_pd(n)
+    mass = W.masses_water(n)
+    vel = W.velocities(mass)
+    n0 = (np.tile([-0.5, 0.25, 0.25], n // 3) + 0.02 * rng.normal(size=n))
+    n0 -= n0.mean()
+    cfg = W.Config(9, "md_small", "water", nlat, L, 5.0, 0.6, 20, 6, 0.8)
+    p = binding.md_params(cfg, dt=0.5)
+    standin = (p.k_oh, p.r_oh, p.k_hh, p.r_hh)
+    c = [p.c[k] for k in range(6)]
+    geo = dict(box=cfg.box, rc=cfg.rc, alpha=cfg.alpha, grid=cfg.grid, order=cfg.order)
+    kw = dict(chi=chi, u=u, ke=W.KE_EV_A, qtot=0.0, standin=standin, kappa=p.kappa, krylov_rank=4, **geo)
+    st = oracle.shadow_md_init(pos, n0, **kw)
+
+    nl = ctx.nl_build(dev(pos), cfg.box, cfg.r_list)
+    x, v = dev(pos), dev(vel)
+    nh, F, en = ctx.shadow_md_init(nl, x, cfg.box, p, dev(chi), dev(u), max_iter=0, n0=n0)
+    assert en[3] == 6
+    assert relrms(F.cpu().numpy(), st["F"]) < 2e-5
+    assert relrms(nh[6].cpu().numpy(), st["nhist"][6]) < 1e-4
+    assert abs(en[0] - st["U"]) < 1e-5 * abs(st["U"])
+    ov = vel.astype(np.float64)
+    for s in range(3):
+        st, ov, ekin = oracle.shadow_md_step(st, ov, mass, 0.5, alpha_diss=p.alpha_diss, c=c, **kw)
+        en = ctx.shadow_md_step(nl, x, v, dev(mass), cfg.box, p, dev(chi), dev(u), nh, F)
+        assert np.abs(x.cpu().numpy() - st["pos"]).max() < 5e-6 * L            # fp32 positions
+        assert relrms(v.cpu().numpy(), ov) < 1e-5
+        assert relrms(F.cpu().numpy(), st["F"]) < 5e-5
+        assert relrms(nh[0].cpu().numpy(), st["nhist"][0]) < 1e-6
+        assert relrms(nh[6].cpu().numpy(), st["nhist"][6]) < 5e-4
+        assert abs(en[0] - st["U"]) < 2e-5 * abs(st["U"]) and abs(en[1] - ekin) < 1e-4 * ekin
+        assert abs(en[2] - np.linalg.norm(st["res"])) < 1e-3 * en[2]
+    nl.free()
