@@ -182,7 +182,7 @@ def run_reference(args, cfg):
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
-    from paper_2503_21176_b200 import binding
+    from paper_2503_21176_b200 import binding, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -218,8 +218,7 @@ def run_ours(args, cfg):
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
+        replicas.barrier()
         torch.cuda.synchronize()
 
     def timed(nsteps, host=None, k0=0):
@@ -230,12 +229,7 @@ def run_ours(args, cfg):
             step(k0 + k, host)
         e1.record(ctx.stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
 
     # ---- device-resident leg -------------------------------------------------------------------
     for k in range(max(args.warmup, 3)):
