@@ -93,6 +93,18 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_scal, 16 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->scal.p, 16 * sizeof(double));
+    if (e == cudaSuccess) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = device;
+        e = cudaMemPoolCreate(&ctx->pool, &props);
+        if (e == cudaSuccess) {
+            uint64_t keep = UINT64_MAX;       // never hand memory back to the driver between rebuilds
+            e = cudaMemPoolSetAttribute(ctx->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
     if (e != cudaSuccess) {
         sqeq_fail(nullptr, SQEQ_ECUDA, "sqeq_create: %s", cudaGetErrorString(e));
         delete ctx;
@@ -128,6 +140,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
+    if (ctx->pool) cudaMemPoolDestroy(ctx->pool);
     delete ctx;
     return SQEQ_OK;
 }
@@ -244,18 +257,9 @@ int sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, 
 int sqeq_nl_free(sqeq_nlist* nl)
 {
     if (!nl) return SQEQ_OK;
-    if (nl->ctx) {
-        cudaSetDevice(nl->ctx->device);
-        cudaStreamSynchronize(nl->ctx->stream);
-        cudaStreamSynchronize(nl->ctx->stream2);
-    }
-    cudaFree(nl->perm);
-    cudaFree(nl->cell_of);
-    cudaFree(nl->cell_start);
-    cudaFree(nl->wrapc);
-    cudaFree(nl->row_start);
-    cudaFree(nl->nbr);
-    delete nl;
+    if (!nl->ctx) { delete nl; return SQEQ_OK; }
+    cudaSetDevice(nl->ctx->device);
+    nl_release(nl);      // stream-ordered frees into the context's pool: no synchronisation
     return SQEQ_OK;
 }
 

@@ -31,6 +31,9 @@ struct sqeq_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     char err[512] = {0};
     int sm_count = 148;
+    cudaMemPool_t pool = nullptr;         // stream-ordered pool for neighbour-list storage (kept across rebuilds)
+    int64_t nl_last_n = 0, nl_last_total = 0;   // sizes of the previous build: next build's estimate
+    int nl_last_max_row = 0;
 
     // ---- PME state (cached by grid/order/box/alpha) ----
     int K[3] = {0, 0, 0};
@@ -86,8 +89,9 @@ struct sqeq_nlist {
     int*      cell_of = nullptr;     // [n]   cell id of sorted atom
     int*      cell_start = nullptr;  // [ncells+1]
     char4*    wrapc = nullptr;       // [n]   floor(x/L) per axis at build time (sorted order)
-    int64_t*  row_start = nullptr;   // [n+1] CSR offsets (sorted order)
-    uint32_t* nbr = nullptr;         // [n_directed]  j (27 bits) | image code (5 bits) << 27
+    int64_t*  row_start = nullptr;   // [n]   offset of row s in nbr (rows are packed, in no particular order)
+    int*      row_len = nullptr;     // [n]   entries of row s
+    uint32_t* nbr = nullptr;         // [>= n_directed]  j (27 bits) | image code (5 bits) << 27
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -131,6 +135,7 @@ static inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b)
 // ---- stage entry points (implemented in the .cu files) ----
 int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
                   sqeq_nlist** out);
+void nl_release(sqeq_nlist* nl);
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
 
 // Re-gather positions/charges into the list's order (and PME fractional coordinates if K != null).

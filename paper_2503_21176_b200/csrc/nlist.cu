@@ -2,13 +2,14 @@
 //
 // a-1  wrap + bin (fp64 cell index) -> counting sort by cell -> per-cell sort by caller index
 //      (deterministic order) -> cell-major float4 positions, permutation, wrap counts.
-// a-2  pair enumeration: one warp per atom walks the 27 (cell, image) neighbours; candidates are
-//      contiguous float4 runs (coalesced 512 B per warp load); distance test in fp32 on wrapped
-//      coordinates with a guard band, inside which the decision is taken by the exact fp64
+//      Cells have edge >= r_list/2 (stencil half-width w = 2 cells per axis), z fastest in memory.
+// a-2  pair enumeration in ONE pass: one warp per atom sweeps the contiguous atom runs of the
+//      stencil columns that can reach the cutoff sphere (see k_pairs); the distance test is fp32 on
+//      wrapped coordinates with a guard band, inside which the decision is taken by the exact fp64
 //      predicate of DESIGN.md R-NL on the raw caller positions (individually rounded IEEE ops, no
 //      FMA contraction) -- this is what makes the set bit-identical to the O(N^2) definition.
-//      Count pass -> scan -> fill pass; output is a directed CSR, entry = j | shift_code << 27,
-//      shift_code = (sx+1)*9 + (sy+1)*3 + (sz+1) with s the periodic image shift in box lengths.
+//      Output: directed rows (row_start, row_len) into one packed array, entry = j | code << 27,
+//      code = (sx+1)*9 + (sy+1)*3 + (sz+1) with s the periodic image shift in box lengths.
 //
 // Unlike Alg. 1 there is no [N,27,Cmax] candidate tensor and no padded cells[nx,ny,nz,Cmax].
 #include <math.h>
@@ -17,11 +18,15 @@
 
 struct NLGeom {
     double L[3];
-    int    nc[3];
-    float  Lf[3];
-    float  rl2f;
-    float  band;
     double rl2;
+    int    nc[3];
+    int    w[3];      // stencil half-width in cells: ceil(r_list / cell edge), 1 or 2
+    float  Lf[3];
+    float  a[3];      // cell edge
+    float  inva[3];
+    float  rl2f;
+    float  band;      // guard band of the fp32 distance test
+    float  marg;      // safety margin (Angstrom) of the fp32 column pruning
 };
 
 // wrapped coordinate in [0, L] and the integer wrap count w with x = xw + w*L (up to rounding)
@@ -191,71 +196,167 @@ static int exclusive_scan(sqeq_ctx* ctx, int64_t n1, const Tin* in, int64_t* out
 // The exact predicate (DESIGN.md R-NL): d = pos[b]-pos[a] for caller indices a<b, s = -rint(d/L),
 // d += s*L, r2 = (dx*dx + dy*dy) + dz*dz, every operation individually rounded; in range <=> r2 < rl2.
 __device__ __noinline__ bool exact_in_range(const float* __restrict__ pos, int oi, int oj,
-                                            const NLGeom& g)
+                                            double L0, double L1, double L2, double rl2)
 {
     int a = oi < oj ? oi : oj, b = oi < oj ? oj : oi;
+    const double L[3] = {L0, L1, L2};
     double d[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         double dk = __dsub_rn((double)pos[3 * (int64_t)b + k], (double)pos[3 * (int64_t)a + k]);
-        double sk = -rint(__ddiv_rn(dk, g.L[k]));
-        d[k] = __dadd_rn(dk, __dmul_rn(sk, g.L[k]));
+        double sk = -rint(__ddiv_rn(dk, L[k]));
+        d[k] = __dadd_rn(dk, __dmul_rn(sk, L[k]));
     }
     double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
-    return r2 < g.rl2;
+    return r2 < rl2;
 }
 
-template <bool FILL>
-__global__ void __launch_bounds__(256)
+__device__ __forceinline__ int floordiv(int a, int b) { int q = a / b; return (a % b != 0 && (a < 0)) ? q - 1 : q; }
+
+// Single-pass pair enumeration.  One warp per atom i (cell-major index s):
+//  1. lanes build the warp's SEGMENT list in shared memory: one lane per (x,y) column of the
+//     (2w+1)^2 cell stencil; a column is pruned when its rectangle is farther than r_list from
+//     atom i, its z-range is trimmed to the chord of the cutoff sphere, and -- cells being
+//     z-fastest in memory -- what is left is at most 3 contiguous runs of atoms (one per periodic
+//     image along z), each a segment (begin, end, image code);
+//  2. the warp sweeps the segments 32 candidates at a time (coalesced float4 loads), decides in
+//     fp32 outside the guard band and by the exact fp64 predicate inside it, and compacts the
+//     hits with ballot/popc into a per-warp staging row in shared memory;
+//  3. one atomicAdd on a global cursor reserves the row's slice of `nbr`, the staged row is copied
+//     out with coalesced stores, and (row_start, row_len) are recorded.
+// If the cursor passes `capacity` or a row outgrows the staging row the kernel keeps counting and
+// the host re-runs it with the now known sizes.
+#define NL_MAXSEG 96
+struct NLCounters {
+    unsigned long long cursor;
+    int max_row;
+    int flag;
+};
+
+template <int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 4 : 1)
 k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
-        const float* __restrict__ pos, NLGeom g, int* __restrict__ row_count,
-        const int64_t* __restrict__ row_start, uint32_t* __restrict__ nbr, int* __restrict__ max_row)
+        const float* __restrict__ pos, NLGeom g, int cap_row, unsigned long long capacity,
+        NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
+        uint32_t* __restrict__ nbr)
 {
-    const int lane = threadIdx.x & 31;
-    const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (s >= n) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4* shtab = (float4*)smem_raw;                                  // [32] image shift vectors
+    int4* segs_all = (int4*)(smem_raw + 32 * sizeof(float4));           // [WARPS][NL_MAXSEG]
+    uint32_t* stage_all = (uint32_t*)(segs_all + WARPS * NL_MAXSEG);    // [WARPS][cap_row]
+    if (threadIdx.x < 32) {
+        int img = threadIdx.x < 27 ? threadIdx.x : 13;
+        shtab[threadIdx.x] = make_float4((img / 9 - 1) * g.Lf[0], ((img / 3) % 3 - 1) * g.Lf[1],
+                                         (img % 3 - 1) * g.Lf[2], 0.f);
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t s64 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    if (s64 >= n) return;
+    const int s = (int)s64;
+    int4* segs = segs_all + wid * NL_MAXSEG;
+    uint32_t* stage = stage_all + (size_t)wid * cap_row;
     const float4 xi = xq[s];
     const int c = cell_of[s];
     const int cz = c % g.nc[2], cy = (c / g.nc[2]) % g.nc[1], cx = c / (g.nc[2] * g.nc[1]);
+
+    // ---- 1. segments
+    const int ny_st = 2 * g.w[1] + 1;
+    const int ncol = (2 * g.w[0] + 1) * ny_st;
+    int nloc = 0;
+    int4 loc0 = make_int4(0, 0, 0, 0), loc1 = loc0, loc2 = loc0;
+    if (lane < ncol) {
+        const int ox = lane / ny_st - g.w[0], oy = lane % ny_st - g.w[1];
+        const int ux = cx + ox, uy = cy + oy;
+        const int shx = floordiv(ux, g.nc[0]), shy = floordiv(uy, g.nc[1]);
+        bool valid = shx >= -1 && shx <= 1 && shy >= -1 && shy <= 1;
+        float dxm = fmaxf(fmaxf((float)ux * g.a[0] - xi.x, xi.x - (float)(ux + 1) * g.a[0]) - g.marg, 0.f);
+        float dym = fmaxf(fmaxf((float)uy * g.a[1] - xi.y, xi.y - (float)(uy + 1) * g.a[1]) - g.marg, 0.f);
+        if (ox == 0) dxm = 0.f;
+        if (oy == 0) dym = 0.f;
+        const float rem = (g.rl2f + g.band) - (dxm * dxm + dym * dym);
+        valid = valid && rem > 0.f;
+        if (valid) {
+            const float zr = sqrtf(rem) + g.marg;
+            int zlo = (int)floorf((xi.z - zr) * g.inva[2]), zhi = (int)floorf((xi.z + zr) * g.inva[2]);
+            zlo = max(zlo, cz - g.w[2]); zlo = min(zlo, cz);
+            zhi = min(zhi, cz + g.w[2]); zhi = max(zhi, cz);
+            const int colbase = ((ux - shx * g.nc[0]) * g.nc[1] + (uy - shy * g.nc[1])) * g.nc[2];
+            int zc = zlo;
+            while (zc <= zhi && nloc < 3) {
+                const int shz = floordiv(zc, g.nc[2]);
+                const int zlast = min(zhi, (shz + 1) * g.nc[2] - 1);
+                if (shz >= -1 && shz <= 1) {
+                    const int zf = zc - shz * g.nc[2];
+                    const int beg = cell_start[colbase + zf], end = cell_start[colbase + zf + (zlast - zc) + 1];
+                    if (end > beg) {
+                        const int4 v = make_int4(beg, end, (shx + 1) * 9 + (shy + 1) * 3 + (shz + 1), 0);
+                        if (nloc == 0) loc0 = v; else if (nloc == 1) loc1 = v; else loc2 = v;
+                        ++nloc;
+                    }
+                }
+                zc = zlast + 1;
+            }
+        }
+    }
+    int incl = nloc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += y;
+    }
+    const int nseg = __shfl_sync(0xffffffffu, incl, 31);
+    {
+        const int at = incl - nloc;
+        if (nloc > 0) segs[at] = loc0;
+        if (nloc > 1) segs[at + 1] = loc1;
+        if (nloc > 2) segs[at + 2] = loc2;
+    }
+    __syncwarp();
+
+    // ---- 2. sweep
     int count = 0;
-    const int64_t base = FILL ? row_start[s] : 0;
     const unsigned lt = (1u << lane) - 1u;
-    for (int img = 0; img < 27; ++img) {
-        int ox = img / 9 - 1, oy = (img / 3) % 3 - 1, oz = img % 3 - 1;
-        int nx = cx + ox, ny = cy + oy, nz = cz + oz;
-        // image shift of the neighbour cell (in box lengths): non-zero only where the stencil wraps
-        int wx = 0, wy = 0, wz = 0;
-        if (nx < 0) { nx += g.nc[0]; wx = -1; } else if (nx >= g.nc[0]) { nx -= g.nc[0]; wx = 1; }
-        if (ny < 0) { ny += g.nc[1]; wy = -1; } else if (ny >= g.nc[1]) { ny -= g.nc[1]; wy = 1; }
-        if (nz < 0) { nz += g.nc[2]; wz = -1; } else if (nz >= g.nc[2]) { nz -= g.nc[2]; wz = 1; }
-        const float sx = wx * g.Lf[0], sy = wy * g.Lf[1], sz = wz * g.Lf[2];
-        const uint32_t scode = (uint32_t)((wx + 1) * 9 + (wy + 1) * 3 + (wz + 1));
-        const int nc = (nx * g.nc[1] + ny) * g.nc[2] + nz;
-        const int beg = cell_start[nc], end = cell_start[nc + 1];
-        for (int t0 = beg; t0 < end; t0 += 32) {
+    const float hi_thr = g.rl2f + g.band, lo_thr = g.rl2f - g.band;
+    for (int sg = 0; sg < nseg; ++sg) {
+        const int4 seg = segs[sg];
+        const float4 sh = shtab[seg.z];
+        const float x0 = xi.x - sh.x, y0 = xi.y - sh.y, z0 = xi.z - sh.z;   // d = xj + shift - xi
+        const int self = seg.z == 13 ? s : -1;
+        const uint32_t codebits = (uint32_t)seg.z << 27;
+#pragma unroll 2
+        for (int t0 = seg.x; t0 < seg.y; t0 += 32) {
             const int t = t0 + lane;
             bool ok = false;
-            if (t < end) {
-                const float4 xj = xq[t];
-                const float dx = (xj.x - xi.x) + sx;
-                const float dy = (xj.y - xi.y) + sy;
-                const float dz = (xj.z - xi.z) + sz;
+            if (t < seg.y) {
+                const float4 xj = __ldg(xq + t);
+                const float dx = xj.x - x0, dy = xj.y - y0, dz = xj.z - z0;
                 const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                if (r2 < g.rl2f + g.band) {
-                    if (r2 < g.rl2f - g.band) ok = !(t == s && scode == 13u);
-                    else if (!(t == s)) ok = exact_in_range(pos, perm[s], perm[t], g);
-                }
+                ok = r2 < hi_thr && t != self;
+                if (ok && r2 >= lo_thr) ok = exact_in_range(pos, perm[s], perm[t], g.L[0], g.L[1], g.L[2], g.rl2);
             }
             const unsigned m = __ballot_sync(0xffffffffu, ok);
-            if (FILL && ok) nbr[base + count + __popc(m & lt)] = (uint32_t)t | (scode << 27);
+            if (ok) {
+                const int at = count + __popc(m & lt);
+                if (at < cap_row) stage[at] = (uint32_t)t | codebits;
+            }
             count += __popc(m);
         }
     }
-    if (!FILL && lane == 0) {
-        row_count[s] = count;
-        atomicMax(max_row, count);
+    __syncwarp();
+
+    // ---- 3. reserve and copy out
+    unsigned long long off = 0;
+    if (lane == 0) {
+        off = atomicAdd(&ctr->cursor, (unsigned long long)count);
+        atomicMax(&ctr->max_row, count);
+        row_start[s] = (int64_t)off;
+        row_len[s] = count;
     }
+    off = __shfl_sync(0xffffffffu, off, 0);
+    if (count <= cap_row && off + (unsigned long long)count <= capacity)
+        for (int k = lane; k < count; k += 32) nbr[off + k] = stage[k];
 }
 
 // ------------------------------------------------------------------------------------------ export
@@ -270,6 +371,7 @@ __device__ __forceinline__ void decode_img(uint32_t e, int& t, int& ox, int& oy,
 
 // counts, per CALLER index, the neighbours with a larger caller index
 __global__ void k_export_count(int64_t n, const int64_t* __restrict__ row_start,
+                               const int* __restrict__ row_len,
                                const uint32_t* __restrict__ nbr, const int* __restrict__ perm,
                                int* __restrict__ cnt_orig)
 {
@@ -278,7 +380,8 @@ __global__ void k_export_count(int64_t n, const int64_t* __restrict__ row_start,
     if (s >= n) return;
     const int oi = perm[s];
     int c = 0;
-    for (int64_t k = row_start[s] + lane; k < row_start[s + 1]; k += 32)
+    const int64_t beg = row_start[s], end = beg + row_len[s];
+    for (int64_t k = beg + lane; k < end; k += 32)
         c += perm[nbr[k] & 0x07ffffffu] > oi;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
@@ -288,7 +391,8 @@ __global__ void k_export_count(int64_t n, const int64_t* __restrict__ row_start,
 #define EXPORT_CAP 4096
 // one block per (sorted) atom: collect upper neighbours, sort by caller index j, write canonical rows
 __global__ void __launch_bounds__(256)
-k_export_fill(int64_t n, const int64_t* __restrict__ row_start, const uint32_t* __restrict__ nbr,
+k_export_fill(int64_t n, const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
+              const uint32_t* __restrict__ nbr,
               const int* __restrict__ perm, const char4* __restrict__ wrapc,
               const int64_t* __restrict__ off_orig, int32_t* __restrict__ out_i,
               int32_t* __restrict__ out_j, int8_t* __restrict__ out_s, int* __restrict__ flag)
@@ -298,7 +402,7 @@ k_export_fill(int64_t n, const int64_t* __restrict__ row_start, const uint32_t* 
     __shared__ int cnt;
     const int64_t s = blockIdx.x;
     const int oi = perm[s];
-    const int64_t beg = row_start[s], end = row_start[s + 1];
+    const int64_t beg = row_start[s], end = beg + row_len[s];
     const int64_t o0 = off_orig[oi];
     const int m = (int)(off_orig[oi + 1] - o0);
     if (m == 0) return;
@@ -351,21 +455,72 @@ k_export_fill(int64_t n, const int64_t* __restrict__ row_start, const uint32_t* 
 }
 
 // ------------------------------------------------------------------------------------------ host
-static void fill_geom(NLGeom& g, const double box[3], double cutoff)
+static void fill_geom(NLGeom& g, const double box[3], double cutoff, int64_t n)
 {
     double lmax = 0;
+    const double rl = cutoff * (1.0 + 1e-6);
     for (int d = 0; d < 3; ++d) {
         g.L[d] = box[d];
         g.Lf[d] = (float)box[d];
-        int nc = (int)floor(box[d] / (cutoff * (1.0 + 1e-6)));
-        g.nc[d] = nc < 1 ? 1 : nc;
+        int nc = (int)floor(2.0 * box[d] / rl);          // edge >= r_list/2
+        g.nc[d] = nc < 1 ? 1 : (nc > 1024 ? 1024 : nc);
         lmax = fmax(lmax, box[d]);
+    }
+    // keep cells from becoming absurdly many for huge dilute boxes: at most ~ 4n cells + 64
+    while ((int64_t)g.nc[0] * g.nc[1] * g.nc[2] > 4 * n + 64) {
+        int dmax = 0;
+        for (int d = 1; d < 3; ++d) if (g.nc[d] > g.nc[dmax]) dmax = d;
+        g.nc[dmax] = (g.nc[dmax] + 1) / 2;
+    }
+    for (int d = 0; d < 3; ++d) {
+        const double a = box[d] / g.nc[d];
+        g.a[d] = (float)a;
+        g.inva[d] = (float)(1.0 / a);
+        g.w[d] = a >= rl ? 1 : 2;
     }
     g.rl2 = cutoff * cutoff;
     g.rl2f = (float)g.rl2;
     // fp32 error of r2 on wrapped coordinates: |delta d| <= 1.5 ulp(L) per axis, so
     // |delta r2| <= 2 sqrt(3) r 1.5 L 2^-23 + 3 r^2 2^-24 ~ 5.2 r L 2^-23; band = 3x that.
     g.band = (float)((16.0 * cutoff * lmax + 8.0 * cutoff * cutoff) * ldexp(1.0, -23));
+    // column pruning compares fp32 cell faces (index * edge) with fp32 wrapped coordinates: both are
+    // within a few ulp(L) of the fp64 values the binning used; 64 ulp(L) + 1e-4 of an edge is safe.
+    g.marg = (float)(64.0 * lmax * ldexp(1.0, -23) + 1e-4 * lmax / 64.0);
+}
+
+static int pool_alloc(sqeq_ctx* ctx, void** p, size_t bytes)
+{
+    cudaError_t e = cudaMallocFromPoolAsync(p, bytes > 0 ? bytes : 4, ctx->pool, ctx->stream);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        *p = nullptr;
+        return sqeq_fail(ctx, e == cudaErrorMemoryAllocation ? SQEQ_ENOMEM : SQEQ_ECUDA,
+                         "neighbour-list allocation of %zu bytes failed: %s", bytes, cudaGetErrorString(e));
+    }
+    return SQEQ_OK;
+}
+
+void nl_release(sqeq_nlist* nl)
+{
+    cudaStream_t st = nl->ctx->stream;
+    void* ptrs[] = {nl->perm, nl->cell_of, nl->cell_start, nl->wrapc, nl->row_start, nl->row_len, nl->nbr};
+    for (void* p : ptrs)
+        if (p) cudaFreeAsync(p, st);     // stream-ordered: safe after every evaluation already enqueued
+    delete nl;
+}
+
+template <int WARPS>
+static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, int cap_row,
+                        size_t capacity, NLCounters* ctr, cudaStream_t st)
+{
+    const size_t smem = 32 * sizeof(float4) + (size_t)WARPS * NL_MAXSEG * sizeof(int4) +
+                        (size_t)WARPS * cap_row * sizeof(uint32_t);
+    CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_pairs<WARPS><<<ceil_div(nl->n, WARPS), WARPS * 32, smem, st>>>(
+        nl->n, (const float4*)ctx->xq.p, nl->cell_of, nl->cell_start, nl->perm, pos, g, cap_row,
+        (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
 }
 
 int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
@@ -373,44 +528,39 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
 {
     cudaStream_t st = ctx->stream;
     NLGeom g;
-    fill_geom(g, box, cutoff);
-    // keep cells from becoming absurdly many for huge dilute boxes: at most ~ n cells + 64
-    int64_t ncells = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
-    while (ncells > 4 * n + 64) {
-        int dmax = 0;
-        for (int d = 1; d < 3; ++d) if (g.nc[d] > g.nc[dmax]) dmax = d;
-        g.nc[dmax] = (g.nc[dmax] + 1) / 2;
-        ncells = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
-    }
+    fill_geom(g, box, cutoff, n);
+    const int64_t ncells = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
     sqeq_nlist* nl = new sqeq_nlist();
     nl->ctx = ctx;
     nl->n = n;
     nl->cutoff = cutoff;
     for (int d = 0; d < 3; ++d) { nl->box[d] = box[d]; nl->ncell[d] = g.nc[d]; }
 
-    int *cell_id = nullptr, *cell_count = nullptr, *cell_fill = nullptr, *flag = nullptr, *row_count = nullptr;
+    int *cell_id = nullptr, *cell_count = nullptr, *cell_fill = nullptr, *flag = nullptr;
     int64_t* tmp64 = nullptr;
+    NLCounters* ctr = nullptr;
     auto cleanup = [&](int code) {
-        cudaFree(cell_id); cudaFree(cell_count); cudaFree(cell_fill); cudaFree(flag);
-        cudaFree(row_count); cudaFree(tmp64);
-        if (code != SQEQ_OK) sqeq_nl_free(nl);
+        void* tmp[] = {cell_id, cell_count, cell_fill, flag, tmp64, ctr};
+        for (void* p : tmp) if (p) cudaFreeAsync(p, st);
+        if (code != SQEQ_OK) nl_release(nl);
         return code;
     };
 #define NL_TRY(expr) do { int _r = (expr); if (_r != SQEQ_OK) return cleanup(_r); } while (0)
 #define NL_CUDA(expr) do { cudaError_t _e = (expr); if (_e != cudaSuccess) return cleanup(sqeq_fail(ctx, \
         _e == cudaErrorMemoryAllocation ? SQEQ_ENOMEM : SQEQ_ECUDA, "%s: %s", #expr, cudaGetErrorString(_e))); } while (0)
 
-    NL_CUDA(cudaMalloc((void**)&cell_id, sizeof(int) * n));
-    NL_CUDA(cudaMalloc((void**)&cell_count, sizeof(int) * (ncells + 1)));
-    NL_CUDA(cudaMalloc((void**)&cell_fill, sizeof(int) * (ncells + 1)));
-    NL_CUDA(cudaMalloc((void**)&flag, sizeof(int) * 2));
-    NL_CUDA(cudaMalloc((void**)&row_count, sizeof(int) * (n + 1)));
-    NL_CUDA(cudaMalloc((void**)&tmp64, sizeof(int64_t) * (ncells + 1)));
-    NL_CUDA(cudaMalloc((void**)&nl->perm, sizeof(int) * n));
-    NL_CUDA(cudaMalloc((void**)&nl->cell_of, sizeof(int) * n));
-    NL_CUDA(cudaMalloc((void**)&nl->cell_start, sizeof(int) * (ncells + 1)));
-    NL_CUDA(cudaMalloc((void**)&nl->wrapc, sizeof(char4) * n));
-    NL_CUDA(cudaMalloc((void**)&nl->row_start, sizeof(int64_t) * (n + 1)));
+    NL_TRY(pool_alloc(ctx, (void**)&cell_id, sizeof(int) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&cell_count, sizeof(int) * (ncells + 1)));
+    NL_TRY(pool_alloc(ctx, (void**)&cell_fill, sizeof(int) * (ncells + 1)));
+    NL_TRY(pool_alloc(ctx, (void**)&flag, sizeof(int) * 2));
+    NL_TRY(pool_alloc(ctx, (void**)&tmp64, sizeof(int64_t) * (ncells + 1)));
+    NL_TRY(pool_alloc(ctx, (void**)&ctr, sizeof(NLCounters)));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->perm, sizeof(int) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->cell_of, sizeof(int) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->cell_start, sizeof(int) * (ncells + 1)));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->wrapc, sizeof(char4) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->row_start, sizeof(int64_t) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->row_len, sizeof(int) * n));
     NL_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * n));
     float4* xq = (float4*)ctx->xq.p;
 
@@ -427,38 +577,64 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         ctx->launches++;
         k_scatter<<<nb, 256, 0, st>>>(n, cell_id, nl->cell_start, cell_fill, nl->perm);
         ctx->launches++;
-        k_sort_cells<<<(int)ncells, 256, 0, st>>>(nl->cell_start, nl->perm);
+        // per-cell sort: block size from the mean occupancy (cells hold ~10 atoms at liquid density)
+        int sort_threads = 32;
+        while (sort_threads < 256 && sort_threads < 2 * n / ncells) sort_threads <<= 1;
+        k_sort_cells<<<(int)ncells, sort_threads, 0, st>>>(nl->cell_start, nl->perm);
         ctx->launches++;
         k_reorder<<<nb, 256, 0, st>>>(n, pos, nl->perm, g, xq, nl->cell_of, nl->wrapc);
         ctx->launches++;
         NL_CUDA(cudaGetLastError());
     }
-    int h_flag[2] = {0, 0};
     {
         StageTimer tm(ctx, SQEQ_T_NL_PAIRS);
-        int* max_row = flag + 1;
-        NL_CUDA(cudaMemsetAsync(row_count, 0, sizeof(int) * (n + 1), st));
-        const int nbw = ceil_div(n * 32, 256);
-        k_pairs<false><<<nbw, 256, 0, st>>>(n, xq, nl->cell_of, nl->cell_start, nl->perm, pos, g,
-                                             row_count, nullptr, nullptr, max_row);
-        ctx->launches++;
-        NL_TRY(exclusive_scan<int>(ctx, n + 1, row_count, nl->row_start, st));
-        int64_t total = 0;
-        NL_CUDA(cudaMemcpyAsync(&total, nl->row_start + n, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-        NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int) * 2, cudaMemcpyDeviceToHost, st));
-        NL_CUDA(cudaStreamSynchronize(st));
-        if (h_flag[0] & 1)
-            return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
-                                     "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
-        nl->n_directed = total;
-        nl->max_row = h_flag[1];
-        NL_CUDA(cudaMalloc((void**)&nl->nbr, sizeof(uint32_t) * (size_t)(total > 0 ? total : 1)));
-        k_pairs<true><<<nbw, 256, 0, st>>>(n, xq, nl->cell_of, nl->cell_start, nl->perm, pos, g,
-                                            nullptr, nl->row_start, nl->nbr, nullptr);
-        ctx->launches++;
-        NL_CUDA(cudaGetLastError());
+        // sizes: from the previous build of the same system if there was one, else from the mean
+        // density; the kernel reports the exact sizes and is re-run if either estimate was short
+        const double vol = box[0] * box[1] * box[2];
+        const double mean_row = 4.0 / 3.0 * M_PI * cutoff * cutoff * cutoff * (double)n / vol;
+        size_t capacity;
+        int cap_row;
+        if (ctx->nl_last_n == n && ctx->nl_last_total > 0) {
+            capacity = (size_t)(1.08 * (double)ctx->nl_last_total) + 4096;
+            cap_row = (int)(1.2 * ctx->nl_last_max_row) + 32;
+        } else {
+            capacity = (size_t)(1.2 * mean_row * (double)n) + 64 * (size_t)n + 4096;
+            cap_row = (int)(1.5 * mean_row) + 128;
+        }
+        cap_row = (cap_row + 31) & ~31;
+        NLCounters* h = (NLCounters*)(ctx->h_scal + 12);
+        int* h_flag = (int*)(ctx->h_scal + 14);
+        for (int attempt = 0;; ++attempt) {
+            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, sizeof(uint32_t) * capacity));
+            NL_CUDA(cudaMemsetAsync(ctr, 0, sizeof(NLCounters), st));
+            // staging rows: 8 warps per block up to 6656 entries per row, 2 warps per block beyond
+            if (cap_row <= 6656) NL_TRY(launch_pairs<8>(ctx, nl, pos, g, cap_row, capacity, ctr, st));
+            else if (cap_row <= 27648) NL_TRY(launch_pairs<2>(ctx, nl, pos, g, cap_row, capacity, ctr, st));
+            else return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
+                        "sqeq_nl_build: a row has %d neighbours; rows above 27648 are not supported", cap_row));
+            NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
+            NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+            NL_CUDA(cudaStreamSynchronize(st));
+            if (h_flag[0] & 1)
+                return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
+                                         "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
+            const bool row_ok = h->max_row <= cap_row, cap_ok = h->cursor <= capacity;
+            if (row_ok && cap_ok) break;
+            if (attempt >= 2)
+                return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY, "sqeq_nl_build: sizing did not converge"));
+            if (!row_ok) cap_row = (h->max_row + 31) & ~31;
+            if (!cap_ok) {
+                NL_CUDA(cudaFreeAsync(nl->nbr, st));
+                nl->nbr = nullptr;
+                capacity = (size_t)h->cursor;
+            }
+        }
+        nl->n_directed = (int64_t)h->cursor;
+        nl->max_row = h->max_row;
+        ctx->nl_last_n = n;
+        ctx->nl_last_total = nl->n_directed;
+        ctx->nl_last_max_row = nl->max_row;
     }
-    NL_CUDA(cudaStreamSynchronize(st));
     *out = nl;
     cleanup(SQEQ_OK);
     return SQEQ_OK;
@@ -479,11 +655,11 @@ int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj
     CUDA_TRY(ctx, cudaMalloc((void**)&flag, sizeof(int)));
     CUDA_TRY(ctx, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
     CUDA_TRY(ctx, cudaMemsetAsync(flag, 0, sizeof(int), st));
-    k_export_count<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, nl->row_start, nl->nbr, nl->perm, cnt);
+    k_export_count<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, nl->row_start, nl->row_len, nl->nbr, nl->perm, cnt);
     KERNEL_CHECK(ctx);
     int r = exclusive_scan<int>(ctx, n + 1, cnt, off, st);
     if (r == SQEQ_OK) {
-        k_export_fill<<<(unsigned)n, 256, 0, st>>>(n, nl->row_start, nl->nbr, nl->perm, nl->wrapc, off,
+        k_export_fill<<<(unsigned)n, 256, 0, st>>>(n, nl->row_start, nl->row_len, nl->nbr, nl->perm, nl->wrapc, off,
                                                     oi, oj, shift3, flag);
         ctx->launches++;
     }

@@ -96,25 +96,51 @@ struct RealParams {
     float rc2;
     float alpha;
     float c2;        // 2 alpha / sqrt(pi)
+    float na2l2e;    // -alpha^2 log2(e):  exp(-alpha^2 r^2) = 2^(na2l2e r^2)
 };
+
+// MUFU wrappers (one XU instruction each, <= 2 ulp; flush-to-zero is harmless here)
+__device__ __forceinline__ float mufu_rsqrt(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rcp(float x)   { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_ex2(float x)   { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// erfc(x) = exp(-x^2) t P6(t), t = 1/(1 + 0.3275911 x), x >= 0, given ex = exp(-x^2).
+// The form is Abramowitz & Stegun 7.1.26 extended to 7 terms; the coefficients are a weighted
+// minimax fit of erfcx(x) = exp(x^2) erfc(x) made for this library (max |error| of erfc 3.5e-9 in
+// exact arithmetic, ~5e-8 rms once evaluated in fp32) -- 1 MUFU.RCP + 8 FP32 ops instead of the
+// ~40-instruction erfcf, and it shares the exp(-alpha^2 r^2) the force needs anyway.
+__device__ __forceinline__ float erfc_from_exp(float x, float ex)
+{
+    const float t = mufu_rcp(fmaf(0.3275911f, x, 1.f));
+    float p = -0.2984510018424136f;
+    p = fmaf(p, t, 1.504820963708936f);
+    p = fmaf(p, t, -2.085553381950119f);
+    p = fmaf(p, t, 2.0401082452998613f);
+    p = fmaf(p, t, -0.7490695346520456f);
+    p = fmaf(p, t, 0.4311045009554423f);
+    p = fmaf(p, t, 0.1570402119784954f);
+    return p * t * ex;
+}
 
 template <bool FORCE>
 __global__ void __launch_bounds__(256)
 k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row_start,
-       const uint32_t* __restrict__ nbr, RealParams p, float4* __restrict__ out)
+       const int* __restrict__ row_len, const uint32_t* __restrict__ nbr, RealParams p,
+       float4* __restrict__ out)
 {
     __shared__ float4 sh[32];
-    if (threadIdx.x < 27) {
-        int img = threadIdx.x;
-        sh[img] = make_float4((img / 9 - 1) * p.Lx, ((img / 3) % 3 - 1) * p.Ly, (img % 3 - 1) * p.Lz, 0.f);
+    if (threadIdx.x < 32) {
+        int img = threadIdx.x < 27 ? threadIdx.x : 13;
+        sh[threadIdx.x] = make_float4((img / 9 - 1) * p.Lx, ((img / 3) % 3 - 1) * p.Ly, (img % 3 - 1) * p.Lz, 0.f);
     }
     __syncthreads();
     const int lane = threadIdx.x & 31;
     const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     if (s >= n) return;
     const float4 xi = xq[s];
-    const int64_t beg = row_start[s], end = row_start[s + 1];
+    const int64_t beg = row_start[s], end = beg + row_len[s];
     float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+    // branch-free body: a lane outside rc contributes q_j * 0, so the two unrolled iterations interleave
 #pragma unroll 2
     for (int64_t k = beg + lane; k < end; k += 32) {
         const uint32_t e = __ldg(nbr + k);
@@ -125,19 +151,16 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
         const float dy = (xi.y - xj.y) - s4.y;
         const float dz = (xi.z - xj.z) - s4.z;
         const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-        if (r2 < p.rc2) {
-            const float rinv = rsqrtf(r2);
-            const float r = r2 * rinv;
-            const float ar = p.alpha * r;
-            const float t = erfcf(ar) * rinv;                 // erfc(alpha r)/r
-            phi = fmaf(xj.w, t, phi);
-            if (FORCE) {
-                const float ex = expf(-ar * ar);
-                const float gq = xj.w * fmaf(p.c2, ex, t) * (rinv * rinv);
-                fx = fmaf(gq, dx, fx);
-                fy = fmaf(gq, dy, fy);
-                fz = fmaf(gq, dz, fz);
-            }
+        const float qj = r2 < p.rc2 ? xj.w : 0.f;
+        const float rinv = mufu_rsqrt(r2);
+        const float ex = mufu_ex2(p.na2l2e * r2);             // exp(-alpha^2 r^2)
+        const float t = erfc_from_exp(p.alpha * (r2 * rinv), ex) * rinv;   // erfc(alpha r)/r
+        phi = fmaf(qj, t, phi);
+        if (FORCE) {
+            const float gq = qj * fmaf(p.c2, ex, t) * (rinv * rinv);
+            fx = fmaf(gq, dx, fx);
+            fy = fmaf(gq, dy, fy);
+            fz = fmaf(gq, dz, fz);
         }
     }
 #pragma unroll
@@ -163,13 +186,14 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     p.rc2 = (float)(rc * rc);
     p.alpha = (float)alpha;
     p.c2 = (float)(2.0 * alpha / sqrt(M_PI));
+    p.na2l2e = (float)(-alpha * alpha * 1.4426950408889634);
     StageTimer tm(ctx, SQEQ_T_REAL, st);
     const int nb = ceil_div(n * 32, 256);
     if (want_force)
-        k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->nbr, p,
+        k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, nl->nbr, p,
                                           (float4*)ctx->real_out.p);
     else
-        k_real<false><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->nbr, p,
+        k_real<false><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, nl->nbr, p,
                                            (float4*)ctx->real_out.p);
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
