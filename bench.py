@@ -44,53 +44,70 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
-         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled DURING the timed region, in-process through NVML (the
+    same counters as the nvidia-smi clocks line of B200_PROFILING.md; a polling nvidia-smi
+    subprocess stalls the driver for ~0.3 s when it is started or torn down, which a run of a few
+    dozen 1 ms steps cannot absorb)."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
-    def __init__(self, gpu_index):
-        self.gpu = gpu_index
-        self.proc = None
-        self.lines = []
+    def __init__(self, gpu_index, period_s=0.01):
+        self.gpu, self.period = gpu_index, period_s
+        self.sm, self.pw, self.bits = [], [], 0
+        self.h = self.nv = None
+        self.stop_flag = threading.Event()
+        self.thr = None
+        self.sm_max = None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.thr = threading.Thread(target=self._read, daemon=True)
+            import pynvml
+            pynvml.nvmlInit()
+            idx = self.gpu
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            if vis:
+                try:
+                    idx = int(vis.split(",")[self.gpu])
+                except ValueError:
+                    idx = self.gpu
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self._one()          # first query outside the timed region (it initialises NVML state)
+            self.sm, self.pw, self.bits = [], [], 0
+            self.thr = threading.Thread(target=self._loop, daemon=True)
             self.thr.start()
-        except Exception:
-            self.proc = None
+        except Exception as ex:  # reported in the JSON line, never hidden
+            self.h = None
+            self.err = str(ex)
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.lines.append(line.strip())
+    def _one(self):
+        nv = self.nv
+        self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+        try:
+            self.pw.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
+        except Exception:
+            pass
+        try:
+            self.bits |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+        except Exception:
+            self.bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+
+    def _loop(self):
+        while not self.stop_flag.is_set():
+            try:
+                self._one()
+            except Exception:
+                break
+            self.stop_flag.wait(self.period)
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.25)
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except Exception:
-            self.proc.kill()
-        sm, mx, reasons, pw = [], [], set(), []
-        for ln in self.lines:
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 9:
-                continue
-            try:
-                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
-            except ValueError:
-                continue
-            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[5:9]):
-                if v.lower().startswith("active"):
-                    reasons.add(name)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+        if self.h is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + getattr(self, "err", "?")]}
+        self.stop_flag.set()
+        self.thr.join(timeout=2)
+        reasons = sorted(name for bit, name in self.REASONS.items() if self.bits & bit)
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.sm_max,
+                "power_w_max": max(self.pw) if self.pw else None, "samples": len(self.sm), "reasons": reasons}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -231,27 +248,25 @@ def run_ours(args, cfg):
         barrier()
         return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
 
-    # ---- device-resident leg -------------------------------------------------------------------
+    # ---- device-resident leg: the reported value (no stage events), clocks sampled during it ------
     for k in range(max(args.warmup, 3)):
         step(k)
-    ctx.profile_enable(True)
-    ctx.profile_reset()
     ctx.launch_count(reset=True)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    ms = timed(args.steps)
+    ms_value = timed(args.steps)
     launches = ctx.launch_count()
+    clocks = sampler.stop() if rank == 0 else {}
+    value = world * 1e3 * args.steps / ms_value
+    ms_step = ms_value / args.steps
+
+    # ---- same loop again with a CUDA-event pair around every stage (per-kernel durations) ---------
+    ctx.profile_enable(True)
+    ctx.profile_reset()
+    ms = timed(args.steps)
     prof = ctx.profile_read()
     ctx.profile_enable(False)
-    clocks = sampler.stop() if rank == 0 else {}
-    ms_step = ms / args.steps
-    value = world * 1e3 / ms_step
-
-    # same loop without the stage events (they add two event records per kernel)
-    ms_noprof = timed(args.steps)
-    value = max(value, world * 1e3 * args.steps / ms_noprof) if args.best_of_two else world * 1e3 * args.steps / ms_noprof
-    ms_step = 1e3 * world / value
 
     # ---- end-to-end leg: C-ABI call with HOST buffers, copies inside the timed region -----------
     hp = [p.cpu().pin_memory() for p in possets]
@@ -406,7 +421,6 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-md", action="store_true")
-    ap.add_argument("--best-of-two", action="store_true")
     ap.add_argument("--krylov-iters", type=int, default=50)
     ap.add_argument("--md-steps", type=int, default=20)
     args = ap.parse_args()

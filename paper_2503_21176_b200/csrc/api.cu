@@ -2,6 +2,7 @@
 // per-stage event timing, and the sqeq_coulomb orchestration (include/sqeq.h).
 #include <math.h>
 #include <stdarg.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 
@@ -111,6 +112,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
         return SQEQ_ECUDA;
     }
     ctx->scal.cap = 16 * sizeof(double);
+    const char* env = getenv("SQEQ_PME_TILES");
+    ctx->pme_tiles_off = env && env[0] == '0';
     *out = ctx;
     return SQEQ_OK;
 }
@@ -295,13 +298,19 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
                  double alpha, float* phi, float* force, bool want_energy, bool field_mode)
 {
     const bool want_force = force != nullptr;
-    // fork: PME on the side stream, real space on the main stream
-    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
-    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream2, ctx->ev_fork, 0));
-    SQEQ_TRY(pme_run(ctx, n, box, want_force, false, ctx->stream2));
-    CUDA_TRY(ctx, cudaEventRecord(ctx->ev_join, ctx->stream2));
-    SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
-    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+    // fork: PME on the side stream, real space on the main stream.  With stage timing on, both run
+    // on the main stream so that every event pair brackets one kernel running alone.
+    if (ctx->profiling) {
+        SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream));
+        SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
+    } else {
+        CUDA_TRY(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
+        CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream2, ctx->ev_fork, 0));
+        SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream2));
+        CUDA_TRY(ctx, cudaEventRecord(ctx->ev_join, ctx->stream2));
+        SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
+        CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
+    }
     SQEQ_TRY(assemble_run(ctx, nl, alpha, phi, force, want_energy, field_mode, ctx->stream));
     ctx->last_had_force = want_force;
     ctx->last_n = n;

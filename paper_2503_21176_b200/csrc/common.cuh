@@ -42,6 +42,7 @@ struct sqeq_ctx {
     double tab_alpha = 0;
     cufftHandle plan_r2c = 0, plan_c2r = 0;
     bool plans_ok = false;
+    bool pme_tiles_off = false;           // SQEQ_PME_TILES=0: global-memory spread/gather only (testing)
     DevBuf grid;      // float  [K0][K1][K2]        charge grid Q, then potential grid Phi
     DevBuf gridQ;     // float  copy of Q kept for sqeq_pme_grid (diagnostics only when enabled)
     DevBuf spec;      // float2 [K0][K1][K2/2+1]
@@ -147,8 +148,9 @@ int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const do
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
                   cudaStream_t st);
 int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3], int order);
-int pme_run(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_force, bool want_energy,
-            cudaStream_t st);
+// nl supplies the cell-major atom runs the shared-memory tiles are built on (NULL: global kernels)
+int pme_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,
+            bool want_energy, cudaStream_t st);
 int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, float* force,
                  bool want_energy, bool field_mode, cudaStream_t st);
 // Full evaluation on prepared geometry (used by coulomb, qeq and md drivers).

@@ -38,35 +38,69 @@ __device__ __forceinline__ void bspline_weights(float w, float* theta, float* dt
 }
 
 // -------------------------------------------------------------------------------------- spread
-// a-4, Alg. 2 step 1.  One warp per atom; lanes 0..2 evaluate the three axes'
-// weights into shared memory, then the 32 lanes sweep the P^3 points z-fastest (contiguous rows of P
-// floats) and reduce into the grid with red.global.add.f32.
+// a-4, Alg. 2 step 1.  A block takes SPREAD_APB consecutive atoms: 3 threads per
+// atom evaluate the per-axis weights into shared memory, then the block sweeps the atoms' P^2 (x,y)
+// ROWS, one row of P z-contiguous points per thread (flat row index -> every lane busy, index
+// arithmetic paid once per row instead of once per point).  A row is added to the grid with
+// 8-byte vector reductions (red.global.add.v2.f32) on even-aligned pairs; K2 is even, so a pair
+// never straddles the periodic boundary, and an odd row start is padded with a zero on each side.
+#define SPREAD_APB 64
+__device__ __forceinline__ void red_add_v2(float* addr, float a, float b)
+{
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(a), "f"(b) : "memory");
+}
+
 template <int P>
 __global__ void __launch_bounds__(256)
 k_spread(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ base, int K0, int K1, int K2,
          float* __restrict__ grid)
 {
-    __shared__ float wt[8][3][P];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (s >= n) return;
-    const float4 fw = frac[s];
-    const int4 f = base[s];
-    if (lane < 3) {
-        float th[P], dth[P];
-        bspline_weights<P>(lane == 0 ? fw.x : (lane == 1 ? fw.y : fw.z), th, dth);
+    __shared__ float wt[SPREAD_APB][3][P];
+    __shared__ int4 sb[SPREAD_APB];
+    const int64_t s0 = blockIdx.x * (int64_t)SPREAD_APB;
+    const int na = (int)min((int64_t)SPREAD_APB, n - s0);
+    if (threadIdx.x < 3 * SPREAD_APB) {
+        const int at = threadIdx.x / 3, ax = threadIdx.x % 3;
+        if (at < na) {
+            const float4 fw = frac[s0 + at];
+            float th[P], dth[P];
+            bspline_weights<P>(ax == 0 ? fw.x : (ax == 1 ? fw.y : fw.z), th, dth);
 #pragma unroll
-        for (int j = 0; j < P; ++j) wt[wid][lane][j] = th[j];
+            for (int j = 0; j < P; ++j) wt[at][ax][j] = th[j];
+            if (ax == 0) {
+                int4 f = base[s0 + at];
+                f.w = __float_as_int(fw.w);
+                sb[at] = f;
+            }
+        }
     }
-    __syncwarp();
-    if (fw.w == 0.f) return;
-    for (int pidx = lane; pidx < P * P * P; pidx += 32) {
-        const int c = pidx % P, b = (pidx / P) % P, a = pidx / (P * P);
+    __syncthreads();
+    const int rows = na * P * P;
+    for (int R = threadIdx.x; R < rows; R += blockDim.x) {
+        const int at = R / (P * P), row = R % (P * P);
+        const int a = row / P, b = row % P;
+        const int4 f = sb[at];
+        const float w2 = __int_as_float(f.w) * wt[at][0][a] * wt[at][1][b];
+        if (w2 == 0.f) continue;
         int gx = f.x - a; gx += gx < 0 ? K0 : 0;
         int gy = f.y - b; gy += gy < 0 ? K1 : 0;
-        int gz = f.z - c; gz += gz < 0 ? K2 : 0;
-        const float v = fw.w * wt[wid][0][a] * wt[wid][1][b] * wt[wid][2][c];
-        atomicAdd(grid + ((size_t)gx * K1 + gy) * K2 + gz, v);
+        float* rowp = grid + ((size_t)gx * K1 + gy) * K2;
+        // ascending z: point i (0..P-1) is grid index zs+i and carries theta_z[P-1-i]
+        int zs = f.z - (P - 1); zs += zs < 0 ? K2 : 0;
+        const int odd = zs & 1;
+        float ext[P + 2];
+        ext[0] = 0.f; ext[P + 1] = 0.f;
+#pragma unroll
+        for (int i = 0; i < P; ++i) ext[i + 1] = w2 * wt[at][2][P - 1 - i];
+        int pz = zs - odd;                       // even start of the first pair
+#pragma unroll
+        for (int j = 0; j <= P / 2; ++j) {
+            if (j == P / 2 && !odd) break;
+            const float lo = odd ? ext[2 * j] : ext[2 * j + 1];
+            const float hi = odd ? ext[2 * j + 1] : ext[2 * j + 2];
+            red_add_v2(rowp + pz, lo, hi);
+            pz += 2; pz -= pz >= K2 ? K2 : 0;
+        }
     }
 }
 
@@ -117,6 +151,36 @@ k_influence(int K0, int K1, int K2h, int K2, const double* __restrict__ tab, dou
 
 // -------------------------------------------------------------------------------------- gather
 // a-8, Alg. 2 step 5: phi_i = sum W Phi;  F_i,x = -q_i (K_x/L_x) sum dW_x Phi.
+// One warp per atom, one (x,y) ROW of P z-contiguous points per lane: per row the z sums
+// s0 = sum_c theta_z Phi and s1 = sum_c dtheta_z Phi cost 2 FMAs per point, and the x,y factors are
+// applied once per row.  For P = 6 the 4 rows beyond the first 32 are handed out point by point to
+// lanes 0..23 so that no pass runs with 4 active lanes.
+template <int P, bool FORCE>
+__device__ __forceinline__ void gather_row(const float* __restrict__ grid, const float (*w)[P], int a, int b,
+                                           int c0, int c1, const int4 f, int K0, int K1, int K2,
+                                           float& ph, float& gx_, float& gy_, float& gz_)
+{
+    int gx = f.x - a; gx += gx < 0 ? K0 : 0;
+    int gy = f.y - b; gy += gy < 0 ? K1 : 0;
+    const float* rowp = grid + ((size_t)gx * K1 + gy) * K2;
+    float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+    for (int c = 0; c < P; ++c) {
+        if (c < c0 || c >= c1) continue;
+        int gz = f.z - c; gz += gz < 0 ? K2 : 0;
+        const float v = __ldg(rowp + gz);
+        s0 = fmaf(w[2][c], v, s0);
+        if (FORCE) s1 = fmaf(w[5][c], v, s1);
+    }
+    const float tx = w[0][a], ty = w[1][b];
+    ph = fmaf(tx * ty, s0, ph);
+    if (FORCE) {
+        gx_ = fmaf(w[3][a] * ty, s0, gx_);
+        gy_ = fmaf(tx * w[4][b], s0, gy_);
+        gz_ = fmaf(tx * ty, s1, gz_);
+    }
+}
+
 template <int P, bool FORCE>
 __global__ void __launch_bounds__(256)
 k_gather(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ base, int K0, int K1, int K2,
@@ -135,20 +199,17 @@ k_gather(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ ba
         for (int j = 0; j < P; ++j) { wt[wid][lane][j] = th[j]; wt[wid][3 + lane][j] = dth[j]; }
     }
     __syncwarp();
+    const float (*w)[P] = wt[wid];
     float ph = 0.f, gx_ = 0.f, gy_ = 0.f, gz_ = 0.f;
-    for (int pidx = lane; pidx < P * P * P; pidx += 32) {
-        const int c = pidx % P, b = (pidx / P) % P, a = pidx / (P * P);
-        int gx = f.x - a; gx += gx < 0 ? K0 : 0;
-        int gy = f.y - b; gy += gy < 0 ? K1 : 0;
-        int gz = f.z - c; gz += gz < 0 ? K2 : 0;
-        const float v = __ldg(grid + ((size_t)gx * K1 + gy) * K2 + gz);
-        const float tx = wt[wid][0][a], ty = wt[wid][1][b], tz = wt[wid][2][c];
-        ph = fmaf(tx * ty * tz, v, ph);
-        if (FORCE) {
-            gx_ = fmaf(wt[wid][3][a] * ty * tz, v, gx_);
-            gy_ = fmaf(tx * wt[wid][4][b] * tz, v, gy_);
-            gz_ = fmaf(tx * ty * wt[wid][5][c], v, gz_);
+    if (P == 6) {
+        gather_row<P, FORCE>(grid, w, lane / P, lane % P, 0, P, f, K0, K1, K2, ph, gx_, gy_, gz_);
+        if (lane < 24) {                       // rows 32..35 = (a = 5, b = 2..5), one point per lane
+            const int c = lane % P;
+            gather_row<P, FORCE>(grid, w, 5, 2 + lane / P, c, c + 1, f, K0, K1, K2, ph, gx_, gy_, gz_);
         }
+    } else {
+        for (int row = lane; row < P * P; row += 32)
+            gather_row<P, FORCE>(grid, w, row / P, row % P, 0, P, f, K0, K1, K2, ph, gx_, gy_, gz_);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -160,6 +221,317 @@ k_gather(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ ba
         }
     }
     if (lane == 0) out[s] = make_float4(-sx * gx_, -sy * gy_, -sz * gz_, ph);   // per unit charge; a-9 applies q_i
+}
+
+// -------------------------------------------------------------------------------------- tiles
+// Shared-memory tiles for spread and gather.  The atoms arrive in the neighbour list's cell-major
+// order (cells z-fastest), so a GROUP of g0 x g1 x g2 cells is g0*g1 contiguous atom runs that sit
+// in one compact region of the grid.  A block takes one group: its tile is the grid window
+//   [o_d, o_d + T_d),  o_d = floor(c0_d K_d / nc_d) - M - (P-1),  T_d = floor(g_d K_d / nc_d) + 2 + 2M + (P-1)
+// i.e. every point an atom of the group can touch while it has drifted less than M grid spacings
+// since the list was built.  Spread accumulates into the tile (shared-memory atomics) and flushes
+// it once with coalesced reductions; gather loads the tile once with coalesced loads and
+// interpolates out of shared memory.  An atom whose footprint is not inside the window (it drifted
+// further) takes the global-memory path inside the same kernel, so the result never depends on
+// the drift bound.  Tile strides are padded on the host so that the 32 (x,y) rows a warp touches
+// at once fall into distinct banks.  Atoms are processed in chunks of TILE_CHUNK: three threads
+// per atom evaluate its spline weights into a shared record (all lanes busy), then the rows follow.
+struct TileGeom {
+    int K[3];
+    int nc[3];     // neighbour-list cells per axis
+    int g[3];      // cells per group
+    int ng[3];     // groups per axis
+    int T[3];      // tile extent in grid points
+    int ZS, XS;    // shared-memory strides: element (tx,ty,tz) at tx*XS + ty*ZS + tz
+    int M;         // drift margin in grid points
+};
+#define TILE_MAXRANGES 16
+#define TILE_CHUNK 64
+// per-atom record (floats): theta_z[8] | dtheta_z[8] | theta_x[P] | theta_y[P] | dtheta_x[P] | dtheta_y[P]
+#define REC_Z 0
+#define REC_DZ 8
+#define REC_X 16
+#define REC_LEN(P) (16 + 4 * (P))
+
+struct TileBlock {
+    int o[3];          // tile origin (grid index of element 0; may be negative)
+    int natoms;        // atoms of this group
+};
+
+// a in (-K, 2K) -> [0, K)
+__device__ __forceinline__ int wrap1(int a, int K) { a += a < 0 ? K : 0; a -= a >= K ? K : 0; return a; }
+
+// ranges of sorted-atom indices of the block's group; rpre = exclusive prefix of their lengths
+__device__ __forceinline__ TileBlock tile_block_setup(const TileGeom& tg, const int* __restrict__ cell_start,
+                                                       int P, int* rbeg, int* rpre)
+{
+    TileBlock tb;
+    int b = blockIdx.x;
+    const int bz = b % tg.ng[2]; b /= tg.ng[2];
+    const int by = b % tg.ng[1];
+    const int bx = b / tg.ng[1];
+    const int c0[3] = {bx * tg.g[0], by * tg.g[1], bz * tg.g[2]};
+    int gc[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        gc[d] = min(tg.g[d], tg.nc[d] - c0[d]);
+        tb.o[d] = (int)(((long long)c0[d] * tg.K[d]) / tg.nc[d]) - tg.M - (P - 1);
+    }
+    const int nr = gc[0] * gc[1];
+    if (threadIdx.x < nr) {
+        const int cx = c0[0] + threadIdx.x / gc[1], cy = c0[1] + threadIdx.x % gc[1];
+        const int col = (cx * tg.nc[1] + cy) * tg.nc[2] + c0[2];
+        const int beg = cell_start[col];
+        rbeg[threadIdx.x] = beg;
+        rpre[threadIdx.x + 1] = cell_start[col + gc[2]] - beg;     // length, scanned below
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        rpre[0] = 0;
+        for (int r = 0; r < nr; ++r) { acc += rpre[r + 1]; rpre[r + 1] = acc; }
+        for (int r = nr; r < TILE_MAXRANGES; ++r) rpre[r + 1] = acc;
+    }
+    __syncthreads();
+    tb.natoms = rpre[TILE_MAXRANGES];
+    return tb;
+}
+
+__device__ __forceinline__ int tile_atom(int i, const int* rbeg, const int* rpre)
+{
+    int r = 0;
+#pragma unroll
+    for (int k = 1; k < TILE_MAXRANGES; ++k) r += (i >= rpre[k]);
+    return rbeg[r] + (i - rpre[r]);
+}
+
+// Chunk setup by threads 0 .. 3*TILE_CHUNK-1 (thread = atom*3 + axis): spline weights into the atom's
+// record, and by the axis-0 thread the atom's sorted index, raw base index + charge bits, and the
+// linear tile offset of its base point (-1: footprint not inside the window).
+template <int P, bool DERIV>
+__device__ __forceinline__ void tile_chunk_setup(int ch, int na, const TileBlock& tb, const TileGeom& tg,
+                                                 const float4* __restrict__ frac, const int4* __restrict__ base,
+                                                 const int* rbeg, const int* rpre, float* rec, int4* sb,
+                                                 int* stoff, int* sidx)
+{
+    if (threadIdx.x >= 3 * TILE_CHUNK) return;
+    const int at = threadIdx.x / 3, ax = threadIdx.x % 3;
+    if (at >= na) return;
+    const int s = tile_atom(ch + at, rbeg, rpre);
+    const float4 fw = frac[s];
+    float th[P], dth[P];
+    bspline_weights<P>(ax == 0 ? fw.x : (ax == 1 ? fw.y : fw.z), th, dth);
+    float* r = rec + at * REC_LEN(P);
+    const int o_t = ax == 2 ? REC_Z : REC_X + ax * P;
+    const int o_d = ax == 2 ? REC_DZ : REC_X + (2 + ax) * P;
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        r[o_t + j] = th[j];
+        if (DERIV) r[o_d + j] = dth[j];
+    }
+    if (ax == 0) {
+        int4 f = base[s];
+        const int tx = wrap1(f.x - tb.o[0], tg.K[0]), ty = wrap1(f.y - tb.o[1], tg.K[1]),
+                  tz = wrap1(f.z - tb.o[2], tg.K[2]);
+        const bool in = tx >= P - 1 && tx < tg.T[0] && ty >= P - 1 && ty < tg.T[1] && tz >= P - 1 && tz < tg.T[2];
+        stoff[at] = in ? tx * tg.XS + ty * tg.ZS + tz : -1;
+        sidx[at] = s;
+        f.w = __float_as_int(fw.w);
+        sb[at] = f;
+    }
+}
+
+template <int P>
+__global__ void __launch_bounds__(256)
+k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
+              const int* __restrict__ cell_start, TileGeom tg, float* __restrict__ grid)
+{
+    extern __shared__ __align__(16) float tile[];
+    __shared__ __align__(16) float rec[TILE_CHUNK * REC_LEN(P)];
+    __shared__ int4 sb[TILE_CHUNK];
+    __shared__ int stoff[TILE_CHUNK], sidx[TILE_CHUNK];
+    __shared__ int rbeg[TILE_MAXRANGES], rpre[TILE_MAXRANGES + 1];
+    const TileBlock tb = tile_block_setup(tg, cell_start, P, rbeg, rpre);
+    if (tb.natoms == 0) return;
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
+    const int tsize = tg.XS * tg.T[0];
+    for (int e = threadIdx.x; e < tsize; e += blockDim.x) tile[e] = 0.f;
+
+    for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK) {
+        const int na = min(TILE_CHUNK, tb.natoms - ch);
+        __syncthreads();
+        tile_chunk_setup<P, false>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
+        __syncthreads();
+        const int rows = na * P * P;
+        for (int R = threadIdx.x; R < rows; R += blockDim.x) {
+            const int at = R / (P * P), row = R % (P * P);
+            const int a = row / P, b = row % P;
+            const float* r = rec + at * REC_LEN(P);
+            const float w2 = __int_as_float(sb[at].w) * r[REC_X + a] * r[REC_X + P + b];
+            if (w2 == 0.f) continue;
+            float wz[8];
+            *(float4*)wz = *(const float4*)(r + REC_Z);
+            *(float4*)(wz + 4) = *(const float4*)(r + REC_Z + 4);
+            const int t = stoff[at];
+            if (t >= 0) {
+                float* rowp = tile + (t - a * tg.XS - b * tg.ZS);
+#pragma unroll
+                for (int c = 0; c < P; ++c) atomicAdd(rowp - c, w2 * wz[c]);   // CAS loop: no native fp32 shared atomic
+            } else {
+                const int4 f = sb[at];
+                int gx = f.x - a; gx += gx < 0 ? K0 : 0;
+                int gy = f.y - b; gy += gy < 0 ? K1 : 0;
+                float* rowp = grid + ((size_t)gx * K1 + gy) * K2;
+#pragma unroll
+                for (int c = 0; c < P; ++c) {
+                    int gz = f.z - c; gz += gz < 0 ? K2 : 0;
+                    atomicAdd(rowp + gz, w2 * wz[c]);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // flush: one warp per (tx,ty) row, lanes along z (coalesced reductions); untouched points skipped
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    int tx = wid / tg.T[1], ty = wid % tg.T[1];
+    while (tx < tg.T[0]) {
+        const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1);
+        const float* trow = tile + tx * tg.XS + ty * tg.ZS;
+        float* grow = grid + ((size_t)gx * K1 + gy) * K2;
+        for (int tz = lane; tz < tg.T[2]; tz += 32) {
+            const float v = trow[tz];
+            if (v != 0.f) atomicAdd(grow + wrap1(tb.o[2] + tz, K2), v);
+        }
+        ty += nw;
+        while (ty >= tg.T[1]) { ty -= tg.T[1]; ++tx; }
+    }
+}
+
+// gather of one atom by one warp out of the tile (IN_TILE) or out of global memory: full passes of
+// 32 (x,y) rows, then the P*P % 32 leftover rows point by point.  r = the atom's weight record.
+template <int P, bool FORCE, bool IN_TILE>
+__device__ __forceinline__ void gather_atom(const float* __restrict__ src, int toff, const int4 f,
+                                            const float* __restrict__ r, const TileGeom& tg, int lane,
+                                            float& ph, float& gx_, float& gy_, float& gz_)
+{
+    constexpr int FULL = (P * P) / 32 * 32, REST = (P * P - FULL) * P;
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
+    float wz[8], dz[8];
+    if (FULL > 0) {
+        *(float4*)wz = *(const float4*)(r + REC_Z);
+        *(float4*)(wz + 4) = *(const float4*)(r + REC_Z + 4);
+        if (FORCE) {
+            *(float4*)dz = *(const float4*)(r + REC_DZ);
+            *(float4*)(dz + 4) = *(const float4*)(r + REC_DZ + 4);
+        }
+    }
+#pragma unroll
+    for (int row0 = 0; row0 < FULL; row0 += 32) {
+        const int row = row0 + lane, a = row / P, b = row % P;
+        float s0 = 0.f, s1 = 0.f;
+        if (IN_TILE) {
+            const float* rowp = src + (toff - a * tg.XS - b * tg.ZS);
+#pragma unroll
+            for (int c = 0; c < P; ++c) {
+                const float v = rowp[-c];
+                s0 = fmaf(wz[c], v, s0);
+                if (FORCE) s1 = fmaf(dz[c], v, s1);
+            }
+        } else {
+            int gx = f.x - a; gx += gx < 0 ? K0 : 0;
+            int gy = f.y - b; gy += gy < 0 ? K1 : 0;
+            const float* rowp = src + ((size_t)gx * K1 + gy) * K2;
+#pragma unroll
+            for (int c = 0; c < P; ++c) {
+                int gz = f.z - c; gz += gz < 0 ? K2 : 0;
+                const float v = __ldg(rowp + gz);
+                s0 = fmaf(wz[c], v, s0);
+                if (FORCE) s1 = fmaf(dz[c], v, s1);
+            }
+        }
+        const float tx = r[REC_X + a], ty = r[REC_X + P + b];
+        ph = fmaf(tx * ty, s0, ph);
+        if (FORCE) {
+            gx_ = fmaf(r[REC_X + 2 * P + a] * ty, s0, gx_);
+            gy_ = fmaf(tx * r[REC_X + 3 * P + b], s0, gy_);
+            gz_ = fmaf(tx * ty, s1, gz_);
+        }
+    }
+#pragma unroll
+    for (int p0 = 0; p0 < REST; p0 += 32) {
+        const int pt = p0 + lane;
+        if (pt < REST) {
+            const int row = FULL + pt / P, c = pt % P, a = row / P, b = row % P;
+            float v;
+            if (IN_TILE) {
+                v = src[toff - a * tg.XS - b * tg.ZS - c];
+            } else {
+                int gx = f.x - a; gx += gx < 0 ? K0 : 0;
+                int gy = f.y - b; gy += gy < 0 ? K1 : 0;
+                int gz = f.z - c; gz += gz < 0 ? K2 : 0;
+                v = __ldg(src + ((size_t)gx * K1 + gy) * K2 + gz);
+            }
+            const float tx = r[REC_X + a], ty = r[REC_X + P + b], tz = r[REC_Z + c];
+            const float vz = tz * v;
+            ph = fmaf(tx * ty, vz, ph);
+            if (FORCE) {
+                gx_ = fmaf(r[REC_X + 2 * P + a] * ty, vz, gx_);
+                gy_ = fmaf(tx * r[REC_X + 3 * P + b], vz, gy_);
+                gz_ = fmaf(tx * ty, r[REC_DZ + c] * v, gz_);
+            }
+        }
+    }
+}
+
+template <int P, bool FORCE>
+__global__ void __launch_bounds__(256)
+k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
+              const int* __restrict__ cell_start, TileGeom tg, const float* __restrict__ grid,
+              float sx, float sy, float sz, float4* __restrict__ out)
+{
+    extern __shared__ __align__(16) float tile[];
+    __shared__ __align__(16) float rec[TILE_CHUNK * REC_LEN(P)];
+    __shared__ int4 sb[TILE_CHUNK];
+    __shared__ int stoff[TILE_CHUNK], sidx[TILE_CHUNK];
+    __shared__ int rbeg[TILE_MAXRANGES], rpre[TILE_MAXRANGES + 1];
+    const TileBlock tb = tile_block_setup(tg, cell_start, P, rbeg, rpre);
+    if (tb.natoms == 0) return;
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    {   // load the window: one warp per (tx,ty) row, lanes along z
+        int tx = wid / tg.T[1], ty = wid % tg.T[1];
+        while (tx < tg.T[0]) {
+            const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1);
+            float* trow = tile + tx * tg.XS + ty * tg.ZS;
+            const float* grow = grid + ((size_t)gx * K1 + gy) * K2;
+            for (int tz = lane; tz < tg.T[2]; tz += 32) trow[tz] = __ldg(grow + wrap1(tb.o[2] + tz, K2));
+            ty += nw;
+            while (ty >= tg.T[1]) { ty -= tg.T[1]; ++tx; }
+        }
+    }
+    for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK) {
+        const int na = min(TILE_CHUNK, tb.natoms - ch);
+        __syncthreads();
+        tile_chunk_setup<P, FORCE>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
+        __syncthreads();
+        for (int at = wid; at < na; at += nw) {
+            const float* r = rec + at * REC_LEN(P);
+            const int toff = stoff[at];
+            float ph = 0.f, gx_ = 0.f, gy_ = 0.f, gz_ = 0.f;
+            if (toff >= 0) gather_atom<P, FORCE, true>(tile, toff, sb[at], r, tg, lane, ph, gx_, gy_, gz_);
+            else gather_atom<P, FORCE, false>(grid, 0, sb[at], r, tg, lane, ph, gx_, gy_, gz_);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                ph += __shfl_xor_sync(0xffffffffu, ph, o);
+                if (FORCE) {
+                    gx_ += __shfl_xor_sync(0xffffffffu, gx_, o);
+                    gy_ += __shfl_xor_sync(0xffffffffu, gy_, o);
+                    gz_ += __shfl_xor_sync(0xffffffffu, gz_, o);
+                }
+            }
+            if (lane == 0) out[sidx[at]] = make_float4(-sx * gx_, -sy * gy_, -sz * gz_, ph);
+        }
+    }
 }
 
 // -------------------------------------------------------------------------------------- host side
@@ -227,10 +599,67 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
     return SQEQ_OK;
 }
 
-template <int P>
-static int pme_run_t(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_force, bool want_energy,
-                     cudaStream_t st)
+// Chooses the cell group and tile shape for the shared-memory spread/gather kernels; false when the
+// geometry does not suit them (window wider than the grid, no list) and the global kernels run.
+static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeom& best, size_t& best_bytes)
 {
+    if (!nl || !nl->cell_start || ctx->pme_tiles_off) return false;
+    const int M = 1;
+    const size_t limit = 44 * 1024;      // + 12 KB of records: four blocks per SM
+    double best_cost = 1e300;
+    bool found = false;
+    const int64_t want_groups = 3 * (int64_t)ctx->sm_count;
+    for (int pass = 0; pass < 2 && !found; ++pass)       // pass 1 drops the "enough blocks" wish
+        for (int gxy = 1; gxy <= 4; ++gxy)
+            for (int gz = 1; gz <= 12; ++gz) {
+                TileGeom tg;
+                const int g[3] = {gxy, gxy, gz};
+                bool ok = true;
+                int64_t groups = 1;
+                for (int d = 0; d < 3; ++d) {
+                    tg.K[d] = ctx->K[d];
+                    tg.nc[d] = nl->ncell[d];
+                    tg.g[d] = g[d] < tg.nc[d] ? g[d] : tg.nc[d];
+                    tg.ng[d] = (tg.nc[d] + tg.g[d] - 1) / tg.g[d];
+                    tg.T[d] = (int)(((int64_t)tg.g[d] * tg.K[d]) / tg.nc[d]) + 2 + 2 * M + (P - 1);
+                    if (tg.T[d] > tg.K[d] || tg.T[d] > 1023) ok = false;
+                    groups *= tg.ng[d];
+                }
+                if (!ok || tg.g[0] * tg.g[1] > TILE_MAXRANGES) continue;
+                if (pass == 0 && groups < want_groups) continue;
+                tg.M = M;
+                // strides: smallest padding that puts the 32 rows (a,b) of a full pass in distinct banks
+                const int nrow = (P * P >= 32) ? 32 : 0;
+                int bz = -1, bx = -1;
+                for (int zs = tg.T[2]; zs < tg.T[2] + 32 && bz < 0; ++zs)
+                    for (int xs = tg.T[1] * zs; xs < tg.T[1] * zs + 32; ++xs) {
+                        unsigned seen = 0;
+                        bool distinct = true;
+                        for (int r = 0; r < nrow; ++r) {
+                            const int bank = (((-(r / P) * xs - (r % P) * zs) % 32) + 32) % 32;
+                            if (seen & (1u << bank)) { distinct = false; break; }
+                            seen |= 1u << bank;
+                        }
+                        if (distinct) { bz = zs; bx = xs; break; }
+                    }
+                if (bz < 0) { bz = tg.T[2]; bx = tg.T[1] * tg.T[2]; }
+                tg.ZS = bz; tg.XS = bx;
+                const size_t bytes = sizeof(float) * (size_t)tg.XS * tg.T[0];
+                if (bytes > limit) continue;
+                const double cost = (double)tg.T[0] * tg.T[1] * tg.T[2] / ((double)tg.g[0] * tg.g[1] * tg.g[2]);
+                if (cost < best_cost) { best_cost = cost; best = tg; best_bytes = bytes; found = true; }
+            }
+    return found;
+}
+
+template <int P>
+static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,
+                     bool want_energy, cudaStream_t st)
+{
+    TileGeom tg;
+    size_t tile_bytes = 0;
+    const bool tiles = plan_tiles(ctx, nl, P, tg, tile_bytes);
+    const int ngroups = tiles ? tg.ng[0] * tg.ng[1] * tg.ng[2] : 0;
     const int K0 = ctx->K[0], K1 = ctx->K[1], K2 = ctx->K[2], K2h = K2 / 2 + 1;
     const size_t G3 = (size_t)K0 * K1 * K2;
     float* grid = (float*)ctx->grid.p;
@@ -242,7 +671,12 @@ static int pme_run_t(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_fo
     {
         StageTimer tm(ctx, SQEQ_T_SPREAD, st);
         CUDA_TRY(ctx, cudaMemsetAsync(grid, 0, sizeof(float) * G3, st));
-        k_spread<P><<<nbw, 256, 0, st>>>(n, frac, base, K0, K1, K2, grid);
+        if (tiles) {
+            CUDA_TRY(ctx, cudaFuncSetAttribute(k_spread_tile<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+            k_spread_tile<P><<<ngroups, 256, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid);
+        } else {
+            k_spread<P><<<ceil_div(n, SPREAD_APB), 256, 0, st>>>(n, frac, base, K0, K1, K2, grid);
+        }
         KERNEL_CHECK(ctx);
     }
     if (ctx->gridQ.p) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->gridQ.p, grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, st));
@@ -272,23 +706,32 @@ static int pme_run_t(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_fo
     {
         StageTimer tm(ctx, SQEQ_T_GATHER, st);
         const float sx = (float)(K0 / box[0]), sy = (float)(K1 / box[1]), sz = (float)(K2 / box[2]);
-        if (want_force)
-            k_gather<P, true><<<nbw, 256, 0, st>>>(n, frac, base, K0, K1, K2, grid, sx, sy, sz, (float4*)ctx->rec_out.p);
+        float4* rec = (float4*)ctx->rec_out.p;
+        if (tiles) {
+            if (want_force) {
+                CUDA_TRY(ctx, cudaFuncSetAttribute(k_gather_tile<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+                k_gather_tile<P, true><<<ngroups, 256, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
+            } else {
+                CUDA_TRY(ctx, cudaFuncSetAttribute(k_gather_tile<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+                k_gather_tile<P, false><<<ngroups, 256, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
+            }
+        } else if (want_force)
+            k_gather<P, true><<<nbw, 256, 0, st>>>(n, frac, base, K0, K1, K2, grid, sx, sy, sz, rec);
         else
-            k_gather<P, false><<<nbw, 256, 0, st>>>(n, frac, base, K0, K1, K2, grid, sx, sy, sz, (float4*)ctx->rec_out.p);
+            k_gather<P, false><<<nbw, 256, 0, st>>>(n, frac, base, K0, K1, K2, grid, sx, sy, sz, rec);
         KERNEL_CHECK(ctx);
     }
     (void)want_energy;
     return SQEQ_OK;
 }
 
-int pme_run(sqeq_ctx* ctx, int64_t n, const double box[3], bool want_force, bool want_energy,
-            cudaStream_t st)
+int pme_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,
+            bool want_energy, cudaStream_t st)
 {
     switch (ctx->order) {
-        case 4: return pme_run_t<4>(ctx, n, box, want_force, want_energy, st);
-        case 6: return pme_run_t<6>(ctx, n, box, want_force, want_energy, st);
-        case 8: return pme_run_t<8>(ctx, n, box, want_force, want_energy, st);
+        case 4: return pme_run_t<4>(ctx, nl, n, box, want_force, want_energy, st);
+        case 6: return pme_run_t<6>(ctx, nl, n, box, want_force, want_energy, st);
+        case 8: return pme_run_t<8>(ctx, nl, n, box, want_force, want_energy, st);
     }
     return sqeq_fail(ctx, SQEQ_EINVAL, "pme_run: unsupported order %d", ctx->order);
 }

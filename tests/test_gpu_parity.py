@@ -267,3 +267,33 @@ def test_shadow_md_steps_against_oracle(ctx):
         assert abs(en[0] - st["U"]) < 2e-5 * abs(st["U"]) and abs(en[1] - ekin) < 1e-4 * ekin
         assert abs(en[2] - np.linalg.norm(st["res"])) < 1e-3 * en[2]
     nl.free()
+
+
+def test_pme_tile_window_fallbacks(ctx, monkeypatch):
+    """The shared-memory spread/gather tiles assume an atom stays within one grid spacing of the cell
+    it was binned into; beyond that the atom takes the global-memory path inside the same kernels,
+    and SQEQ_PME_TILES=0 selects the global kernels outright.  All three must match the oracle:
+    (a) a rigid translation by 2.7 grid spacings after the list build (every atom leaves its window;
+    the pair list stays valid because relative positions do not change), (b) the global kernels."""
+    from paper_2503_21176_b200 import binding
+    c = W.CONFIGS[2]
+    pos, q = inputs(2)
+    h = c.L / c.grid
+    nl = ctx.nl_build(dev(pos), c.box, c.r_list)
+    moved = (pos.astype(np.float64) + np.array([2.7 * h, -1.6 * h, 0.4 * h])).astype(np.float32)
+    rows = np.sort(np.random.default_rng(3).choice(len(q), 256, replace=False))
+    op, oF, _, _ = oracle.coulomb_pme(moved, q, c.box, c.rc, c.alpha, c.grid, c.order, rows=rows)
+    phi, F, E = ctx.coulomb(nl, dev(moved), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+    # positions were re-rounded to fp32 after the shift, so pair distances differ at the 1e-7 level
+    assert relrms(phi.cpu().numpy()[rows], op) < TOL and relrms(F.cpu().numpy()[rows], oF) < TOL
+    nl.free()
+    monkeypatch.setenv("SQEQ_PME_TILES", "0")
+    c2 = binding.Context(0)
+    try:
+        nl2 = c2.nl_build(dev(pos), c.box, c.r_list)
+        op, oF, _, _ = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order, rows=rows)
+        phi, F, E = c2.coulomb(nl2, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+        assert relrms(phi.cpu().numpy()[rows], op) < TOL and relrms(F.cpu().numpy()[rows], oF) < TOL
+        nl2.free()
+    finally:
+        c2.close()
