@@ -4,6 +4,7 @@
 //   f-j, unnormalised transforms (no 1/K^3), G(m) = B(m) exp(-pi^2 mt^2/alpha^2)/(pi V mt^2), G(0)=0.
 // cuFFT does the two 3-D transforms (north_star allows it; timed as separate stages).
 #include <math.h>
+#include <stdlib.h>
 
 #include <vector>
 
@@ -234,7 +235,7 @@ k_gather(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ ba
 // interpolates out of shared memory.  An atom whose footprint is not inside the window (it drifted
 // further) takes the global-memory path inside the same kernel, so the result never depends on
 // the drift bound.  Tile strides are padded on the host so that the 32 (x,y) rows a warp touches
-// at once fall into distinct banks.  Atoms are processed in chunks of TILE_CHUNK: three threads
+// at once fall into distinct banks.  Atoms are processed in chunks of NT/4: three threads
 // per atom evaluate its spline weights into a shared record (all lanes busy), then the rows follow.
 struct TileGeom {
     int K[3];
@@ -244,9 +245,10 @@ struct TileGeom {
     int T[3];      // tile extent in grid points
     int ZS, XS;    // shared-memory strides: element (tx,ty,tz) at tx*XS + ty*ZS + tz
     int M;         // drift margin in grid points
+    unsigned T1_magic;   // ceil(2^32 / T[1]): r / T[1] = umulhi(r, T1_magic) for r < 2^16
 };
 #define TILE_MAXRANGES 16
-#define TILE_CHUNK 64
+#define TILE_CHUNK(NT) ((NT) / 4)
 // per-atom record (floats): theta_z[8] | dtheta_z[8] | theta_x[P] | theta_y[P] | dtheta_x[P] | dtheta_y[P]
 #define REC_Z 0
 #define REC_DZ 8
@@ -277,6 +279,7 @@ __device__ __forceinline__ TileBlock tile_block_setup(const TileGeom& tg, const 
         gc[d] = min(tg.g[d], tg.nc[d] - c0[d]);
         tb.o[d] = (int)(((long long)c0[d] * tg.K[d]) / tg.nc[d]) - tg.M - (P - 1);
     }
+    tb.o[2] &= ~3;      // z origin on a float4 boundary (K2 % 4 == 0): the window moves as 16-byte vectors
     const int nr = gc[0] * gc[1];
     if (threadIdx.x < nr) {
         const int cx = c0[0] + threadIdx.x / gc[1], cy = c0[1] + threadIdx.x % gc[1];
@@ -305,16 +308,16 @@ __device__ __forceinline__ int tile_atom(int i, const int* rbeg, const int* rpre
     return rbeg[r] + (i - rpre[r]);
 }
 
-// Chunk setup by threads 0 .. 3*TILE_CHUNK-1 (thread = atom*3 + axis): spline weights into the atom's
+// Chunk setup by threads 0 .. 3*TILE_CHUNK(NT)-1 (thread = atom*3 + axis): spline weights into the atom's
 // record, and by the axis-0 thread the atom's sorted index, raw base index + charge bits, and the
 // linear tile offset of its base point (-1: footprint not inside the window).
-template <int P, bool DERIV>
+template <int P, int NT, bool DERIV>
 __device__ __forceinline__ void tile_chunk_setup(int ch, int na, const TileBlock& tb, const TileGeom& tg,
                                                  const float4* __restrict__ frac, const int4* __restrict__ base,
                                                  const int* rbeg, const int* rpre, float* rec, int4* sb,
                                                  int* stoff, int* sidx)
 {
-    if (threadIdx.x >= 3 * TILE_CHUNK) return;
+    if (threadIdx.x >= 3 * TILE_CHUNK(NT)) return;
     const int at = threadIdx.x / 3, ax = threadIdx.x % 3;
     if (at >= na) return;
     const int s = tile_atom(ch + at, rbeg, rpre);
@@ -341,15 +344,49 @@ __device__ __forceinline__ void tile_chunk_setup(int ch, int na, const TileBlock
     }
 }
 
-template <int P>
-__global__ void __launch_bounds__(256)
+// Moves the window between the grid and the tile as float4 vectors: 8 lanes cover 32 z-points of a
+// row, so a warp handles 4 (tx,ty) rows per step.  The z origin and K2 are multiples of 4, so a vector
+// never straddles the periodic boundary; the tile side stays scalar (its row stride is odd).
+// FLUSH: tile -> grid with red.global.add.v4.f32, all-zero vectors skipped; else grid -> tile.
+__device__ __forceinline__ void red_add_v4(float* addr, float4 v)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+template <bool FLUSH>
+__device__ __forceinline__ void tile_move(float* tile, float* grid, const TileBlock& tb, const TileGeom& tg)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
+    const int nrows = tg.T[0] * tg.T[1];
+    const int sub = lane >> 3, z4 = (lane & 7) * 4;
+    for (int r = wid * 4 + sub; r < nrows; r += nw * 4) {
+        const int tx = (int)__umulhi((unsigned)r, tg.T1_magic), ty = r - tx * tg.T[1];
+        const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1);
+        float* trow = tile + tx * tg.XS + ty * tg.ZS;
+        float* grow = grid + ((size_t)gx * K1 + gy) * K2;
+        for (int tz = z4; tz < tg.T[2]; tz += 32) {
+            float* g = grow + wrap1(tb.o[2] + tz, K2);
+            if (FLUSH) {
+                const float4 v = make_float4(trow[tz], trow[tz + 1], trow[tz + 2], trow[tz + 3]);
+                if (v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f) red_add_v4(g, v);
+            } else {
+                const float4 v = __ldg((const float4*)g);
+                trow[tz] = v.x; trow[tz + 1] = v.y; trow[tz + 2] = v.z; trow[tz + 3] = v.w;
+            }
+        }
+    }
+}
+
+template <int P, int NT>
+__global__ void __launch_bounds__(NT)
 k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
               const int* __restrict__ cell_start, TileGeom tg, float* __restrict__ grid)
 {
     extern __shared__ __align__(16) float tile[];
-    __shared__ __align__(16) float rec[TILE_CHUNK * REC_LEN(P)];
-    __shared__ int4 sb[TILE_CHUNK];
-    __shared__ int stoff[TILE_CHUNK], sidx[TILE_CHUNK];
+    __shared__ __align__(16) float rec[TILE_CHUNK(NT) * REC_LEN(P)];
+    __shared__ int4 sb[TILE_CHUNK(NT)];
+    __shared__ int stoff[TILE_CHUNK(NT)], sidx[TILE_CHUNK(NT)];
     __shared__ int rbeg[TILE_MAXRANGES], rpre[TILE_MAXRANGES + 1];
     const TileBlock tb = tile_block_setup(tg, cell_start, P, rbeg, rpre);
     if (tb.natoms == 0) return;
@@ -357,10 +394,10 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
     const int tsize = tg.XS * tg.T[0];
     for (int e = threadIdx.x; e < tsize; e += blockDim.x) tile[e] = 0.f;
 
-    for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK) {
-        const int na = min(TILE_CHUNK, tb.natoms - ch);
+    for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK(NT)) {
+        const int na = min(TILE_CHUNK(NT), tb.natoms - ch);
         __syncthreads();
-        tile_chunk_setup<P, false>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
+        tile_chunk_setup<P, NT, false>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
         __syncthreads();
         const int rows = na * P * P;
         for (int R = threadIdx.x; R < rows; R += blockDim.x) {
@@ -391,20 +428,7 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
         }
     }
     __syncthreads();
-    // flush: one warp per (tx,ty) row, lanes along z (coalesced reductions); untouched points skipped
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    int tx = wid / tg.T[1], ty = wid % tg.T[1];
-    while (tx < tg.T[0]) {
-        const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1);
-        const float* trow = tile + tx * tg.XS + ty * tg.ZS;
-        float* grow = grid + ((size_t)gx * K1 + gy) * K2;
-        for (int tz = lane; tz < tg.T[2]; tz += 32) {
-            const float v = trow[tz];
-            if (v != 0.f) atomicAdd(grow + wrap1(tb.o[2] + tz, K2), v);
-        }
-        ty += nw;
-        while (ty >= tg.T[1]) { ty -= tg.T[1]; ++tx; }
-    }
+    tile_move<true>(tile, grid, tb, tg);
 }
 
 // gather of one atom by one warp out of the tile (IN_TILE) or out of global memory: full passes of
@@ -483,36 +507,25 @@ __device__ __forceinline__ void gather_atom(const float* __restrict__ src, int t
     }
 }
 
-template <int P, bool FORCE>
-__global__ void __launch_bounds__(256)
+template <int P, bool FORCE, int NT>
+__global__ void __launch_bounds__(NT)
 k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
               const int* __restrict__ cell_start, TileGeom tg, const float* __restrict__ grid,
               float sx, float sy, float sz, float4* __restrict__ out)
 {
     extern __shared__ __align__(16) float tile[];
-    __shared__ __align__(16) float rec[TILE_CHUNK * REC_LEN(P)];
-    __shared__ int4 sb[TILE_CHUNK];
-    __shared__ int stoff[TILE_CHUNK], sidx[TILE_CHUNK];
+    __shared__ __align__(16) float rec[TILE_CHUNK(NT) * REC_LEN(P)];
+    __shared__ int4 sb[TILE_CHUNK(NT)];
+    __shared__ int stoff[TILE_CHUNK(NT)], sidx[TILE_CHUNK(NT)];
     __shared__ int rbeg[TILE_MAXRANGES], rpre[TILE_MAXRANGES + 1];
     const TileBlock tb = tile_block_setup(tg, cell_start, P, rbeg, rpre);
     if (tb.natoms == 0) return;
-    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    {   // load the window: one warp per (tx,ty) row, lanes along z
-        int tx = wid / tg.T[1], ty = wid % tg.T[1];
-        while (tx < tg.T[0]) {
-            const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1);
-            float* trow = tile + tx * tg.XS + ty * tg.ZS;
-            const float* grow = grid + ((size_t)gx * K1 + gy) * K2;
-            for (int tz = lane; tz < tg.T[2]; tz += 32) trow[tz] = __ldg(grow + wrap1(tb.o[2] + tz, K2));
-            ty += nw;
-            while (ty >= tg.T[1]) { ty -= tg.T[1]; ++tx; }
-        }
-    }
-    for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK) {
-        const int na = min(TILE_CHUNK, tb.natoms - ch);
+    tile_move<false>(tile, const_cast<float*>(grid), tb, tg);
+    for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK(NT)) {
+        const int na = min(TILE_CHUNK(NT), tb.natoms - ch);
         __syncthreads();
-        tile_chunk_setup<P, FORCE>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
+        tile_chunk_setup<P, NT, FORCE>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
         __syncthreads();
         for (int at = wid; at < na; at += nw) {
             const float* r = rec + at * REC_LEN(P);
@@ -601,54 +614,66 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
 
 // Chooses the cell group and tile shape for the shared-memory spread/gather kernels; false when the
 // geometry does not suit them (window wider than the grid, no list) and the global kernels run.
-static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeom& best, size_t& best_bytes)
+static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeom& best, size_t& best_bytes,
+                       int& best_nt)
 {
     if (!nl || !nl->cell_start || ctx->pme_tiles_off) return false;
+    if (ctx->K[2] % 4 != 0) return false;                 // float4 window rows
     const int M = 1;
-    const size_t limit = 44 * 1024;      // + 12 KB of records: four blocks per SM
     double best_cost = 1e300;
     bool found = false;
-    const int64_t want_groups = 3 * (int64_t)ctx->sm_count;
+    const int64_t want_groups = 2 * (int64_t)ctx->sm_count;
     for (int pass = 0; pass < 2 && !found; ++pass)       // pass 1 drops the "enough blocks" wish
-        for (int gxy = 1; gxy <= 4; ++gxy)
-            for (int gz = 1; gz <= 12; ++gz) {
-                TileGeom tg;
-                const int g[3] = {gxy, gxy, gz};
-                bool ok = true;
-                int64_t groups = 1;
-                for (int d = 0; d < 3; ++d) {
-                    tg.K[d] = ctx->K[d];
-                    tg.nc[d] = nl->ncell[d];
-                    tg.g[d] = g[d] < tg.nc[d] ? g[d] : tg.nc[d];
-                    tg.ng[d] = (tg.nc[d] + tg.g[d] - 1) / tg.g[d];
-                    tg.T[d] = (int)(((int64_t)tg.g[d] * tg.K[d]) / tg.nc[d]) + 2 + 2 * M + (P - 1);
-                    if (tg.T[d] > tg.K[d] || tg.T[d] > 1023) ok = false;
-                    groups *= tg.ng[d];
-                }
-                if (!ok || tg.g[0] * tg.g[1] > TILE_MAXRANGES) continue;
-                if (pass == 0 && groups < want_groups) continue;
-                tg.M = M;
-                // strides: smallest padding that puts the 32 rows (a,b) of a full pass in distinct banks
-                const int nrow = (P * P >= 32) ? 32 : 0;
-                int bz = -1, bx = -1;
-                for (int zs = tg.T[2]; zs < tg.T[2] + 32 && bz < 0; ++zs)
-                    for (int xs = tg.T[1] * zs; xs < tg.T[1] * zs + 32; ++xs) {
-                        unsigned seen = 0;
-                        bool distinct = true;
-                        for (int r = 0; r < nrow; ++r) {
-                            const int bank = (((-(r / P) * xs - (r % P) * zs) % 32) + 32) % 32;
-                            if (seen & (1u << bank)) { distinct = false; break; }
-                            seen |= 1u << bank;
-                        }
-                        if (distinct) { bz = zs; bx = xs; break; }
+        for (int nt = 256; nt <= 512; nt *= 2) {
+            // 227 KB per SM: four 256-thread blocks or two 512-thread blocks, records included
+            const size_t limit = (nt == 256 ? 56 * 1024 : 112 * 1024) - (size_t)(nt / 4) * (REC_LEN(P) * 4 + 24) - 256;
+            for (int gxy = 1; gxy <= 4; ++gxy)
+                for (int gz = 1; gz <= 12; ++gz) {
+                    TileGeom tg;
+                    const int g[3] = {gxy, gxy, gz};
+                    bool ok = true;
+                    int64_t groups = 1;
+                    for (int d = 0; d < 3; ++d) {
+                        tg.K[d] = ctx->K[d];
+                        tg.nc[d] = nl->ncell[d];
+                        tg.g[d] = g[d] < tg.nc[d] ? g[d] : tg.nc[d];
+                        tg.ng[d] = (tg.nc[d] + tg.g[d] - 1) / tg.g[d];
+                        tg.T[d] = (int)(((int64_t)tg.g[d] * tg.K[d]) / tg.nc[d]) + 2 + 2 * M + (P - 1);
+                        if (d == 2) tg.T[d] = (tg.T[d] + 3 + 3) & ~3;     // origin rounded down to 4, extent up
+                        if (tg.T[d] > tg.K[d] || tg.T[d] > 1023) ok = false;
+                        groups *= tg.ng[d];
                     }
-                if (bz < 0) { bz = tg.T[2]; bx = tg.T[1] * tg.T[2]; }
-                tg.ZS = bz; tg.XS = bx;
-                const size_t bytes = sizeof(float) * (size_t)tg.XS * tg.T[0];
-                if (bytes > limit) continue;
-                const double cost = (double)tg.T[0] * tg.T[1] * tg.T[2] / ((double)tg.g[0] * tg.g[1] * tg.g[2]);
-                if (cost < best_cost) { best_cost = cost; best = tg; best_bytes = bytes; found = true; }
-            }
+                    if (!ok || tg.g[0] * tg.g[1] > TILE_MAXRANGES) continue;
+                    if (tg.T[0] * tg.T[1] >= 65536) continue;
+                    if (pass == 0 && groups < want_groups) continue;
+                    tg.M = M;
+                    tg.T1_magic = (unsigned)((0x100000000ull + tg.T[1] - 1) / tg.T[1]);
+                    // strides: smallest padding that puts the 32 rows (a,b) of a full pass in distinct banks
+                    const int nrow = (P * P >= 32) ? 32 : 0;
+                    int bz = -1, bx = -1;
+                    for (int zs = tg.T[2]; zs < tg.T[2] + 32 && bz < 0; ++zs)
+                        for (int xs = tg.T[1] * zs; xs < tg.T[1] * zs + 32; ++xs) {
+                            unsigned seen = 0;
+                            bool distinct = true;
+                            for (int r = 0; r < nrow; ++r) {
+                                const int bank = (((-(r / P) * xs - (r % P) * zs) % 32) + 32) % 32;
+                                if (seen & (1u << bank)) { distinct = false; break; }
+                                seen |= 1u << bank;
+                            }
+                            if (distinct) { bz = zs; bx = xs; break; }
+                        }
+                    if (bz < 0) { bz = tg.T[2]; bx = tg.T[1] * tg.T[2]; }
+                    tg.ZS = bz; tg.XS = bx;
+                    const size_t bytes = sizeof(float) * (size_t)tg.XS * tg.T[0];
+                    if (bytes > limit) continue;
+                    // window points moved per cell, plus a charge for idle SMs when blocks are few
+                    double cost = (double)tg.T[0] * tg.T[1] * tg.T[2] / ((double)tg.g[0] * tg.g[1] * tg.g[2]);
+                    const double slots = (double)ctx->sm_count * (nt == 256 ? 4 : 2);
+                    const double waves = (double)groups / slots;
+                    cost *= ceil(waves) / waves;
+                    if (cost < best_cost) { best_cost = cost; best = tg; best_bytes = bytes; best_nt = nt; found = true; }
+                }
+        }
     return found;
 }
 
@@ -658,8 +683,13 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
 {
     TileGeom tg;
     size_t tile_bytes = 0;
-    const bool tiles = plan_tiles(ctx, nl, P, tg, tile_bytes);
+    int nt = 256;
+    const bool tiles = plan_tiles(ctx, nl, P, tg, tile_bytes, nt);
     const int ngroups = tiles ? tg.ng[0] * tg.ng[1] * tg.ng[2] : 0;
+    static const bool debug = getenv("SQEQ_DEBUG") != nullptr;
+    if (debug)
+        fprintf(stderr, "[sqeq] pme tiles=%d nt=%d g=(%d,%d,%d) groups=%d T=(%d,%d,%d) ZS=%d XS=%d bytes=%zu\n", (int)tiles,
+                nt, tg.g[0], tg.g[1], tg.g[2], ngroups, tg.T[0], tg.T[1], tg.T[2], tg.ZS, tg.XS, tile_bytes);
     const int K0 = ctx->K[0], K1 = ctx->K[1], K2 = ctx->K[2], K2h = K2 / 2 + 1;
     const size_t G3 = (size_t)K0 * K1 * K2;
     float* grid = (float*)ctx->grid.p;
@@ -672,8 +702,9 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         StageTimer tm(ctx, SQEQ_T_SPREAD, st);
         CUDA_TRY(ctx, cudaMemsetAsync(grid, 0, sizeof(float) * G3, st));
         if (tiles) {
-            CUDA_TRY(ctx, cudaFuncSetAttribute(k_spread_tile<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
-            k_spread_tile<P><<<ngroups, 256, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid);
+            auto kern = nt == 256 ? k_spread_tile<P, 256> : k_spread_tile<P, 512>;
+            CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+            kern<<<ngroups, nt, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid);
         } else {
             k_spread<P><<<ceil_div(n, SPREAD_APB), 256, 0, st>>>(n, frac, base, K0, K1, K2, grid);
         }
@@ -708,13 +739,10 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         const float sx = (float)(K0 / box[0]), sy = (float)(K1 / box[1]), sz = (float)(K2 / box[2]);
         float4* rec = (float4*)ctx->rec_out.p;
         if (tiles) {
-            if (want_force) {
-                CUDA_TRY(ctx, cudaFuncSetAttribute(k_gather_tile<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
-                k_gather_tile<P, true><<<ngroups, 256, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
-            } else {
-                CUDA_TRY(ctx, cudaFuncSetAttribute(k_gather_tile<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
-                k_gather_tile<P, false><<<ngroups, 256, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
-            }
+            auto kern = want_force ? (nt == 256 ? k_gather_tile<P, true, 256> : k_gather_tile<P, true, 512>)
+                                   : (nt == 256 ? k_gather_tile<P, false, 256> : k_gather_tile<P, false, 512>);
+            CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+            kern<<<ngroups, nt, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
         } else if (want_force)
             k_gather<P, true><<<nbw, 256, 0, st>>>(n, frac, base, K0, K1, K2, grid, sx, sy, sz, rec);
         else
