@@ -94,6 +94,16 @@ int  sqeq_coulomb  (sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float*
                     const float* q, const double box[3], double rc, double alpha,
                     const int grid[3], int order, float* phi, float* force, double* energy);
 
+/* The same evaluation without any synchronisation: everything, including the fp64 reduction of
+ * E = 1/2 sum q_i phi_i when want_energy != 0, is enqueued on the context's stream and the call
+ * returns.  The energy stays in a context-owned device scalar until sqeq_energy_fetch copies the
+ * value of the LAST enqueued evaluation to the host (that call synchronises the stream).  For
+ * callers that step many evaluations back to back (MD, Krylov loops) and read energies rarely. */
+int  sqeq_coulomb_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                          const float* q, const double box[3], double rc, double alpha,
+                          const int grid[3], int order, float* phi, float* force, int want_energy);
+int  sqeq_energy_fetch(sqeq_ctx* ctx, double* energy);
+
 /* The same evaluation with HOST buffers (pos, q, phi, force are host fp32 arrays, ideally pinned):
  * host->device copies of pos and q, the evaluation, and device->host copies of phi / force all
  * happen inside the call on the context's stream; always synchronises.  This is the end-to-end

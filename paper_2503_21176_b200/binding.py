@@ -59,6 +59,8 @@ def load():
     L.sqeq_nl_info.argtypes = [vp, ip, ctypes.POINTER(i64), ip]
     L.sqeq_nl_free.argtypes = [vp]
     L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
+    L.sqeq_coulomb_enqueue.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
+    L.sqeq_energy_fetch.argtypes = [vp, dp]
     L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_parts.argtypes = [vp, vp, i64, vp, vp, vp, vp, dp]
     L.sqeq_pme_grid.argtypes = [vp, cint, vp]
@@ -198,6 +200,20 @@ class Context:
                                         _ptr(force, torch.float32, 3 * n) if want_force else None,
                                         ctypes.byref(e) if want_energy else None))
         return phi, (force if want_force else None), (e.value if want_energy else None)
+
+    def coulomb_enqueue(self, nl, pos, q, box, rc, alpha, grid, order, phi, force, want_energy=True):
+        """sqeq_coulomb_enqueue: no synchronisation; read the energy later with energy_fetch()."""
+        n = pos.shape[0]
+        self._check(load().sqeq_coulomb_enqueue(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                                _ptr(q, torch.float32, n), _box(box), float(rc), float(alpha),
+                                                _grid(grid), int(order), _ptr(phi, torch.float32, n),
+                                                _ptr(force, torch.float32, 3 * n) if force is not None else None,
+                                                int(want_energy)))
+
+    def energy_fetch(self):
+        e = ctypes.c_double()
+        self._check(load().sqeq_energy_fetch(self.handle, ctypes.byref(e)))
+        return e.value
 
     def coulomb_host(self, nl, pos, q, box, rc, alpha, grid, order, phi, force, want_energy=True):
         """Same evaluation with HOST buffers (pinned CPU tensors): H2D and D2H copies inside the call."""

@@ -93,6 +93,7 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_scal, 16 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_nl, 256);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->scal.p, 16 * sizeof(double));
     if (e == cudaSuccess) {
         cudaMemPoolProps props = {};
@@ -138,6 +139,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
     for (auto& b : ctx->vec_f3) if (b.p) cudaFree(b.p);
     for (auto& b : ctx->stage) if (b.p) cudaFree(b.p);
     if (ctx->h_scal) cudaFreeHost(ctx->h_scal);
+    if (ctx->h_nl) cudaFreeHost(ctx->h_nl);
     for (auto& r : ctx->pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto& e : ctx->free_events) cudaEventDestroy(e);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -317,9 +319,9 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
     return SQEQ_OK;
 }
 
-extern "C" int sqeq_coulomb(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const float* q,
-                 const double box[3], double rc, double alpha, const int grid[3], int order,
-                 float* phi, float* force, double* energy)
+extern "C" int sqeq_coulomb_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                                    const float* q, const double box[3], double rc, double alpha,
+                                    const int grid[3], int order, float* phi, float* force, int want_energy)
 {
     if (!ctx) return SQEQ_EINVAL;
     SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_coulomb"));
@@ -327,13 +329,29 @@ extern "C" int sqeq_coulomb(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, cons
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
     SQEQ_TRY(prep_atoms(ctx, nl, pos, q, ctx->K, ctx->stream));
-    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, phi, force, energy != nullptr));
-    if (energy) {
-        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal.p, 2 * sizeof(double),
-                                      cudaMemcpyDeviceToHost, ctx->stream));
-        CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
-        *energy = ctx->h_scal[0];
-    }
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, phi, force, want_energy != 0));
+    ctx->energy_pending = want_energy != 0;
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_energy_fetch(sqeq_ctx* ctx, double* energy)
+{
+    if (!ctx || !energy) return SQEQ_EINVAL;
+    if (!ctx->energy_pending)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_energy_fetch: the last evaluation did not reduce an energy");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal.p, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    *energy = ctx->h_scal[0];
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_coulomb(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const float* q,
+                 const double box[3], double rc, double alpha, const int grid[3], int order,
+                 float* phi, float* force, double* energy)
+{
+    SQEQ_TRY(sqeq_coulomb_enqueue(ctx, nl, n, pos, q, box, rc, alpha, grid, order, phi, force, energy != nullptr));
+    if (energy) SQEQ_TRY(sqeq_energy_fetch(ctx, energy));
     return SQEQ_OK;
 }
 

@@ -56,7 +56,9 @@ struct sqeq_ctx {
     DevBuf rec_out;   // float4 [n]  F_rec  xyz, phi_rec    (sorted order)
     DevBuf scal;      // double [16] device scalars (energy sums, dots)
     double* h_scal = nullptr;  // pinned host mirror
+    void* h_nl = nullptr;      // pinned scratch of the neighbour build (256 B)
     bool last_had_force = false;
+    bool energy_pending = false;   // scal[0] holds the energy of the last enqueued evaluation
     int64_t last_n = 0;
 
     // ---- Krylov / MD workspaces ----

@@ -123,7 +123,7 @@ __global__ void k_reorder(int64_t n, const float* __restrict__ pos, const int* _
         xw[d] = (float)x;
     }
     xq[s] = make_float4(xw[0], xw[1], xw[2], 0.f);
-    cell_of[s] = (c[0] * g.nc[1] + c[1]) * g.nc[2] + c[2];
+    cell_of[s] = c[0] | (c[1] << 10) | (c[2] << 20);      // packed cell coordinates (nc <= 1024 per axis)
     wrapc[s] = make_char4((signed char)w[0], (signed char)w[1], (signed char)w[2], 0);
 }
 
@@ -195,23 +195,35 @@ static int exclusive_scan(sqeq_ctx* ctx, int64_t n1, const Tin* in, int64_t* out
 // ------------------------------------------------------------------------------------------ pairs
 // The exact predicate (DESIGN.md R-NL): d = pos[b]-pos[a] for caller indices a<b, s = -rint(d/L),
 // d += s*L, r2 = (dx*dx + dy*dy) + dz*dz, every operation individually rounded; in range <=> r2 < rl2.
+// Out of line and fed through a pointer so that the hot loop keeps no fp64 state in registers.
+struct NLExact {
+    double L[3];
+    double rl2;
+};
+
 __device__ __noinline__ bool exact_in_range(const float* __restrict__ pos, int oi, int oj,
-                                            double L0, double L1, double L2, double rl2)
+                                            const NLExact* __restrict__ ex)
 {
     int a = oi < oj ? oi : oj, b = oi < oj ? oj : oi;
-    const double L[3] = {L0, L1, L2};
     double d[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
+        const double L = ex->L[k];
         double dk = __dsub_rn((double)pos[3 * (int64_t)b + k], (double)pos[3 * (int64_t)a + k]);
-        double sk = -rint(__ddiv_rn(dk, L[k]));
-        d[k] = __dadd_rn(dk, __dmul_rn(sk, L[k]));
+        double sk = -rint(__ddiv_rn(dk, L));
+        d[k] = __dadd_rn(dk, __dmul_rn(sk, L));
     }
     double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
-    return r2 < rl2;
+    return r2 < ex->rl2;
 }
 
-__device__ __forceinline__ int floordiv(int a, int b) { int q = a / b; return (a % b != 0 && (a < 0)) ? q - 1 : q; }
+// unwrapped cell index u in [-nc, 2nc) -> wrapped index and image shift; false if |shift| would be > 1
+__device__ __forceinline__ bool wrap_cell(int& u, int nc, int& sh)
+{
+    sh = 0;
+    if (u < 0) { u += nc; sh = -1; } else if (u >= nc) { u -= nc; sh = 1; }
+    return u >= 0 && u < nc;
+}
 
 // Single-pass pair enumeration.  One warp per atom i (cell-major index s):
 //  1. lanes build the warp's SEGMENT list in shared memory: one lane per (x,y) column of the
@@ -220,8 +232,9 @@ __device__ __forceinline__ int floordiv(int a, int b) { int q = a / b; return (a
 //     z-fastest in memory -- what is left is at most 3 contiguous runs of atoms (one per periodic
 //     image along z), each a segment (begin, end, image code);
 //  2. the warp sweeps the segments 32 candidates at a time (coalesced float4 loads), decides in
-//     fp32 outside the guard band and by the exact fp64 predicate inside it, and compacts the
-//     hits with ballot/popc into a per-warp staging row in shared memory;
+//     fp32 outside the guard band and by the exact fp64 predicate inside it (a warp-uniform, rarely
+//     taken branch), and compacts the hits with ballot/popc into a per-warp staging row in shared
+//     memory;
 //  3. one atomicAdd on a global cursor reserves the row's slice of `nbr`, the staged row is copied
 //     out with coalesced stores, and (row_start, row_len) are recorded.
 // If the cursor passes `capacity` or a row outgrows the staging row the kernel keeps counting and
@@ -231,11 +244,12 @@ struct NLCounters {
     unsigned long long cursor;
     int max_row;
     int flag;
+    NLExact ex;
 };
 
 template <int WARPS>
-__global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 4 : 1)
-k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_of,
+__global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 3 : 1)
+k_pairs(int n, const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
         const float* __restrict__ pos, NLGeom g, int cap_row, unsigned long long capacity,
         NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
@@ -252,14 +266,13 @@ k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_o
     }
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int64_t s64 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
-    if (s64 >= n) return;
-    const int s = (int)s64;
+    const int s = blockIdx.x * WARPS + wid;
+    if (s >= n) return;
     int4* segs = segs_all + wid * NL_MAXSEG;
     uint32_t* stage = stage_all + (size_t)wid * cap_row;
     const float4 xi = xq[s];
-    const int c = cell_of[s];
-    const int cz = c % g.nc[2], cy = (c / g.nc[2]) % g.nc[1], cx = c / (g.nc[2] * g.nc[1]);
+    const int c = cell_of[s];                                  // packed cx | cy << 10 | cz << 20
+    const int cx = c & 1023, cy = (c >> 10) & 1023, cz = c >> 20;
 
     // ---- 1. segments
     const int ny_st = 2 * g.w[1] + 1;
@@ -268,13 +281,13 @@ k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_o
     int4 loc0 = make_int4(0, 0, 0, 0), loc1 = loc0, loc2 = loc0;
     if (lane < ncol) {
         const int ox = lane / ny_st - g.w[0], oy = lane % ny_st - g.w[1];
-        const int ux = cx + ox, uy = cy + oy;
-        const int shx = floordiv(ux, g.nc[0]), shy = floordiv(uy, g.nc[1]);
-        bool valid = shx >= -1 && shx <= 1 && shy >= -1 && shy <= 1;
+        int ux = cx + ox, uy = cy + oy, shx, shy;
         float dxm = fmaxf(fmaxf((float)ux * g.a[0] - xi.x, xi.x - (float)(ux + 1) * g.a[0]) - g.marg, 0.f);
         float dym = fmaxf(fmaxf((float)uy * g.a[1] - xi.y, xi.y - (float)(uy + 1) * g.a[1]) - g.marg, 0.f);
         if (ox == 0) dxm = 0.f;
         if (oy == 0) dym = 0.f;
+        bool valid = wrap_cell(ux, g.nc[0], shx);
+        valid = wrap_cell(uy, g.nc[1], shy) && valid;
         const float rem = (g.rl2f + g.band) - (dxm * dxm + dym * dym);
         valid = valid && rem > 0.f;
         if (valid) {
@@ -282,13 +295,15 @@ k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_o
             int zlo = (int)floorf((xi.z - zr) * g.inva[2]), zhi = (int)floorf((xi.z + zr) * g.inva[2]);
             zlo = max(zlo, cz - g.w[2]); zlo = min(zlo, cz);
             zhi = min(zhi, cz + g.w[2]); zhi = max(zhi, cz);
-            const int colbase = ((ux - shx * g.nc[0]) * g.nc[1] + (uy - shy * g.nc[1])) * g.nc[2];
+            const int colbase = (ux * g.nc[1] + uy) * g.nc[2];
+            const int ncz = g.nc[2];
             int zc = zlo;
             while (zc <= zhi && nloc < 3) {
-                const int shz = floordiv(zc, g.nc[2]);
-                const int zlast = min(zhi, (shz + 1) * g.nc[2] - 1);
+                // image of this stretch of z cells: zc in [shz*ncz, (shz+1)*ncz)
+                const int shz = zc < 0 ? (zc < -ncz ? -2 : -1) : (zc >= ncz ? (zc >= 2 * ncz ? 2 : 1) : 0);
+                const int zlast = min(zhi, (shz + 1) * ncz - 1);
                 if (shz >= -1 && shz <= 1) {
-                    const int zf = zc - shz * g.nc[2];
+                    const int zf = zc - shz * ncz;
                     const int beg = cell_start[colbase + zf], end = cell_start[colbase + zf + (zlast - zc) + 1];
                     if (end > beg) {
                         const int4 v = make_int4(beg, end, (shx + 1) * 9 + (shy + 1) * 3 + (shz + 1), 0);
@@ -315,8 +330,11 @@ k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_o
     }
     __syncwarp();
 
-    // ---- 2. sweep
+    // ---- 2. sweep.  The loop keeps every candidate whose fp32 r2 is below rl2 + band; a lane that saw
+    // one inside the guard band only raises a flag (xq carries 32 padding entries, so the tail of a
+    // segment is loaded unclamped and masked).
     int count = 0;
+    bool band_seen = false;
     const unsigned lt = (1u << lane) - 1u;
     const float hi_thr = g.rl2f + g.band, lo_thr = g.rl2f - g.band;
     for (int sg = 0; sg < nseg; ++sg) {
@@ -326,23 +344,44 @@ k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_o
         const int self = seg.z == 13 ? s : -1;
         const uint32_t codebits = (uint32_t)seg.z << 27;
 #pragma unroll 2
-        for (int t0 = seg.x; t0 < seg.y; t0 += 32) {
-            const int t = t0 + lane;
-            bool ok = false;
-            if (t < seg.y) {
-                const float4 xj = __ldg(xq + t);
-                const float dx = xj.x - x0, dy = xj.y - y0, dz = xj.z - z0;
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                ok = r2 < hi_thr && t != self;
-                if (ok && r2 >= lo_thr) ok = exact_in_range(pos, perm[s], perm[t], g.L[0], g.L[1], g.L[2], g.rl2);
-            }
+        for (int t = seg.x + lane; t - lane < seg.y; t += 32) {
+            const float4 xj = __ldg(xq + t);
+            const float dx = xj.x - x0, dy = xj.y - y0, dz = xj.z - z0;
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const bool ok = r2 < hi_thr && t < seg.y && t != self;
+            band_seen |= ok && r2 >= lo_thr;
             const unsigned m = __ballot_sync(0xffffffffu, ok);
-            if (ok) {
-                const int at = count + __popc(m & lt);
-                if (at < cap_row) stage[at] = (uint32_t)t | codebits;
-            }
+            const int at = count + __popc(m & lt);
+            if (ok && at < cap_row) stage[at] = (uint32_t)t | codebits;
             count += __popc(m);
         }
+    }
+    __syncwarp();
+    // guard band (rare): re-decide the staged candidates inside it with the exact fp64 predicate on the
+    // raw caller positions, and compact the staging row in place
+    if (__any_sync(0xffffffffu, band_seen) && count <= cap_row) {
+        const int oi = perm[s];
+        int kept = 0;
+        for (int k0 = 0; k0 < count; k0 += 32) {
+            const int k = k0 + lane;
+            bool ok = k < count;
+            uint32_t e = 0;
+            if (ok) {
+                e = stage[k];
+                const int t = (int)(e & 0x07ffffffu);
+                const float4 xj = __ldg(xq + t);
+                const float4 sh = shtab[e >> 27];
+                const float dx = xj.x - (xi.x - sh.x), dy = xj.y - (xi.y - sh.y), dz = xj.z - (xi.z - sh.z);
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));     // same expression as in the sweep
+                if (r2 >= lo_thr) ok = exact_in_range(pos, oi, perm[t], &ctr->ex);
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, ok);
+            __syncwarp();
+            if (ok) stage[kept + __popc(m & lt)] = e;            // kept + rank <= k: never ahead of a reader
+            __syncwarp();
+            kept += __popc(m);
+        }
+        count = kept;
     }
     __syncwarp();
 
@@ -355,8 +394,10 @@ k_pairs(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_o
         row_len[s] = count;
     }
     off = __shfl_sync(0xffffffffu, off, 0);
-    if (count <= cap_row && off + (unsigned long long)count <= capacity)
-        for (int k = lane; k < count; k += 32) nbr[off + k] = stage[k];
+    if (count <= cap_row && off + (unsigned long long)count <= capacity) {
+        uint32_t* dst = nbr + off;
+        for (int k = lane; k < count; k += 32) dst[k] = stage[k];
+    }
 }
 
 // ------------------------------------------------------------------------------------------ export
@@ -517,7 +558,7 @@ static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const N
                         (size_t)WARPS * cap_row * sizeof(uint32_t);
     CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_pairs<WARPS><<<ceil_div(nl->n, WARPS), WARPS * 32, smem, st>>>(
-        nl->n, (const float4*)ctx->xq.p, nl->cell_of, nl->cell_start, nl->perm, pos, g, cap_row,
+        (int)nl->n, (const float4*)ctx->xq.p, nl->cell_of, nl->cell_start, nl->perm, pos, g, cap_row,
         (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
@@ -561,8 +602,9 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     NL_TRY(pool_alloc(ctx, (void**)&nl->wrapc, sizeof(char4) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_start, sizeof(int64_t) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_len, sizeof(int) * n));
-    NL_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * n));
+    NL_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * (n + 32)));     // 32 padding entries: see k_pairs
     float4* xq = (float4*)ctx->xq.p;
+    NL_CUDA(cudaMemsetAsync(xq + n, 0x7f, sizeof(float4) * 32, st));    // 3.4e38: far from everything
 
     const int nb = ceil_div(n, 256);
     {
@@ -602,11 +644,16 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
             cap_row = (int)(1.5 * mean_row) + 128;
         }
         cap_row = (cap_row + 31) & ~31;
-        NLCounters* h = (NLCounters*)(ctx->h_scal + 12);
-        int* h_flag = (int*)(ctx->h_scal + 14);
+        NLCounters* h = (NLCounters*)ctx->h_nl;                    // pinned: result, init image, bin flag
+        NLCounters* hinit = h + 1;
+        int* h_flag = (int*)(h + 2);
         for (int attempt = 0;; ++attempt) {
             if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, sizeof(uint32_t) * capacity));
-            NL_CUDA(cudaMemsetAsync(ctr, 0, sizeof(NLCounters), st));
+            NLCounters init = {};
+            for (int d = 0; d < 3; ++d) init.ex.L[d] = g.L[d];
+            init.ex.rl2 = g.rl2;
+            *hinit = init;
+            NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
             // staging rows: 8 warps per block up to 6656 entries per row, 2 warps per block beyond
             if (cap_row <= 6656) NL_TRY(launch_pairs<8>(ctx, nl, pos, g, cap_row, capacity, ctr, st));
             else if (cap_row <= 27648) NL_TRY(launch_pairs<2>(ctx, nl, pos, g, cap_row, capacity, ctr, st));

@@ -109,31 +109,34 @@ k_spread(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ ba
 // a-6, Alg. 2 step 3: Qhat(m) *= G(m); E_rec = 1/2 sum_m G |Qhat|^2 with Hermitian
 // weights on the half spectrum.  G is formed in fp64 from three per-axis tables.
 __global__ void __launch_bounds__(256)
-k_influence(int K0, int K1, int K2h, int K2, const double* __restrict__ tab, double inv_piV,
+k_influence(int K0, int K1, int K2h, int K2, const float* __restrict__ tab, float inv_piV,
             float2* __restrict__ spec, double* __restrict__ e_out)
 {
-    const int64_t total = (int64_t)K0 * K1 * K2h;
-    const double* B0 = tab;               const double* g0 = B0 + K0;  const double* s0 = g0 + K0;
-    const double* B1 = s0 + K0;           const double* g1 = B1 + K1;  const double* s1 = g1 + K1;
-    const double* B2 = s1 + K1;           const double* g2 = B2 + K2;  const double* s2 = g2 + K2;
+    // per-axis fp32 tables (built in fp64 on the host): Bg_d[m] = |b_d(m)|^2 exp(-pi^2 mt_d^2/alpha^2), s_d[m] = mt_d^2
+    const int total_rows = K0 * K1;
+    const float* Bg0 = tab;       const float* s0 = Bg0 + K0;
+    const float* Bg1 = s0 + K0;   const float* s1 = Bg1 + K1;
+    const float* Bg2 = s1 + K1;   const float* s2 = Bg2 + K2;
     double e = 0.0;
-    for (int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; idx < total;
-         idx += (int64_t)gridDim.x * blockDim.x) {
-        const int m2 = (int)(idx % K2h);
-        const int m1 = (int)((idx / K2h) % K1);
-        const int m0 = (int)(idx / ((int64_t)K2h * K1));
-        double G = 0.0;
-        if (m0 | m1 | m2) {
-            const double mt2 = s0[m0] + s1[m1] + s2[m2];
-            G = B0[m0] * B1[m1] * B2[m2] * g0[m0] * g1[m1] * g2[m2] * inv_piV / mt2;
+    // one warp per (m0, m1) row, lanes along m2 (coalesced; no per-element division by K2h)
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = (gridDim.x * blockDim.x) >> 5;
+    for (int row = warp; row < total_rows; row += nwarp) {
+        const int m0 = row / K1, m1 = row - m0 * K1;
+        const float bg01 = Bg0[m0] * Bg1[m1] * inv_piV, s01 = s0[m0] + s1[m1];
+        float2* srow = spec + (size_t)row * K2h;
+        float er = 0.f;
+        for (int m2 = lane; m2 < K2h; m2 += 32) {
+            float G = 0.f;
+            if (row | m2) G = __fdividef(bg01 * Bg2[m2], s01 + s2[m2]);
+            float2 z = srow[m2];
+            const float w = (m2 == 0 || 2 * m2 == K2) ? 0.5f : 1.0f;     // 1/2 * (1 or 2)
+            er = fmaf(w * G, fmaf(z.x, z.x, z.y * z.y), er);
+            z.x *= G;
+            z.y *= G;
+            srow[m2] = z;
         }
-        float2 z = spec[idx];
-        const double w = (m2 == 0 || 2 * m2 == K2) ? 0.5 : 1.0;     // 1/2 * (1 or 2)
-        e += w * G * ((double)z.x * z.x + (double)z.y * z.y);
-        const float Gf = (float)G;
-        z.x *= Gf;
-        z.y *= Gf;
-        spec[idx] = z;
+        e += (double)er;
     }
     if (e_out) {
         __shared__ double red[8];
@@ -582,13 +585,14 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
         SQEQ_TRY(sqeq_reserve(ctx, ctx->grid, sizeof(float) * G3));
         SQEQ_TRY(sqeq_reserve(ctx, ctx->spec, sizeof(float2) * S3));
     }
-    // per-axis tables: |b(m)|^2, exp(-pi^2 mt^2/alpha^2), mt^2   (DESIGN.md R-PME)
+    // per-axis tables (DESIGN.md R-PME), evaluated in fp64 and stored as fp32:
+    //   Bg[m] = |b(m)|^2 exp(-pi^2 mt^2/alpha^2),  s[m] = mt^2
     const int Ksum = grid[0] + grid[1] + grid[2];
-    std::vector<double> tab(3 * (size_t)Ksum);
+    std::vector<float> tab(2 * (size_t)Ksum);
     size_t off = 0;
     for (int d = 0; d < 3; ++d) {
         const int K = grid[d];
-        double* B = tab.data() + off; double* g = B + K; double* s = g + K;
+        float* Bg = tab.data() + off; float* s = Bg + K;
         for (int m = 0; m < K; ++m) {
             double re = 0, im = 0;
             for (int k = 0; k <= order - 2; ++k) {
@@ -597,15 +601,14 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
                 re += M * cos(a);
                 im += M * sin(a);
             }
-            B[m] = 1.0 / (re * re + im * im);
             double mp = (m <= K / 2 ? m : m - K) / box[d];
-            s[m] = mp * mp;
-            g[m] = exp(-M_PI * M_PI * mp * mp / (alpha * alpha));
+            s[m] = (float)(mp * mp);
+            Bg[m] = (float)(exp(-M_PI * M_PI * mp * mp / (alpha * alpha)) / (re * re + im * im));
         }
-        off += 3 * (size_t)K;
+        off += 2 * (size_t)K;
     }
-    SQEQ_TRY(sqeq_reserve(ctx, ctx->tabs, sizeof(double) * tab.size()));
-    CUDA_TRY(ctx, cudaMemcpy(ctx->tabs.p, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->tabs, sizeof(float) * tab.size()));
+    CUDA_TRY(ctx, cudaMemcpy(ctx->tabs.p, tab.data(), sizeof(float) * tab.size(), cudaMemcpyHostToDevice));
     ctx->order = order;
     ctx->tab_alpha = alpha;
     for (int d = 0; d < 3; ++d) ctx->tab_box[d] = box[d];
@@ -721,11 +724,10 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         StageTimer tm(ctx, SQEQ_T_INFLUENCE, st);
         double* e_out = (double*)ctx->scal.p + 1;
         CUDA_TRY(ctx, cudaMemsetAsync(e_out, 0, sizeof(double), st));
-        const double inv_piV = 1.0 / (M_PI * box[0] * box[1] * box[2]);
-        const int64_t total = (int64_t)K0 * K1 * K2h;
-        int nb = ceil_div(total, 256);
+        const float inv_piV = (float)(1.0 / (M_PI * box[0] * box[1] * box[2]));
+        int nb = ceil_div((int64_t)K0 * K1, 8);
         if (nb > ctx->sm_count * 8) nb = ctx->sm_count * 8;
-        k_influence<<<nb, 256, 0, st>>>(K0, K1, K2h, K2, (const double*)ctx->tabs.p, inv_piV, spec, e_out);
+        k_influence<<<nb, 256, 0, st>>>(K0, K1, K2h, K2, (const float*)ctx->tabs.p, inv_piV, spec, e_out);
         KERNEL_CHECK(ctx);
     }
     {

@@ -67,7 +67,7 @@ int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const floa
                cudaStream_t st)
 {
     const int64_t n = nl->n;
-    SQEQ_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * n));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * (n + 32)));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->frac, sizeof(float4) * n));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->base, sizeof(int4) * n));
     PrepGeom g;
@@ -138,12 +138,13 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
     const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     if (s >= n) return;
     const float4 xi = xq[s];
-    const int64_t beg = row_start[s], end = beg + row_len[s];
+    const uint32_t* __restrict__ row = nbr + row_start[s];
+    const int len = row_len[s];
     float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
     // branch-free body: a lane outside rc contributes q_j * 0, so the two unrolled iterations interleave
 #pragma unroll 2
-    for (int64_t k = beg + lane; k < end; k += 32) {
-        const uint32_t e = __ldg(nbr + k);
+    for (int k = lane; k < len; k += 32) {
+        const uint32_t e = __ldg(row + k);
         const float4 xj = __ldg(xq + (e & 0x07ffffffu));
         const float4 s4 = sh[e >> 27];
         // d = r_i - (r_j + shift)

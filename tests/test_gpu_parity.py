@@ -297,3 +297,18 @@ def test_pme_tile_window_fallbacks(ctx, monkeypatch):
         nl2.free()
     finally:
         c2.close()
+
+
+def test_enqueue_and_energy_fetch_match_synchronous_call(ctx):
+    c = W.CONFIGS[0]
+    pos, q = inputs(0)
+    nl = ctx.nl_build(dev(pos), c.box, c.r_list)
+    phi, F, E = ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+    phi2 = torch.empty_like(phi); F2 = torch.empty_like(F)
+    for _ in range(3):      # back to back, no synchronisation in between
+        ctx.coulomb_enqueue(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order, phi2, F2)
+    E2 = ctx.energy_fetch()
+    assert abs(E2 - E) <= 1e-6 * abs(E)
+    assert relrms(phi2.cpu().numpy(), phi.cpu().numpy()) < 1e-6
+    assert relrms(F2.cpu().numpy(), F.cpu().numpy()) < 1e-6
+    nl.free()
