@@ -286,10 +286,11 @@ def run_ours(args, cfg):
     # ---- per-kernel roofline (stage events on the launching streams, over the timed region) -----
     info = state["nl"].info()
     P = info["n_directed"]
+    EB = info["entry_bytes"]       # 2: 16-bit local list (staged real-space kernel), 4: atom index | image
     G3 = grid ** 3
     S3 = grid * grid * (grid // 2 + 1)
     alg_bytes = {  # algorithmic bytes per launch
-        "real": 4 * P + 32 * n,
+        "real": EB * P + 32 * n,
         "spread": 16 * n + 4 * G3,
         "fft_fwd": 4 * G3 + 8 * S3,
         "influence": 16 * S3,
@@ -297,7 +298,7 @@ def run_ours(args, cfg):
         "gather": 32 * n + 4 * G3,
         "prep": 16 * n + 16 * n + 16 * n + 16 * n,
         "assemble": 48 * n + 16 * n,
-        "nl_pairs": 4 * P + 2 * 16 * n,
+        "nl_pairs": EB * P + 2 * 16 * n,
         "nl_bin": 12 * n * 2 + 16 * n + 12 * n,
     }
     kernels = {}
@@ -320,8 +321,16 @@ def run_ours(args, cfg):
                 "unit": "GB/s", "frac": kernels[dom]["hbm_frac"], "traffic": traffic,
                 "peak_source": peak_src,
                 "alg_bytes_per_launch": alg_bytes[dom],
-                "note": "4 B x directed list entries + 32 B x atoms for the real-space kernel; "
-                        "ms_avg from CUDA events on the launching stream over the timed region"}
+                "note": "%d B x directed list entries + 32 B x atoms for the real-space kernel; ms_avg from CUDA "
+                        "events on the launching stream over the timed region; the kernel is instruction-issue "
+                        "bound (DESIGN.md section 7), see roofline_alu" % EB}
+    # ALU view of the same kernel: 43 FP32 flops per list entry (FMA = 2) against
+    # 148 SMs x 128 lanes x 2 x max SM clock
+    flops = 43.0 * P
+    fp32_peak = 148 * 128 * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    roofline_alu = {"kernel": dom, "bound": "alu", "achieved": round(flops / (kernels[dom]["ms_avg"] * 1e-3) / 1e12, 2),
+                    "peak": round(fp32_peak, 1), "unit": "TFLOP/s",
+                    "frac": round(flops / (kernels[dom]["ms_avg"] * 1e-3) / 1e12 / fp32_peak, 4)} if dom == "real" else None
 
     extra = {"kernels": kernels,
              "pair_interactions_per_s": None, "grid_points_per_s": None,
@@ -346,12 +355,12 @@ def run_ours(args, cfg):
                                   f"(+{cfg.skin} A skin), alpha {cfg.alpha}, PME {grid}^3 order {order}; one "
                                   f"potential+force+energy evaluation per step, positions perturbed (sigma 0.02 A) "
                                   f"each step, neighbour rebuild every {REBUILD_EVERY} steps inside the timed region",
-                      "l2": "inputs larger than L2: the %.0f MB neighbour list is streamed every step; no flush" % (4 * P / 1e6),
+                      "l2": "inputs larger than L2: the %.0f MB neighbour list is streamed every step; no flush" % (EB * P / 1e6),
                       "parallelism": "replicas only" if world > 1 else "single GPU"},
            "clocks": clocks, "gpu_launches": launches,
            "e2e": {"value": e2e_val, "unit": "evals/s", "h2d_bytes_per_step": 16 * n,
                    "d2h_bytes_per_step": 16 * n + 8},
-           "roofline": roofline, "extra": extra}
+           "roofline": roofline, "roofline_alu": roofline_alu, "extra": extra}
 
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:

@@ -60,9 +60,11 @@ const char* sqeq_version(void);
  *   box     host double[3]
  *   cutoff  list cutoff; must satisfy 0 < cutoff < min(box)/2 (one image per pair)
  *   out     receives a new list handle (free with sqeq_nl_free)
- * Internally: atoms are wrapped, binned into cells of edge >= cutoff, reordered cell-major; the
- * list is a directed CSR over the reordered atoms with the 27-valued image code packed into each
- * 32-bit entry.  Synchronises the stream (the pair count sizes the list allocation). */
+ * Internally: atoms are wrapped, binned into cells of edge >= cutoff/2, reordered cell-major; the
+ * list is directed rows over the reordered atoms, entries either 16-bit indices into the neighbourhood
+ * of the atom's 2x2x2 cell group or 32-bit (atom index | 27-valued image code).  Synchronises the
+ * stream (the pair count sizes the list allocation).  SQEQ_ECAPACITY if an atom has more than 4352
+ * neighbours. */
 int  sqeq_nl_build (sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3],
                     double cutoff, sqeq_nlist** out);
 /* Number of unique (i<j) pairs in the list.  host int64 out. */
@@ -74,6 +76,10 @@ int  sqeq_nl_count (const sqeq_nlist* nl, int64_t* n_pairs_unique);
 int  sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
 /* List introspection (host outputs, any may be NULL): cells per axis, directed entries, max row. */
 int  sqeq_nl_info  (const sqeq_nlist* nl, int ncell[3], int64_t* n_directed, int* max_row);
+/* Bytes per stored list entry: 2 (16-bit index into the cell group's neighbourhood, the format of the
+ * shared-memory-staged real-space kernel) or 4 (atom index | image code; used when a neighbourhood
+ * does not fit 16 bits / shared memory). */
+int  sqeq_nl_entry_bytes(const sqeq_nlist* nl, int* bytes);
 int  sqeq_nl_free  (sqeq_nlist* nl);
 
 /* ---- Coulomb evaluation: Eq. 2 = Eq. 3 (real space, r < rc) + Alg. 2 (smooth PME,

@@ -57,6 +57,7 @@ def load():
     L.sqeq_nl_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.sqeq_nl_export.argtypes = [vp, vp, vp, vp, vp]
     L.sqeq_nl_info.argtypes = [vp, ip, ctypes.POINTER(i64), ip]
+    L.sqeq_nl_entry_bytes.argtypes = [vp, ip]
     L.sqeq_nl_free.argtypes = [vp]
     L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_enqueue.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
@@ -118,7 +119,9 @@ class NeighbourList:
         nd = ctypes.c_int64()
         mr = ctypes.c_int()
         self.ctx._check(load().sqeq_nl_info(self.handle, nc, ctypes.byref(nd), ctypes.byref(mr)))
-        return dict(ncell=list(nc), n_directed=nd.value, max_row=mr.value)
+        eb = ctypes.c_int()
+        self.ctx._check(load().sqeq_nl_entry_bytes(self.handle, ctypes.byref(eb)))
+        return dict(ncell=list(nc), n_directed=nd.value, max_row=mr.value, entry_bytes=eb.value)
 
     def export(self):
         """Canonical (i, j, shift) arrays on the device: unique pairs i<j sorted by (i,j)."""

@@ -115,6 +115,10 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->scal.cap = 16 * sizeof(double);
     const char* env = getenv("SQEQ_PME_TILES");
     ctx->pme_tiles_off = env && env[0] == '0';
+    env = getenv("SQEQ_OVERLAP");
+    ctx->overlap = env && env[0] == '1';
+    env = getenv("SQEQ_REAL_STAGED");
+    ctx->real_staged_off = env && env[0] == '0';
     *out = ctx;
     return SQEQ_OK;
 }
@@ -259,6 +263,13 @@ int sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, 
     return nl_export_impl(ctx, nl, i, j, shift3);
 }
 
+int sqeq_nl_entry_bytes(const sqeq_nlist* nl, int* bytes)
+{
+    if (!nl || !bytes) return SQEQ_EINVAL;
+    *bytes = nl->fmt == 1 ? 2 : 4;
+    return SQEQ_OK;
+}
+
 int sqeq_nl_free(sqeq_nlist* nl)
 {
     if (!nl) return SQEQ_OK;
@@ -300,9 +311,12 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
                  double alpha, float* phi, float* force, bool want_energy, bool field_mode)
 {
     const bool want_force = force != nullptr;
-    // fork: PME on the side stream, real space on the main stream.  With stage timing on, both run
-    // on the main stream so that every event pair brackets one kernel running alone.
-    if (ctx->profiling) {
+    // One stream by default: every kernel of the evaluation is instruction-issue bound and fills the
+    // machine, so running PME beside the real-space kernel gains nothing and costs co-residency (their
+    // shared-memory footprints do not pack).  SQEQ_OVERLAP=1 forks PME onto the side stream (useful for
+    // small systems that do not fill the GPU); never with stage timing on, where every event pair
+    // brackets one kernel running alone.
+    if (ctx->profiling || !ctx->overlap) {
         SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream));
         SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
     } else {

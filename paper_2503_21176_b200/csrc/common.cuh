@@ -10,9 +10,11 @@
 #include <vector>
 
 #include "../../include/sqeq.h"
+#include "cellgroup.cuh"
 
 #define SQEQ_MAX_ORDER 8
 #define SQEQ_NHIST 7
+#define REAL_STAGE_MAX_BYTES (160 * 1024)   // staged neighbourhood of the real-space kernel
 
 struct DevBuf {
     void*  p = nullptr;
@@ -34,6 +36,9 @@ struct sqeq_ctx {
     cudaMemPool_t pool = nullptr;         // stream-ordered pool for neighbour-list storage (kept across rebuilds)
     int64_t nl_last_n = 0, nl_last_total = 0;   // sizes of the previous build: next build's estimate
     int nl_last_max_row = 0;
+    int nl_last_fmt = 1;
+    bool overlap = false;                 // SQEQ_OVERLAP=1: PME on the side stream beside the real-space kernel
+    bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
 
     // ---- PME state (cached by grid/order/box/alpha) ----
     int K[3] = {0, 0, 0};
@@ -94,7 +99,11 @@ struct sqeq_nlist {
     char4*    wrapc = nullptr;       // [n]   floor(x/L) per axis at build time (sorted order)
     int64_t*  row_start = nullptr;   // [n]   offset of row s in nbr (rows are packed, in no particular order)
     int*      row_len = nullptr;     // [n]   entries of row s
-    uint32_t* nbr = nullptr;         // [>= n_directed]  j (27 bits) | image code (5 bits) << 27
+    void*     nbr = nullptr;         // [>= n_directed] entries: fmt 0: uint32 j (27 bits) | image code << 27;
+                                     //                          fmt 1: uint16 local index in the group's neighbourhood
+    int       fmt = 0;
+    int       max_pop = 0;           // fmt 1: largest neighbourhood population of a group
+    GroupGeom gg;                    // cell groups (cellgroup.cuh)
 };
 
 // ---------------------------------------------------------------------------------------------

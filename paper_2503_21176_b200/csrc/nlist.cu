@@ -15,6 +15,7 @@
 #include <math.h>
 
 #include "common.cuh"
+#include "cellgroup.cuh"
 
 struct NLGeom {
     double L[3];
@@ -217,187 +218,257 @@ __device__ __noinline__ bool exact_in_range(const float* __restrict__ pos, int o
     return r2 < ex->rl2;
 }
 
-// unwrapped cell index u in [-nc, 2nc) -> wrapped index and image shift; false if |shift| would be > 1
-__device__ __forceinline__ bool wrap_cell(int& u, int nc, int& sh)
-{
-    sh = 0;
-    if (u < 0) { u += nc; sh = -1; } else if (u >= nc) { u -= nc; sh = 1; }
-    return u >= 0 && u < nc;
-}
-
-// Single-pass pair enumeration.  One warp per atom i (cell-major index s):
-//  1. lanes build the warp's SEGMENT list in shared memory: one lane per (x,y) column of the
-//     (2w+1)^2 cell stencil; a column is pruned when its rectangle is farther than r_list from
-//     atom i, its z-range is trimmed to the chord of the cutoff sphere, and -- cells being
-//     z-fastest in memory -- what is left is at most 3 contiguous runs of atoms (one per periodic
-//     image along z), each a segment (begin, end, image code);
-//  2. the warp sweeps the segments 32 candidates at a time (coalesced float4 loads), decides in
-//     fp32 outside the guard band and by the exact fp64 predicate inside it (a warp-uniform, rarely
-//     taken branch), and compacts the hits with ballot/popc into a per-warp staging row in shared
-//     memory;
-//  3. one atomicAdd on a global cursor reserves the row's slice of `nbr`, the staged row is copied
-//     out with coalesced stores, and (row_start, row_len) are recorded.
-// If the cursor passes `capacity` or a row outgrows the staging row the kernel keeps counting and
-// the host re-runs it with the now known sizes.
+// Single-pass pair enumeration.  One block per GROUP of 2x2x2 cells (cellgroup.cuh), one warp per atom
+// of the group at a time:
+//  0. the block lays out the group's neighbourhood (columns x periodic images = pieces) in shared memory;
+//  1. lanes build the atom's SEGMENT list: one lane per (x,y) column of its (2w+1)^2 cell stencil; a
+//     column is pruned when its rectangle is farther than r_list from the atom, its z-range is trimmed
+//     to the chord of the cutoff sphere, and what is left of each piece is one contiguous run of atoms:
+//     a segment (begin, end, image code, local-index offset);
+//  2. the warp sweeps the segments 32 candidates at a time (coalesced float4 loads), keeps what the fp32
+//     test cannot exclude, compacts with ballot/popc into a per-warp staging row in shared memory, and
+//     afterwards settles the candidates inside the guard band by the exact fp64 predicate (rare);
+//  3. one atomicAdd on a global cursor reserves the row's slice of `nbr`, the staged row is copied out
+//     with coalesced stores, and (row_start, row_len) are recorded.
+// LOCAL = true emits 16-bit local indices into the group's neighbourhood (for the shared-memory-staged
+// real-space kernel), LOCAL = false 32-bit entries j | image code << 27.
+// If the cursor passes `capacity`, a row outgrows the staging row or a neighbourhood outgrows 16 bits,
+// the kernel keeps counting and the host re-runs it with the now known sizes / the other format.
 #define NL_MAXSEG 96
+#define NL_WARPS 8
 struct NLCounters {
     unsigned long long cursor;
     int max_row;
-    int flag;
+    int max_pop;
     NLExact ex;
 };
 
-template <int WARPS>
-__global__ void __launch_bounds__(WARPS * 32, WARPS == 8 ? 3 : 1)
-k_pairs(int n, const float4* __restrict__ xq, const int* __restrict__ cell_of,
+template <bool LOCAL>
+__global__ void __launch_bounds__(NL_WARPS * 32, 3)
+k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
-        const float* __restrict__ pos, NLGeom g, int cap_row, unsigned long long capacity,
+        const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, unsigned long long capacity,
         NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
-        uint32_t* __restrict__ nbr)
+        void* __restrict__ nbr_out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4* shtab = (float4*)smem_raw;                                  // [32] image shift vectors
-    int4* segs_all = (int4*)(smem_raw + 32 * sizeof(float4));           // [WARPS][NL_MAXSEG]
-    uint32_t* stage_all = (uint32_t*)(segs_all + WARPS * NL_MAXSEG);    // [WARPS][cap_row]
+    float4* shtab = (float4*)smem_raw;                                        // [32] image shift vectors
+    GroupPiece* pieces = (GroupPiece*)(smem_raw + 32 * sizeof(float4));       // [GRP_MAXPIECE]
+    int4* segs_all = (int4*)(pieces + GRP_MAXPIECE);                          // [NL_WARPS][NL_MAXSEG]
+    uint32_t* stage_all = (uint32_t*)(segs_all + NL_WARPS * NL_MAXSEG);       // [NL_WARPS][cap_row] j | code
+    uint16_t* stage16_all = (uint16_t*)(stage_all + (size_t)NL_WARPS * cap_row);   // [NL_WARPS][cap_row] local
+    __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
     if (threadIdx.x < 32) {
         int img = threadIdx.x < 27 ? threadIdx.x : 13;
         shtab[threadIdx.x] = make_float4((img / 9 - 1) * g.Lf[0], ((img / 3) % 3 - 1) * g.Lf[1],
                                          (img % 3 - 1) * g.Lf[2], 0.f);
     }
+    const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
+    // the group's own atoms: ge0*ge1 columns, cells c0z .. c0z+ge2-1 of the zero-image piece
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int r = 0; r < GRP_G * GRP_G; ++r) {
+            s_rpre[r] = acc;
+            const int ix = r / GRP_G, iy = r % GRP_G;
+            if (ix < gi.ge[0] && iy < gi.ge[1]) {
+                const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+                const int beg = cell_start[colw];
+                s_rbeg[r] = beg;
+                acc += cell_start[colw + gi.ge[2]] - beg;
+            } else {
+                s_rbeg[r] = 0;
+            }
+        }
+        s_rpre[GRP_G * GRP_G] = acc;
+        if (LOCAL) atomicMax(&ctr->max_pop, gi.pop);
+    }
     __syncthreads();
+    const int natoms = s_rpre[GRP_G * GRP_G];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int s = blockIdx.x * WARPS + wid;
-    if (s >= n) return;
     int4* segs = segs_all + wid * NL_MAXSEG;
     uint32_t* stage = stage_all + (size_t)wid * cap_row;
-    const float4 xi = xq[s];
-    const int c = cell_of[s];                                  // packed cx | cy << 10 | cz << 20
-    const int cx = c & 1023, cy = (c >> 10) & 1023, cz = c >> 20;
-
-    // ---- 1. segments
-    const int ny_st = 2 * g.w[1] + 1;
-    const int ncol = (2 * g.w[0] + 1) * ny_st;
-    int nloc = 0;
-    int4 loc0 = make_int4(0, 0, 0, 0), loc1 = loc0, loc2 = loc0;
-    if (lane < ncol) {
-        const int ox = lane / ny_st - g.w[0], oy = lane % ny_st - g.w[1];
-        int ux = cx + ox, uy = cy + oy, shx, shy;
-        float dxm = fmaxf(fmaxf((float)ux * g.a[0] - xi.x, xi.x - (float)(ux + 1) * g.a[0]) - g.marg, 0.f);
-        float dym = fmaxf(fmaxf((float)uy * g.a[1] - xi.y, xi.y - (float)(uy + 1) * g.a[1]) - g.marg, 0.f);
-        if (ox == 0) dxm = 0.f;
-        if (oy == 0) dym = 0.f;
-        bool valid = wrap_cell(ux, g.nc[0], shx);
-        valid = wrap_cell(uy, g.nc[1], shy) && valid;
-        const float rem = (g.rl2f + g.band) - (dxm * dxm + dym * dym);
-        valid = valid && rem > 0.f;
-        if (valid) {
-            const float zr = sqrtf(rem) + g.marg;
-            int zlo = (int)floorf((xi.z - zr) * g.inva[2]), zhi = (int)floorf((xi.z + zr) * g.inva[2]);
-            zlo = max(zlo, cz - g.w[2]); zlo = min(zlo, cz);
-            zhi = min(zhi, cz + g.w[2]); zhi = max(zhi, cz);
-            const int colbase = (ux * g.nc[1] + uy) * g.nc[2];
-            const int ncz = g.nc[2];
-            int zc = zlo;
-            while (zc <= zhi && nloc < 3) {
-                // image of this stretch of z cells: zc in [shz*ncz, (shz+1)*ncz)
-                const int shz = zc < 0 ? (zc < -ncz ? -2 : -1) : (zc >= ncz ? (zc >= 2 * ncz ? 2 : 1) : 0);
-                const int zlast = min(zhi, (shz + 1) * ncz - 1);
-                if (shz >= -1 && shz <= 1) {
-                    const int zf = zc - shz * ncz;
-                    const int beg = cell_start[colbase + zf], end = cell_start[colbase + zf + (zlast - zc) + 1];
-                    if (end > beg) {
-                        const int4 v = make_int4(beg, end, (shx + 1) * 9 + (shy + 1) * 3 + (shz + 1), 0);
-                        if (nloc == 0) loc0 = v; else if (nloc == 1) loc1 = v; else loc2 = v;
-                        ++nloc;
-                    }
-                }
-                zc = zlast + 1;
-            }
-        }
-    }
-    int incl = nloc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int y = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += y;
-    }
-    const int nseg = __shfl_sync(0xffffffffu, incl, 31);
-    {
-        const int at = incl - nloc;
-        if (nloc > 0) segs[at] = loc0;
-        if (nloc > 1) segs[at + 1] = loc1;
-        if (nloc > 2) segs[at + 2] = loc2;
-    }
-    __syncwarp();
-
-    // ---- 2. sweep.  The loop keeps every candidate whose fp32 r2 is below rl2 + band; a lane that saw
-    // one inside the guard band only raises a flag (xq carries 32 padding entries, so the tail of a
-    // segment is loaded unclamped and masked).
-    int count = 0;
-    bool band_seen = false;
+    uint16_t* stage16 = stage16_all + (size_t)wid * cap_row;
     const unsigned lt = (1u << lane) - 1u;
     const float hi_thr = g.rl2f + g.band, lo_thr = g.rl2f - g.band;
-    for (int sg = 0; sg < nseg; ++sg) {
-        const int4 seg = segs[sg];
-        const float4 sh = shtab[seg.z];
-        const float x0 = xi.x - sh.x, y0 = xi.y - sh.y, z0 = xi.z - sh.z;   // d = xj + shift - xi
-        const int self = seg.z == 13 ? s : -1;
-        const uint32_t codebits = (uint32_t)seg.z << 27;
-#pragma unroll 2
-        for (int t = seg.x + lane; t - lane < seg.y; t += 32) {
-            const float4 xj = __ldg(xq + t);
-            const float dx = xj.x - x0, dy = xj.y - y0, dz = xj.z - z0;
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            const bool ok = r2 < hi_thr && t < seg.y && t != self;
-            band_seen |= ok && r2 >= lo_thr;
-            const unsigned m = __ballot_sync(0xffffffffu, ok);
-            const int at = count + __popc(m & lt);
-            if (ok && at < cap_row) stage[at] = (uint32_t)t | codebits;
-            count += __popc(m);
-        }
-    }
-    __syncwarp();
-    // guard band (rare): re-decide the staged candidates inside it with the exact fp64 predicate on the
-    // raw caller positions, and compact the staging row in place
-    if (__any_sync(0xffffffffu, band_seen) && count <= cap_row) {
-        const int oi = perm[s];
-        int kept = 0;
-        for (int k0 = 0; k0 < count; k0 += 32) {
-            const int k = k0 + lane;
-            bool ok = k < count;
-            uint32_t e = 0;
-            if (ok) {
-                e = stage[k];
-                const int t = (int)(e & 0x07ffffffu);
-                const float4 xj = __ldg(xq + t);
-                const float4 sh = shtab[e >> 27];
-                const float dx = xj.x - (xi.x - sh.x), dy = xj.y - (xi.y - sh.y), dz = xj.z - (xi.z - sh.z);
-                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));     // same expression as in the sweep
-                if (r2 >= lo_thr) ok = exact_in_range(pos, oi, perm[t], &ctr->ex);
-            }
-            const unsigned m = __ballot_sync(0xffffffffu, ok);
-            __syncwarp();
-            if (ok) stage[kept + __popc(m & lt)] = e;            // kept + rank <= k: never ahead of a reader
-            __syncwarp();
-            kept += __popc(m);
-        }
-        count = kept;
-    }
-    __syncwarp();
+    const int ny_st = 2 * gg.w[1] + 1;
+    const int ncol_atom = (2 * gg.w[0] + 1) * ny_st;
+    const int ncz = gg.nc[2];
 
-    // ---- 3. reserve and copy out
-    unsigned long long off = 0;
-    if (lane == 0) {
-        off = atomicAdd(&ctr->cursor, (unsigned long long)count);
-        atomicMax(&ctr->max_row, count);
-        row_start[s] = (int64_t)off;
-        row_len[s] = count;
+    for (int ia = wid; ia < natoms; ia += NL_WARPS) {
+        int r = 0;
+#pragma unroll
+        for (int k = 1; k < GRP_G * GRP_G; ++k) r += (ia >= s_rpre[k]);
+        const int s = s_rbeg[r] + (ia - s_rpre[r]);
+        const float4 xi = xq[s];
+        const int c = cell_of[s];                                  // packed cx | cy << 10 | cz << 20
+        const int cx = c & 1023, cy = (c >> 10) & 1023, cz = c >> 20;
+
+        // ---- 1. segments
+        int nloc = 0;
+        int4 loc0 = make_int4(0, 0, 0, 0), loc1 = loc0, loc2 = loc0;
+        if (lane < ncol_atom) {
+            const int ox = lane / ny_st - gg.w[0], oy = lane % ny_st - gg.w[1];
+            const int ux = cx + ox, uy = cy + oy;
+            float dxm = fmaxf(fmaxf((float)ux * g.a[0] - xi.x, xi.x - (float)(ux + 1) * g.a[0]) - g.marg, 0.f);
+            float dym = fmaxf(fmaxf((float)uy * g.a[1] - xi.y, xi.y - (float)(uy + 1) * g.a[1]) - g.marg, 0.f);
+            if (ox == 0) dxm = 0.f;
+            if (oy == 0) dym = 0.f;
+            const float rem = hi_thr - (dxm * dxm + dym * dym);
+            if (rem > 0.f) {
+                const float zr = sqrtf(rem) + g.marg;
+                int zlo = (int)floorf((xi.z - zr) * g.inva[2]), zhi = (int)floorf((xi.z + zr) * g.inva[2]);
+                zlo = max(zlo, cz - gg.w[2]); zlo = min(zlo, cz);
+                zhi = min(zhi, cz + gg.w[2]); zhi = max(zhi, cz);
+                const int col = (ux - (gi.c0[0] - gg.w[0])) * gi.ncoly + (uy - (gi.c0[1] - gg.w[1]));
+                int uxw = ux, uyw = uy, shx, shy;
+                const bool valid = grp_wrap(uxw, gg.nc[0], shx) & grp_wrap(uyw, gg.nc[1], shy);
+#pragma unroll
+                for (int p = 0; p < 3; ++p) {
+                    const GroupPiece pc = pieces[col * 3 + p];
+                    const int shz = p - 1;
+                    const int a = max(zlo, shz * ncz), b = min(zhi, (shz + 1) * ncz - 1);
+                    if (valid && pc.len > 0 && a <= b) {
+                        const int colw = (uxw * gg.nc[1] + uyw) * ncz - shz * ncz;
+                        const int beg = cell_start[colw + a], end = cell_start[colw + b + 1];
+                        if (end > beg) {
+                            const int4 v = make_int4(beg, end, pc.code, pc.lbase - pc.gbeg);
+                            if (nloc == 0) loc0 = v; else if (nloc == 1) loc1 = v; else loc2 = v;
+                            ++nloc;
+                        }
+                    }
+                }
+            }
+        }
+        int incl = nloc;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        const int nseg = __shfl_sync(0xffffffffu, incl, 31);
+        __syncwarp();
+        {
+            const int at = incl - nloc;
+            if (nloc > 0) segs[at] = loc0;
+            if (nloc > 1) segs[at + 1] = loc1;
+            if (nloc > 2) segs[at + 2] = loc2;
+        }
+        __syncwarp();
+
+        // ---- 2. sweep.  The loop keeps every candidate whose fp32 r2 is below rl2 + band; a lane that saw
+        // one inside the guard band only raises a flag (xq carries 32 padding entries, so the tail of a
+        // segment is loaded unclamped and masked).
+        int count = 0;
+        bool band_seen = false;
+        for (int sg = 0; sg < nseg; ++sg) {
+            const int4 seg = segs[sg];
+            const float4 sh = shtab[seg.z];
+            const float x0 = xi.x - sh.x, y0 = xi.y - sh.y, z0 = xi.z - sh.z;   // d = xj + shift - xi
+            const int self = seg.z == 13 ? s : -1;
+            const uint32_t codebits = (uint32_t)seg.z << 27;
+#pragma unroll 2
+            for (int t = seg.x + lane; t - lane < seg.y; t += 32) {
+                const float4 xj = __ldg(xq + t);
+                const float dx = xj.x - x0, dy = xj.y - y0, dz = xj.z - z0;
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                const bool ok = r2 < hi_thr && t < seg.y && t != self;
+                band_seen |= ok && r2 >= lo_thr;
+                const unsigned m = __ballot_sync(0xffffffffu, ok);
+                const int at = count + __popc(m & lt);
+                if (ok && at < cap_row) {
+                    stage[at] = (uint32_t)t | codebits;
+                    if (LOCAL) stage16[at] = (uint16_t)(t + seg.w);
+                }
+                count += __popc(m);
+            }
+        }
+        __syncwarp();
+        // guard band (rare): re-decide the staged candidates inside it with the exact fp64 predicate on
+        // the raw caller positions, and compact the staging row in place
+        if (__any_sync(0xffffffffu, band_seen) && count <= cap_row) {
+            const int oi = perm[s];
+            int kept = 0;
+            for (int k0 = 0; k0 < count; k0 += 32) {
+                const int k = k0 + lane;
+                bool ok = k < count;
+                uint32_t e = 0;
+                uint16_t e16 = 0;
+                if (ok) {
+                    e = stage[k];
+                    if (LOCAL) e16 = stage16[k];
+                    const int t = (int)(e & 0x07ffffffu);
+                    const float4 xj = __ldg(xq + t);
+                    const float4 sh = shtab[e >> 27];
+                    const float dx = xj.x - (xi.x - sh.x), dy = xj.y - (xi.y - sh.y), dz = xj.z - (xi.z - sh.z);
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));     // same expression as in the sweep
+                    if (r2 >= lo_thr) ok = exact_in_range(pos, oi, perm[t], &ctr->ex);
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, ok);
+                __syncwarp();
+                if (ok) {                                             // kept + rank <= k: never ahead of a reader
+                    stage[kept + __popc(m & lt)] = e;
+                    if (LOCAL) stage16[kept + __popc(m & lt)] = e16;
+                }
+                __syncwarp();
+                kept += __popc(m);
+            }
+            count = kept;
+        }
+        __syncwarp();
+
+        // ---- 3. reserve and copy out
+        unsigned long long off = 0;
+        if (lane == 0) {
+            off = atomicAdd(&ctr->cursor, (unsigned long long)count);
+            atomicMax(&ctr->max_row, count);
+            row_start[s] = (int64_t)off;
+            row_len[s] = count;
+        }
+        off = __shfl_sync(0xffffffffu, off, 0);
+        if (count <= cap_row && off + (unsigned long long)count <= capacity) {
+            if (LOCAL) {
+                uint16_t* dst = (uint16_t*)nbr_out + off;
+                for (int k = lane; k < count; k += 32) dst[k] = stage16[k];
+            } else {
+                uint32_t* dst = (uint32_t*)nbr_out + off;
+                for (int k = lane; k < count; k += 32) dst[k] = stage[k];
+            }
+        }
+        __syncwarp();
     }
-    off = __shfl_sync(0xffffffffu, off, 0);
-    if (count <= cap_row && off + (unsigned long long)count <= capacity) {
-        uint32_t* dst = nbr + off;
-        for (int k = lane; k < count; k += 32) dst[k] = stage[k];
-    }
+}
+
+// Expands a 16-bit local list to 32-bit entries j | image code << 27 with the same row offsets (used by
+// the canonical export only): one block per group, binary search of each entry in the piece table.
+__global__ void __launch_bounds__(256)
+k_local_to_global(const int* __restrict__ cell_start, GroupGeom gg, const int64_t* __restrict__ row_start,
+                  const int* __restrict__ row_len, const uint16_t* __restrict__ nbr16,
+                  uint32_t* __restrict__ nbr32)
+{
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_scratch;
+    const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
+    const int np = gi.ncol * 3;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int ix = 0; ix < gi.ge[0]; ++ix)
+        for (int iy = 0; iy < gi.ge[1]; ++iy) {
+            const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+            const int beg = cell_start[colw], end = cell_start[colw + gi.ge[2]];
+            for (int s = beg + wid; s < end; s += 8) {
+                const int64_t r0 = row_start[s];
+                const int len = row_len[s];
+                for (int k = lane; k < len; k += 32) {
+                    const int e = nbr16[r0 + k];
+                    int lo = 0, hi = np - 1;                 // last piece with lbase <= e
+                    while (lo < hi) {
+                        const int mid = (lo + hi + 1) >> 1;
+                        if (pieces[mid].lbase <= e) lo = mid; else hi = mid - 1;
+                    }
+                    const GroupPiece pc = pieces[lo];
+                    nbr32[r0 + k] = (uint32_t)(pc.gbeg + (e - pc.lbase)) | ((uint32_t)pc.code << 27);
+                }
+            }
+        }
 }
 
 // ------------------------------------------------------------------------------------------ export
@@ -550,16 +621,35 @@ void nl_release(sqeq_nlist* nl)
     delete nl;
 }
 
-template <int WARPS>
-static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, int cap_row,
-                        size_t capacity, NLCounters* ctr, cudaStream_t st)
+static void fill_group_geom(GroupGeom& gg, const NLGeom& g)
 {
-    const size_t smem = 32 * sizeof(float4) + (size_t)WARPS * NL_MAXSEG * sizeof(int4) +
-                        (size_t)WARPS * cap_row * sizeof(uint32_t);
-    CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_pairs<WARPS><<<ceil_div(nl->n, WARPS), WARPS * 32, smem, st>>>(
-        (int)nl->n, (const float4*)ctx->xq.p, nl->cell_of, nl->cell_start, nl->perm, pos, g, cap_row,
-        (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+    for (int d = 0; d < 3; ++d) {
+        gg.nc[d] = g.nc[d];
+        gg.ng[d] = (g.nc[d] + GRP_G - 1) / GRP_G;
+        gg.w[d] = g.w[d];
+    }
+}
+
+static size_t pairs_smem(int cap_row)
+{
+    return 32 * sizeof(float4) + GRP_MAXPIECE * sizeof(GroupPiece) + (size_t)NL_WARPS * NL_MAXSEG * sizeof(int4) +
+           (size_t)NL_WARPS * cap_row * (sizeof(uint32_t) + sizeof(uint16_t));
+}
+
+static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, bool local,
+                        int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
+{
+    const size_t smem = pairs_smem(cap_row);
+    const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
+    if (local) {
+        CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_pairs<true><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
+            nl->perm, pos, g, nl->gg, cap_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+    } else {
+        CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        k_pairs<false><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
+            nl->perm, pos, g, nl->gg, cap_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+    }
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
 }
@@ -576,6 +666,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     nl->n = n;
     nl->cutoff = cutoff;
     for (int d = 0; d < 3; ++d) { nl->box[d] = box[d]; nl->ncell[d] = g.nc[d]; }
+    fill_group_geom(nl->gg, g);
 
     int *cell_id = nullptr, *cell_count = nullptr, *cell_fill = nullptr, *flag = nullptr;
     int64_t* tmp64 = nullptr;
@@ -647,18 +738,22 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         NLCounters* h = (NLCounters*)ctx->h_nl;                    // pinned: result, init image, bin flag
         NLCounters* hinit = h + 1;
         int* h_flag = (int*)(h + 2);
+        // entry format: 16-bit local indices for the shared-memory-staged real-space kernel unless a
+        // group's neighbourhood is too populous for 16 bits / shared memory (or SQEQ_REAL_STAGED=0)
+        bool local = !ctx->real_staged_off && !(ctx->nl_last_n == n && ctx->nl_last_fmt == 0);
+        const int cap_row_max = 4352;      // 8 staging rows of 6 B entries in 227 KB of shared memory
         for (int attempt = 0;; ++attempt) {
-            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, sizeof(uint32_t) * capacity));
+            if (cap_row > cap_row_max)
+                return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
+                        "sqeq_nl_build: a row has %d neighbours; rows above %d are not supported", cap_row, cap_row_max));
+            const size_t esize = local ? sizeof(uint16_t) : sizeof(uint32_t);
+            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, esize * capacity));
             NLCounters init = {};
             for (int d = 0; d < 3; ++d) init.ex.L[d] = g.L[d];
             init.ex.rl2 = g.rl2;
             *hinit = init;
             NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
-            // staging rows: 8 warps per block up to 6656 entries per row, 2 warps per block beyond
-            if (cap_row <= 6656) NL_TRY(launch_pairs<8>(ctx, nl, pos, g, cap_row, capacity, ctr, st));
-            else if (cap_row <= 27648) NL_TRY(launch_pairs<2>(ctx, nl, pos, g, cap_row, capacity, ctr, st));
-            else return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
-                        "sqeq_nl_build: a row has %d neighbours; rows above 27648 are not supported", cap_row));
+            NL_TRY(launch_pairs(ctx, nl, pos, g, local, cap_row, capacity, ctr, st));
             NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaStreamSynchronize(st));
@@ -666,16 +761,21 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
                 return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
                                          "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
             const bool row_ok = h->max_row <= cap_row, cap_ok = h->cursor <= capacity;
-            if (row_ok && cap_ok) break;
-            if (attempt >= 2)
+            const bool fmt_ok = !local || (h->max_pop <= 65535 && (size_t)h->max_pop * sizeof(float4) <= REAL_STAGE_MAX_BYTES);
+            if (row_ok && cap_ok && fmt_ok) break;
+            if (attempt >= 3)
                 return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY, "sqeq_nl_build: sizing did not converge"));
             if (!row_ok) cap_row = (h->max_row + 31) & ~31;
-            if (!cap_ok) {
+            if (!cap_ok || !fmt_ok) {
                 NL_CUDA(cudaFreeAsync(nl->nbr, st));
                 nl->nbr = nullptr;
-                capacity = (size_t)h->cursor;
+                if (!cap_ok) capacity = (size_t)h->cursor;
+                if (!fmt_ok) local = false;
             }
         }
+        nl->fmt = local ? 1 : 0;
+        nl->max_pop = local ? h->max_pop : 0;
+        ctx->nl_last_fmt = nl->fmt;
         nl->n_directed = (int64_t)h->cursor;
         nl->max_row = h->max_row;
         ctx->nl_last_n = n;
@@ -702,11 +802,21 @@ int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj
     CUDA_TRY(ctx, cudaMalloc((void**)&flag, sizeof(int)));
     CUDA_TRY(ctx, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
     CUDA_TRY(ctx, cudaMemsetAsync(flag, 0, sizeof(int), st));
-    k_export_count<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, nl->row_start, nl->row_len, nl->nbr, nl->perm, cnt);
+    // a 16-bit local list is expanded to j | code entries first (same row offsets)
+    uint32_t* nbr32 = (uint32_t*)nl->nbr;
+    uint32_t* expanded = nullptr;
+    if (nl->fmt == 1) {
+        CUDA_TRY(ctx, cudaMalloc((void**)&expanded, sizeof(uint32_t) * (size_t)nl->n_directed));
+        k_local_to_global<<<nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2], 256, 0, st>>>(
+            nl->cell_start, nl->gg, nl->row_start, nl->row_len, (const uint16_t*)nl->nbr, expanded);
+        KERNEL_CHECK(ctx);
+        nbr32 = expanded;
+    }
+    k_export_count<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, nl->row_start, nl->row_len, nbr32, nl->perm, cnt);
     KERNEL_CHECK(ctx);
     int r = exclusive_scan<int>(ctx, n + 1, cnt, off, st);
     if (r == SQEQ_OK) {
-        k_export_fill<<<(unsigned)n, 256, 0, st>>>(n, nl->row_start, nl->row_len, nl->nbr, nl->perm, nl->wrapc, off,
+        k_export_fill<<<(unsigned)n, 256, 0, st>>>(n, nl->row_start, nl->row_len, nbr32, nl->perm, nl->wrapc, off,
                                                     oi, oj, shift3, flag);
         ctx->launches++;
     }
@@ -715,7 +825,7 @@ int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj
     cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(&total, off + n, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
     cudaError_t e = cudaStreamSynchronize(st);
-    cudaFree(cnt); cudaFree(off); cudaFree(flag);
+    cudaFree(cnt); cudaFree(off); cudaFree(flag); cudaFree(expanded);
     if (r != SQEQ_OK) return r;
     if (e != cudaSuccess) return sqeq_fail(ctx, SQEQ_ECUDA, "sqeq_nl_export: %s", cudaGetErrorString(e));
     if (h_flag & 2) return sqeq_fail(ctx, SQEQ_ECAPACITY, "sqeq_nl_export: a row has more than %d upper neighbours", EXPORT_CAP);

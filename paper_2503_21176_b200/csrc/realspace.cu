@@ -177,6 +177,93 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
     if (lane == 0) out[s] = make_float4(fx, fy, fz, phi);
 }
 
+// The same sum with the neighbourhood STAGED IN SHARED MEMORY (list format 1, cellgroup.cuh): one block
+// per group of 2x2x2 cells.  The block copies the group's neighbourhood -- every piece a contiguous run
+// of the cell-major float4 array, coalesced -- into shared memory with the piece's image shift already
+// added, then each warp takes rows of the group's own atoms: 16-bit local indices from the list (64 B
+// per warp load), neighbour (x,y,z,q) by LDS.128 instead of a scattered global gather, no per-pair
+// shift, same arithmetic as k_real.
+#define REAL_NT 512
+template <bool FORCE>
+__global__ void __launch_bounds__(REAL_NT, 4)
+k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
+              const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
+              const uint16_t* __restrict__ nbr, RealParams p, float4* __restrict__ out)
+{
+    extern __shared__ __align__(16) float4 xs[];               // [neighbourhood population]
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int r = 0; r < GRP_G * GRP_G; ++r) {
+            s_rpre[r] = acc;
+            const int ix = r / GRP_G, iy = r % GRP_G;
+            if (ix < gi.ge[0] && iy < gi.ge[1]) {
+                const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+                const int beg = cell_start[colw];
+                s_rbeg[r] = beg;
+                acc += cell_start[colw + gi.ge[2]] - beg;
+            } else {
+                s_rbeg[r] = 0;
+            }
+        }
+        s_rpre[GRP_G * GRP_G] = acc;
+    }
+    // stage: one warp per piece at a time
+    const int np = gi.ncol * 3;
+    for (int ip = wid; ip < np; ip += REAL_NT / 32) {
+        const GroupPiece pc = pieces[ip];
+        if (pc.len == 0) continue;
+        const float sx = (pc.code / 9 - 1) * p.Lx, sy = ((pc.code / 3) % 3 - 1) * p.Ly, sz = (pc.code % 3 - 1) * p.Lz;
+        for (int k = lane; k < pc.len; k += 32) {
+            float4 v = __ldg(xq + pc.gbeg + k);
+            v.x += sx; v.y += sy; v.z += sz;
+            xs[pc.lbase + k] = v;
+        }
+    }
+    __syncthreads();
+    const int natoms = s_rpre[GRP_G * GRP_G];
+    for (int ia = wid; ia < natoms; ia += REAL_NT / 32) {
+        int r = 0;
+#pragma unroll
+        for (int k = 1; k < GRP_G * GRP_G; ++k) r += (ia >= s_rpre[k]);
+        const int s = s_rbeg[r] + (ia - s_rpre[r]);
+        const float4 xi = __ldg(xq + s);
+        const uint16_t* __restrict__ row = nbr + row_start[s];
+        const int len = row_len[s];
+        float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+#pragma unroll 4
+        for (int k = lane; k < len; k += 32) {
+            const float4 xj = xs[__ldg(row + k)];
+            const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const float qj = r2 < p.rc2 ? xj.w : 0.f;
+            const float rinv = mufu_rsqrt(r2);
+            const float ex = mufu_ex2(p.na2l2e * r2);             // exp(-alpha^2 r^2)
+            const float t = erfc_from_exp(p.alpha * (r2 * rinv), ex) * rinv;   // erfc(alpha r)/r
+            phi = fmaf(qj, t, phi);
+            if (FORCE) {
+                const float gq = qj * fmaf(p.c2, ex, t) * (rinv * rinv);
+                fx = fmaf(gq, dx, fx);
+                fy = fmaf(gq, dy, fy);
+                fz = fmaf(gq, dz, fz);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            phi += __shfl_xor_sync(0xffffffffu, phi, o);
+            if (FORCE) {
+                fx += __shfl_xor_sync(0xffffffffu, fx, o);
+                fy += __shfl_xor_sync(0xffffffffu, fy, o);
+                fz += __shfl_xor_sync(0xffffffffu, fz, o);
+            }
+        }
+        if (lane == 0) out[s] = make_float4(fx, fy, fz, phi);
+    }
+}
+
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
                   cudaStream_t st)
 {
@@ -190,11 +277,18 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     p.na2l2e = (float)(-alpha * alpha * 1.4426950408889634);
     StageTimer tm(ctx, SQEQ_T_REAL, st);
     const int nb = ceil_div(n * 32, 256);
-    if (want_force)
-        k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, nl->nbr, p,
+    if (nl->fmt == 1) {
+        const size_t smem = sizeof(float4) * (size_t)nl->max_pop;
+        const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
+        auto kern = want_force ? k_real_staged<true> : k_real_staged<false>;
+        CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<ngroups, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, nl->row_len,
+                                         (const uint16_t*)nl->nbr, p, (float4*)ctx->real_out.p);
+    } else if (want_force)
+        k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, (const uint32_t*)nl->nbr, p,
                                           (float4*)ctx->real_out.p);
     else
-        k_real<false><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, nl->nbr, p,
+        k_real<false><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, (const uint32_t*)nl->nbr, p,
                                            (float4*)ctx->real_out.p);
     KERNEL_CHECK(ctx);
     return SQEQ_OK;

@@ -312,3 +312,27 @@ def test_enqueue_and_energy_fetch_match_synchronous_call(ctx):
     assert relrms(phi2.cpu().numpy(), phi.cpu().numpy()) < 1e-6
     assert relrms(F2.cpu().numpy(), F.cpu().numpy()) < 1e-6
     nl.free()
+
+
+def test_neighbour_build_resizes_for_clustered_systems(ctx):
+    """The single-pass build sizes the list and the per-warp staging rows from the MEAN density; a system
+    clustered into one corner of the box overflows both estimates and must be re-run with the exact
+    sizes the first pass counted (and still be bit-exact).  A second build of the same system then
+    starts from the remembered sizes."""
+    rng = np.random.default_rng(17)
+    box = [60.0, 64.0, 70.0]
+    n = 6000
+    pos = np.concatenate([rng.uniform(0, 14, (n - 50, 3)),            # dense blob: ~2.2 atoms/A^3 x ...
+                          rng.uniform(0, 1, (50, 3)) * np.array(box)]).astype(np.float32)
+    q = rng.normal(size=n).astype(np.float32)
+    for _ in range(2):
+        nl, m = check_nl_exact(ctx, pos, box, 6.0)
+        info = nl.info()
+        assert info["max_row"] > 1.5 * (4.0 / 3.0 * math.pi * 6.0 ** 3 * n / np.prod(box)) + 128
+        nl.free()
+    nl = ctx.nl_build(dev(pos), box, 6.0)
+    phi, F, E = ctx.coulomb(nl, dev(pos), dev(q), box, 5.5, 0.55, [64, 64, 72], 6)
+    rows = np.sort(rng.choice(n, 128, replace=False))
+    op, oF, _, _ = oracle.coulomb_pme(pos, q, box, 5.5, 0.55, [64, 64, 72], 6, rows=rows)
+    assert relrms(phi.cpu().numpy()[rows], op) < TOL and relrms(F.cpu().numpy()[rows], oF) < TOL
+    nl.free()
