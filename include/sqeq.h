@@ -63,7 +63,7 @@ const char* sqeq_version(void);
  * Internally: atoms are wrapped, binned into cells of edge >= cutoff/2, reordered cell-major; the
  * list is directed rows over the reordered atoms, entries either 16-bit indices into the neighbourhood
  * of the atom's 2x2x2 cell group or 32-bit (atom index | 27-valued image code).  Synchronises the
- * stream (the pair count sizes the list allocation).  SQEQ_ECAPACITY if an atom has more than 4352
+ * stream (the pair count sizes the list allocation).  SQEQ_ECAPACITY if an atom has more than 6528
  * neighbours. */
 int  sqeq_nl_build (sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3],
                     double cutoff, sqeq_nlist** out);

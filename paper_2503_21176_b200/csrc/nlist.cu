@@ -13,6 +13,8 @@
 //
 // Unlike Alg. 1 there is no [N,27,Cmax] candidate tensor and no padded cells[nx,ny,nz,Cmax].
 #include <math.h>
+#include <stdlib.h>
+#include <type_traits>
 
 #include "common.cuh"
 #include "cellgroup.cuh"
@@ -180,7 +182,7 @@ static int exclusive_scan(sqeq_ctx* ctx, int64_t n1, const Tin* in, int64_t* out
 {
     int nb = ceil_div(n1, 1024);
     int64_t* sums = nullptr;
-    if (nb > 1) CUDA_TRY(ctx, cudaMallocAsync((void**)&sums, sizeof(int64_t) * 2 * (size_t)nb, st));
+    if (nb > 1) CUDA_TRY(ctx, cudaMallocFromPoolAsync((void**)&sums, sizeof(int64_t) * 2 * (size_t)nb, ctx->pool, st));
     k_scan_blocks<Tin><<<nb, 1024, 0, st>>>(n1, in, out, sums);
     KERNEL_CHECK(ctx);
     if (nb > 1) {
@@ -255,8 +257,8 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
     float4* shtab = (float4*)smem_raw;                                        // [32] image shift vectors
     GroupPiece* pieces = (GroupPiece*)(smem_raw + 32 * sizeof(float4));       // [GRP_MAXPIECE]
     int4* segs_all = (int4*)(pieces + GRP_MAXPIECE);                          // [NL_WARPS][NL_MAXSEG]
-    uint32_t* stage_all = (uint32_t*)(segs_all + NL_WARPS * NL_MAXSEG);       // [NL_WARPS][cap_row] j | code
-    uint16_t* stage16_all = (uint16_t*)(stage_all + (size_t)NL_WARPS * cap_row);   // [NL_WARPS][cap_row] local
+    typedef typename std::conditional<LOCAL, uint16_t, uint32_t>::type entry_t;
+    entry_t* stage_all = (entry_t*)(segs_all + NL_WARPS * NL_MAXSEG);          // [NL_WARPS][cap_row] list entries
     __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
     if (threadIdx.x < 32) {
         int img = threadIdx.x < 27 ? threadIdx.x : 13;
@@ -286,8 +288,8 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
     const int natoms = s_rpre[GRP_G * GRP_G];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     int4* segs = segs_all + wid * NL_MAXSEG;
-    uint32_t* stage = stage_all + (size_t)wid * cap_row;
-    uint16_t* stage16 = stage16_all + (size_t)wid * cap_row;
+    entry_t* stage = stage_all + (size_t)wid * cap_row;
+    const int np_grp = gi.ncol * 3;
     const unsigned lt = (1u << lane) - 1u;
     const float hi_thr = g.rl2f + g.band, lo_thr = g.rl2f - g.band;
     const int ny_st = 2 * gg.w[1] + 1;
@@ -374,11 +376,8 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
                 const bool ok = r2 < hi_thr && t < seg.y && t != self;
                 band_seen |= ok && r2 >= lo_thr;
                 const unsigned m = __ballot_sync(0xffffffffu, ok);
-                const int at = count + __popc(m & lt);
-                if (ok && at < cap_row) {
-                    stage[at] = (uint32_t)t | codebits;
-                    if (LOCAL) stage16[at] = (uint16_t)(t + seg.w);
-                }
+                const int at = min(count + __popc(m & lt), cap_row - 1);   // an overflowing row is re-run anyway
+                if (ok) stage[at] = LOCAL ? (entry_t)(t + seg.w) : (entry_t)((uint32_t)t | codebits);
                 count += __popc(m);
             }
         }
@@ -391,24 +390,31 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
             for (int k0 = 0; k0 < count; k0 += 32) {
                 const int k = k0 + lane;
                 bool ok = k < count;
-                uint32_t e = 0;
-                uint16_t e16 = 0;
+                entry_t e = 0;
                 if (ok) {
                     e = stage[k];
-                    if (LOCAL) e16 = stage16[k];
-                    const int t = (int)(e & 0x07ffffffu);
+                    int t, code;
+                    if (LOCAL) {                                      // local index -> piece -> atom, image
+                        int lo = 0, hi = np_grp - 1;
+                        while (lo < hi) {
+                            const int mid = (lo + hi + 1) >> 1;
+                            if (pieces[mid].lbase <= (int)e) lo = mid; else hi = mid - 1;
+                        }
+                        t = pieces[lo].gbeg + ((int)e - pieces[lo].lbase);
+                        code = pieces[lo].code;
+                    } else {
+                        t = (int)((uint32_t)e & 0x07ffffffu);
+                        code = (int)((uint32_t)e >> 27);
+                    }
                     const float4 xj = __ldg(xq + t);
-                    const float4 sh = shtab[e >> 27];
+                    const float4 sh = shtab[code];
                     const float dx = xj.x - (xi.x - sh.x), dy = xj.y - (xi.y - sh.y), dz = xj.z - (xi.z - sh.z);
                     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));     // same expression as in the sweep
                     if (r2 >= lo_thr) ok = exact_in_range(pos, oi, perm[t], &ctr->ex);
                 }
                 const unsigned m = __ballot_sync(0xffffffffu, ok);
                 __syncwarp();
-                if (ok) {                                             // kept + rank <= k: never ahead of a reader
-                    stage[kept + __popc(m & lt)] = e;
-                    if (LOCAL) stage16[kept + __popc(m & lt)] = e16;
-                }
+                if (ok) stage[kept + __popc(m & lt)] = e;              // kept + rank <= k: never ahead of a reader
                 __syncwarp();
                 kept += __popc(m);
             }
@@ -426,13 +432,8 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         }
         off = __shfl_sync(0xffffffffu, off, 0);
         if (count <= cap_row && off + (unsigned long long)count <= capacity) {
-            if (LOCAL) {
-                uint16_t* dst = (uint16_t*)nbr_out + off;
-                for (int k = lane; k < count; k += 32) dst[k] = stage16[k];
-            } else {
-                uint32_t* dst = (uint32_t*)nbr_out + off;
-                for (int k = lane; k < count; k += 32) dst[k] = stage[k];
-            }
+            entry_t* dst = (entry_t*)nbr_out + off;
+            for (int k = lane; k < count; k += 32) dst[k] = stage[k];
         }
         __syncwarp();
     }
@@ -630,16 +631,16 @@ static void fill_group_geom(GroupGeom& gg, const NLGeom& g)
     }
 }
 
-static size_t pairs_smem(int cap_row)
+static size_t pairs_smem(int cap_row, bool local)
 {
     return 32 * sizeof(float4) + GRP_MAXPIECE * sizeof(GroupPiece) + (size_t)NL_WARPS * NL_MAXSEG * sizeof(int4) +
-           (size_t)NL_WARPS * cap_row * (sizeof(uint32_t) + sizeof(uint16_t));
+           (size_t)NL_WARPS * cap_row * (local ? sizeof(uint16_t) : sizeof(uint32_t));
 }
 
 static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, bool local,
                         int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
 {
-    const size_t smem = pairs_smem(cap_row);
+    const size_t smem = pairs_smem(cap_row, local);
     const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
     if (local) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -654,10 +655,16 @@ static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const N
     return SQEQ_OK;
 }
 
+#include <chrono>
+static double now_ms() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
+
 int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
                   sqeq_nlist** out)
 {
     cudaStream_t st = ctx->stream;
+    static const bool dbg = getenv("SQEQ_DEBUG") != nullptr;
+    const double t_0 = now_ms();
+    double t_alloc = 0, t_bin = 0, t_launch = 0, t_sync = 0;
     NLGeom g;
     fill_geom(g, box, cutoff, n);
     const int64_t ncells = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
@@ -698,6 +705,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     NL_CUDA(cudaMemsetAsync(xq + n, 0x7f, sizeof(float4) * 32, st));    // 3.4e38: far from everything
 
     const int nb = ceil_div(n, 256);
+    t_alloc = now_ms();
     {
         StageTimer tm(ctx, SQEQ_T_NL_BIN);
         NL_CUDA(cudaMemsetAsync(cell_count, 0, sizeof(int) * (ncells + 1), st));
@@ -719,6 +727,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         ctx->launches++;
         NL_CUDA(cudaGetLastError());
     }
+    t_bin = now_ms();
     {
         StageTimer tm(ctx, SQEQ_T_NL_PAIRS);
         // sizes: from the previous build of the same system if there was one, else from the mean
@@ -741,7 +750,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         // entry format: 16-bit local indices for the shared-memory-staged real-space kernel unless a
         // group's neighbourhood is too populous for 16 bits / shared memory (or SQEQ_REAL_STAGED=0)
         bool local = !ctx->real_staged_off && !(ctx->nl_last_n == n && ctx->nl_last_fmt == 0);
-        const int cap_row_max = 4352;      // 8 staging rows of 6 B entries in 227 KB of shared memory
+        const int cap_row_max = 6528;      // 8 staging rows of 4 B entries in 227 KB of shared memory
         for (int attempt = 0;; ++attempt) {
             if (cap_row > cap_row_max)
                 return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
@@ -754,9 +763,11 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
             *hinit = init;
             NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
             NL_TRY(launch_pairs(ctx, nl, pos, g, local, cap_row, capacity, ctr, st));
+            t_launch = now_ms();
             NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaStreamSynchronize(st));
+            t_sync = now_ms();
             if (h_flag[0] & 1)
                 return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
                                          "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
@@ -784,6 +795,9 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     }
     *out = nl;
     cleanup(SQEQ_OK);
+    if (dbg)
+        fprintf(stderr, "[sqeq] nl_build host ms: alloc %.3f bin-enqueue %.3f pairs-enqueue %.3f sync-wait %.3f tail %.3f\n",
+                t_alloc - t_0, t_bin - t_alloc, t_launch - t_bin, t_sync - t_launch, now_ms() - t_sync);
     return SQEQ_OK;
 #undef NL_TRY
 #undef NL_CUDA

@@ -336,3 +336,26 @@ def test_neighbour_build_resizes_for_clustered_systems(ctx):
     op, oF, _, _ = oracle.coulomb_pme(pos, q, box, 5.5, 0.55, [64, 64, 72], 6, rows=rows)
     assert relrms(phi.cpu().numpy()[rows], op) < TOL and relrms(F.cpu().numpy()[rows], oF) < TOL
     nl.free()
+
+
+def test_global_list_format_and_side_stream(ctx, monkeypatch):
+    """SQEQ_REAL_STAGED=0 keeps the 32-bit (atom | image code) list and the global-gather real-space
+    kernel (the path taken when a cell group's neighbourhood does not fit 16 bits / shared memory);
+    SQEQ_OVERLAP=1 runs PME on the side stream.  Same bars as the default path."""
+    from paper_2503_21176_b200 import binding
+    monkeypatch.setenv("SQEQ_REAL_STAGED", "0")
+    monkeypatch.setenv("SQEQ_OVERLAP", "1")
+    c2 = binding.Context(0)
+    try:
+        for k in (0, 1):
+            c = W.CONFIGS[k]
+            pos, q = inputs(k)
+            nl, npairs = check_nl_exact(c2, pos, c.box, c.r_list)
+            assert nl.info()["entry_bytes"] == 4
+            check_coulomb(c2, nl, pos, q, c)
+            nl.free()
+        nl = ctx.nl_build(dev(inputs(1)[0]), W.CONFIGS[1].box, W.CONFIGS[1].r_list)
+        assert nl.info()["entry_bytes"] == 2
+        nl.free()
+    finally:
+        c2.close()
