@@ -115,6 +115,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->scal.cap = 16 * sizeof(double);
     const char* env = getenv("SQEQ_PME_TILES");
     ctx->pme_tiles_off = env && env[0] == '0';
+    env = getenv("SQEQ_SPREAD_FLOAT");
+    ctx->spread_float = env && env[0] == '1';
     env = getenv("SQEQ_OVERLAP");
     ctx->overlap = env && env[0] == '1';
     env = getenv("SQEQ_REAL_STAGED");

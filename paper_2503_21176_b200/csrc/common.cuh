@@ -37,6 +37,7 @@ struct sqeq_ctx {
     int64_t nl_last_n = 0, nl_last_total = 0;   // sizes of the previous build: next build's estimate
     int nl_last_max_row = 0;
     int nl_last_fmt = 1;
+    bool spread_float = false;            // SQEQ_SPREAD_FLOAT=1: fp32 (CAS) instead of fixed-point shared accumulation
     bool overlap = false;                 // SQEQ_OVERLAP=1: PME on the side stream beside the real-space kernel
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
 

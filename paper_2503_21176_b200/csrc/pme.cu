@@ -356,8 +356,9 @@ __device__ __forceinline__ void red_add_v4(float* addr, float4 v)
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
-template <bool FLUSH>
-__device__ __forceinline__ void tile_move(float* tile, float* grid, const TileBlock& tb, const TileGeom& tg)
+template <bool FLUSH, bool FIXED = false>
+__device__ __forceinline__ void tile_move(float* tile, float* grid, const TileBlock& tb, const TileGeom& tg,
+                                          float inv_scale = 1.f)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
@@ -371,7 +372,14 @@ __device__ __forceinline__ void tile_move(float* tile, float* grid, const TileBl
         for (int tz = z4; tz < tg.T[2]; tz += 32) {
             float* g = grow + wrap1(tb.o[2] + tz, K2);
             if (FLUSH) {
-                const float4 v = make_float4(trow[tz], trow[tz + 1], trow[tz + 2], trow[tz + 3]);
+                float4 v;
+                if (FIXED) {
+                    const int* irow = (const int*)trow;
+                    v = make_float4(inv_scale * (float)irow[tz], inv_scale * (float)irow[tz + 1],
+                                    inv_scale * (float)irow[tz + 2], inv_scale * (float)irow[tz + 3]);
+                } else {
+                    v = make_float4(trow[tz], trow[tz + 1], trow[tz + 2], trow[tz + 3]);
+                }
                 if (v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f) red_add_v4(g, v);
             } else {
                 const float4 v = __ldg((const float4*)g);
@@ -381,7 +389,12 @@ __device__ __forceinline__ void tile_move(float* tile, float* grid, const TileBl
     }
 }
 
-template <int P, int NT>
+// FIXED: the tile accumulates 32-bit fixed point with the native shared integer atomic (one ATOMS.ADD
+// instead of a 7-instruction fp32 compare-and-swap loop that retries under contention).  The scale is
+// per block: |tile point| <= sum_i |q_i| theta_x theta_y theta_z <= (2/3)^3 sum_i |q_i| over the block's
+// atoms (2/3 = max of M_4, the largest cardinal B-spline peak of the supported orders), so
+// S = 2^30 / ((2/3)^3 sum|q|) cannot overflow; one addition rounds by <= 0.5/S.
+template <int P, int NT, bool FIXED>
 __global__ void __launch_bounds__(NT)
 k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
               const int* __restrict__ cell_start, TileGeom tg, float* __restrict__ grid)
@@ -395,7 +408,21 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
     if (tb.natoms == 0) return;
     const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
     const int tsize = tg.XS * tg.T[0];
-    for (int e = threadIdx.x; e < tsize; e += blockDim.x) tile[e] = 0.f;
+    for (int e = threadIdx.x; e < tsize; e += blockDim.x) tile[e] = 0.f;       // 0.f and 0 share a bit pattern
+    float scale = 1.f;
+    if (FIXED) {
+        __shared__ float s_part[NT / 32];
+        float aq = 0.f;
+        for (int i = threadIdx.x; i < tb.natoms; i += NT) aq += fabsf(frac[tile_atom(i, rbeg, rpre)].w);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) aq += __shfl_xor_sync(0xffffffffu, aq, o);
+        if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = aq;
+        __syncthreads();
+        aq = 0.f;
+#pragma unroll
+        for (int k = 0; k < NT / 32; ++k) aq += s_part[k];
+        scale = aq > 0.f ? 1073741824.f / (0.2962963f * aq * 1.0001f) : 1.f;
+    }
 
     for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK(NT)) {
         const int na = min(TILE_CHUNK(NT), tb.natoms - ch);
@@ -403,6 +430,7 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
         tile_chunk_setup<P, NT, false>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
         __syncthreads();
         const int rows = na * P * P;
+        float carry = 0.f;
         for (int R = threadIdx.x; R < rows; R += blockDim.x) {
             const int at = R / (P * P), row = R % (P * P);
             const int a = row / P, b = row % P;
@@ -415,8 +443,22 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
             const int t = stoff[at];
             if (t >= 0) {
                 float* rowp = tile + (t - a * tg.XS - b * tg.ZS);
+                if (FIXED) {
+                    // error feedback: the rounding residual of one point is carried into the thread's next
+                    // point (its neighbour along z), so the quantisation noise is a field of tiny dipoles --
+                    // pushed to the high wavenumbers that the influence function damps
+                    const float w2s = w2 * scale;
 #pragma unroll
-                for (int c = 0; c < P; ++c) atomicAdd(rowp - c, w2 * wz[c]);   // CAS loop: no native fp32 shared atomic
+                    for (int c = 0; c < P; ++c) {
+                        const float v = fmaf(w2s, wz[c], carry);
+                        const float vr = rintf(v);
+                        carry = v - vr;
+                        atomicAdd((int*)rowp - c, (int)vr);
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < P; ++c) atomicAdd(rowp - c, w2 * wz[c]);   // CAS loop: no native fp32 shared atomic
+                }
             } else {
                 const int4 f = sb[at];
                 int gx = f.x - a; gx += gx < 0 ? K0 : 0;
@@ -431,7 +473,7 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
         }
     }
     __syncthreads();
-    tile_move<true>(tile, grid, tb, tg);
+    tile_move<true, FIXED>(tile, grid, tb, tg, 1.f / scale);
 }
 
 // gather of one atom by one warp out of the tile (IN_TILE) or out of global memory: full passes of
@@ -705,7 +747,8 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         StageTimer tm(ctx, SQEQ_T_SPREAD, st);
         CUDA_TRY(ctx, cudaMemsetAsync(grid, 0, sizeof(float) * G3, st));
         if (tiles) {
-            auto kern = nt == 256 ? k_spread_tile<P, 256> : k_spread_tile<P, 512>;
+            auto kern = ctx->spread_float ? (nt == 256 ? k_spread_tile<P, 256, false> : k_spread_tile<P, 512, false>)
+                                          : (nt == 256 ? k_spread_tile<P, 256, true> : k_spread_tile<P, 512, true>);
             CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
             kern<<<ngroups, nt, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid);
         } else {
