@@ -143,6 +143,26 @@ struct StageTimer {
     ~StageTimer();
 };
 
+#ifdef __CUDACC__
+// Sums four per-lane values over the warp with 6 shuffles instead of 20: the first two butterfly steps
+// halve the number of values a lane carries (lanes keep one half of the values and send the other),
+// the last three are an ordinary butterfly.  On return lane 0 holds the sum of a, lane 8 of b, lane 16 of
+// c and lane 24 of d (in the returned value).
+__device__ __forceinline__ float warp_reduce4(float a, float b, float c, float d, int lane)
+{
+    const bool hi16 = lane & 16, hi8 = lane & 8;
+    float k0 = hi16 ? c : a, k1 = hi16 ? d : b;             // keep
+    k0 += __shfl_xor_sync(0xffffffffu, hi16 ? a : c, 16);
+    k1 += __shfl_xor_sync(0xffffffffu, hi16 ? b : d, 16);
+    float k = hi8 ? k1 : k0;
+    k += __shfl_xor_sync(0xffffffffu, hi8 ? k0 : k1, 8);
+    k += __shfl_xor_sync(0xffffffffu, k, 4);
+    k += __shfl_xor_sync(0xffffffffu, k, 2);
+    k += __shfl_xor_sync(0xffffffffu, k, 1);
+    return k;
+}
+#endif
+
 static inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // ---- stage entry points (implemented in the .cu files) ----

@@ -578,16 +578,19 @@ k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
             float ph = 0.f, gx_ = 0.f, gy_ = 0.f, gz_ = 0.f;
             if (toff >= 0) gather_atom<P, FORCE, true>(tile, toff, sb[at], r, tg, lane, ph, gx_, gy_, gz_);
             else gather_atom<P, FORCE, false>(grid, 0, sb[at], r, tg, lane, ph, gx_, gy_, gz_);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                ph += __shfl_xor_sync(0xffffffffu, ph, o);
-                if (FORCE) {
-                    gx_ += __shfl_xor_sync(0xffffffffu, gx_, o);
-                    gy_ += __shfl_xor_sync(0xffffffffu, gy_, o);
-                    gz_ += __shfl_xor_sync(0xffffffffu, gz_, o);
+            if (FORCE) {
+                // lanes 0 / 8 / 16 / 24 end up with the sums of gx / gy / gz / phi: one 16-byte store by four lanes
+                const float v = warp_reduce4(gx_, gy_, gz_, ph, lane);
+                if ((lane & 7) == 0) {
+                    const int comp = lane >> 3;
+                    const float sc = comp == 0 ? -sx : (comp == 1 ? -sy : (comp == 2 ? -sz : 1.f));
+                    ((float*)(out + sidx[at]))[comp] = sc * v;
                 }
+            } else {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) ph += __shfl_xor_sync(0xffffffffu, ph, o);
+                if (lane == 0) out[sidx[at]] = make_float4(0.f, 0.f, 0.f, ph);
             }
-            if (lane == 0) out[sidx[at]] = make_float4(-sx * gx_, -sy * gy_, -sz * gz_, ph);
         }
     }
 }
@@ -670,6 +673,8 @@ static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeo
     const int64_t want_groups = 2 * (int64_t)ctx->sm_count;
     for (int pass = 0; pass < 2 && !found; ++pass)       // pass 1 drops the "enough blocks" wish
         for (int nt = 256; nt <= 512; nt *= 2) {
+            static const int force_nt = getenv("SQEQ_TILE_NT") ? atoi(getenv("SQEQ_TILE_NT")) : 0;
+            if (force_nt && nt != force_nt) continue;
             // 227 KB per SM: four 256-thread blocks or two 512-thread blocks, records included
             const size_t limit = (nt == 256 ? 56 * 1024 : 112 * 1024) - (size_t)(nt / 4) * (REC_LEN(P) * 4 + 24) - 256;
             for (int gxy = 1; gxy <= 4; ++gxy)

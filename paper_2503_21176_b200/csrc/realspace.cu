@@ -251,16 +251,14 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
                 fz = fmaf(gq, dz, fz);
             }
         }
+        if (FORCE) {
+            const float v = warp_reduce4(fx, fy, fz, phi, lane);        // lanes 0 / 8 / 16 / 24: fx / fy / fz / phi
+            if ((lane & 7) == 0) ((float*)(out + s))[lane >> 3] = v;
+        } else {
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            phi += __shfl_xor_sync(0xffffffffu, phi, o);
-            if (FORCE) {
-                fx += __shfl_xor_sync(0xffffffffu, fx, o);
-                fy += __shfl_xor_sync(0xffffffffu, fy, o);
-                fz += __shfl_xor_sync(0xffffffffu, fz, o);
-            }
+            for (int o = 16; o > 0; o >>= 1) phi += __shfl_xor_sync(0xffffffffu, phi, o);
+            if (lane == 0) out[s] = make_float4(0.f, 0.f, 0.f, phi);
         }
-        if (lane == 0) out[s] = make_float4(fx, fy, fz, phi);
     }
 }
 
