@@ -567,6 +567,7 @@ k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
     if (tb.natoms == 0) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     tile_move<false>(tile, const_cast<float*>(grid), tb, tg);
+    const float sc_lane = (lane >> 3) == 0 ? -sx : ((lane >> 3) == 1 ? -sy : ((lane >> 3) == 2 ? -sz : 1.f));   // writers: lanes 0/8/16/24
     for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK(NT)) {
         const int na = min(TILE_CHUNK(NT), tb.natoms - ch);
         __syncthreads();
@@ -581,11 +582,7 @@ k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
             if (FORCE) {
                 // lanes 0 / 8 / 16 / 24 end up with the sums of gx / gy / gz / phi: one 16-byte store by four lanes
                 const float v = warp_reduce4(gx_, gy_, gz_, ph, lane);
-                if ((lane & 7) == 0) {
-                    const int comp = lane >> 3;
-                    const float sc = comp == 0 ? -sx : (comp == 1 ? -sy : (comp == 2 ? -sz : 1.f));
-                    ((float*)(out + sidx[at]))[comp] = sc * v;
-                }
+                if ((lane & 7) == 0) ((float*)out)[4 * sidx[at] + (lane >> 3)] = sc_lane * v;
             } else {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) ph += __shfl_xor_sync(0xffffffffu, ph, o);
