@@ -246,7 +246,7 @@ struct NLCounters {
 };
 
 template <bool LOCAL>
-__global__ void __launch_bounds__(NL_WARPS * 32, 3)
+__global__ void __launch_bounds__(NL_WARPS * 32, 5)
 k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
         const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, unsigned long long capacity,

@@ -94,7 +94,7 @@ int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const do
 struct RealParams {
     float Lx, Ly, Lz;
     float rc2;
-    float alpha;
+    float pa;        // 0.3275911 alpha (erfc_from_exp)
     float c2;        // 2 alpha / sqrt(pi)
     float na2l2e;    // -alpha^2 log2(e):  exp(-alpha^2 r^2) = 2^(na2l2e r^2)
 };
@@ -109,9 +109,10 @@ __device__ __forceinline__ float mufu_ex2(float x)   { float y; asm("ex2.approx.
 // minimax fit of erfcx(x) = exp(x^2) erfc(x) made for this library (max |error| of erfc 3.5e-9 in
 // exact arithmetic, ~5e-8 rms once evaluated in fp32) -- 1 MUFU.RCP + 8 FP32 ops instead of the
 // ~40-instruction erfcf, and it shares the exp(-alpha^2 r^2) the force needs anyway.
-__device__ __forceinline__ float erfc_from_exp(float x, float ex)
+// Called with r and pa = 0.3275911 alpha, so that the product alpha r is never formed on its own.
+__device__ __forceinline__ float erfc_from_exp(float r, float pa, float ex)
 {
-    const float t = mufu_rcp(fmaf(0.3275911f, x, 1.f));
+    const float t = mufu_rcp(fmaf(pa, r, 1.f));
     float p = -0.2984510018424136f;
     p = fmaf(p, t, 1.504820963708936f);
     p = fmaf(p, t, -2.085553381950119f);
@@ -155,7 +156,7 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
         const float qj = r2 < p.rc2 ? xj.w : 0.f;
         const float rinv = mufu_rsqrt(r2);
         const float ex = mufu_ex2(p.na2l2e * r2);             // exp(-alpha^2 r^2)
-        const float t = erfc_from_exp(p.alpha * (r2 * rinv), ex) * rinv;   // erfc(alpha r)/r
+        const float t = erfc_from_exp(r2 * rinv, p.pa, ex) * rinv;   // erfc(alpha r)/r
         phi = fmaf(qj, t, phi);
         if (FORCE) {
             const float gq = qj * fmaf(p.c2, ex, t) * (rinv * rinv);
@@ -242,7 +243,7 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
             const float qj = r2 < p.rc2 ? xj.w : 0.f;
             const float rinv = mufu_rsqrt(r2);
             const float ex = mufu_ex2(p.na2l2e * r2);             // exp(-alpha^2 r^2)
-            const float t = erfc_from_exp(p.alpha * (r2 * rinv), ex) * rinv;   // erfc(alpha r)/r
+            const float t = erfc_from_exp(r2 * rinv, p.pa, ex) * rinv;   // erfc(alpha r)/r
             phi = fmaf(qj, t, phi);
             if (FORCE) {
                 const float gq = qj * fmaf(p.c2, ex, t) * (rinv * rinv);
@@ -270,7 +271,7 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     RealParams p;
     p.Lx = (float)nl->box[0]; p.Ly = (float)nl->box[1]; p.Lz = (float)nl->box[2];
     p.rc2 = (float)(rc * rc);
-    p.alpha = (float)alpha;
+    p.pa = (float)(0.3275911 * alpha);
     p.c2 = (float)(2.0 * alpha / sqrt(M_PI));
     p.na2l2e = (float)(-alpha * alpha * 1.4426950408889634);
     StageTimer tm(ctx, SQEQ_T_REAL, st);
