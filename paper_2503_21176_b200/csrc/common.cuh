@@ -37,6 +37,7 @@ struct sqeq_ctx {
     int64_t nl_last_n = 0, nl_last_total = 0;   // sizes of the previous build: next build's estimate
     int nl_last_max_row = 0;
     int nl_last_fmt = 1;
+    int nl_last_max_pop = 0;
     bool spread_float = false;            // SQEQ_SPREAD_FLOAT=1: fp32 (CAS) instead of fixed-point shared accumulation
     bool overlap = false;                 // SQEQ_OVERLAP=1: PME on the side stream beside the real-space kernel
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
@@ -91,19 +92,21 @@ struct sqeq_nlist {
     double box[3] = {0, 0, 0};
     double cutoff = 0;
     int ncell[3] = {1, 1, 1};
-    int64_t n_directed = 0;
+    int64_t n_directed = 0;          // directed pairs (sum of row_len)
+    int64_t n_slots = 0;             // list slots in use (fmt 1 pads every row to a multiple of 32)
     int max_row = 0;
     // device arrays
     int*      perm = nullptr;        // [n]   sorted index -> caller index
     int*      cell_of = nullptr;     // [n]   cell id of sorted atom
     int*      cell_start = nullptr;  // [ncells+1]
     char4*    wrapc = nullptr;       // [n]   floor(x/L) per axis at build time (sorted order)
-    int64_t*  row_start = nullptr;   // [n]   offset of row s in nbr (rows are packed, in no particular order)
+    int64_t*  row_start = nullptr;   // [n]   offset of row s in nbr (rows in no particular order; fmt 1: multiples of 32)
     int*      row_len = nullptr;     // [n]   entries of row s
-    void*     nbr = nullptr;         // [>= n_directed] entries: fmt 0: uint32 j (27 bits) | image code << 27;
+    void*     nbr = nullptr;         // [>= n_slots] entries: fmt 0: uint32 j (27 bits) | image code << 27;
                                      //                          fmt 1: uint16 local index in the group's neighbourhood
     int       fmt = 0;
     int       max_pop = 0;           // fmt 1: largest neighbourhood population of a group
+    int       lshift = 0;            // fmt 1: entries are local index << lshift (4: byte offsets of float4 slots)
     GroupGeom gg;                    // cell groups (cellgroup.cuh)
 };
 

@@ -238,8 +238,10 @@ __device__ __noinline__ bool exact_in_range(const float* __restrict__ pos, int o
 // the kernel keeps counting and the host re-runs it with the now known sizes / the other format.
 #define NL_MAXSEG 96
 #define NL_WARPS 8
+#define NL_SLACK 256      // slots past the last row: the real-space kernel prefetches list entries ahead of its row
 struct NLCounters {
-    unsigned long long cursor;
+    unsigned long long cursor;     // list slots handed out (fmt 1 rows are padded to whole warps)
+    unsigned long long pairs;      // directed pairs
     int max_row;
     int max_pop;
     NLExact ex;
@@ -249,7 +251,7 @@ template <bool LOCAL>
 __global__ void __launch_bounds__(NL_WARPS * 32, 5)
 k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
-        const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, unsigned long long capacity,
+        const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, int lshift, unsigned long long capacity,
         NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
         void* __restrict__ nbr_out)
 {
@@ -423,17 +425,22 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         __syncwarp();
 
         // ---- 3. reserve and copy out
+        // a local row is padded to a multiple of 32 slots with the index of the neighbourhood's dummy slot
+        // (one past its population: an atom far from everything with charge 0), so that the real-space
+        // kernel runs whole warps over it and every row starts on a 64-byte boundary
+        const int padn = LOCAL ? (count + 31) & ~31 : count;
         unsigned long long off = 0;
         if (lane == 0) {
-            off = atomicAdd(&ctr->cursor, (unsigned long long)count);
+            off = atomicAdd(&ctr->cursor, (unsigned long long)padn);
+            atomicAdd(&ctr->pairs, (unsigned long long)count);
             atomicMax(&ctr->max_row, count);
             row_start[s] = (int64_t)off;
             row_len[s] = count;
         }
         off = __shfl_sync(0xffffffffu, off, 0);
-        if (count <= cap_row && off + (unsigned long long)count <= capacity) {
+        if (count <= cap_row && off + (unsigned long long)padn <= capacity) {
             entry_t* dst = (entry_t*)nbr_out + off;
-            for (int k = lane; k < count; k += 32) dst[k] = stage[k];
+            for (int k = lane; k < padn; k += 32) dst[k] = (entry_t)((k < count ? stage[k] : (entry_t)gi.pop) << lshift);
         }
         __syncwarp();
     }
@@ -443,7 +450,7 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
 // the canonical export only): one block per group, binary search of each entry in the piece table.
 __global__ void __launch_bounds__(256)
 k_local_to_global(const int* __restrict__ cell_start, GroupGeom gg, const int64_t* __restrict__ row_start,
-                  const int* __restrict__ row_len, const uint16_t* __restrict__ nbr16,
+                  const int* __restrict__ row_len, const uint16_t* __restrict__ nbr16, int lshift,
                   uint32_t* __restrict__ nbr32)
 {
     __shared__ GroupPiece pieces[GRP_MAXPIECE];
@@ -459,7 +466,7 @@ k_local_to_global(const int* __restrict__ cell_start, GroupGeom gg, const int64_
                 const int64_t r0 = row_start[s];
                 const int len = row_len[s];
                 for (int k = lane; k < len; k += 32) {
-                    const int e = nbr16[r0 + k];
+                    const int e = nbr16[r0 + k] >> lshift;
                     int lo = 0, hi = np - 1;                 // last piece with lbase <= e
                     while (lo < hi) {
                         const int mid = (lo + hi + 1) >> 1;
@@ -638,18 +645,18 @@ static size_t pairs_smem(int cap_row, bool local)
 }
 
 static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, bool local,
-                        int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
+                        int lshift, int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
 {
     const size_t smem = pairs_smem(cap_row, local);
     const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
     if (local) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<true><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-            nl->perm, pos, g, nl->gg, cap_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+            nl->perm, pos, g, nl->gg, cap_row, lshift, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
     } else {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<false><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-            nl->perm, pos, g, nl->gg, cap_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+            nl->perm, pos, g, nl->gg, cap_row, lshift, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
     }
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
@@ -750,19 +757,22 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         // entry format: 16-bit local indices for the shared-memory-staged real-space kernel unless a
         // group's neighbourhood is too populous for 16 bits / shared memory (or SQEQ_REAL_STAGED=0)
         bool local = !ctx->real_staged_off && !(ctx->nl_last_n == n && ctx->nl_last_fmt == 0);
+        // local entries are stored as byte offsets of the staged float4 slots (index << 4) while the most
+        // populous neighbourhood, dummy slot included, stays below 4096 atoms
+        int lshift = (ctx->nl_last_n == n && ctx->nl_last_max_pop > 4094) ? 0 : 4;
         const int cap_row_max = 6528;      // 8 staging rows of 4 B entries in 227 KB of shared memory
         for (int attempt = 0;; ++attempt) {
             if (cap_row > cap_row_max)
                 return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
                         "sqeq_nl_build: a row has %d neighbours; rows above %d are not supported", cap_row, cap_row_max));
             const size_t esize = local ? sizeof(uint16_t) : sizeof(uint32_t);
-            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, esize * capacity));
+            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, esize * (capacity + NL_SLACK)));
             NLCounters init = {};
             for (int d = 0; d < 3; ++d) init.ex.L[d] = g.L[d];
             init.ex.rl2 = g.rl2;
             *hinit = init;
             NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
-            NL_TRY(launch_pairs(ctx, nl, pos, g, local, cap_row, capacity, ctr, st));
+            NL_TRY(launch_pairs(ctx, nl, pos, g, local, local ? lshift : 0, cap_row, capacity, ctr, st));
             t_launch = now_ms();
             NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -772,8 +782,9 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
                 return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
                                          "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
             const bool row_ok = h->max_row <= cap_row, cap_ok = h->cursor <= capacity;
-            const bool fmt_ok = !local || (h->max_pop <= 65535 && (size_t)h->max_pop * sizeof(float4) <= REAL_STAGE_MAX_BYTES);
-            if (row_ok && cap_ok && fmt_ok) break;
+            const bool fmt_ok = !local || (h->max_pop <= 65534 && ((size_t)h->max_pop + 1) * sizeof(float4) <= REAL_STAGE_MAX_BYTES);
+            const bool shift_ok = !local || !fmt_ok || lshift == 0 || h->max_pop <= 4094;
+            if (row_ok && cap_ok && fmt_ok && shift_ok) break;
             if (attempt >= 3)
                 return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY, "sqeq_nl_build: sizing did not converge"));
             if (!row_ok) cap_row = (h->max_row + 31) & ~31;
@@ -783,14 +794,18 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
                 if (!cap_ok) capacity = (size_t)h->cursor;
                 if (!fmt_ok) local = false;
             }
+            if (!shift_ok) lshift = 0;
         }
         nl->fmt = local ? 1 : 0;
         nl->max_pop = local ? h->max_pop : 0;
+        nl->lshift = local ? lshift : 0;
+        ctx->nl_last_max_pop = h->max_pop;
         ctx->nl_last_fmt = nl->fmt;
-        nl->n_directed = (int64_t)h->cursor;
+        nl->n_directed = (int64_t)h->pairs;
+        nl->n_slots = (int64_t)h->cursor;
         nl->max_row = h->max_row;
         ctx->nl_last_n = n;
-        ctx->nl_last_total = nl->n_directed;
+        ctx->nl_last_total = nl->n_slots;
         ctx->nl_last_max_row = nl->max_row;
     }
     *out = nl;
@@ -820,9 +835,9 @@ int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj
     uint32_t* nbr32 = (uint32_t*)nl->nbr;
     uint32_t* expanded = nullptr;
     if (nl->fmt == 1) {
-        CUDA_TRY(ctx, cudaMalloc((void**)&expanded, sizeof(uint32_t) * (size_t)nl->n_directed));
+        CUDA_TRY(ctx, cudaMalloc((void**)&expanded, sizeof(uint32_t) * (size_t)nl->n_slots));
         k_local_to_global<<<nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2], 256, 0, st>>>(
-            nl->cell_start, nl->gg, nl->row_start, nl->row_len, (const uint16_t*)nl->nbr, expanded);
+            nl->cell_start, nl->gg, nl->row_start, nl->row_len, (const uint16_t*)nl->nbr, nl->lshift, expanded);
         KERNEL_CHECK(ctx);
         nbr32 = expanded;
     }

@@ -673,7 +673,9 @@ static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeo
             static const int force_nt = getenv("SQEQ_TILE_NT") ? atoi(getenv("SQEQ_TILE_NT")) : 0;
             if (force_nt && nt != force_nt) continue;
             // 227 KB per SM: four 256-thread blocks or two 512-thread blocks, records included
-            const size_t limit = (nt == 256 ? 56 * 1024 : 112 * 1024) - (size_t)(nt / 4) * (REC_LEN(P) * 4 + 24) - 256;
+            static const int force_blocks = getenv("SQEQ_TILE_BLOCKS") ? atoi(getenv("SQEQ_TILE_BLOCKS")) : 0;
+            const int blocks_per_sm = force_blocks ? force_blocks : (nt == 256 ? 4 : 2);
+            const size_t limit = (size_t)(224 * 1024 / blocks_per_sm) - (size_t)(nt / 4) * (REC_LEN(P) * 4 + 24) - 256;
             for (int gxy = 1; gxy <= 4; ++gxy)
                 for (int gz = 1; gz <= 12; ++gz) {
                     TileGeom tg;
@@ -715,7 +717,7 @@ static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeo
                     if (bytes > limit) continue;
                     // window points moved per cell, plus a charge for idle SMs when blocks are few
                     double cost = (double)tg.T[0] * tg.T[1] * tg.T[2] / ((double)tg.g[0] * tg.g[1] * tg.g[2]);
-                    const double slots = (double)ctx->sm_count * (nt == 256 ? 4 : 2);
+                    const double slots = (double)ctx->sm_count * blocks_per_sm;
                     const double waves = (double)groups / slots;
                     cost *= ceil(waves) / waves;
                     if (cost < best_cost) { best_cost = cost; best = tg; best_bytes = bytes; best_nt = nt; found = true; }
@@ -758,6 +760,7 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         }
         KERNEL_CHECK(ctx);
     }
+    if (ctx->gridQ.p) SQEQ_TRY(sqeq_reserve(ctx, ctx->gridQ, sizeof(float) * G3));    // the grid may have grown since the capture was enabled
     if (ctx->gridQ.p) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->gridQ.p, grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, st));
     {
         StageTimer tm(ctx, SQEQ_T_FFT_FWD, st);

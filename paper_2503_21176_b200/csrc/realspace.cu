@@ -94,7 +94,7 @@ int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const do
 struct RealParams {
     float Lx, Ly, Lz;
     float rc2;
-    float pa;        // 0.3275911 alpha (erfc_from_exp)
+    float pa;        // ERFC_P alpha (erfc_from_exp)
     float c2;        // 2 alpha / sqrt(pi)
     float na2l2e;    // -alpha^2 log2(e):  exp(-alpha^2 r^2) = 2^(na2l2e r^2)
 };
@@ -104,22 +104,23 @@ __device__ __forceinline__ float mufu_rsqrt(float x) { float y; asm("rsqrt.appro
 __device__ __forceinline__ float mufu_rcp(float x)   { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float mufu_ex2(float x)   { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-// erfc(x) = exp(-x^2) t P6(t), t = 1/(1 + 0.3275911 x), x >= 0, given ex = exp(-x^2).
-// The form is Abramowitz & Stegun 7.1.26 extended to 7 terms; the coefficients are a weighted
-// minimax fit of erfcx(x) = exp(x^2) erfc(x) made for this library (max |error| of erfc 3.5e-9 in
-// exact arithmetic, ~5e-8 rms once evaluated in fp32) -- 1 MUFU.RCP + 8 FP32 ops instead of the
-// ~40-instruction erfcf, and it shares the exp(-alpha^2 r^2) the force needs anyway.
-// Called with r and pa = 0.3275911 alpha, so that the product alpha r is never formed on its own.
+// erfc(x) = exp(-x^2) t P5(t), t = 1/(1 + 0.4 x), x >= 0, given ex = exp(-x^2).
+// The form is Abramowitz & Stegun 7.1.26 with one more term and its own constant in t; the coefficients
+// are a weighted minimax (Lawson) fit of erfcx(x) = exp(x^2) erfc(x) made for this library: max |error|
+// of erfc 2.8e-8 in exact arithmetic, 3.6e-8 rms / 4.2e-7 max once evaluated in fp32 (the fp32 rounding
+// of the product dominates) -- 1 MUFU.RCP + 7 FP32 ops instead of the ~40-instruction erfcf, and it
+// shares the exp(-alpha^2 r^2) the force needs anyway.
+// Called with r and pa = 0.4 alpha, so that the product alpha r is never formed on its own.
+#define ERFC_P 0.4
 __device__ __forceinline__ float erfc_from_exp(float r, float pa, float ex)
 {
     const float t = mufu_rcp(fmaf(pa, r, 1.f));
-    float p = -0.2984510018424136f;
-    p = fmaf(p, t, 1.504820963708936f);
-    p = fmaf(p, t, -2.085553381950119f);
-    p = fmaf(p, t, 2.0401082452998613f);
-    p = fmaf(p, t, -0.7490695346520456f);
-    p = fmaf(p, t, 0.4311045009554423f);
-    p = fmaf(p, t, 0.1570402119784954f);
+    float p = -0.20025848511103075f;
+    p = fmaf(p, t, 0.7091442915149763f);
+    p = fmaf(p, t, -0.370903111156111f);
+    p = fmaf(p, t, 0.468270358550566f);
+    p = fmaf(p, t, 0.16182505660344682f);
+    p = fmaf(p, t, 0.23192186199974116f);
     return p * t * ex;
 }
 
@@ -184,16 +185,37 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
 // added, then each warp takes rows of the group's own atoms: 16-bit local indices from the list (64 B
 // per warp load), neighbour (x,y,z,q) by LDS.128 instead of a scattered global gather, no per-pair
 // shift, same arithmetic as k_real.
+#ifndef REAL_NT
 #define REAL_NT 512
-template <bool FORCE>
-__global__ void __launch_bounds__(REAL_NT, 4)
+#endif
+#ifndef REAL_BPS
+#define REAL_BPS 4          // blocks per SM the register budget is set for
+#endif
+#ifndef REAL_UNROLL
+#define REAL_UNROLL 4
+#endif
+#define REAL_PRAGMA_(x) _Pragma(#x)
+#define REAL_PRAGMA_UNROLL(n) REAL_PRAGMA_(unroll n)
+#ifndef REAL_PF
+#define REAL_PF 0           // list entries are loaded this many 32-pair steps ahead of their use
+#endif
+__device__ __forceinline__ float4 lds128(unsigned addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+// SCALED: the list entries are byte offsets into the staged array (local index * 16, nl->lshift = 4)
+template <bool FORCE, bool SCALED>
+__global__ void __launch_bounds__(REAL_NT, REAL_BPS)
 k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
               const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
               const uint16_t* __restrict__ nbr, RealParams p, float4* __restrict__ out)
 {
-    extern __shared__ __align__(16) float4 xs[];               // [neighbourhood population]
+    extern __shared__ __align__(16) float4 xs[];               // [neighbourhood population + 1]
     __shared__ GroupPiece pieces[GRP_MAXPIECE];
-    __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
     const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
@@ -204,13 +226,15 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
             if (ix < gi.ge[0] && iy < gi.ge[1]) {
                 const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
                 const int beg = cell_start[colw];
-                s_rbeg[r] = beg;
+                s_roff[r] = beg - acc;                         // sorted index = own-atom number + s_roff[range]
                 acc += cell_start[colw + gi.ge[2]] - beg;
             } else {
-                s_rbeg[r] = 0;
+                s_roff[r] = 0;
             }
         }
         s_rpre[GRP_G * GRP_G] = acc;
+        // the dummy slot the padding entries of the rows point to: outside every cutoff, charge 0
+        xs[gi.pop] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
     }
     // stage: one warp per piece at a time
     const int np = gi.ncol * 3;
@@ -226,18 +250,29 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
     }
     __syncthreads();
     const int natoms = s_rpre[GRP_G * GRP_G];
+    const int p1 = s_rpre[1], p2 = s_rpre[2], p3 = s_rpre[3];
+    static_assert(GRP_G * GRP_G == 4, "range lookup below is written for four ranges");
     for (int ia = wid; ia < natoms; ia += REAL_NT / 32) {
-        int r = 0;
-#pragma unroll
-        for (int k = 1; k < GRP_G * GRP_G; ++k) r += (ia >= s_rpre[k]);
-        const int s = s_rbeg[r] + (ia - s_rpre[r]);
+        const int s = ia + s_roff[(ia >= p1) + (ia >= p2) + (ia >= p3)];
         const float4 xi = __ldg(xq + s);
-        const uint16_t* __restrict__ row = nbr + row_start[s];
-        const int len = row_len[s];
+        // rows are padded to whole 32-entry steps (the padding points at the dummy slot), so the loop is
+        // uniform over the warp; entries are fetched REAL_PF steps ahead (the list buffer carries slack
+        // for the look-ahead past the last row), which takes the DRAM latency of the list stream off the
+        // critical path
+        const uint16_t* __restrict__ row = nbr + row_start[s] + lane;
+        const int nst = (row_len[s] + 31) >> 5;
+        const unsigned xs_addr = (unsigned)__cvta_generic_to_shared(xs);
+        unsigned e[REAL_PF + 1];
+#pragma unroll
+        for (int k = 0; k < REAL_PF; ++k) e[k] = __ldg(row + 32 * k);
+        row += 32 * REAL_PF;
         float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
-#pragma unroll 4
-        for (int k = lane; k < len; k += 32) {
-            const float4 xj = xs[__ldg(row + k)];
+REAL_PRAGMA_UNROLL(REAL_UNROLL)
+        for (int it = 0; it < nst; ++it) {
+            e[REAL_PF] = __ldg(row + 32 * it);
+            const float4 xj = SCALED ? lds128(xs_addr + e[0]) : xs[e[0]];
+#pragma unroll
+            for (int k = 0; k < REAL_PF; ++k) e[k] = e[k + 1];
             const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float qj = r2 < p.rc2 ? xj.w : 0.f;
@@ -271,15 +306,16 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     RealParams p;
     p.Lx = (float)nl->box[0]; p.Ly = (float)nl->box[1]; p.Lz = (float)nl->box[2];
     p.rc2 = (float)(rc * rc);
-    p.pa = (float)(0.3275911 * alpha);
+    p.pa = (float)(ERFC_P * alpha);
     p.c2 = (float)(2.0 * alpha / sqrt(M_PI));
     p.na2l2e = (float)(-alpha * alpha * 1.4426950408889634);
     StageTimer tm(ctx, SQEQ_T_REAL, st);
     const int nb = ceil_div(n * 32, 256);
     if (nl->fmt == 1) {
-        const size_t smem = sizeof(float4) * (size_t)nl->max_pop;
+        const size_t smem = sizeof(float4) * ((size_t)nl->max_pop + 1);
         const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
-        auto kern = want_force ? k_real_staged<true> : k_real_staged<false>;
+        auto kern = nl->lshift ? (want_force ? k_real_staged<true, true> : k_real_staged<false, true>)
+                               : (want_force ? k_real_staged<true, false> : k_real_staged<false, false>);
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kern<<<ngroups, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, nl->row_len,
                                          (const uint16_t*)nl->nbr, p, (float4*)ctx->real_out.p);

@@ -221,6 +221,19 @@ def test_full_size_sampled_rows(ctx, k):
         o = np.argsort(allj, kind="stable")
         assert np.array_equal(allj[o], jr) and np.array_equal(alls[o], sr)
     check_coulomb(ctx, nl, pos, q, c, rows=rows)
+    # properties that hold at any size: E = 1/2 sum q phi; Newton's third law for the real-space part
+    # (the reciprocal part does not conserve momentum exactly); neutrality of Q
+    phi, F, E = ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+    half_q_phi = 0.5 * float((phi.double().cpu().numpy() * q.astype(np.float64)).sum())
+    assert abs(E - half_q_phi) < 1e-6 * abs(E)
+    g = ctx.coulomb_parts(nl)
+    Fr = g["F_real"].double().cpu().numpy()
+    assert np.abs(Fr.sum(0)).max() < 1e-4 * np.abs(Fr).sum(0).max() / math.sqrt(n) * 10
+    Q = ctx.pme_grid(0, c.grid)
+    if Q is None:                               # first request only switches the capture on
+        ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+        Q = ctx.pme_grid(0, c.grid)
+    assert abs(float(Q.double().sum()) - float(q.astype(np.float64).sum())) < 1e-3
     nl.free()
 
 
