@@ -314,11 +314,12 @@ __device__ __forceinline__ int tile_atom(int i, const int* rbeg, const int* rpre
 // Chunk setup by threads 0 .. 3*TILE_CHUNK(NT)-1 (thread = atom*3 + axis): spline weights into the atom's
 // record, and by the axis-0 thread the atom's sorted index, raw base index + charge bits, and the
 // linear tile offset of its base point (-1: footprint not inside the window).
-template <int P, int NT, bool DERIV>
+// QSCALE (spread): theta_x is stored multiplied by q_i * qscale, so that a row's weight is one product.
+template <int P, int NT, bool DERIV, bool QSCALE = false>
 __device__ __forceinline__ void tile_chunk_setup(int ch, int na, const TileBlock& tb, const TileGeom& tg,
                                                  const float4* __restrict__ frac, const int4* __restrict__ base,
                                                  const int* rbeg, const int* rpre, float* rec, int4* sb,
-                                                 int* stoff, int* sidx)
+                                                 int* stoff, int* sidx, float qscale = 1.f)
 {
     if (threadIdx.x >= 3 * TILE_CHUNK(NT)) return;
     const int at = threadIdx.x / 3, ax = threadIdx.x % 3;
@@ -330,9 +331,10 @@ __device__ __forceinline__ void tile_chunk_setup(int ch, int na, const TileBlock
     float* r = rec + at * REC_LEN(P);
     const int o_t = ax == 2 ? REC_Z : REC_X + ax * P;
     const int o_d = ax == 2 ? REC_DZ : REC_X + (2 + ax) * P;
+    const float ts = (QSCALE && ax == 0) ? fw.w * qscale : 1.f;
 #pragma unroll
     for (int j = 0; j < P; ++j) {
-        r[o_t + j] = th[j];
+        r[o_t + j] = QSCALE ? th[j] * ts : th[j];
         if (DERIV) r[o_d + j] = dth[j];
     }
     if (ax == 0) {
@@ -424,36 +426,41 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
         scale = aq > 0.f ? 1073741824.f / (0.2962963f * aq * 1.0001f) : 1.f;
     }
 
+    // thread <-> (atom slot, (x,y) row): the row (a, b) of a thread is fixed, NT / P^2 atoms are in flight per
+    // pass, and the index arithmetic of a row is paid once per kernel instead of once per row
+    constexpr int PP = P * P, APP = NT / PP;
+    const int slot = threadIdx.x / PP, row = threadIdx.x - slot * PP;
+    const int a = row / P, b = row - a * P;
+    const int off_ab = a * tg.XS + b * tg.ZS;
+    const float inv_scale = 1.f / scale;
     for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK(NT)) {
         const int na = min(TILE_CHUNK(NT), tb.natoms - ch);
         __syncthreads();
-        tile_chunk_setup<P, NT, false>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
+        tile_chunk_setup<P, NT, false, true>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx, scale);
         __syncthreads();
-        const int rows = na * P * P;
-        float carry = 0.f;
-        for (int R = threadIdx.x; R < rows; R += blockDim.x) {
-            const int at = R / (P * P), row = R % (P * P);
-            const int a = row / P, b = row % P;
+        if (slot >= APP) continue;
+        for (int at = slot; at < na; at += APP) {
             const float* r = rec + at * REC_LEN(P);
-            const float w2 = __int_as_float(sb[at].w) * r[REC_X + a] * r[REC_X + P + b];
-            if (w2 == 0.f) continue;
+            const float w2 = r[REC_X + a] * r[REC_X + P + b];          // q_i * scale * theta_x * theta_y
             float wz[8];
             *(float4*)wz = *(const float4*)(r + REC_Z);
             *(float4*)(wz + 4) = *(const float4*)(r + REC_Z + 4);
             const int t = stoff[at];
             if (t >= 0) {
-                float* rowp = tile + (t - a * tg.XS - b * tg.ZS);
+                float* rowp = tile + (t - off_ab);
                 if (FIXED) {
-                    // error feedback: the rounding residual of one point is carried into the thread's next
-                    // point (its neighbour along z), so the quantisation noise is a field of tiny dipoles --
-                    // pushed to the high wavenumbers that the influence function damps
-                    const float w2s = w2 * scale;
+                    // error feedback: the row's points are the differences of the ROUNDED running sum
+                    // K_c = rint(sum_{j<=c} x_j), so the rounding residual of one point is carried into the
+                    // next one along z and the quantisation noise is a field of tiny dipoles -- pushed to
+                    // the high wavenumbers that the influence function damps
+                    float run = 0.f;
+                    int kprev = 0;
 #pragma unroll
                     for (int c = 0; c < P; ++c) {
-                        const float v = fmaf(w2s, wz[c], carry);
-                        const float vr = rintf(v);
-                        carry = v - vr;
-                        atomicAdd((int*)rowp - c, (int)vr);
+                        run = fmaf(w2, wz[c], run);
+                        const int k = __float2int_rn(run);
+                        atomicAdd((int*)rowp - c, k - kprev);
+                        kprev = k;
                     }
                 } else {
 #pragma unroll
@@ -464,92 +471,17 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
                 int gx = f.x - a; gx += gx < 0 ? K0 : 0;
                 int gy = f.y - b; gy += gy < 0 ? K1 : 0;
                 float* rowp = grid + ((size_t)gx * K1 + gy) * K2;
+                const float w2g = w2 * inv_scale;
 #pragma unroll
                 for (int c = 0; c < P; ++c) {
                     int gz = f.z - c; gz += gz < 0 ? K2 : 0;
-                    atomicAdd(rowp + gz, w2 * wz[c]);
+                    atomicAdd(rowp + gz, w2g * wz[c]);
                 }
             }
         }
     }
     __syncthreads();
-    tile_move<true, FIXED>(tile, grid, tb, tg, 1.f / scale);
-}
-
-// gather of one atom by one warp out of the tile (IN_TILE) or out of global memory: full passes of
-// 32 (x,y) rows, then the P*P % 32 leftover rows point by point.  r = the atom's weight record.
-template <int P, bool FORCE, bool IN_TILE>
-__device__ __forceinline__ void gather_atom(const float* __restrict__ src, int toff, const int4 f,
-                                            const float* __restrict__ r, const TileGeom& tg, int lane,
-                                            float& ph, float& gx_, float& gy_, float& gz_)
-{
-    constexpr int FULL = (P * P) / 32 * 32, REST = (P * P - FULL) * P;
-    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
-    float wz[8], dz[8];
-    if (FULL > 0) {
-        *(float4*)wz = *(const float4*)(r + REC_Z);
-        *(float4*)(wz + 4) = *(const float4*)(r + REC_Z + 4);
-        if (FORCE) {
-            *(float4*)dz = *(const float4*)(r + REC_DZ);
-            *(float4*)(dz + 4) = *(const float4*)(r + REC_DZ + 4);
-        }
-    }
-#pragma unroll
-    for (int row0 = 0; row0 < FULL; row0 += 32) {
-        const int row = row0 + lane, a = row / P, b = row % P;
-        float s0 = 0.f, s1 = 0.f;
-        if (IN_TILE) {
-            const float* rowp = src + (toff - a * tg.XS - b * tg.ZS);
-#pragma unroll
-            for (int c = 0; c < P; ++c) {
-                const float v = rowp[-c];
-                s0 = fmaf(wz[c], v, s0);
-                if (FORCE) s1 = fmaf(dz[c], v, s1);
-            }
-        } else {
-            int gx = f.x - a; gx += gx < 0 ? K0 : 0;
-            int gy = f.y - b; gy += gy < 0 ? K1 : 0;
-            const float* rowp = src + ((size_t)gx * K1 + gy) * K2;
-#pragma unroll
-            for (int c = 0; c < P; ++c) {
-                int gz = f.z - c; gz += gz < 0 ? K2 : 0;
-                const float v = __ldg(rowp + gz);
-                s0 = fmaf(wz[c], v, s0);
-                if (FORCE) s1 = fmaf(dz[c], v, s1);
-            }
-        }
-        const float tx = r[REC_X + a], ty = r[REC_X + P + b];
-        ph = fmaf(tx * ty, s0, ph);
-        if (FORCE) {
-            gx_ = fmaf(r[REC_X + 2 * P + a] * ty, s0, gx_);
-            gy_ = fmaf(tx * r[REC_X + 3 * P + b], s0, gy_);
-            gz_ = fmaf(tx * ty, s1, gz_);
-        }
-    }
-#pragma unroll
-    for (int p0 = 0; p0 < REST; p0 += 32) {
-        const int pt = p0 + lane;
-        if (pt < REST) {
-            const int row = FULL + pt / P, c = pt % P, a = row / P, b = row % P;
-            float v;
-            if (IN_TILE) {
-                v = src[toff - a * tg.XS - b * tg.ZS - c];
-            } else {
-                int gx = f.x - a; gx += gx < 0 ? K0 : 0;
-                int gy = f.y - b; gy += gy < 0 ? K1 : 0;
-                int gz = f.z - c; gz += gz < 0 ? K2 : 0;
-                v = __ldg(src + ((size_t)gx * K1 + gy) * K2 + gz);
-            }
-            const float tx = r[REC_X + a], ty = r[REC_X + P + b], tz = r[REC_Z + c];
-            const float vz = tz * v;
-            ph = fmaf(tx * ty, vz, ph);
-            if (FORCE) {
-                gx_ = fmaf(r[REC_X + 2 * P + a] * ty, vz, gx_);
-                gy_ = fmaf(tx * r[REC_X + 3 * P + b], vz, gy_);
-                gz_ = fmaf(tx * ty, r[REC_DZ + c] * v, gz_);
-            }
-        }
-    }
+    tile_move<true, FIXED>(tile, grid, tb, tg, inv_scale);
 }
 
 template <int P, bool FORCE, int NT>
@@ -567,26 +499,97 @@ k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
     if (tb.natoms == 0) return;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     tile_move<false>(tile, const_cast<float*>(grid), tb, tg);
-    const float sc_lane = (lane >> 3) == 0 ? -sx : ((lane >> 3) == 1 ? -sy : ((lane >> 3) == 2 ? -sz : 1.f));   // writers: lanes 0/8/16/24
+    // LPA lanes per atom, lane <-> x index a: a lane walks the P x P (y,z) plane of its x index (2 FMAs per
+    // point for the z sums, 3 per row for the y sums, no idle passes), the LPA lanes of an atom are summed
+    // with 4 shuffles, and 32/LPA atoms are in flight per warp.
+    constexpr int LPA = P <= 4 ? 4 : 8, APW = 32 / LPA;
+    const int sub = lane / LPA, a = lane % LPA;
+    const bool hA = lane & (LPA / 2), hB = lane & (LPA / 4);
+    const int comp = (hA ? 2 : 0) + (hB ? 1 : 0);                 // component this lane ends up holding
+    const float sc_lane = comp == 0 ? -sx : (comp == 1 ? -sy : (comp == 2 ? -sz : 1.f));
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
     for (int ch = 0; ch < tb.natoms; ch += TILE_CHUNK(NT)) {
         const int na = min(TILE_CHUNK(NT), tb.natoms - ch);
         __syncthreads();
         tile_chunk_setup<P, NT, FORCE>(ch, na, tb, tg, frac, base, rbeg, rpre, rec, sb, stoff, sidx);
         __syncthreads();
-        for (int at = wid; at < na; at += nw) {
-            const float* r = rec + at * REC_LEN(P);
-            const int toff = stoff[at];
+        for (int at0 = wid * APW; at0 < na; at0 += nw * APW) {
+            const int at = at0 + sub;
             float ph = 0.f, gx_ = 0.f, gy_ = 0.f, gz_ = 0.f;
-            if (toff >= 0) gather_atom<P, FORCE, true>(tile, toff, sb[at], r, tg, lane, ph, gx_, gy_, gz_);
-            else gather_atom<P, FORCE, false>(grid, 0, sb[at], r, tg, lane, ph, gx_, gy_, gz_);
+            if (at < na && a < P) {
+                const float* r = rec + at * REC_LEN(P);
+                float wz[8], dz[8];
+                *(float4*)wz = *(const float4*)(r + REC_Z);
+                *(float4*)(wz + 4) = *(const float4*)(r + REC_Z + 4);
+                if (FORCE) {
+                    *(float4*)dz = *(const float4*)(r + REC_DZ);
+                    *(float4*)(dz + 4) = *(const float4*)(r + REC_DZ + 4);
+                }
+                const int toff = stoff[at];
+                float pa = 0.f, gya = 0.f, gza = 0.f;             // sums over the plane: ty s0, dty s0, ty s1
+                if (toff >= 0) {
+                    const float* plane = tile + (toff - a * tg.XS);
+#pragma unroll
+                    for (int b = 0; b < P; ++b) {
+                        const float* rowp = plane - b * tg.ZS;
+                        float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+                        for (int c = 0; c < P; ++c) {
+                            const float v = rowp[-c];
+                            s0 = fmaf(wz[c], v, s0);
+                            if (FORCE) s1 = fmaf(dz[c], v, s1);
+                        }
+                        const float ty = r[REC_X + P + b];
+                        pa = fmaf(ty, s0, pa);
+                        if (FORCE) {
+                            gya = fmaf(r[REC_X + 3 * P + b], s0, gya);
+                            gza = fmaf(ty, s1, gza);
+                        }
+                    }
+                } else {                                           // footprint outside the window: global grid
+                    const int4 f = sb[at];
+                    int gx = f.x - a; gx += gx < 0 ? K0 : 0;
+                    for (int b = 0; b < P; ++b) {
+                        int gy = f.y - b; gy += gy < 0 ? K1 : 0;
+                        const float* rowp = grid + ((size_t)gx * K1 + gy) * K2;
+                        float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+                        for (int c = 0; c < P; ++c) {
+                            int gz = f.z - c; gz += gz < 0 ? K2 : 0;
+                            const float v = __ldg(rowp + gz);
+                            s0 = fmaf(wz[c], v, s0);
+                            if (FORCE) s1 = fmaf(dz[c], v, s1);
+                        }
+                        const float ty = r[REC_X + P + b];
+                        pa = fmaf(ty, s0, pa);
+                        if (FORCE) {
+                            gya = fmaf(r[REC_X + 3 * P + b], s0, gya);
+                            gza = fmaf(ty, s1, gza);
+                        }
+                    }
+                }
+                const float tx = r[REC_X + a];
+                ph = tx * pa;
+                if (FORCE) {
+                    gx_ = r[REC_X + 2 * P + a] * pa;
+                    gy_ = tx * gya;
+                    gz_ = tx * gza;
+                }
+            }
             if (FORCE) {
-                // lanes 0 / 8 / 16 / 24 end up with the sums of gx / gy / gz / phi: one 16-byte store by four lanes
-                const float v = warp_reduce4(gx_, gy_, gz_, ph, lane);
-                if ((lane & 7) == 0) ((float*)out)[4 * sidx[at] + (lane >> 3)] = sc_lane * v;
+                // four values over LPA lanes: the first two steps halve what a lane carries (comp above)
+                float k0 = hA ? gz_ : gx_, k1 = hA ? ph : gy_;
+                k0 += __shfl_xor_sync(0xffffffffu, hA ? gx_ : gz_, LPA / 2);
+                k1 += __shfl_xor_sync(0xffffffffu, hA ? gy_ : ph, LPA / 2);
+                float k = hB ? k1 : k0;
+                k += __shfl_xor_sync(0xffffffffu, hB ? k0 : k1, LPA / 4);
+#pragma unroll
+                for (int o = LPA / 8; o > 0; o >>= 1) k += __shfl_xor_sync(0xffffffffu, k, o);
+                if ((lane & (LPA / 4 - 1)) == 0 && at < na) ((float*)out)[4 * sidx[at] + comp] = sc_lane * k;
             } else {
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) ph += __shfl_xor_sync(0xffffffffu, ph, o);
-                if (lane == 0) out[sidx[at]] = make_float4(0.f, 0.f, 0.f, ph);
+                for (int o = LPA / 2; o > 0; o >>= 1) ph += __shfl_xor_sync(0xffffffffu, ph, o);
+                if (a == 0 && at < na) out[sidx[at]] = make_float4(0.f, 0.f, 0.f, ph);
             }
         }
     }

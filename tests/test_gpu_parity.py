@@ -233,7 +233,8 @@ def test_full_size_sampled_rows(ctx, k):
     if Q is None:                               # first request only switches the capture on
         ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
         Q = ctx.pme_grid(0, c.grid)
-    assert abs(float(Q.double().sum()) - float(q.astype(np.float64).sum())) < 1e-3
+    # fp32 weights, fp32 grid accumulation: the total is exact to a few ulp of the spread charge sum |q_i|
+    assert abs(float(Q.double().sum()) - float(q.astype(np.float64).sum())) < 2e-7 * float(np.abs(q).sum())
     nl.free()
 
 
