@@ -249,6 +249,7 @@ struct TileGeom {
     int ZS, XS;    // shared-memory strides: element (tx,ty,tz) at tx*XS + ty*ZS + tz
     int M;         // drift margin in grid points
     unsigned T1_magic;   // ceil(2^32 / T[1]): r / T[1] = umulhi(r, T1_magic) for r < 2^16
+    unsigned nvz_magic;  // ceil(2^32 / (T[2]/4)): i / (T[2]/4) = umulhi(i, nvz_magic) for i < T[0] T[1] T[2]/4
 };
 #define TILE_MAXRANGES 16
 #define TILE_CHUNK(NT) ((NT) / 4)
@@ -280,7 +281,7 @@ __device__ __forceinline__ TileBlock tile_block_setup(const TileGeom& tg, const 
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         gc[d] = min(tg.g[d], tg.nc[d] - c0[d]);
-        tb.o[d] = (int)(((long long)c0[d] * tg.K[d]) / tg.nc[d]) - tg.M - (P - 1);
+        tb.o[d] = (int)((unsigned)(c0[d] * tg.K[d]) / (unsigned)tg.nc[d]) - tg.M - (P - 1);    // c0, K < 2^10
     }
     tb.o[2] &= ~3;      // z origin on a float4 boundary (K2 % 4 == 0): the window moves as 16-byte vectors
     const int nr = gc[0] * gc[1];
@@ -349,9 +350,9 @@ __device__ __forceinline__ void tile_chunk_setup(int ch, int na, const TileBlock
     }
 }
 
-// Moves the window between the grid and the tile as float4 vectors: 8 lanes cover 32 z-points of a
-// row, so a warp handles 4 (tx,ty) rows per step.  The z origin and K2 are multiples of 4, so a vector
-// never straddles the periodic boundary; the tile side stays scalar (its row stride is odd).
+// Moves the window between the grid and the tile as float4 vectors.  The z origin and K2 are multiples
+// of 4, so a vector never straddles the periodic boundary; the tile side stays scalar (its row stride is
+// odd).
 // FLUSH: tile -> grid with red.global.add.v4.f32, all-zero vectors skipped; else grid -> tile.
 __device__ __forceinline__ void red_add_v4(float* addr, float4 v)
 {
@@ -362,30 +363,42 @@ template <bool FLUSH, bool FIXED = false>
 __device__ __forceinline__ void tile_move(float* tile, float* grid, const TileBlock& tb, const TileGeom& tg,
                                           float inv_scale = 1.f)
 {
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    // flat index over the window's float4 vectors (z fastest): consecutive threads take consecutive vectors
+    // of a row, TILE_MOVE_U vectors per thread are in flight at once (loads first, then the shared stores)
+    constexpr int U = 4;
     const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
-    const int nrows = tg.T[0] * tg.T[1];
-    const int sub = lane >> 3, z4 = (lane & 7) * 4;
-    for (int r = wid * 4 + sub; r < nrows; r += nw * 4) {
-        const int tx = (int)__umulhi((unsigned)r, tg.T1_magic), ty = r - tx * tg.T[1];
-        const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1);
-        float* trow = tile + tx * tg.XS + ty * tg.ZS;
-        float* grow = grid + ((size_t)gx * K1 + gy) * K2;
-        for (int tz = z4; tz < tg.T[2]; tz += 32) {
-            float* g = grow + wrap1(tb.o[2] + tz, K2);
+    const int nvz = tg.T[2] >> 2;
+    const int nvec = tg.T[0] * tg.T[1] * nvz;
+    for (int i0 = threadIdx.x; i0 < nvec; i0 += blockDim.x * U) {
+        float4 v[U];
+        float* tp[U];
+        float* gp[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int i = min(i0 + u * (int)blockDim.x, nvec - 1);        // clamped: the store is predicated below
+            const int r = (int)__umulhi((unsigned)i, tg.nvz_magic), tz = (i - r * nvz) << 2;
+            const int tx = (int)__umulhi((unsigned)r, tg.T1_magic), ty = r - tx * tg.T[1];
+            const int gx = wrap1(tb.o[0] + tx, K0), gy = wrap1(tb.o[1] + ty, K1), gz = wrap1(tb.o[2] + tz, K2);
+            tp[u] = tile + tx * tg.XS + ty * tg.ZS + tz;
+            gp[u] = grid + ((size_t)(gx * K1 + gy) * K2 + gz);
+            if (!FLUSH) v[u] = __ldg((const float4*)gp[u]);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (i0 + u * (int)blockDim.x >= nvec) break;
+            float* t = tp[u];
             if (FLUSH) {
-                float4 v;
+                float4 w;
                 if (FIXED) {
-                    const int* irow = (const int*)trow;
-                    v = make_float4(inv_scale * (float)irow[tz], inv_scale * (float)irow[tz + 1],
-                                    inv_scale * (float)irow[tz + 2], inv_scale * (float)irow[tz + 3]);
+                    const int* it = (const int*)t;
+                    w = make_float4(inv_scale * (float)it[0], inv_scale * (float)it[1], inv_scale * (float)it[2],
+                                    inv_scale * (float)it[3]);
                 } else {
-                    v = make_float4(trow[tz], trow[tz + 1], trow[tz + 2], trow[tz + 3]);
+                    w = make_float4(t[0], t[1], t[2], t[3]);
                 }
-                if (v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f) red_add_v4(g, v);
+                if (w.x != 0.f || w.y != 0.f || w.z != 0.f || w.w != 0.f) red_add_v4(gp[u], w);
             } else {
-                const float4 v = __ldg((const float4*)g);
-                trow[tz] = v.x; trow[tz + 1] = v.y; trow[tz + 2] = v.z; trow[tz + 3] = v.w;
+                t[0] = v[u].x; t[1] = v[u].y; t[2] = v[u].z; t[3] = v[u].w;
             }
         }
     }
@@ -410,7 +423,8 @@ k_spread_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
     if (tb.natoms == 0) return;
     const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
     const int tsize = tg.XS * tg.T[0];
-    for (int e = threadIdx.x; e < tsize; e += blockDim.x) tile[e] = 0.f;       // 0.f and 0 share a bit pattern
+    for (int e = threadIdx.x; e < (tsize >> 2); e += blockDim.x) ((float4*)tile)[e] = make_float4(0.f, 0.f, 0.f, 0.f);   // 0.f and 0 share a bit pattern
+    if (threadIdx.x < (tsize & 3)) tile[(tsize & ~3) + threadIdx.x] = 0.f;
     float scale = 1.f;
     if (FIXED) {
         __shared__ float s_part[NT / 32];
@@ -700,6 +714,8 @@ static bool plan_tiles(const sqeq_ctx* ctx, const sqeq_nlist* nl, int P, TileGeo
                     if (pass == 0 && groups < want_groups) continue;
                     tg.M = M;
                     tg.T1_magic = (unsigned)((0x100000000ull + tg.T[1] - 1) / tg.T[1]);
+                    tg.nvz_magic = (unsigned)((0x100000000ull + tg.T[2] / 4 - 1) / (tg.T[2] / 4));
+                    if ((uint64_t)tg.T[0] * tg.T[1] * (tg.T[2] / 4) * (tg.T[2] / 4) >= 0x100000000ull) continue;   // magic division exact
                     // strides: smallest padding that puts the 32 rows (a,b) of a full pass in distinct banks
                     const int nrow = (P * P >= 32) ? 32 : 0;
                     int bz = -1, bx = -1;
