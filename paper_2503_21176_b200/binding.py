@@ -58,6 +58,7 @@ def load():
     L.sqeq_nl_export.argtypes = [vp, vp, vp, vp, vp]
     L.sqeq_nl_info.argtypes = [vp, ip, ctypes.POINTER(i64), ip]
     L.sqeq_nl_entry_bytes.argtypes = [vp, ip]
+    L.sqeq_nl_layout.argtypes = [vp, ctypes.POINTER(i64), ip, ip]
     L.sqeq_nl_free.argtypes = [vp]
     L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_enqueue.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
@@ -121,7 +122,11 @@ class NeighbourList:
         self.ctx._check(load().sqeq_nl_info(self.handle, nc, ctypes.byref(nd), ctypes.byref(mr)))
         eb = ctypes.c_int()
         self.ctx._check(load().sqeq_nl_entry_bytes(self.handle, ctypes.byref(eb)))
-        return dict(ncell=list(nc), n_directed=nd.value, max_row=mr.value, entry_bytes=eb.value)
+        ns = ctypes.c_int64()
+        sh, mp = ctypes.c_int(), ctypes.c_int()
+        self.ctx._check(load().sqeq_nl_layout(self.handle, ctypes.byref(ns), ctypes.byref(sh), ctypes.byref(mp)))
+        return dict(ncell=list(nc), n_directed=nd.value, max_row=mr.value, entry_bytes=eb.value,
+                    n_slots=ns.value, entry_shift=sh.value, max_neighbourhood=mp.value)
 
     def export(self):
         """Canonical (i, j, shift) arrays on the device: unique pairs i<j sorted by (i,j)."""

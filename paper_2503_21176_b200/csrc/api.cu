@@ -272,6 +272,15 @@ int sqeq_nl_entry_bytes(const sqeq_nlist* nl, int* bytes)
     return SQEQ_OK;
 }
 
+int sqeq_nl_layout(const sqeq_nlist* nl, int64_t* n_slots, int* entry_shift, int* max_neighbourhood)
+{
+    if (!nl) return SQEQ_EINVAL;
+    if (n_slots) *n_slots = nl->n_slots;
+    if (entry_shift) *entry_shift = nl->lshift;
+    if (max_neighbourhood) *max_neighbourhood = nl->max_pop;
+    return SQEQ_OK;
+}
+
 int sqeq_nl_free(sqeq_nlist* nl)
 {
     if (!nl) return SQEQ_OK;

@@ -373,3 +373,38 @@ def test_global_list_format_and_side_stream(ctx, monkeypatch):
         nl.free()
     finally:
         c2.close()
+
+
+def test_local_list_layouts(ctx):
+    """The 16-bit list: rows padded to whole warps with entries of a far-away dummy slot, entries stored as
+    byte offsets (index << 4) while the largest neighbourhood has fewer than 4095 atoms and as plain indices
+    above that.  Both layouts, rows of length 0 and of an exact multiple of 32, against the oracle."""
+    c = W.CONFIGS[2]
+    pos, q = inputs(2)
+    rows = np.sort(np.random.default_rng(5).choice(len(q), 128, replace=False))
+    seen = set()
+    for rl in (c.r_list, 12.5):                       # 12.5 A: (3 x 12.5 A)^3 x 0.1 atoms/A^3 > 4095 atoms
+        nl = ctx.nl_build(dev(pos), c.box, rl)
+        info = nl.info()
+        assert info["entry_bytes"] == 2
+        assert info["n_slots"] % 32 == 0 and 0 <= info["n_slots"] - info["n_directed"] < 32 * len(q)
+        assert info["entry_shift"] == (4 if info["max_neighbourhood"] <= 4094 else 0)
+        seen.add(info["entry_shift"])
+        check_coulomb(ctx, nl, pos, q, c, rows=rows)
+        nl.free()
+    assert seen == {0, 4}
+    # a cluster whose rows have exactly 32 and 64 neighbours, and two isolated atoms with empty rows
+    rng = np.random.default_rng(6)
+    box = [40.0, 44.0, 48.0]
+    blob33 = 10.0 + rng.uniform(0, 1.5, (33, 3))       # 33 atoms within 2.6 A of each other: rows of 32
+    blob65 = 30.0 + rng.uniform(0, 1.5, (65, 3))       # rows of 64
+    lone = np.array([[20.0, 2.0, 40.0], [2.0, 30.0, 5.0]])
+    p2 = np.concatenate([blob33, blob65, lone]).astype(np.float32)
+    q2 = rng.normal(size=len(p2)).astype(np.float32)
+    nl, m = check_nl_exact(ctx, p2, box, 6.0)
+    assert m == (33 * 32 + 65 * 64) // 2
+    assert nl.info()["n_slots"] == 33 * 32 + 65 * 64
+    phi, F, E = ctx.coulomb(nl, dev(p2), dev(q2), box, 6.0, 0.5, [40, 44, 48], 6)
+    op, oF, oE, _ = oracle.coulomb_pme(p2, q2, box, 6.0, 0.5, [40, 44, 48], 6)
+    assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL and abs(E / oE - 1) < TOL
+    nl.free()
