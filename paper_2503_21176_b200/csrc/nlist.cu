@@ -238,6 +238,9 @@ __device__ __noinline__ bool exact_in_range(const float* __restrict__ pos, int o
 // the kernel keeps counting and the host re-runs it with the now known sizes / the other format.
 #define NL_MAXSEG 96
 #define NL_WARPS 8
+#ifndef NL_BPS
+#define NL_BPS 4
+#endif
 #define NL_SLACK 256      // slots past the last row: the real-space kernel prefetches list entries ahead of its row
 struct NLCounters {
     unsigned long long cursor;     // list slots handed out (fmt 1 rows are padded to whole warps)
@@ -248,7 +251,7 @@ struct NLCounters {
 };
 
 template <bool LOCAL>
-__global__ void __launch_bounds__(NL_WARPS * 32, 5)
+__global__ void __launch_bounds__(NL_WARPS * 32, NL_BPS)
 k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
         const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, int lshift, unsigned long long capacity,
@@ -260,7 +263,8 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
     GroupPiece* pieces = (GroupPiece*)(smem_raw + 32 * sizeof(float4));       // [GRP_MAXPIECE]
     int4* segs_all = (int4*)(pieces + GRP_MAXPIECE);                          // [NL_WARPS][NL_MAXSEG]
     typedef typename std::conditional<LOCAL, uint16_t, uint32_t>::type entry_t;
-    entry_t* stage_all = (entry_t*)(segs_all + NL_WARPS * NL_MAXSEG);          // [NL_WARPS][cap_row] list entries
+    float4* segx_all = (float4*)(segs_all + NL_WARPS * NL_MAXSEG);            // [NL_WARPS][NL_MAXSEG] xi - image shift
+    entry_t* stage_all = (entry_t*)(segx_all + NL_WARPS * NL_MAXSEG);          // [NL_WARPS][cap_row] list entries
     __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
     if (threadIdx.x < 32) {
         int img = threadIdx.x < 27 ? threadIdx.x : 13;
@@ -290,6 +294,7 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
     const int natoms = s_rpre[GRP_G * GRP_G];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     int4* segs = segs_all + wid * NL_MAXSEG;
+    float4* segx = segx_all + wid * NL_MAXSEG;
     entry_t* stage = stage_all + (size_t)wid * cap_row;
     const int np_grp = gi.ncol * 3;
     const unsigned lt = (1u << lane) - 1u;
@@ -343,44 +348,82 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
                 }
             }
         }
-        int incl = nloc;
+        // slots and candidate offsets of the lane's segments: two warp scans (segments, candidates)
+        int incl = nloc, cinc = (loc0.y - loc0.x) + (loc1.y - loc1.x) + (loc2.y - loc2.x);
+        const int clen = cinc;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            int y = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += y;
+            const int y = __shfl_up_sync(0xffffffffu, incl, o), yc = __shfl_up_sync(0xffffffffu, cinc, o);
+            if (lane >= o) { incl += y; cinc += yc; }
         }
         const int nseg = __shfl_sync(0xffffffffu, incl, 31);
+        const int total = __shfl_sync(0xffffffffu, cinc, 31);      // candidates of this atom
         __syncwarp();
         {
-            const int at = incl - nloc;
-            if (nloc > 0) segs[at] = loc0;
-            if (nloc > 1) segs[at + 1] = loc1;
-            if (nloc > 2) segs[at + 2] = loc2;
+            // record: x = first atom - first candidate number (t = c + x), y = one past its last candidate
+            // number, z = image code, w = local-index offset; segx = xi - image shift
+            int at = incl - nloc, cpre = cinc - clen;
+            const int4 loc[3] = {loc0, loc1, loc2};
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+                if (k < nloc) {
+                    const float4 sh = shtab[loc[k].z];
+                    const int len = loc[k].y - loc[k].x;
+                    // (the atom's last segment never ends: lanes past the last candidate stay on it)
+                    segs[at] = make_int4(loc[k].x - cpre, at + 1 == nseg ? 0x7fffffff : cpre + len, loc[k].z, loc[k].w);
+                    segx[at] = make_float4(xi.x - sh.x, xi.y - sh.y, xi.z - sh.z, 0.f);   // d = xj + shift - xi
+                    cpre += len;
+                    ++at;
+                }
         }
         __syncwarp();
 
-        // ---- 2. sweep.  The loop keeps every candidate whose fp32 r2 is below rl2 + band; a lane that saw
-        // one inside the guard band only raises a flag (xq carries 32 padding entries, so the tail of a
-        // segment is loaded unclamped and masked).
+        // ---- 2. sweep over the atom's candidates NUMBERED ACROSS SEGMENTS, 32 per step, so that every step
+        // but the last runs with all lanes busy whatever the segment lengths.  A lane keeps the record of
+        // the segment its candidate number falls in and moves on when the number passes the segment's end.
+        // Every candidate whose fp32 r2 is below rl2 + band is kept; a lane that saw one inside the guard
+        // band only raises a flag (xq carries 32 padding entries, so the tail is loaded unclamped and masked).
         int count = 0;
         bool band_seen = false;
-        for (int sg = 0; sg < nseg; ++sg) {
-            const int4 seg = segs[sg];
-            const float4 sh = shtab[seg.z];
-            const float x0 = xi.x - sh.x, y0 = xi.y - sh.y, z0 = xi.z - sh.z;   // d = xj + shift - xi
-            const int self = seg.z == 13 ? s : -1;
-            const uint32_t codebits = (uint32_t)seg.z << 27;
-#pragma unroll 2
-            for (int t = seg.x + lane; t - lane < seg.y; t += 32) {
-                const float4 xj = __ldg(xq + t);
-                const float dx = xj.x - x0, dy = xj.y - y0, dz = xj.z - z0;
+        uint32_t self_entry = (uint32_t)s | (13u << 27);
+        if (LOCAL) {
+            // local index of the atom itself: its column of the group, zero-image piece
+            const int col = (cx - (gi.c0[0] - gg.w[0])) * gi.ncoly + (cy - (gi.c0[1] - gg.w[1]));
+            const GroupPiece pc = pieces[col * 3 + 1];
+            self_entry = (uint32_t)(s + pc.lbase - pc.gbeg);
+        }
+        if (total > 0) {
+            int sg = 0;
+            int4 cur = segs[0];
+            float4 xs0 = segx[0];
+            // software pipeline: the candidate of the NEXT step is located and its load issued before the
+            // current one is tested, so the L2 latency of xq overlaps the test/compaction of the step before
+            int c = lane;
+            while (c >= cur.y) { ++sg; cur = segs[sg]; xs0 = segx[sg]; }
+            int t = c + cur.x;
+            float4 xj = __ldg(xq + t);
+            for (;;) {
+                const float4 xjc = xj;
+                const float x0 = xs0.x, y0 = xs0.y, z0 = xs0.z;
+                const uint32_t e = LOCAL ? (uint32_t)(t + cur.w) : ((uint32_t)t | ((uint32_t)cur.z << 27));
+                const bool valid = c < total;
+                c += 32;
+                const bool more = c - lane < total;                 // warp-uniform
+                if (more) {
+                    while (c >= cur.y) { ++sg; cur = segs[sg]; xs0 = segx[sg]; }
+                    t = c + cur.x;
+                    xj = __ldg(xq + t);
+                }
+                const float dx = xjc.x - x0, dy = xjc.y - y0, dz = xjc.z - z0;
                 const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                const bool ok = r2 < hi_thr && t < seg.y && t != self;
+                // the entry itself tells the atom from its own zero-image copy
+                const bool ok = r2 < hi_thr && valid && e != self_entry;
                 band_seen |= ok && r2 >= lo_thr;
                 const unsigned m = __ballot_sync(0xffffffffu, ok);
                 const int at = min(count + __popc(m & lt), cap_row - 1);   // an overflowing row is re-run anyway
-                if (ok) stage[at] = LOCAL ? (entry_t)(t + seg.w) : (entry_t)((uint32_t)t | codebits);
+                if (ok) stage[at] = (entry_t)e;
                 count += __popc(m);
+                if (!more) break;
             }
         }
         __syncwarp();
@@ -439,8 +482,24 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         }
         off = __shfl_sync(0xffffffffu, off, 0);
         if (count <= cap_row && off + (unsigned long long)padn <= capacity) {
-            entry_t* dst = (entry_t*)nbr_out + off;
-            for (int k = lane; k < padn; k += 32) dst[k] = (entry_t)((k < count ? stage[k] : (entry_t)gi.pop) << lshift);
+            if (LOCAL) {
+                // pad in the staging row, then move 4 entries per lane (rows and staging rows are 64-byte
+                // aligned); the shift is applied to both halves of a word at once (indices < 4096 when shifted)
+                if (count + lane < padn) stage[count + lane] = (entry_t)gi.pop;
+                __syncwarp();
+                const uint32_t keep = lshift ? 0x0fff0fffu : 0xffffffffu;
+                const uint2* src = (const uint2*)stage;
+                uint2* dst = (uint2*)((entry_t*)nbr_out + off);
+                for (int k = lane; 4 * k < padn; k += 32) {
+                    uint2 w = src[k];
+                    w.x = (w.x & keep) << lshift;
+                    w.y = (w.y & keep) << lshift;
+                    dst[k] = w;
+                }
+            } else {
+                entry_t* dst = (entry_t*)nbr_out + off;
+                for (int k = lane; k < count; k += 32) dst[k] = stage[k];
+            }
         }
         __syncwarp();
     }
@@ -640,7 +699,7 @@ static void fill_group_geom(GroupGeom& gg, const NLGeom& g)
 
 static size_t pairs_smem(int cap_row, bool local)
 {
-    return 32 * sizeof(float4) + GRP_MAXPIECE * sizeof(GroupPiece) + (size_t)NL_WARPS * NL_MAXSEG * sizeof(int4) +
+    return 32 * sizeof(float4) + GRP_MAXPIECE * sizeof(GroupPiece) + (size_t)NL_WARPS * NL_MAXSEG * (sizeof(int4) + sizeof(float4)) +
            (size_t)NL_WARPS * cap_row * (local ? sizeof(uint16_t) : sizeof(uint32_t));
 }
 
