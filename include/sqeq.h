@@ -82,7 +82,7 @@ int  sqeq_nl_info  (const sqeq_nlist* nl, int ncell[3], int64_t* n_directed, int
 int  sqeq_nl_entry_bytes(const sqeq_nlist* nl, int* bytes);
 /* Storage layout of a built list (host outputs, any may be NULL).  n_slots: list slots in use -- the 16-bit
  * format pads every row to a multiple of 32 slots (padding entries point at a far-away dummy atom), so
- * n_slots >= directed entries.  entry_shift: a 16-bit entry is (local index << entry_shift); 4 (byte offset
+ * n_slots >= directed entries (it also counts the unused tail of each cell group's reserved slice).  entry_shift: a 16-bit entry is (local index << entry_shift); 4 (byte offset
  * of a 16-byte staged atom) while the most populous neighbourhood stays below 4095 atoms, else 0.
  * max_neighbourhood: atoms (all periodic images) the staged real-space kernel holds per cell group. */
 int  sqeq_nl_layout(const sqeq_nlist* nl, int64_t* n_slots, int* entry_shift, int* max_neighbourhood);

@@ -38,6 +38,7 @@ struct sqeq_ctx {
     int nl_last_max_row = 0;
     int nl_last_fmt = 1;
     int nl_last_max_pop = 0;
+    int64_t nl_last_pairs = 0;
     bool spread_float = false;            // SQEQ_SPREAD_FLOAT=1: fp32 (CAS) instead of fixed-point shared accumulation
     bool overlap = false;                 // SQEQ_OVERLAP=1: PME on the side stream beside the real-space kernel
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel

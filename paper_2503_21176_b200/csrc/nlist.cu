@@ -254,8 +254,8 @@ template <bool LOCAL>
 __global__ void __launch_bounds__(NL_WARPS * 32, NL_BPS)
 k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
-        const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, int lshift, unsigned long long capacity,
-        NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
+        const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, int lshift, int est_row,
+        unsigned long long capacity, NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
         void* __restrict__ nbr_out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -266,6 +266,8 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
     float4* segx_all = (float4*)(segs_all + NL_WARPS * NL_MAXSEG);            // [NL_WARPS][NL_MAXSEG] xi - image shift
     entry_t* stage_all = (entry_t*)(segx_all + NL_WARPS * NL_MAXSEG);          // [NL_WARPS][cap_row] list entries
     __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    __shared__ unsigned long long s_base, s_pairs;      // the block's reserved slice of the list; its pair count
+    __shared__ int s_used, s_res, s_maxrow;
     if (threadIdx.x < 32) {
         int img = threadIdx.x < 27 ? threadIdx.x : 13;
         shtab[threadIdx.x] = make_float4((img / 9 - 1) * g.Lf[0], ((img / 3) % 3 - 1) * g.Lf[1],
@@ -289,6 +291,15 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         }
         s_rpre[GRP_G * GRP_G] = acc;
         if (LOCAL) atomicMax(&ctr->max_pop, gi.pop);
+        // ONE global reservation per block (est_row slots per atom, a multiple of 32): the rows then take
+        // their slices with a shared-memory counter.  Per-row reservations on the global cursor -- a third
+        // of a million atomics on one address -- were what bounded this kernel.  Rows that do not fit the
+        // estimate fall back to the global cursor; unused slots at the end of a slice stay empty.
+        s_res = acc * est_row;
+        s_base = s_res > 0 ? atomicAdd(&ctr->cursor, (unsigned long long)s_res) : 0ull;
+        s_used = 0;
+        s_maxrow = 0;
+        s_pairs = 0ull;
     }
     __syncthreads();
     const int natoms = s_rpre[GRP_G * GRP_G];
@@ -474,9 +485,11 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int padn = LOCAL ? (count + 31) & ~31 : count;
         unsigned long long off = 0;
         if (lane == 0) {
-            off = atomicAdd(&ctr->cursor, (unsigned long long)padn);
-            atomicAdd(&ctr->pairs, (unsigned long long)count);
-            atomicMax(&ctr->max_row, count);
+            const int old = atomicAdd(&s_used, padn);
+            off = old + padn <= s_res ? s_base + (unsigned long long)old
+                                      : atomicAdd(&ctr->cursor, (unsigned long long)padn);
+            atomicAdd(&s_pairs, (unsigned long long)count);
+            atomicMax(&s_maxrow, count);
             row_start[s] = (int64_t)off;
             row_len[s] = count;
         }
@@ -502,6 +515,11 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
             }
         }
         __syncwarp();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && natoms > 0) {
+        atomicAdd(&ctr->pairs, s_pairs);
+        atomicMax(&ctr->max_row, s_maxrow);
     }
 }
 
@@ -704,18 +722,18 @@ static size_t pairs_smem(int cap_row, bool local)
 }
 
 static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, bool local,
-                        int lshift, int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
+                        int lshift, int est_row, int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
 {
     const size_t smem = pairs_smem(cap_row, local);
     const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
     if (local) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<true><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-            nl->perm, pos, g, nl->gg, cap_row, lshift, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+            nl->perm, pos, g, nl->gg, cap_row, lshift, est_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
     } else {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<false><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-            nl->perm, pos, g, nl->gg, cap_row, lshift, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+            nl->perm, pos, g, nl->gg, cap_row, lshift, est_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
     }
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
@@ -802,13 +820,17 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         const double mean_row = 4.0 / 3.0 * M_PI * cutoff * cutoff * cutoff * (double)n / vol;
         size_t capacity;
         int cap_row;
+        int est_row;                   // slots a block reserves per atom (k_pairs), a multiple of 32
         if (ctx->nl_last_n == n && ctx->nl_last_total > 0) {
             capacity = (size_t)(1.08 * (double)ctx->nl_last_total) + 4096;
             cap_row = (int)(1.2 * ctx->nl_last_max_row) + 32;
+            est_row = (int)(1.06 * (double)ctx->nl_last_pairs / (double)n) + 32;
         } else {
-            capacity = (size_t)(1.2 * mean_row * (double)n) + 64 * (size_t)n + 4096;
+            capacity = (size_t)(1.3 * mean_row * (double)n) + 128 * (size_t)n + 4096;
             cap_row = (int)(1.5 * mean_row) + 128;
+            est_row = (int)(1.1 * mean_row) + 48;
         }
+        est_row = (est_row + 31) & ~31;
         cap_row = (cap_row + 31) & ~31;
         NLCounters* h = (NLCounters*)ctx->h_nl;                    // pinned: result, init image, bin flag
         NLCounters* hinit = h + 1;
@@ -831,7 +853,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
             init.ex.rl2 = g.rl2;
             *hinit = init;
             NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
-            NL_TRY(launch_pairs(ctx, nl, pos, g, local, local ? lshift : 0, cap_row, capacity, ctr, st));
+            NL_TRY(launch_pairs(ctx, nl, pos, g, local, local ? lshift : 0, est_row, cap_row, capacity, ctr, st));
             t_launch = now_ms();
             NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -865,6 +887,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         nl->max_row = h->max_row;
         ctx->nl_last_n = n;
         ctx->nl_last_total = nl->n_slots;
+        ctx->nl_last_pairs = nl->n_directed;
         ctx->nl_last_max_row = nl->max_row;
     }
     *out = nl;

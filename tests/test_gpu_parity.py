@@ -387,7 +387,7 @@ def test_local_list_layouts(ctx):
         nl = ctx.nl_build(dev(pos), c.box, rl)
         info = nl.info()
         assert info["entry_bytes"] == 2
-        assert info["n_slots"] % 32 == 0 and 0 <= info["n_slots"] - info["n_directed"] < 32 * len(q)
+        assert info["n_slots"] % 32 == 0 and info["n_slots"] >= info["n_directed"]     # padding + unused reservations
         assert info["entry_shift"] == (4 if info["max_neighbourhood"] <= 4094 else 0)
         seen.add(info["entry_shift"])
         check_coulomb(ctx, nl, pos, q, c, rows=rows)
@@ -403,7 +403,7 @@ def test_local_list_layouts(ctx):
     q2 = rng.normal(size=len(p2)).astype(np.float32)
     nl, m = check_nl_exact(ctx, p2, box, 6.0)
     assert m == (33 * 32 + 65 * 64) // 2
-    assert nl.info()["n_slots"] == 33 * 32 + 65 * 64
+    assert nl.info()["n_slots"] >= 33 * 32 + 65 * 64 and nl.info()["n_slots"] % 32 == 0
     phi, F, E = ctx.coulomb(nl, dev(p2), dev(q2), box, 6.0, 0.5, [40, 44, 48], 6)
     op, oF, oE, _ = oracle.coulomb_pme(p2, q2, box, 6.0, 0.5, [40, 44, 48], 6)
     assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL and abs(E / oE - 1) < TOL
