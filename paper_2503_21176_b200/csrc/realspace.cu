@@ -191,14 +191,6 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
 #ifndef REAL_BPS
 #define REAL_BPS 4          // blocks per SM the register budget is set for
 #endif
-#ifndef REAL_UNROLL
-#define REAL_UNROLL 4
-#endif
-#define REAL_PRAGMA_(x) _Pragma(#x)
-#define REAL_PRAGMA_UNROLL(n) REAL_PRAGMA_(unroll n)
-#ifndef REAL_PF
-#define REAL_PF 0           // list entries are loaded this many 32-pair steps ahead of their use
-#endif
 __device__ __forceinline__ float4 lds128(unsigned addr)
 {
     float4 v;
@@ -256,23 +248,13 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
         const int s = ia + s_roff[(ia >= p1) + (ia >= p2) + (ia >= p3)];
         const float4 xi = __ldg(xq + s);
         // rows are padded to whole 32-entry steps (the padding points at the dummy slot), so the loop is
-        // uniform over the warp; entries are fetched REAL_PF steps ahead (the list buffer carries slack
-        // for the look-ahead past the last row), which takes the DRAM latency of the list stream off the
-        // critical path
+        // uniform over the warp
         const uint16_t* __restrict__ row = nbr + row_start[s] + lane;
         const int nst = (row_len[s] + 31) >> 5;
         const unsigned xs_addr = (unsigned)__cvta_generic_to_shared(xs);
-        unsigned e[REAL_PF + 1];
-#pragma unroll
-        for (int k = 0; k < REAL_PF; ++k) e[k] = __ldg(row + 32 * k);
-        row += 32 * REAL_PF;
         float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
-REAL_PRAGMA_UNROLL(REAL_UNROLL)
-        for (int it = 0; it < nst; ++it) {
-            e[REAL_PF] = __ldg(row + 32 * it);
-            const float4 xj = SCALED ? lds128(xs_addr + e[0]) : xs[e[0]];
-#pragma unroll
-            for (int k = 0; k < REAL_PF; ++k) e[k] = e[k + 1];
+        auto pair = [&](unsigned e) {
+            const float4 xj = SCALED ? lds128(xs_addr + e) : xs[e];
             const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float qj = r2 < p.rc2 ? xj.w : 0.f;
@@ -286,7 +268,15 @@ REAL_PRAGMA_UNROLL(REAL_UNROLL)
                 fy = fmaf(gq, dy, fy);
                 fz = fmaf(gq, dz, fz);
             }
+        };
+        // four entry loads in flight ahead of the four pair evaluations that use them
+        int it = 0;
+        for (; it + 4 <= nst; it += 4) {
+            const unsigned e0 = __ldg(row + 32 * it), e1 = __ldg(row + 32 * it + 32), e2 = __ldg(row + 32 * it + 64),
+                           e3 = __ldg(row + 32 * it + 96);
+            pair(e0); pair(e1); pair(e2); pair(e3);
         }
+        for (; it < nst; ++it) pair(__ldg(row + 32 * it));
         if (FORCE) {
             const float v = warp_reduce4(fx, fy, fz, phi, lane);        // lanes 0 / 8 / 16 / 24: fx / fy / fz / phi
             if ((lane & 7) == 0) ((float*)(out + s))[lane >> 3] = v;
