@@ -188,8 +188,17 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
 #ifndef REAL_NT
 #define REAL_NT 512
 #endif
-#ifndef REAL_BPS
-#define REAL_BPS 4          // blocks per SM the register budget is set for
+#ifndef REAL_BATCH_F
+#define REAL_BATCH_F 8      // entry loads in flight, force kernel
+#endif
+#ifndef REAL_BATCH_P
+#define REAL_BATCH_P 16     // entry loads in flight, potential-only kernel
+#endif
+#ifndef REAL_BPS_F
+#define REAL_BPS_F 3        // blocks per SM the register budget is set for, force kernel
+#endif
+#ifndef REAL_BPS_P
+#define REAL_BPS_P 4        // ... potential-only kernel
 #endif
 __device__ __forceinline__ float4 lds128(unsigned addr)
 {
@@ -200,7 +209,7 @@ __device__ __forceinline__ float4 lds128(unsigned addr)
 
 // SCALED: the list entries are byte offsets into the staged array (local index * 16, nl->lshift = 4)
 template <bool FORCE, bool SCALED>
-__global__ void __launch_bounds__(REAL_NT, REAL_BPS)
+__global__ void __launch_bounds__(REAL_NT, FORCE ? REAL_BPS_F : REAL_BPS_P)
 k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
               const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
               const uint16_t* __restrict__ nbr, RealParams p, float4* __restrict__ out)
@@ -270,7 +279,27 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
             }
         };
         // four entry loads in flight ahead of the four pair evaluations that use them
+        // the entry loads of B steps are issued together ahead of the B pair evaluations that use them
+        // (B = 16/8/4 while the row lasts): the potential-only kernel has registers for 16 in flight, the
+        // force kernel for 4
+        constexpr int BMAX = FORCE ? REAL_BATCH_F : REAL_BATCH_P;
         int it = 0;
+        if (BMAX >= 16)
+            for (; it + 16 <= nst; it += 16) {
+                unsigned e[16];
+#pragma unroll
+                for (int k = 0; k < 16; ++k) e[k] = __ldg(row + 32 * (it + k));
+#pragma unroll
+                for (int k = 0; k < 16; ++k) pair(e[k]);
+            }
+        if (BMAX >= 8)
+            for (; it + 8 <= nst; it += 8) {
+                unsigned e[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) e[k] = __ldg(row + 32 * (it + k));
+#pragma unroll
+                for (int k = 0; k < 8; ++k) pair(e[k]);
+            }
         for (; it + 4 <= nst; it += 4) {
             const unsigned e0 = __ldg(row + 32 * it), e1 = __ldg(row + 32 * it + 32), e2 = __ldg(row + 32 * it + 64),
                            e3 = __ldg(row + 32 * it + 96);
