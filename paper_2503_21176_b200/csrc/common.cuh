@@ -103,6 +103,7 @@ struct sqeq_nlist {
     char4*    wrapc = nullptr;       // [n]   floor(x/L) per axis at build time (sorted order)
     int64_t*  row_start = nullptr;   // [n]   offset of row s in nbr (rows in no particular order; fmt 1: multiples of 32)
     int*      row_len = nullptr;     // [n]   entries of row s
+    longlong2* grp_slice = nullptr;  // [cell groups] (first slot, slots used) of the group's reserved slice of nbr
     void*     nbr = nullptr;         // [>= n_slots] entries: fmt 0: uint32 j (27 bits) | image code << 27;
                                      //                          fmt 1: uint16 local index in the group's neighbourhood
     int       fmt = 0;

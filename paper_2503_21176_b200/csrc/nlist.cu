@@ -255,8 +255,8 @@ __global__ void __launch_bounds__(NL_WARPS * 32, NL_BPS)
 k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         const int* __restrict__ cell_start, const int* __restrict__ perm,
         const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, int lshift, int est_row,
-        unsigned long long capacity, NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start, int* __restrict__ row_len,
-        void* __restrict__ nbr_out)
+        unsigned long long capacity, NLCounters* __restrict__ ctr, int64_t* __restrict__ row_start,
+        int* __restrict__ row_len, longlong2* __restrict__ grp_slice, void* __restrict__ nbr_out)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* shtab = (float4*)smem_raw;                                        // [32] image shift vectors
@@ -517,9 +517,13 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
         __syncwarp();
     }
     __syncthreads();
-    if (threadIdx.x == 0 && natoms > 0) {
-        atomicAdd(&ctr->pairs, s_pairs);
-        atomicMax(&ctr->max_row, s_maxrow);
+    if (threadIdx.x == 0) {
+        if (natoms > 0) {
+            atomicAdd(&ctr->pairs, s_pairs);
+            atomicMax(&ctr->max_row, s_maxrow);
+        }
+        // where the group's rows are (those that fitted the reservation): the real-space kernel prefetches it
+        grp_slice[blockIdx.x] = make_longlong2((long long)s_base, (long long)min(s_used, s_res));
     }
 }
 
@@ -700,7 +704,7 @@ static int pool_alloc(sqeq_ctx* ctx, void** p, size_t bytes)
 void nl_release(sqeq_nlist* nl)
 {
     cudaStream_t st = nl->ctx->stream;
-    void* ptrs[] = {nl->perm, nl->cell_of, nl->cell_start, nl->wrapc, nl->row_start, nl->row_len, nl->nbr};
+    void* ptrs[] = {nl->perm, nl->cell_of, nl->cell_start, nl->wrapc, nl->row_start, nl->row_len, nl->grp_slice, nl->nbr};
     for (void* p : ptrs)
         if (p) cudaFreeAsync(p, st);     // stream-ordered: safe after every evaluation already enqueued
     delete nl;
@@ -729,11 +733,11 @@ static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const N
     if (local) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<true><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-            nl->perm, pos, g, nl->gg, cap_row, lshift, est_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+            nl->perm, pos, g, nl->gg, cap_row, lshift, est_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->grp_slice, nl->nbr);
     } else {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<false><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-            nl->perm, pos, g, nl->gg, cap_row, lshift, est_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->nbr);
+            nl->perm, pos, g, nl->gg, cap_row, lshift, est_row, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->grp_slice, nl->nbr);
     }
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
@@ -784,6 +788,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     NL_TRY(pool_alloc(ctx, (void**)&nl->wrapc, sizeof(char4) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_start, sizeof(int64_t) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_len, sizeof(int) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->grp_slice, sizeof(longlong2) * (size_t)nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2]));
     NL_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * (n + 32)));     // 32 padding entries: see k_pairs
     float4* xq = (float4*)ctx->xq.p;
     NL_CUDA(cudaMemsetAsync(xq + n, 0x7f, sizeof(float4) * 32, st));    // 3.4e38: far from everything

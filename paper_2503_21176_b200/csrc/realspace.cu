@@ -212,9 +212,19 @@ template <bool FORCE, bool SCALED>
 __global__ void __launch_bounds__(REAL_NT, FORCE ? REAL_BPS_F : REAL_BPS_P)
 k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
               const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
-              const uint16_t* __restrict__ nbr, RealParams p, float4* __restrict__ out)
+              const uint16_t* __restrict__ nbr, const longlong2* __restrict__ grp_slice, RealParams p,
+              float4* __restrict__ out)
 {
     extern __shared__ __align__(16) float4 xs[];               // [neighbourhood population + 1]
+    {
+        // the group's rows sit in one contiguous slice of the list (k_pairs reserves it per group): ask for it
+        // in L2 now, so that the entry loads below meet L2 latency instead of DRAM latency
+        const longlong2 sl = grp_slice[blockIdx.x];
+        const char* base = (const char*)(nbr + sl.x);
+        const long long bytes = sl.y * (long long)sizeof(uint16_t);
+        for (long long o = (long long)threadIdx.x * 128; o < bytes; o += (long long)REAL_NT * 128)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(base + o));
+    }
     __shared__ GroupPiece pieces[GRP_MAXPIECE];
     __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
     const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
@@ -337,7 +347,7 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
                                : (want_force ? k_real_staged<true, false> : k_real_staged<false, false>);
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         kern<<<ngroups, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, nl->row_len,
-                                         (const uint16_t*)nl->nbr, p, (float4*)ctx->real_out.p);
+                                         (const uint16_t*)nl->nbr, nl->grp_slice, p, (float4*)ctx->real_out.p);
     } else if (want_force)
         k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, (const uint32_t*)nl->nbr, p,
                                           (float4*)ctx->real_out.p);
