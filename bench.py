@@ -324,9 +324,9 @@ def run_ours(args, cfg):
                 "note": "%d B x directed list entries + 32 B x atoms for the real-space kernel; ms_avg from CUDA "
                         "events on the launching stream over the timed region; the kernel is instruction-issue "
                         "bound (DESIGN.md section 7), see roofline_alu" % EB}
-    # ALU view of the same kernel: 43 FP32 flops per list entry (FMA = 2) against
+    # ALU view of the same kernel: 41 FP32 flops per list entry (38 FP32 + 3 MUFU) (FMA = 2) against
     # 148 SMs x 128 lanes x 2 x max SM clock
-    flops = 43.0 * P
+    flops = 41.0 * P
     fp32_peak = 148 * 128 * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
     roofline_alu = {"kernel": dom, "bound": "alu", "achieved": round(flops / (kernels[dom]["ms_avg"] * 1e-3) / 1e12, 2),
                     "peak": round(fp32_peak, 1), "unit": "TFLOP/s",
