@@ -250,6 +250,19 @@ struct NLCounters {
     NLExact ex;
 };
 
+__device__ __forceinline__ int4 lds_int4(unsigned addr)
+{
+    int4 v;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float4 lds_float4(unsigned addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 template <bool LOCAL>
 __global__ void __launch_bounds__(NL_WARPS * 32, NL_BPS)
 k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
@@ -404,37 +417,30 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
             self_entry = (uint32_t)(s + pc.lbase - pc.gbeg);
         }
         if (total > 0) {
-            int sg = 0;
-            int4 cur = segs[0];
-            float4 xs0 = segx[0];
-            // software pipeline: the candidate of the NEXT step is located and its load issued before the
-            // current one is tested, so the L2 latency of xq overlaps the test/compaction of the step before
-            int c = lane;
-            while (c >= cur.y) { ++sg; cur = segs[sg]; xs0 = segx[sg]; }
-            int t = c + cur.x;
-            float4 xj = __ldg(xq + t);
-            for (;;) {
-                const float4 xjc = xj;
-                const float x0 = xs0.x, y0 = xs0.y, z0 = xs0.z;
-                const uint32_t e = LOCAL ? (uint32_t)(t + cur.w) : ((uint32_t)t | ((uint32_t)cur.z << 27));
-                const bool valid = c < total;
-                c += 32;
-                const bool more = c - lane < total;                 // warp-uniform
-                if (more) {
-                    while (c >= cur.y) { ++sg; cur = segs[sg]; xs0 = segx[sg]; }
-                    t = c + cur.x;
-                    xj = __ldg(xq + t);
+            // the lane's current segment record, addressed by its 32-bit shared address (one add per advance)
+            unsigned sa = (unsigned)__cvta_generic_to_shared(segs);
+            constexpr unsigned SEGX = NL_WARPS * NL_MAXSEG * sizeof(int4);      // segx_all - segs_all, bytes
+            int4 cur = lds_int4(sa);
+            float4 xs0 = lds_float4(sa + SEGX);
+#pragma unroll 2
+            for (int c = lane; c - lane < total; c += 32) {
+                while (c >= cur.y) {
+                    sa += sizeof(int4);
+                    cur = lds_int4(sa);
+                    xs0 = lds_float4(sa + SEGX);
                 }
-                const float dx = xjc.x - x0, dy = xjc.y - y0, dz = xjc.z - z0;
+                const int t = c + cur.x;
+                const float4 xj = __ldg(xq + t);
+                const float dx = xj.x - xs0.x, dy = xj.y - xs0.y, dz = xj.z - xs0.z;
                 const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                 // the entry itself tells the atom from its own zero-image copy
-                const bool ok = r2 < hi_thr && valid && e != self_entry;
+                const uint32_t e = LOCAL ? (uint32_t)(t + cur.w) : ((uint32_t)t | ((uint32_t)cur.z << 27));
+                const bool ok = r2 < hi_thr && c < total && e != self_entry;
                 band_seen |= ok && r2 >= lo_thr;
                 const unsigned m = __ballot_sync(0xffffffffu, ok);
                 const int at = min(count + __popc(m & lt), cap_row - 1);   // an overflowing row is re-run anyway
                 if (ok) stage[at] = (entry_t)e;
                 count += __popc(m);
-                if (!more) break;
             }
         }
         __syncwarp();
