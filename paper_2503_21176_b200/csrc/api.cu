@@ -146,6 +146,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
     for (auto& b : ctx->stage) if (b.p) cudaFree(b.p);
     if (ctx->h_scal) cudaFreeHost(ctx->h_scal);
     if (ctx->h_nl) cudaFreeHost(ctx->h_nl);
+    if (ctx->h_kry) cudaFreeHost(ctx->h_kry);
     for (auto& r : ctx->pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto& e : ctx->free_events) cudaEventDestroy(e);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);

@@ -161,6 +161,41 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
     if (bnorm == 0.0) { converged = true; relres = 0.0; }
     bool first_cycle = true;
     std::vector<double> H((size_t)(m + 1) * m), cs(m), sn(m), gvec(m + 1), y(m);
+    // Column j of the Hessenberg matrix from the coefficients of iteration j (hc), its Givens rotation and the
+    // residual estimate; true when the cycle ends at this column (converged or exact breakdown).
+    const size_t HL = (size_t)2 * (m + 2) + 1;
+    auto process_column = [&](int j, const double* hc) {
+        double* Hj = H.data() + (size_t)j * (m + 1);
+        for (int k = 0; k <= j; ++k) Hj[k] = hc[k] + hc[(m + 2) + k];
+        Hj[j + 1] = sqrt(hc[2 * (m + 2)]);
+        for (int k = 0; k < j; ++k) {
+            double t = cs[k] * Hj[k] + sn[k] * Hj[k + 1];
+            Hj[k + 1] = -sn[k] * Hj[k] + cs[k] * Hj[k + 1];
+            Hj[k] = t;
+        }
+        double a = Hj[j], b = Hj[j + 1], rr = hypot(a, b);
+        cs[j] = rr > 0 ? a / rr : 1.0;
+        sn[j] = rr > 0 ? b / rr : 0.0;
+        Hj[j] = rr;
+        Hj[j + 1] = 0.0;
+        gvec[j + 1] = -sn[j] * gvec[j];
+        gvec[j] = cs[j] * gvec[j];
+        relres = fabs(gvec[j + 1]) / bnorm;
+        if (relres <= tol || b == 0.0) { converged = relres <= tol; return true; }
+        return false;
+    };
+    // tol <= 0 asks for a FIXED number of iterations (the rank-m updates of Eq. 27, timed Krylov loops): the
+    // host has nothing to decide between iterations, so the coefficients of every iteration are copied to
+    // pinned memory without synchronising and the columns are processed after the cycle -- the GPU never
+    // waits for the host to launch the next iteration.
+    const bool deferred = tol <= 0.0;
+    if (deferred && ctx->h_kry_cap < HL * (size_t)m) {
+        if (ctx->h_kry) cudaFreeHost(ctx->h_kry);
+        ctx->h_kry = nullptr;
+        ctx->h_kry_cap = 0;
+        CUDA_TRY(ctx, cudaMallocHost((void**)&ctx->h_kry, sizeof(double) * HL * (size_t)m));
+        ctx->h_kry_cap = HL * (size_t)m;
+    }
     while (!converged && iters < max_iter) {
         // r = b - A x  (x = 0 in the first cycle: r = b, already in w)
         double beta = bnorm;
@@ -208,28 +243,21 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
                 KERNEL_CHECK(ctx);
                 k_normalise<<<nbl, 256, 0, st>>>(len, w, nrm2, V + (int64_t)(j + 1) * ld);
                 KERNEL_CHECK(ctx);
-                CUDA_TRY(ctx, cudaMemcpyAsync(hh.data(), h, sizeof(double) * (2 * (m + 2) + 1),
-                                              cudaMemcpyDeviceToHost, st));
-                CUDA_TRY(ctx, cudaStreamSynchronize(st));
+                if (deferred) {
+                    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_kry + HL * (size_t)j, h, sizeof(double) * HL,
+                                                  cudaMemcpyDeviceToHost, st));
+                } else {
+                    CUDA_TRY(ctx, cudaMemcpyAsync(hh.data(), h, sizeof(double) * HL, cudaMemcpyDeviceToHost, st));
+                    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+                }
             }
-            // Hessenberg column j (column-major, leading dimension m+1)
-            double* Hj = H.data() + (size_t)j * (m + 1);
-            for (int k = 0; k <= j; ++k) Hj[k] = hh[k] + hh[(m + 2) + k];
-            Hj[j + 1] = sqrt(hh[2 * (m + 2)]);
-            for (int k = 0; k < j; ++k) {
-                double t = cs[k] * Hj[k] + sn[k] * Hj[k + 1];
-                Hj[k + 1] = -sn[k] * Hj[k] + cs[k] * Hj[k + 1];
-                Hj[k] = t;
-            }
-            double a = Hj[j], b = Hj[j + 1], rr = hypot(a, b);
-            cs[j] = rr > 0 ? a / rr : 1.0;
-            sn[j] = rr > 0 ? b / rr : 0.0;
-            Hj[j] = rr;
-            Hj[j + 1] = 0.0;
-            gvec[j + 1] = -sn[j] * gvec[j];
-            gvec[j] = cs[j] * gvec[j];
-            relres = fabs(gvec[j + 1]) / bnorm;
-            if (relres <= tol || b == 0.0) { ++j; converged = relres <= tol; break; }
+            if (!deferred && process_column(j, hh.data())) { ++j; break; }
+        }
+        if (deferred) {
+            CUDA_TRY(ctx, cudaStreamSynchronize(st));
+            const int done = j;
+            for (j = 0; j < done; ++j)
+                if (process_column(j, ctx->h_kry + HL * (size_t)j)) { ++j; break; }     // exact breakdown: stop there
         }
         // y = R^{-1} g ;  x += V y
         const int k = j;
