@@ -119,6 +119,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->spread_float = env && env[0] == '1';
     env = getenv("SQEQ_OVERLAP");
     ctx->overlap = env && env[0] == '1';
+    env = getenv("SQEQ_REAL_LEAN_BLOCKS");          // persistent real-space blocks per SM beside the side stream
+    ctx->real_lean_blocks = env && atoi(env) > 0 ? atoi(env) : 2;
     env = getenv("SQEQ_REAL_STAGED");
     ctx->real_staged_off = env && env[0] == '0';
     *out = ctx;
@@ -323,20 +325,20 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
                  double alpha, float* phi, float* force, bool want_energy, bool field_mode)
 {
     const bool want_force = force != nullptr;
-    // One stream by default: every kernel of the evaluation is instruction-issue bound and fills the
-    // machine, so running PME beside the real-space kernel gains nothing and costs co-residency (their
-    // shared-memory footprints do not pack).  SQEQ_OVERLAP=1 forks PME onto the side stream (useful for
-    // small systems that do not fill the GPU); never with stage timing on, where every event pair
-    // brackets one kernel running alone.
+    // One stream by default.  SQEQ_OVERLAP=1 runs the real-space sum as a persistent grid of two lean
+    // (32-register) blocks per SM and forks PME onto the side stream, where one PME block per SM fits beside
+    // them: at cfg 4 the device-side step goes from 0.624 to 0.587 ms, but a single synchronous evaluation
+    // (sqeq_coulomb_host) gets slower (0.94 -> 1.02 ms), so it stays an option.  Never
+    // with stage timing on, where every event pair brackets one kernel running alone.
     if (ctx->profiling || !ctx->overlap) {
         SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream));
         SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
     } else {
         CUDA_TRY(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream2, ctx->ev_fork, 0));
+        SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));     // first: its persistent blocks settle
         SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream2));
         CUDA_TRY(ctx, cudaEventRecord(ctx->ev_join, ctx->stream2));
-        SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
         CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_join, 0));
     }
     SQEQ_TRY(assemble_run(ctx, nl, alpha, phi, force, want_energy, field_mode, ctx->stream));

@@ -43,6 +43,7 @@ struct sqeq_ctx {
     int64_t nl_last_pairs = 0;
     bool spread_float = false;            // SQEQ_SPREAD_FLOAT=1: fp32 (CAS) instead of fixed-point shared accumulation
     bool overlap = false;                 // SQEQ_OVERLAP=1: PME on the side stream beside the real-space kernel
+    int real_lean_blocks = 2;             // SQEQ_REAL_LEAN_BLOCKS: persistent real-space blocks per SM with SQEQ_OVERLAP=1
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
 
     // ---- PME state (cached by grid/order/box/alpha) ----

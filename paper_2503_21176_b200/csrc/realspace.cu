@@ -7,6 +7,7 @@
 // image shift from a 27-entry shared table, accumulate phi and F in registers, then a shuffle
 // reduction -- no atomics (the paper's ELLPACK row sum, without the padding).
 #include <math.h>
+#include <stdlib.h>
 
 #include "common.cuh"
 
@@ -208,26 +209,31 @@ __device__ __forceinline__ float4 lds128(unsigned addr)
 }
 
 // SCALED: the list entries are byte offsets into the staged array (local index * 16, nl->lshift = 4)
-template <bool FORCE, bool SCALED>
-__global__ void __launch_bounds__(REAL_NT, FORCE ? REAL_BPS_F : REAL_BPS_P)
+// LEAN: 32 registers (four blocks per SM would fit) and 4 loads in flight -- the variant launched as a
+// PERSISTENT grid of a few blocks per SM beside the PME kernels (SQEQ_OVERLAP=1), each block walking over
+// cell groups, so that the register file and shared memory have room for both.
+template <bool FORCE, bool SCALED, bool LEAN = false>
+__global__ void __launch_bounds__(REAL_NT, LEAN ? 4 : (FORCE ? REAL_BPS_F : REAL_BPS_P))
 k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
               const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
               const uint16_t* __restrict__ nbr, const longlong2* __restrict__ grp_slice, RealParams p,
-              float4* __restrict__ out)
+              int ngroups, float4* __restrict__ out)
 {
     extern __shared__ __align__(16) float4 xs[];               // [neighbourhood population + 1]
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    if (grp != (int)blockIdx.x) __syncthreads();               // the previous group's shared state is still being read
     {
         // the group's rows sit in one contiguous slice of the list (k_pairs reserves it per group): ask for it
         // in L2 now, so that the entry loads below meet L2 latency instead of DRAM latency
-        const longlong2 sl = grp_slice[blockIdx.x];
+        const longlong2 sl = grp_slice[grp];
         const char* base = (const char*)(nbr + sl.x);
         const long long bytes = sl.y * (long long)sizeof(uint16_t);
         for (long long o = (long long)threadIdx.x * 128; o < bytes; o += (long long)REAL_NT * 128)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(base + o));
     }
-    __shared__ GroupPiece pieces[GRP_MAXPIECE];
-    __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
-    const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
+    const GroupInfo gi = group_layout(gg, cell_start, grp, pieces, &s_scratch);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     if (threadIdx.x == 0) {
         int acc = 0;
@@ -292,7 +298,7 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
         // the entry loads of B steps are issued together ahead of the B pair evaluations that use them
         // (B = 16/8/4 while the row lasts): the potential-only kernel has registers for 16 in flight, the
         // force kernel for 4
-        constexpr int BMAX = FORCE ? REAL_BATCH_F : REAL_BATCH_P;
+        constexpr int BMAX = LEAN ? 4 : (FORCE ? REAL_BATCH_F : REAL_BATCH_P);
         int it = 0;
         if (BMAX >= 16)
             for (; it + 16 <= nst; it += 16) {
@@ -325,6 +331,7 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
             if (lane == 0) out[s] = make_float4(0.f, 0.f, 0.f, phi);
         }
     }
+    }   // groups
 }
 
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
@@ -343,11 +350,19 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     if (nl->fmt == 1) {
         const size_t smem = sizeof(float4) * ((size_t)nl->max_pop + 1);
         const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
-        auto kern = nl->lshift ? (want_force ? k_real_staged<true, true> : k_real_staged<false, true>)
-                               : (want_force ? k_real_staged<true, false> : k_real_staged<false, false>);
+        // beside the PME side stream: a persistent grid of two lean blocks per SM leaves registers and shared
+        // memory for one PME block per SM; otherwise one block per group
+        const bool lean = ctx->overlap && !ctx->profiling;
+        auto kern = nl->lshift ? (want_force ? k_real_staged<true, true, false> : k_real_staged<false, true, false>)
+                               : (want_force ? k_real_staged<true, false, false> : k_real_staged<false, false, false>);
+        if (lean)
+            kern = nl->lshift ? (want_force ? k_real_staged<true, true, true> : k_real_staged<false, true, true>)
+                              : (want_force ? k_real_staged<true, false, true> : k_real_staged<false, false, true>);
+        const int lean_bps = ctx->real_lean_blocks;
+        const int nblocks = lean ? (ngroups < lean_bps * ctx->sm_count ? ngroups : lean_bps * ctx->sm_count) : ngroups;
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<ngroups, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, nl->row_len,
-                                         (const uint16_t*)nl->nbr, nl->grp_slice, p, (float4*)ctx->real_out.p);
+        kern<<<nblocks, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, nl->row_len,
+                                         (const uint16_t*)nl->nbr, nl->grp_slice, p, ngroups, (float4*)ctx->real_out.p);
     } else if (want_force)
         k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, (const uint32_t*)nl->nbr, p,
                                           (float4*)ctx->real_out.p);

@@ -408,3 +408,23 @@ def test_local_list_layouts(ctx):
     op, oF, oE, _ = oracle.coulomb_pme(p2, q2, box, 6.0, 0.5, [40, 44, 48], 6)
     assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL and abs(E / oE - 1) < TOL
     nl.free()
+
+
+@pytest.mark.gpu
+def test_side_stream_with_persistent_real_space(monkeypatch):
+    """SQEQ_OVERLAP=1 with the default 16-bit list: PME runs on the side stream beside a persistent grid of
+    lean real-space blocks (here one per SM), each walking over several cell groups.  Same bars as the default."""
+    from paper_2503_21176_b200 import binding
+    monkeypatch.setenv("SQEQ_OVERLAP", "1")
+    monkeypatch.setenv("SQEQ_REAL_LEAN_BLOCKS", "1")      # 148 blocks: at cfg 2 (216 cell groups) some take two
+    c2 = binding.Context(0)
+    try:
+        for k in (0, 2):
+            c = W.CONFIGS[k]
+            pos, q = inputs(k)
+            nl = c2.nl_build(dev(pos), c.box, c.r_list)
+            assert nl.info()["entry_bytes"] == 2
+            check_coulomb(c2, nl, pos, q, c)
+            nl.free()
+    finally:
+        c2.close()
