@@ -321,7 +321,12 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
                            e3 = __ldg(row + 32 * it + 96);
             pair(e0); pair(e1); pair(e2); pair(e3);
         }
-        for (; it < nst; ++it) pair(__ldg(row + 32 * it));
+        if (it + 2 <= nst) {
+            const unsigned e0 = __ldg(row + 32 * it), e1 = __ldg(row + 32 * it + 32);
+            pair(e0); pair(e1);
+            it += 2;
+        }
+        if (it < nst) pair(__ldg(row + 32 * it));
         if (FORCE) {
             const float v = warp_reduce4(fx, fy, fz, phi, lane);        // lanes 0 / 8 / 16 / 24: fx / fy / fz / phi
             if ((lane & 7) == 0) ((float*)(out + s))[lane >> 3] = v;
