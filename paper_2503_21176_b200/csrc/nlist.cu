@@ -8,8 +8,11 @@
 //      wrapped coordinates with a guard band, inside which the decision is taken by the exact fp64
 //      predicate of DESIGN.md R-NL on the raw caller positions (individually rounded IEEE ops, no
 //      FMA contraction) -- this is what makes the set bit-identical to the O(N^2) definition.
-//      Output: directed rows (row_start, row_len) into one packed array, entry = j | code << 27,
-//      code = (sx+1)*9 + (sy+1)*3 + (sz+1) with s the periodic image shift in box lengths.
+//      Output: directed rows (row_start, row_len) in one array.  Default format: 16-bit indices into the
+//      neighbourhood of the atom's 2x2x2 cell group (cellgroup.cuh; stored << 4 while neighbourhoods have
+//      fewer than 4095 atoms), rows padded to multiples of 32 entries, each group's rows in one reserved
+//      slice.  Fallback format: entry = j | code << 27, code = (sx+1)*9 + (sy+1)*3 + (sz+1) with s the
+//      periodic image shift in box lengths.
 //
 // Unlike Alg. 1 there is no [N,27,Cmax] candidate tensor and no padded cells[nx,ny,nz,Cmax].
 #include <math.h>
@@ -241,7 +244,6 @@ __device__ __noinline__ bool exact_in_range(const float* __restrict__ pos, int o
 #ifndef NL_BPS
 #define NL_BPS 4
 #endif
-#define NL_SLACK 256      // slots past the last row: the real-space kernel prefetches list entries ahead of its row
 struct NLCounters {
     unsigned long long cursor;     // list slots handed out (fmt 1 rows are padded to whole warps)
     unsigned long long pairs;      // directed pairs
@@ -858,7 +860,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
                 return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
                         "sqeq_nl_build: a row has %d neighbours; rows above %d are not supported", cap_row, cap_row_max));
             const size_t esize = local ? sizeof(uint16_t) : sizeof(uint32_t);
-            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, esize * (capacity + NL_SLACK)));
+            if (!nl->nbr) NL_TRY(pool_alloc(ctx, (void**)&nl->nbr, esize * capacity));
             NLCounters init = {};
             for (int d = 0; d < 3; ++d) init.ex.L[d] = g.L[d];
             init.ex.rl2 = g.rl2;
