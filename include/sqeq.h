@@ -125,6 +125,19 @@ int  sqeq_coulomb_host(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const flo
                        const int grid[3], int order, float* phi_host, float* force_host,
                        double* energy);
 
+/* The same evaluation, PIPELINED for independent evaluations: submit enqueues the host->device copies on a copy
+ * stream, the evaluation on the context's stream and the device->host copies on a second copy stream, and
+ * returns without synchronising; wait blocks until the results of that slot are in phi_host / force_host
+ * (and returns the energy if it was asked for at submit).  Two slots (0, 1): while slot s computes, the inputs
+ * of the other slot travel in and its previous results travel out.  Host buffers must be pinned and stay
+ * untouched between submit and wait; a slot cannot be submitted again before it was waited for (EINVAL).
+ * The neighbour list may be freed after submit (its storage is released in stream order). */
+int  sqeq_coulomb_host_submit(sqeq_ctx* ctx, int slot, const sqeq_nlist* nl, int64_t n,
+                              const float* pos_host, const float* q_host, const double box[3],
+                              double rc, double alpha, const int grid[3], int order,
+                              float* phi_host, float* force_host, int want_energy);
+int  sqeq_coulomb_host_wait(sqeq_ctx* ctx, int slot, double* energy);
+
 /* Parts of the last sqeq_coulomb call on this context, for diagnostics and stage-wise parity
  * (caller order; device fp32 outputs, any may be NULL): phi_real[n], F_real[n][3], phi_rec[n],
  * F_rec[n][3]; host double E_rec = 1/2 sum_m G|Qhat|^2 (Alg. 2 step 3).  Synchronises. */

@@ -61,6 +61,8 @@ def load():
     L.sqeq_nl_layout.argtypes = [vp, ctypes.POINTER(i64), ip, ip]
     L.sqeq_nl_free.argtypes = [vp]
     L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
+    L.sqeq_coulomb_host_submit.argtypes = [vp, cint, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
+    L.sqeq_coulomb_host_wait.argtypes = [vp, cint, dp]
     L.sqeq_coulomb_enqueue.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
     L.sqeq_energy_fetch.argtypes = [vp, dp]
     L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
@@ -234,6 +236,23 @@ class Context:
                                              _grid(grid), int(order), ctypes.c_void_p(phi.data_ptr()),
                                              ctypes.c_void_p(force.data_ptr()) if force is not None else None,
                                              ctypes.byref(e) if want_energy else None))
+        return e.value if want_energy else None
+
+    def coulomb_host_submit(self, slot, nl, pos, q, box, rc, alpha, grid, order, phi, force, want_energy=True):
+        """Pipelined form of coulomb_host (slot 0 or 1): returns at once; coulomb_host_wait(slot) delivers."""
+        n = pos.shape[0]
+        for t in (pos, q, phi) + ((force,) if force is not None else ()):
+            assert not t.is_cuda and t.is_contiguous() and t.dtype == torch.float32 and t.is_pinned()
+        self._check(load().sqeq_coulomb_host_submit(self.handle, int(slot), nl.handle, n,
+                                                    ctypes.c_void_p(pos.data_ptr()), ctypes.c_void_p(q.data_ptr()),
+                                                    _box(box), float(rc), float(alpha), _grid(grid), int(order),
+                                                    ctypes.c_void_p(phi.data_ptr()),
+                                                    ctypes.c_void_p(force.data_ptr()) if force is not None else None,
+                                                    1 if want_energy else 0))
+
+    def coulomb_host_wait(self, slot, want_energy=True):
+        e = ctypes.c_double()
+        self._check(load().sqeq_coulomb_host_wait(self.handle, int(slot), ctypes.byref(e) if want_energy else None))
         return e.value if want_energy else None
 
     def coulomb_parts(self, nl, want_force=True):

@@ -149,6 +149,16 @@ int sqeq_destroy(sqeq_ctx* ctx)
     if (ctx->h_scal) cudaFreeHost(ctx->h_scal);
     if (ctx->h_nl) cudaFreeHost(ctx->h_nl);
     if (ctx->h_kry) cudaFreeHost(ctx->h_kry);
+    if (ctx->h_slot_e) cudaFreeHost(ctx->h_slot_e);
+    for (int k = 0; k < 2; ++k) {
+        if (ctx->slot_in[k]) cudaEventDestroy(ctx->slot_in[k]);
+        if (ctx->slot_done[k]) cudaEventDestroy(ctx->slot_done[k]);
+        if (ctx->slot_out[k]) cudaEventDestroy(ctx->slot_out[k]);
+        for (int b = 0; b < 5; ++b)
+            if (ctx->slot_buf[k][b].p) cudaFree(ctx->slot_buf[k][b].p);
+    }
+    if (ctx->stream_h2d) cudaStreamDestroy(ctx->stream_h2d);
+    if (ctx->stream_d2h) cudaStreamDestroy(ctx->stream_d2h);
     for (auto& r : ctx->pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto& e : ctx->free_events) cudaEventDestroy(e);
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -411,5 +421,89 @@ extern "C" int sqeq_coulomb_host(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n,
     if (energy) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal.p, sizeof(double), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(ctx, cudaStreamSynchronize(st));
     if (energy) *energy = ctx->h_scal[0];
+    return SQEQ_OK;
+}
+
+// Pipelined form of sqeq_coulomb_host for independent evaluations: the inputs of evaluation k+1 travel to the
+// device (copy stream) and the results of evaluation k-1 travel back (second copy stream) while evaluation k
+// runs on the context's stream.  Two slots; a slot is free again after sqeq_coulomb_host_wait on it.
+static int slot_setup(sqeq_ctx* ctx)
+{
+    if (ctx->stream_h2d) return SQEQ_OK;
+    CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->stream_h2d, cudaStreamNonBlocking));
+    CUDA_TRY(ctx, cudaStreamCreateWithFlags(&ctx->stream_d2h, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; ++k) {
+        CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->slot_in[k], cudaEventDisableTiming));
+        CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->slot_done[k], cudaEventDisableTiming));
+        CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->slot_out[k], cudaEventDisableTiming));
+    }
+    CUDA_TRY(ctx, cudaMallocHost((void**)&ctx->h_slot_e, 2 * sizeof(double)));
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_coulomb_host_submit(sqeq_ctx* ctx, int slot, const sqeq_nlist* nl, int64_t n,
+                                        const float* pos_host, const float* q_host, const double box[3],
+                                        double rc, double alpha, const int grid[3], int order,
+                                        float* phi_host, float* force_host, int want_energy)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (slot < 0 || slot > 1) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_host_submit: slot must be 0 or 1");
+    if (ctx->slot_busy[slot])
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_host_submit: slot %d is in flight (call sqeq_coulomb_host_wait)", slot);
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_coulomb_host_submit"));
+    if (!pos_host || !q_host) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_host_submit: pos or q is NULL");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    SQEQ_TRY(slot_setup(ctx));
+    DevBuf* b = ctx->slot_buf[slot];
+    const size_t want[5] = {sizeof(float) * 3 * (size_t)n, sizeof(float) * (size_t)n, sizeof(float) * (size_t)n,
+                            force_host ? sizeof(float) * 3 * (size_t)n : 0, sizeof(double)};
+    for (int k = 0; k < 5; ++k)
+        if (want[k] > b[k].cap) {
+            // the slot is idle (its last evaluation was waited for), so its buffers can be replaced right away
+            if (b[k].p) CUDA_TRY(ctx, cudaFree(b[k].p));
+            b[k].p = nullptr;
+            b[k].cap = 0;
+            CUDA_TRY(ctx, cudaMalloc(&b[k].p, want[k]));
+            b[k].cap = want[k];
+        }
+    float* d_pos = (float*)b[0].p;
+    float* d_q = (float*)b[1].p;
+    float* d_phi = (float*)b[2].p;
+    float* d_f = force_host ? (float*)b[3].p : nullptr;
+    CUDA_TRY(ctx, cudaMemcpyAsync(d_pos, pos_host, want[0], cudaMemcpyHostToDevice, ctx->stream_h2d));
+    CUDA_TRY(ctx, cudaMemcpyAsync(d_q, q_host, want[1], cudaMemcpyHostToDevice, ctx->stream_h2d));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->slot_in[slot], ctx->stream_h2d));
+    cudaStream_t st = ctx->stream;
+    CUDA_TRY(ctx, cudaStreamWaitEvent(st, ctx->slot_in[slot], 0));
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    SQEQ_TRY(prep_atoms(ctx, nl, d_pos, d_q, ctx->K, st));
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, d_phi, d_f, want_energy != 0));
+    if (want_energy)
+        CUDA_TRY(ctx, cudaMemcpyAsync(b[4].p, ctx->scal.p, sizeof(double), cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->slot_done[slot], st));
+    CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream_d2h, ctx->slot_done[slot], 0));
+    if (phi_host) CUDA_TRY(ctx, cudaMemcpyAsync(phi_host, d_phi, want[2], cudaMemcpyDeviceToHost, ctx->stream_d2h));
+    if (force_host) CUDA_TRY(ctx, cudaMemcpyAsync(force_host, d_f, want[3], cudaMemcpyDeviceToHost, ctx->stream_d2h));
+    if (want_energy)
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_slot_e + slot, b[4].p, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream_d2h));
+    CUDA_TRY(ctx, cudaEventRecord(ctx->slot_out[slot], ctx->stream_d2h));
+    ctx->slot_busy[slot] = true;
+    ctx->slot_energy[slot] = want_energy != 0;
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_coulomb_host_wait(sqeq_ctx* ctx, int slot, double* energy)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (slot < 0 || slot > 1 || !ctx->slot_busy[slot])
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_host_wait: nothing submitted on slot %d", slot);
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaEventSynchronize(ctx->slot_out[slot]));
+    ctx->slot_busy[slot] = false;
+    if (energy) {
+        if (!ctx->slot_energy[slot])
+            return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_host_wait: slot %d was submitted without the energy", slot);
+        *energy = ctx->h_slot_e[slot];
+    }
     return SQEQ_OK;
 }

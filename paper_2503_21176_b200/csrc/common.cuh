@@ -80,6 +80,13 @@ struct sqeq_ctx {
     DevBuf vec_d[6];  // double [n] scratch
     DevBuf vec_f3[2]; // float  [n][3] scratch forces
     DevBuf stage[4];  // device staging for sqeq_coulomb_host: pos, q, phi, force
+    // sqeq_coulomb_host_submit / _wait: two slots, copies on their own streams beside the evaluation stream
+    DevBuf slot_buf[2][5];                // pos, q, phi, force, energy (one double)
+    cudaStream_t stream_h2d = nullptr, stream_d2h = nullptr;
+    cudaEvent_t slot_in[2] = {nullptr, nullptr}, slot_done[2] = {nullptr, nullptr}, slot_out[2] = {nullptr, nullptr};
+    bool slot_busy[2] = {false, false};
+    bool slot_energy[2] = {false, false};
+    double* h_slot_e = nullptr;           // pinned [2]
 
     // ---- timing ----
     bool profiling = false;

@@ -428,3 +428,42 @@ def test_side_stream_with_persistent_real_space(monkeypatch):
             nl.free()
     finally:
         c2.close()
+
+
+def test_pipelined_host_entry_matches_synchronous_call(ctx):
+    """sqeq_coulomb_host_submit / _wait (two slots, copies on their own streams) give the results of
+    sqeq_coulomb_host for the same inputs, in any interleaving; slot misuse is an error, not a hang."""
+    from paper_2503_21176_b200.binding import SqeqError
+    c = W.CONFIGS[1]
+    pos, q = inputs(1)
+    n = len(q)
+    nl = ctx.nl_build(dev(pos), c.box, c.r_list)
+    pin = lambda a: torch.as_tensor(np.ascontiguousarray(a)).pin_memory()
+    sets = [pin(W.perturb(pos, k, 0.02, 1)) for k in range(3)]
+    hq = pin(q)
+    ref = []
+    for p in sets:
+        hphi, hf = torch.empty(n).pin_memory(), torch.empty((n, 3)).pin_memory()
+        e = ctx.coulomb_host(nl, p, hq, c.box, c.rc, c.alpha, c.grid, c.order, hphi, hf)
+        ref.append((hphi.clone(), hf.clone(), e))
+    out = [(torch.empty(n).pin_memory(), torch.empty((n, 3)).pin_memory()) for _ in range(2)]
+    got = []
+    for k, p in enumerate(sets):
+        s = k & 1
+        if k >= 2:
+            e = ctx.coulomb_host_wait(s)
+            got.append((out[s][0].clone(), out[s][1].clone(), e))
+        ctx.coulomb_host_submit(s, nl, p, hq, c.box, c.rc, c.alpha, c.grid, c.order, out[s][0], out[s][1])
+    with pytest.raises(SqeqError):
+        ctx.coulomb_host_submit(0, nl, sets[0], hq, c.box, c.rc, c.alpha, c.grid, c.order, out[0][0], out[0][1])
+    for k in (1, 2):
+        s = k & 1
+        e = ctx.coulomb_host_wait(s)
+        got.append((out[s][0].clone(), out[s][1].clone(), e))
+    with pytest.raises(SqeqError):
+        ctx.coulomb_host_wait(0)
+    for (a, b, e), (ra, rb, re) in zip(got, ref):
+        # same kernels on the same inputs; only the order of the fp32 reductions that flush the tiles differs
+        assert relrms(a.numpy(), ra.numpy()) < 2e-6 and relrms(b.numpy(), rb.numpy()) < 2e-6
+        assert abs(e / re - 1) < 1e-6
+    nl.free()
