@@ -227,6 +227,7 @@ def run_ours(args, cfg):
             if state["nl"] is not None:
                 state["nl"].free()
             state["nl"] = ctx.nl_build(possets[k % N_POSSETS], box, rl)
+            state["nl_set"] = k % N_POSSETS
         if host is None:
             # potential, force and the fp64 energy reduction, all enqueued; the energy of the last
             # step is read back once at the end of the timed region (sqeq_energy_fetch)
@@ -298,6 +299,7 @@ def run_ours(args, cfg):
             if k % REBUILD_EVERY == 0:
                 state["nl"].free()
                 state["nl"] = ctx.nl_build(possets[k % N_POSSETS], box, rl)
+                state["nl_set"] = k % N_POSSETS
             ctx.coulomb_host_submit(s, state["nl"], hp[k % N_POSSETS], hq, box, rc, alpha, grid, order,
                                     hphi2[s], hf2[s])
         for k in range(max(0, nsteps - 2), nsteps):
@@ -364,7 +366,22 @@ def run_ours(args, cfg):
              "pair_interactions_per_s": None, "grid_points_per_s": None,
              "n_directed_list_entries": P, "ms_per_step_with_stage_events": round(ms / args.steps, 4)}
     if "real" in kernels:
-        extra["pair_interactions_per_s"] = (P / 2) / (kernels["real"]["ms_avg"] * 1e-3)
+        # unique pairs with r < rc per second of the real-space kernel; counted here from
+        # the exported list (the list itself also holds the skin pairs between rc and r_list)
+        gi, gj, gs = state["nl"].export()
+        pb = possets[state["nl_set"]]
+        boxv = torch.tensor(box, dtype=torch.float32, device=dev)
+        n_in = 0
+        CH = 1 << 24
+        for a in range(0, gi.numel(), CH):
+            sl = slice(a, min(a + CH, gi.numel()))
+            d = pb[gj[sl].long()] + gs[sl].float() * boxv - pb[gi[sl].long()]
+            n_in += int(((d * d).sum(1) < rc * rc).sum())
+        del gi, gj, gs
+        extra["unique_pairs_within_rc"] = n_in
+        extra["unique_pairs_in_list"] = P // 2
+        extra["pair_interactions_per_s"] = n_in / (kernels["real"]["ms_avg"] * 1e-3)
+        extra["list_pairs_per_s"] = (P / 2) / (kernels["real"]["ms_avg"] * 1e-3)
     pme_ms = sum(kernels[k]["ms_avg"] for k in ("spread", "fft_fwd", "influence", "fft_inv", "gather") if k in kernels)
     if pme_ms > 0:
         extra["grid_points_per_s"] = G3 / (pme_ms * 1e-3)
