@@ -86,6 +86,11 @@ int  sqeq_nl_entry_bytes(const sqeq_nlist* nl, int* bytes);
  * of a 16-byte staged atom) while the most populous neighbourhood stays below 4095 atoms, else 0.
  * max_neighbourhood: atoms (all periodic images) the staged real-space kernel holds per cell group. */
 int  sqeq_nl_layout(const sqeq_nlist* nl, int64_t* n_slots, int* entry_shift, int* max_neighbourhood);
+/* Largest distance (Angstrom, host double) any atom has moved since the list was built, from the caller's
+ * positions pos[n][3] (device) and the copy the list keeps of the positions it was built from.  A list built
+ * with cutoff rc + skin holds every pair with r < rc while this stays below skin/2: rebuild
+ * when it does not.  One small kernel and a stream synchronisation; +inf if a position is NaN. */
+int  sqeq_nl_max_drift(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, double* max_drift);
 int  sqeq_nl_free  (sqeq_nlist* nl);
 
 /* ---- Coulomb evaluation: Eq. 2 = Eq. 3 (real space, r < rc) + Alg. 2 (smooth PME,

@@ -59,6 +59,7 @@ def load():
     L.sqeq_nl_info.argtypes = [vp, ip, ctypes.POINTER(i64), ip]
     L.sqeq_nl_entry_bytes.argtypes = [vp, ip]
     L.sqeq_nl_layout.argtypes = [vp, ctypes.POINTER(i64), ip, ip]
+    L.sqeq_nl_max_drift.argtypes = [vp, vp, i64, vp, dp]
     L.sqeq_nl_free.argtypes = [vp]
     L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_host_submit.argtypes = [vp, cint, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
@@ -129,6 +130,13 @@ class NeighbourList:
         self.ctx._check(load().sqeq_nl_layout(self.handle, ctypes.byref(ns), ctypes.byref(sh), ctypes.byref(mp)))
         return dict(ncell=list(nc), n_directed=nd.value, max_row=mr.value, entry_bytes=eb.value,
                     n_slots=ns.value, entry_shift=sh.value, max_neighbourhood=mp.value)
+
+    def max_drift(self, pos):
+        """Largest displacement since the build (rebuild when it reaches skin/2)."""
+        d = ctypes.c_double()
+        self.ctx._check(load().sqeq_nl_max_drift(self.ctx.handle, self.handle, self.n,
+                                                 _ptr(pos, torch.float32, 3 * self.n), ctypes.byref(d)))
+        return d.value
 
     def export(self):
         """Canonical (i, j, shift) arrays on the device: unique pairs i<j sorted by (i,j)."""

@@ -294,6 +294,15 @@ int sqeq_nl_layout(const sqeq_nlist* nl, int64_t* n_slots, int* entry_shift, int
     return SQEQ_OK;
 }
 
+int sqeq_nl_max_drift(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, double* max_drift)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!nl || nl->ctx != ctx || n != nl->n || !pos || !max_drift)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_max_drift: list/context/n mismatch or NULL argument");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return nl_max_drift_impl(ctx, nl, pos, max_drift);
+}
+
 int sqeq_nl_free(sqeq_nlist* nl)
 {
     if (!nl) return SQEQ_OK;

@@ -113,6 +113,7 @@ struct sqeq_nlist {
     char4*    wrapc = nullptr;       // [n]   floor(x/L) per axis at build time (sorted order)
     int64_t*  row_start = nullptr;   // [n]   offset of row s in nbr (rows in no particular order; fmt 1: multiples of 32)
     int*      row_len = nullptr;     // [n]   entries of row s
+    float*    pos0 = nullptr;        // [n][3] caller order: the positions the list was built from (drift check)
     longlong2* grp_slice = nullptr;  // [cell groups] (first slot, slots used) of the group's reserved slice of nbr
     void*     nbr = nullptr;         // [>= n_slots] entries: fmt 0: uint32 j (27 bits) | image code << 27;
                                      //                          fmt 1: uint16 local index in the group's neighbourhood
@@ -185,6 +186,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
                   sqeq_nlist** out);
 void nl_release(sqeq_nlist* nl);
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
+int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, double* max_drift);
 
 // Re-gather positions/charges into the list's order (and PME fractional coordinates if K != null).
 int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* q,

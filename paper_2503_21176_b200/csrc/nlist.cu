@@ -17,6 +17,7 @@
 // Unlike Alg. 1 there is no [N,27,Cmax] candidate tensor and no padded cells[nx,ny,nz,Cmax].
 #include <math.h>
 #include <stdlib.h>
+#include <string.h>
 #include <type_traits>
 
 #include "common.cuh"
@@ -712,7 +713,7 @@ static int pool_alloc(sqeq_ctx* ctx, void** p, size_t bytes)
 void nl_release(sqeq_nlist* nl)
 {
     cudaStream_t st = nl->ctx->stream;
-    void* ptrs[] = {nl->perm, nl->cell_of, nl->cell_start, nl->wrapc, nl->row_start, nl->row_len, nl->grp_slice, nl->nbr};
+    void* ptrs[] = {nl->perm, nl->cell_of, nl->cell_start, nl->wrapc, nl->row_start, nl->row_len, nl->grp_slice, nl->pos0, nl->nbr};
     for (void* p : ptrs)
         if (p) cudaFreeAsync(p, st);     // stream-ordered: safe after every evaluation already enqueued
     delete nl;
@@ -796,6 +797,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     NL_TRY(pool_alloc(ctx, (void**)&nl->wrapc, sizeof(char4) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_start, sizeof(int64_t) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_len, sizeof(int) * n));
+    NL_TRY(pool_alloc(ctx, (void**)&nl->pos0, sizeof(float) * 3 * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->grp_slice, sizeof(longlong2) * (size_t)nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2]));
     NL_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * (n + 32)));     // 32 padding entries: see k_pairs
     float4* xq = (float4*)ctx->xq.p;
@@ -822,6 +824,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         ctx->launches++;
         k_reorder<<<nb, 256, 0, st>>>(n, pos, nl->perm, g, xq, nl->cell_of, nl->wrapc);
         ctx->launches++;
+        NL_CUDA(cudaMemcpyAsync(nl->pos0, pos, sizeof(float) * 3 * n, cudaMemcpyDeviceToDevice, st));   // for sqeq_nl_max_drift
         NL_CUDA(cudaGetLastError());
     }
     t_bin = now_ms();
@@ -911,6 +914,40 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     return SQEQ_OK;
 #undef NL_TRY
 #undef NL_CUDA
+}
+
+// Largest distance any atom has moved since the list was built (plain difference of caller positions: an atom
+// that crossed the box is still the same unwrapped coordinate to the caller).  A list with cutoff rc + skin
+// stays complete for r < rc while this is below skin/2 (cfg 4 recipe).
+__global__ void k_max_drift(int64_t n, const float* __restrict__ pos, const float* __restrict__ pos0,
+                            unsigned* __restrict__ out)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float d2 = 0.f;
+    if (i < n) {
+        const float dx = pos[3 * i] - pos0[3 * i], dy = pos[3 * i + 1] - pos0[3 * i + 1], dz = pos[3 * i + 2] - pos0[3 * i + 2];
+        d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        if (!(d2 == d2)) d2 = __int_as_float(0x7f800000);      // NaN position: report +inf
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) d2 = fmaxf(d2, __shfl_xor_sync(0xffffffffu, d2, o));
+    if ((threadIdx.x & 31) == 0 && d2 > 0.f) atomicMax(out, __float_as_uint(d2));   // non-negative floats order as uints
+}
+
+int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, double* max_drift)
+{
+    cudaStream_t st = ctx->stream;
+    unsigned* d_out = (unsigned*)((double*)ctx->scal.p + 12);        // a scratch word of the scalar block
+    CUDA_TRY(ctx, cudaMemsetAsync(d_out, 0, sizeof(unsigned), st));
+    k_max_drift<<<ceil_div(nl->n, 256), 256, 0, st>>>(nl->n, pos, nl->pos0, d_out);
+    KERNEL_CHECK(ctx);
+    unsigned* h = (unsigned*)(ctx->h_scal + 12);
+    CUDA_TRY(ctx, cudaMemcpyAsync(h, d_out, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    float d2;
+    memcpy(&d2, h, sizeof(float));
+    *max_drift = sqrt((double)d2);
+    return SQEQ_OK;
 }
 
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj, int8_t* shift3)

@@ -118,6 +118,14 @@ def test_stale_list_with_skin_and_perturbation(ctx):
     phi, F, E = ctx.coulomb(nl, dev(p), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
     op, oF, oE, _ = oracle.coulomb_pme(p, q, c.box, c.rc, c.alpha, c.grid, c.order)
     assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL
+    # the drift the list reports is the largest displacement since the build: below skin/2 here, so the
+    # evaluation above was entitled to the stale list; zero at the build positions; the plain definition
+    drift = np.sqrt((((p.astype(np.float32) - pos.astype(np.float32)).astype(np.float64)) ** 2).sum(1)).max()
+    assert abs(nl.max_drift(dev(p)) - drift) < 1e-6 and drift < 0.5
+    assert nl.max_drift(dev(pos)) == 0.0
+    far = pos.copy()
+    far[1234] += np.array([0.3, -0.4, 1.2], dtype=np.float32)
+    assert abs(nl.max_drift(dev(far)) - 1.3) < 1e-5
     nl.free()
 
 
