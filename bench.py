@@ -281,7 +281,12 @@ def run_ours(args, cfg):
     host = (hp, hq, hphi, hf)
     for k in range(3):
         step(k, host)
-    ms_e2e_sync = timed(args.steps, host)            # one synchronous call per step (sqeq_coulomb_host)
+    # the host-side legs are timed three times each and the median repetition is reported (all three are in the
+    # JSON line): the first repetition still pays first-use costs of the host path (pinned position sets touched
+    # for the first time, slot buffers), which the three warm-up steps do not cover
+    E2E_REPS = 3
+    reps_sync = [timed(args.steps, host) for _ in range(E2E_REPS)]    # one synchronous sqeq_coulomb_host call per step
+    ms_e2e_sync = sorted(reps_sync)[E2E_REPS // 2]
     # the same steps through the pipelined entry (sqeq_coulomb_host_submit / _wait, two slots): the evaluations
     # are independent, so the inputs of step k+1 and the results of step k-1 cross PCIe while step k computes;
     # every step still copies its 16 B/atom in and 16 B/atom + 8 B out inside the timed region
@@ -309,7 +314,8 @@ def run_ours(args, cfg):
         return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
 
     timed_pipelined(4)
-    ms_e2e = timed_pipelined(args.steps)
+    reps_pipe = [timed_pipelined(args.steps) for _ in range(E2E_REPS)]
+    ms_e2e = sorted(reps_pipe)[E2E_REPS // 2]
     e2e_val = world * 1e3 * args.steps / ms_e2e
     e2e_sync_val = world * 1e3 * args.steps / ms_e2e_sync
 
@@ -406,6 +412,9 @@ def run_ours(args, cfg):
            "e2e": {"value": e2e_val, "unit": "evals/s", "h2d_bytes_per_step": 16 * n,
                    "d2h_bytes_per_step": 16 * n + 8,
                    "api": "sqeq_coulomb_host_submit/_wait, two slots (independent evaluations pipelined over PCIe)",
+                   "timing": "median of %d repetitions of the %d-step loop" % (E2E_REPS, args.steps),
+                   "ms_per_step_repetitions": [round(t / args.steps, 4) for t in reps_pipe],
+                   "sync_ms_per_step_repetitions": [round(t / args.steps, 4) for t in reps_sync],
                    "sync_value": e2e_sync_val,
                    "sync_api": "sqeq_coulomb_host, one synchronous call per step"},
            "roofline": roofline, "roofline_alu": roofline_alu, "extra": extra}
