@@ -432,6 +432,18 @@ def shadow_md_force_and_ndd(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, orde
     return ev
 
 
+def xl_n_update(nh, ndd_dt2, alpha_diss, c):
+    """Verlet step with dissipation for the extended charges (DESIGN.md R-MD; the form of the
+    integration the paper cites for Eq. 27):
+        n(t+dt) = 2 n(t) - n(t-dt) + dt^2 ndd(t) + alpha_diss * sum_{k=0}^{5} c_k n(t - k dt),
+    nh[k] = n(t - k dt), k = 0..5.  alpha_diss = 0 is the plain time-reversible Verlet step."""
+    nh = np.asarray(nh, dtype=np.float64)
+    diss = np.zeros_like(nh[0])
+    for k in range(6):
+        diss = diss + float(c[k]) * nh[k]
+    return 2.0 * nh[0] - nh[1] + _f64(ndd_dt2) + float(alpha_diss) * diss
+
+
 def shadow_md_init(pos, n0, chi, u, ke, qtot, box, rc, alpha, grid, order, standin, kappa,
                    krylov_rank):
     """History rows 0..5 = n0 (PAPER.md is silent on the start: DESIGN.md R-MD), row 6 = dt^2 ndd."""
@@ -453,7 +465,7 @@ def shadow_md_step(state, vel, mass, dt, chi, u, ke, qtot, box, rc, alpha, grid,
     a = ACC_CONV * state["F"] / mass[:, None]
     vel = vel + 0.5 * dt * a
     pos = pos + dt * vel
-    n_new = 2.0 * nh[0] - nh[1] + nh[6] + alpha_diss * sum(c[k] * nh[k] for k in range(6))
+    n_new = xl_n_update(nh[0:6], nh[6], alpha_diss, c)
     ev = shadow_md_force_and_ndd(pos, n_new, chi, u, ke, qtot, box, rc, alpha, grid, order,
                                  standin, kappa, krylov_rank)
     nhist = np.vstack([n_new[None, :], nh[0:5], ev["ndd_dt2"][None, :]])

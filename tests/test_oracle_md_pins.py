@@ -125,3 +125,72 @@ def test_short_nve_run_conserves_shadow_energy():
     # kinetic and potential energy exchange O(0.1-1 eV) while their sum stays flat
     assert np.ptp(k) > 0.3
     assert e.std() < 0.02 * np.ptp(k), (e.std(), np.ptp(k))
+
+
+# ---- the n(t) integrator (oracle.xl_n_update): what the mathematics fixes ---------------------------
+# kappa, alpha_diss and c_k are not printed in the paper (DESIGN.md R-MD); they are the K = 5 set of the
+# XL-BOMD literature it cites.  What can be checked without that literature: the dissipation term must
+# not move a stationary n (sum c = 0), must be invisible to time reversal up to high order in dt (the odd
+# moments sum k^p c_k, p = 1, 3, 5 vanish -- the design condition that determines such a set up to its
+# scale and one free parameter), the step at alpha_diss = 0 is exactly reversible, and the homogeneous
+# recursion with the exact kernel (dt^2 ndd = -kappa (n - q)) must be stable: all roots of its
+# characteristic polynomial inside the closed unit disc, strictly inside when alpha_diss > 0.
+XL_KAPPA, XL_ALPHA, XL_C = 1.82, 0.018, [-6.0, 14.0, -8.0, -3.0, 4.0, -1.0]
+
+
+def test_xl_coefficients_moments():
+    c = np.array(XL_C)
+    k = np.arange(6.0)
+    assert c.sum() == 0.0
+    for p in (1, 3, 5):
+        assert (k ** p * c).sum() == 0.0, p
+    assert (k ** 2 * c).sum() != 0.0          # the even moment carries the dissipation
+    # stationary n, no acceleration: stays put for any alpha_diss
+    n = np.array([0.3, -0.7, 0.4])
+    assert np.abs(oracle.xl_n_update(np.tile(n, (6, 1)), np.zeros(3), 0.5, XL_C) - n).max() < 1e-15
+
+
+def test_xl_step_is_time_reversible_without_dissipation():
+    rng = np.random.default_rng(0)
+    nh = rng.normal(size=(6, 50))
+    acc = rng.normal(size=50) * 0.1
+    fwd = oracle.xl_n_update(nh, acc, 0.0, XL_C)                       # n(t+dt)
+    back_hist = np.vstack([nh[0:1], fwd[None, :], nh[1:5]])            # time reversed: n(t), n(t+dt), ...
+    back = oracle.xl_n_update(back_hist, acc, 0.0, XL_C)               # same acceleration at t
+    assert np.abs(back - nh[1]).max() < 1e-15
+    # with dissipation the reversed step does NOT return (the term breaks time reversal on purpose)
+    fwd_d = oracle.xl_n_update(nh, acc, XL_ALPHA, XL_C)
+    back_d = oracle.xl_n_update(np.vstack([nh[0:1], fwd_d[None, :], nh[1:5]]), acc, XL_ALPHA, XL_C)
+    assert np.abs(back_d - nh[1]).max() > 1e-4
+
+
+def _char_roots(kappa, alpha, c):
+    # n_{j+1} = (2 - kappa) n_j - n_{j-1} + alpha sum_k c_k n_{j-k}   =>   polynomial in z of degree 6
+    p = [1.0, -(2.0 - kappa + alpha * c[0]), 1.0 - alpha * c[1], -alpha * c[2], -alpha * c[3], -alpha * c[4],
+         -alpha * c[5]]
+    return np.roots(p)
+
+
+def test_xl_recursion_is_stable_and_damped():
+    r0 = _char_roots(XL_KAPPA, 0.0, XL_C)
+    assert np.abs(np.abs(r0[np.abs(r0) > 1e-8]) - 1.0).max() < 1e-12      # undamped Verlet: on the unit circle
+    r = _char_roots(XL_KAPPA, XL_ALPHA, XL_C)
+    rho = np.abs(r).max()
+    assert rho < 0.92                                        # strictly inside: noise in n is damped
+    # sign or index slips in c, or kappa beyond the Verlet limit, leave the disc
+    assert np.abs(_char_roots(XL_KAPPA, XL_ALPHA, [-x for x in XL_C])).max() > 1.0
+    assert np.abs(_char_roots(XL_KAPPA, XL_ALPHA, XL_C[::-1])).max() > 1.0
+    assert np.abs(_char_roots(4.2, XL_ALPHA, XL_C)).max() > 1.0
+    # the oracle's recursion itself, run on the exact-kernel model problem dt^2 ndd = -kappa (n - q):
+    # the error decays at the rate of the largest root
+    q = np.array([0.4, -0.1])
+    nh = np.tile(q + np.array([0.05, -0.02]), (6, 1))
+    err = []
+    for _ in range(120):
+        n_new = oracle.xl_n_update(nh, -XL_KAPPA * (nh[0] - q), XL_ALPHA, XL_C)
+        nh = np.vstack([n_new[None, :], nh[0:5]])
+        err.append(np.abs(n_new - q).max())
+    err = np.array(err)
+    assert err[-1] < 1e-4 * err[0]
+    rate = (err[100:120].max() / err[40:60].max()) ** (1.0 / 60.0)
+    assert abs(rate - rho) < 0.02, (rate, rho)
