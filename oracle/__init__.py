@@ -49,6 +49,8 @@ def lib():
         L.orc_nl_row.argtypes = [i64, c_dp, c_dp, ctypes.c_double, i64, i64,
                                  ctypes.c_void_p, ctypes.c_void_p]
         L.orc_nl_row.restype = i64
+        L.orc_nl_rows_upper.argtypes = [i64, c_dp, c_dp, ctypes.c_double, i64, i64, i64,
+                                        ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         L.orc_realspace.argtypes = [i64, c_dp, c_dp, c_dp, ctypes.c_double,
                                     ctypes.c_double, c_dp, c_dp]
         L.orc_realspace_rows.argtypes = [i64, c_dp, c_dp, c_dp, ctypes.c_double,
@@ -116,6 +118,27 @@ def neighbour_list(pos, box, rlist):
     lib().orc_nl_fill(n, _dp(pos), _dp(box), float(rlist), offsets.ctypes.data,
                       pi.ctypes.data, pj.ctypes.data, sh.ctypes.data)
     return pi, pj, sh
+
+
+def neighbour_rows_upper(pos, box, rlist, i0, i1, cap=1024):
+    """Rows i0 <= i < i1 of the canonical list (j > i) in one pass: (i, j, shift) arrays sorted by
+    (i, j), exactly the slice of neighbour_list() with i0 <= i < i1."""
+    pos = _f64(pos, (-1, 3))
+    box = _box(box)
+    n = pos.shape[0]
+    while True:
+        m = int(i1 - i0)
+        counts = np.zeros(m, dtype=np.int64)
+        pj = np.empty((m, cap), dtype=np.int32)
+        sh = np.empty((m, cap, 3), dtype=np.int8)
+        lib().orc_nl_rows_upper(n, _dp(pos), _dp(box), float(rlist), int(i0), int(i1), int(cap),
+                                counts.ctypes.data, pj.ctypes.data, sh.ctypes.data)
+        if counts.max(initial=0) <= cap:
+            break
+        cap = int(counts.max())
+    mask = np.arange(cap)[None, :] < counts[:, None]
+    oi = np.repeat(np.arange(i0, i1, dtype=np.int32), counts)
+    return oi, pj[mask], sh[mask]
 
 
 def neighbour_row(pos, box, rlist, i, cap=4096):

@@ -115,6 +115,37 @@ void orc_nl_fill(int64_t n, const double *pos, const double box[3],
     }
 }
 
+/* Rows i0 <= i < i1 of the canonical list (j > i, ascending j) in ONE O((i1-i0) N) pass with
+ * a fixed capacity per row: row i's entries go to pj[(i-i0)*cap ...], shift likewise, and
+ * counts[i-i0] is the number found (entries beyond cap are counted, not written).  The same
+ * predicate as orc_nl_fill; lets a test walk a large system chunk by chunk in bounded memory. */
+void orc_nl_rows_upper(int64_t n, const double *pos, const double box[3],
+                       double rlist, int64_t i0, int64_t i1, int64_t cap,
+                       int64_t *counts, int32_t *pj, int8_t *shift)
+{
+    const double rr = rlist * rlist;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = i0; i < i1; ++i) {
+        int64_t c = 0;
+        int s[3];
+        double d[3], r2;
+        int32_t *oj = pj + (i - i0) * cap;
+        int8_t *os = shift + 3 * (i - i0) * cap;
+        for (int64_t j = i + 1; j < n; ++j) {
+            if (orc_pair(pos + 3 * i, pos + 3 * j, box, rr, s, d, &r2)) {
+                if (c < cap) {
+                    oj[c] = (int32_t)j;
+                    os[3 * c + 0] = (int8_t)s[0];
+                    os[3 * c + 1] = (int8_t)s[1];
+                    os[3 * c + 2] = (int8_t)s[2];
+                }
+                ++c;
+            }
+        }
+        counts[i - i0] = c;
+    }
+}
+
 /* All neighbours j != i of ONE atom i (directed row), ascending j, with the
  * shift for the ordered pair (i,j).  Returns the number found (writes at most
  * cap of them).  O(N) -- used to check sampled rows at sizes where the full

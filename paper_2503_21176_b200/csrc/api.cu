@@ -133,6 +133,13 @@ int sqeq_destroy(sqeq_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     if (ctx->stream2) cudaStreamSynchronize(ctx->stream2);
+    // lists that outlive their context: release the device storage now, leave a detached handle behind
+    for (sqeq_nlist* nl : ctx->lists) {
+        nl_release_storage(nl);
+        nl->ctx = nullptr;
+    }
+    ctx->lists.clear();
+    cudaStreamSynchronize(ctx->stream);
     if (ctx->plans_ok) {
         cufftDestroy(ctx->plan_r2c);
         cufftDestroy(ctx->plan_c2r);

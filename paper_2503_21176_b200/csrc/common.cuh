@@ -21,6 +21,8 @@ struct DevBuf {
     size_t cap = 0;
 };
 
+struct sqeq_nlist;
+
 struct TimerRec {
     int stage;
     cudaEvent_t a, b;
@@ -95,6 +97,10 @@ struct sqeq_ctx {
     double t_total[SQEQ_T_COUNT] = {0};
     int64_t t_count[SQEQ_T_COUNT] = {0};
     int64_t launches = 0;
+
+    // live neighbour lists of this context: sqeq_destroy releases their device storage and detaches them, so a
+    // handle freed after its context is only deleted (no use of a dead stream or pool)
+    std::vector<sqeq_nlist*> lists;
 };
 
 struct sqeq_nlist {
@@ -185,6 +191,7 @@ static inline int ceil_div(int64_t a, int64_t b) { return (int)((a + b - 1) / b)
 int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
                   sqeq_nlist** out);
 void nl_release(sqeq_nlist* nl);
+void nl_release_storage(sqeq_nlist* nl);
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
 int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, double* max_drift);
 

@@ -710,12 +710,24 @@ static int pool_alloc(sqeq_ctx* ctx, void** p, size_t bytes)
     return SQEQ_OK;
 }
 
-void nl_release(sqeq_nlist* nl)
+// stream-ordered frees: safe after every evaluation already enqueued; the handle itself stays
+void nl_release_storage(sqeq_nlist* nl)
 {
     cudaStream_t st = nl->ctx->stream;
-    void* ptrs[] = {nl->perm, nl->cell_of, nl->cell_start, nl->wrapc, nl->row_start, nl->row_len, nl->grp_slice, nl->pos0, nl->nbr};
-    for (void* p : ptrs)
-        if (p) cudaFreeAsync(p, st);     // stream-ordered: safe after every evaluation already enqueued
+    void** ptrs[] = {(void**)&nl->perm, (void**)&nl->cell_of, (void**)&nl->cell_start, (void**)&nl->wrapc, (void**)&nl->row_start,
+                     (void**)&nl->row_len, (void**)&nl->grp_slice, (void**)&nl->pos0, &nl->nbr};
+    for (void** p : ptrs) {
+        if (*p) cudaFreeAsync(*p, st);
+        *p = nullptr;
+    }
+}
+
+void nl_release(sqeq_nlist* nl)
+{
+    sqeq_ctx* ctx = nl->ctx;
+    nl_release_storage(nl);
+    for (size_t k = 0; k < ctx->lists.size(); ++k)
+        if (ctx->lists[k] == nl) { ctx->lists[k] = ctx->lists.back(); ctx->lists.pop_back(); break; }
     delete nl;
 }
 
@@ -752,16 +764,10 @@ static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const N
     return SQEQ_OK;
 }
 
-#include <chrono>
-static double now_ms() { return std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
-
 int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3], double cutoff,
                   sqeq_nlist** out)
 {
     cudaStream_t st = ctx->stream;
-    static const bool dbg = getenv("SQEQ_DEBUG") != nullptr;
-    const double t_0 = now_ms();
-    double t_alloc = 0, t_bin = 0, t_launch = 0, t_sync = 0;
     NLGeom g;
     fill_geom(g, box, cutoff, n);
     const int64_t ncells = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
@@ -778,7 +784,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     auto cleanup = [&](int code) {
         void* tmp[] = {cell_id, cell_count, cell_fill, flag, tmp64, ctr};
         for (void* p : tmp) if (p) cudaFreeAsync(p, st);
-        if (code != SQEQ_OK) nl_release(nl);
+        if (code != SQEQ_OK) { nl_release_storage(nl); delete nl; }
         return code;
     };
 #define NL_TRY(expr) do { int _r = (expr); if (_r != SQEQ_OK) return cleanup(_r); } while (0)
@@ -804,7 +810,6 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     NL_CUDA(cudaMemsetAsync(xq + n, 0x7f, sizeof(float4) * 32, st));    // 3.4e38: far from everything
 
     const int nb = ceil_div(n, 256);
-    t_alloc = now_ms();
     {
         StageTimer tm(ctx, SQEQ_T_NL_BIN);
         NL_CUDA(cudaMemsetAsync(cell_count, 0, sizeof(int) * (ncells + 1), st));
@@ -827,7 +832,6 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         NL_CUDA(cudaMemcpyAsync(nl->pos0, pos, sizeof(float) * 3 * n, cudaMemcpyDeviceToDevice, st));   // for sqeq_nl_max_drift
         NL_CUDA(cudaGetLastError());
     }
-    t_bin = now_ms();
     {
         StageTimer tm(ctx, SQEQ_T_NL_PAIRS);
         // sizes: from the previous build of the same system if there was one, else from the mean
@@ -857,8 +861,9 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         // local entries are stored as byte offsets of the staged float4 slots (index << 4) while the most
         // populous neighbourhood, dummy slot included, stays below 4096 atoms
         int lshift = (ctx->nl_last_n == n && ctx->nl_last_max_pop > 4094) ? 0 : 4;
-        const int cap_row_max = 6528;      // 8 staging rows of 4 B entries in 227 KB of shared memory
         for (int attempt = 0;; ++attempt) {
+            // the staging rows must fit the 227 KB a block can opt into (minus the kernel's static shared memory)
+            const int cap_row_max = (int)(((size_t)232448 - 1024 - pairs_smem(0, local)) / (NL_WARPS * (local ? sizeof(uint16_t) : sizeof(uint32_t)))) & ~31;
             if (cap_row > cap_row_max)
                 return cleanup(sqeq_fail(ctx, SQEQ_ECAPACITY,
                         "sqeq_nl_build: a row has %d neighbours; rows above %d are not supported", cap_row, cap_row_max));
@@ -870,11 +875,9 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
             *hinit = init;
             NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
             NL_TRY(launch_pairs(ctx, nl, pos, g, local, local ? lshift : 0, est_row, cap_row, capacity, ctr, st));
-            t_launch = now_ms();
             NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaStreamSynchronize(st));
-            t_sync = now_ms();
             if (h_flag[0] & 1)
                 return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
                                          "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
@@ -888,7 +891,11 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
             if (!cap_ok || !fmt_ok) {
                 NL_CUDA(cudaFreeAsync(nl->nbr, st));
                 nl->nbr = nullptr;
-                if (!cap_ok) capacity = (size_t)h->cursor;
+                // the cursor of a failed pass is not reproducible (rows take their places in the order warps
+                // finish, so which rows fall back to the global cursor varies): leave room for every group to
+                // spill one padded row, plus 2 %
+                if (!cap_ok) capacity = (size_t)h->cursor + (size_t)h->cursor / 50 +
+                                        (size_t)nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2] * (size_t)cap_row;
                 if (!fmt_ok) local = false;
             }
             if (!shift_ok) lshift = 0;
@@ -907,10 +914,8 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         ctx->nl_last_max_row = nl->max_row;
     }
     *out = nl;
+    ctx->lists.push_back(nl);
     cleanup(SQEQ_OK);
-    if (dbg)
-        fprintf(stderr, "[sqeq] nl_build host ms: alloc %.3f bin-enqueue %.3f pairs-enqueue %.3f sync-wait %.3f tail %.3f\n",
-                t_alloc - t_0, t_bin - t_alloc, t_launch - t_bin, t_sync - t_launch, now_ms() - t_sync);
     return SQEQ_OK;
 #undef NL_TRY
 #undef NL_CUDA
@@ -958,35 +963,41 @@ int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj
     int* cnt = nullptr;
     int64_t* off = nullptr;
     int* flag = nullptr;
-    CUDA_TRY(ctx, cudaMalloc((void**)&cnt, sizeof(int) * (n + 1)));
-    CUDA_TRY(ctx, cudaMalloc((void**)&off, sizeof(int64_t) * (n + 1)));
-    CUDA_TRY(ctx, cudaMalloc((void**)&flag, sizeof(int)));
-    CUDA_TRY(ctx, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
-    CUDA_TRY(ctx, cudaMemsetAsync(flag, 0, sizeof(int), st));
-    // a 16-bit local list is expanded to j | code entries first (same row offsets)
-    uint32_t* nbr32 = (uint32_t*)nl->nbr;
     uint32_t* expanded = nullptr;
-    if (nl->fmt == 1) {
-        CUDA_TRY(ctx, cudaMalloc((void**)&expanded, sizeof(uint32_t) * (size_t)nl->n_slots));
-        k_local_to_global<<<nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2], 256, 0, st>>>(
-            nl->cell_start, nl->gg, nl->row_start, nl->row_len, (const uint16_t*)nl->nbr, nl->lshift, expanded);
+    // temporaries from the context's stream-ordered pool, released on every path
+    auto body = [&]() -> int {
+        SQEQ_TRY(pool_alloc(ctx, (void**)&cnt, sizeof(int) * (n + 1)));
+        SQEQ_TRY(pool_alloc(ctx, (void**)&off, sizeof(int64_t) * (n + 1)));
+        SQEQ_TRY(pool_alloc(ctx, (void**)&flag, sizeof(int)));
+        CUDA_TRY(ctx, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
+        CUDA_TRY(ctx, cudaMemsetAsync(flag, 0, sizeof(int), st));
+        // a 16-bit local list is expanded to j | code entries first (same row offsets)
+        const uint32_t* nbr32 = (const uint32_t*)nl->nbr;
+        if (nl->fmt == 1) {
+            SQEQ_TRY(pool_alloc(ctx, (void**)&expanded, sizeof(uint32_t) * (size_t)nl->n_slots));
+            k_local_to_global<<<nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2], 256, 0, st>>>(
+                nl->cell_start, nl->gg, nl->row_start, nl->row_len, (const uint16_t*)nl->nbr, nl->lshift, expanded);
+            KERNEL_CHECK(ctx);
+            nbr32 = expanded;
+        }
+        k_export_count<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, nl->row_start, nl->row_len, nbr32, nl->perm, cnt);
         KERNEL_CHECK(ctx);
-        nbr32 = expanded;
-    }
-    k_export_count<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, nl->row_start, nl->row_len, nbr32, nl->perm, cnt);
-    KERNEL_CHECK(ctx);
-    int r = exclusive_scan<int>(ctx, n + 1, cnt, off, st);
-    if (r == SQEQ_OK) {
+        SQEQ_TRY(exclusive_scan<int>(ctx, n + 1, cnt, off, st));
         k_export_fill<<<(unsigned)n, 256, 0, st>>>(n, nl->row_start, nl->row_len, nbr32, nl->perm, nl->wrapc, off,
                                                     oi, oj, shift3, flag);
-        ctx->launches++;
-    }
+        KERNEL_CHECK(ctx);
+        return SQEQ_OK;
+    };
+    const int r = body();
     int h_flag = 0;
     int64_t total = 0;
-    cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
-    cudaMemcpyAsync(&total, off + n, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    if (r == SQEQ_OK) {
+        cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(&total, off + n, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    }
     cudaError_t e = cudaStreamSynchronize(st);
-    cudaFree(cnt); cudaFree(off); cudaFree(flag); cudaFree(expanded);
+    for (void* p : {(void*)cnt, (void*)off, (void*)flag, (void*)expanded})
+        if (p) cudaFreeAsync(p, st);
     if (r != SQEQ_OK) return r;
     if (e != cudaSuccess) return sqeq_fail(ctx, SQEQ_ECUDA, "sqeq_nl_export: %s", cudaGetErrorString(e));
     if (h_flag & 2) return sqeq_fail(ctx, SQEQ_ECAPACITY, "sqeq_nl_export: a row has more than %d upper neighbours", EXPORT_CAP);

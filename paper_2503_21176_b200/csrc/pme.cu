@@ -754,10 +754,6 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     int nt = 256;
     const bool tiles = plan_tiles(ctx, nl, P, tg, tile_bytes, nt);
     const int ngroups = tiles ? tg.ng[0] * tg.ng[1] * tg.ng[2] : 0;
-    static const bool debug = getenv("SQEQ_DEBUG") != nullptr;
-    if (debug)
-        fprintf(stderr, "[sqeq] pme tiles=%d nt=%d g=(%d,%d,%d) groups=%d T=(%d,%d,%d) ZS=%d XS=%d bytes=%zu\n", (int)tiles,
-                nt, tg.g[0], tg.g[1], tg.g[2], ngroups, tg.T[0], tg.T[1], tg.T[2], tg.ZS, tg.XS, tile_bytes);
     const int K0 = ctx->K[0], K1 = ctx->K[1], K2 = ctx->K[2], K2h = K2 / 2 + 1;
     const size_t G3 = (size_t)K0 * K1 * K2;
     float* grid = (float*)ctx->grid.p;

@@ -250,6 +250,18 @@ def test_neighbour_rows_are_the_symmetric_closure():
         assert np.array_equal(sr[jr < a], -s[j == a])
 
 
+def test_neighbour_rows_upper_is_a_slice_of_the_list():
+    """The chunked walk used by the full-size GPU list tests returns exactly rows i0..i1 of the list
+    (also when the first capacity guess is too small)."""
+    pos, q = W.make(0)
+    box = W.CONFIGS[0].box
+    i, j, s = oracle.neighbour_list(pos, box, 9.0)
+    for i0, i1, cap in ((0, 648, 400), (100, 230, 16), (640, 648, 4)):
+        m = (i >= i0) & (i < i1)
+        oi, oj, os_ = oracle.neighbour_rows_upper(pos, box, 9.0, i0, i1, cap=cap)
+        assert np.array_equal(oi, i[m]) and np.array_equal(oj, j[m]) and np.array_equal(os_, s[m])
+
+
 # ---------------------------------------------------------------- PME pieces
 def test_bspline_vs_scipy_and_knot_values():
     for p in (4, 5, 6, 8):
