@@ -44,6 +44,8 @@ typedef struct sqeq_nlist sqeq_nlist;  /* opaque: device neighbour list + cell-m
 /* device: CUDA ordinal.  cuda_stream: a cudaStream_t (may be NULL = legacy default stream); the
  * caller keeps ownership of the stream. */
 int  sqeq_create (sqeq_ctx** out, int device, void* cuda_stream);
+/* Synchronises, releases everything the context owns -- including the device storage of neighbour lists that
+ * are still alive: their handles stay valid for sqeq_nl_free / sqeq_nl_count only. */
 int  sqeq_destroy(sqeq_ctx* ctx);
 /* Context-owned NUL-terminated message of the last failing call; never freed by the caller.
  * ctx may be NULL (returns the message of the last failing sqeq_create in this thread). */
@@ -142,6 +144,22 @@ int  sqeq_coulomb_host_submit(sqeq_ctx* ctx, int slot, const sqeq_nlist* nl, int
                               double rc, double alpha, const int grid[3], int order,
                               float* phi_host, float* force_host, int want_energy);
 int  sqeq_coulomb_host_wait(sqeq_ctx* ctx, int slot, double* energy);
+
+/* ---- fixed geometry, many charge vectors ("Each iteration involves
+ * calculating a Coulomb-like potential") ------------------------------------------------------
+ * Every Krylov iteration of a QEq solve and all 2 + m evaluations of a shadow-MD step repeat the evaluation on
+ * the SAME positions with another charge vector.  sqeq_geometry_set prepares the positions once (re-gather,
+ * fractional grid coordinates; arguments as for sqeq_coulomb); each sqeq_coulomb_fixed then evaluates one
+ * charge vector q (device fp32 [n]) on them.  The first evaluation also writes the GEOMETRY CACHE -- per row
+ * of the list the entries with r < rc and their erfc(alpha r)/r (and the field factor when forces are asked
+ * for) -- and the later ones run the real-space part as a sparse product over it: no erfc/exp/rsqrt, no skin
+ * entries (10 B per list slot of device memory, owned by the context).  phi may be NULL when force is given
+ * (field only).  The cache is dropped by any other evaluation or neighbour build on the context.  No
+ * synchronisation; the energy, if asked for, is read with sqeq_energy_fetch.  sqeq_qeq_solve and
+ * sqeq_shadow_md_* use the same mechanism internally. */
+int  sqeq_geometry_set (sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
+                        double rc, double alpha, const int grid[3], int order);
+int  sqeq_coulomb_fixed(sqeq_ctx* ctx, int64_t n, const float* q, float* phi, float* force, int want_energy);
 
 /* Parts of the last sqeq_coulomb call on this context, for diagnostics and stage-wise parity
  * (caller order; device fp32 outputs, any may be NULL): phi_real[n], F_real[n][3], phi_rec[n],

@@ -66,6 +66,8 @@ def load():
     L.sqeq_coulomb_host_wait.argtypes = [vp, cint, dp]
     L.sqeq_coulomb_enqueue.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
     L.sqeq_energy_fetch.argtypes = [vp, dp]
+    L.sqeq_geometry_set.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint]
+    L.sqeq_coulomb_fixed.argtypes = [vp, i64, vp, vp, vp, cint]
     L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_parts.argtypes = [vp, vp, i64, vp, vp, vp, vp, dp]
     L.sqeq_pme_grid.argtypes = [vp, cint, vp]
@@ -227,6 +229,20 @@ class Context:
                                                 _grid(grid), int(order), _ptr(phi, torch.float32, n),
                                                 _ptr(force, torch.float32, 3 * n) if force is not None else None,
                                                 int(want_energy)))
+
+    def geometry_set(self, nl, pos, box, rc, alpha, grid, order=6):
+        """sqeq_geometry_set: prepare the positions once for many charge vectors (coulomb_fixed)."""
+        n = pos.shape[0]
+        self._check(load().sqeq_geometry_set(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n), _box(box),
+                                             float(rc), float(alpha), _grid(grid), int(order)))
+
+    def coulomb_fixed(self, q, phi=None, force=None, want_energy=False):
+        """sqeq_coulomb_fixed: one charge vector on the geometry of geometry_set; no synchronisation."""
+        n = q.shape[0]
+        self._check(load().sqeq_coulomb_fixed(self.handle, n, _ptr(q, torch.float32, n),
+                                              _ptr(phi, torch.float32, n) if phi is not None else None,
+                                              _ptr(force, torch.float32, 3 * n) if force is not None else None,
+                                              int(want_energy)))
 
     def energy_fetch(self):
         e = ctypes.c_double()

@@ -144,7 +144,8 @@ int sqeq_destroy(sqeq_ctx* ctx)
         cufftDestroy(ctx->plan_r2c);
         cufftDestroy(ctx->plan_c2r);
     }
-    DevBuf* bufs[] = {&ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
+    DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len,
+                      &ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
                       &ctx->base, &ctx->real_out, &ctx->rec_out, &ctx->scal, &ctx->kry_V,
                       &ctx->kry_w, &ctx->kry_h};
     for (DevBuf* b : bufs)
@@ -348,9 +349,10 @@ int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const 
 }
 
 int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc,
-                 double alpha, float* phi, float* force, bool want_energy, bool field_mode)
+                 double alpha, float* phi, float* force, bool want_energy, bool field_mode, int geom)
 {
     const bool want_force = force != nullptr;
+    const bool want_phi = phi != nullptr || want_energy;
     // One stream by default.  SQEQ_OVERLAP=1 runs the real-space sum as a persistent grid of two lean
     // (32-register) blocks per SM and forks PME onto the side stream, where one PME block per SM fits beside
     // them: at cfg 4 the device-side step goes from 0.624 to 0.587 ms, but a single synchronous evaluation
@@ -358,7 +360,7 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
     // with stage timing on, where every event pair brackets one kernel running alone.
     if (ctx->profiling || !ctx->overlap) {
         SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream));
-        SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream));
+        SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream, geom, want_phi));
     } else {
         CUDA_TRY(ctx, cudaEventRecord(ctx->ev_fork, ctx->stream));
         CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->stream2, ctx->ev_fork, 0));
@@ -384,6 +386,42 @@ extern "C" int sqeq_coulomb_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t
     SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
     SQEQ_TRY(prep_atoms(ctx, nl, pos, q, ctx->K, ctx->stream));
     SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, phi, force, want_energy != 0));
+    ctx->energy_pending = want_energy != 0;
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_geometry_set(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
+                                 double rc, double alpha, const int grid[3], int order)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    ctx->fixed.nl = nullptr;
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_geometry_set"));
+    if (!pos) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_geometry_set: pos is NULL");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    SQEQ_TRY(prep_atoms(ctx, nl, pos, nullptr, ctx->K, ctx->stream));      // charges come with each evaluation
+    ctx->fixed.nl = nl; ctx->fixed.serial = nl->serial; ctx->fixed.n = n;
+    ctx->fixed.geom_serial = ctx->geom_serial;
+    for (int d = 0; d < 3; ++d) ctx->fixed.box[d] = box[d];
+    ctx->fixed.rc = rc; ctx->fixed.alpha = alpha;
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_coulomb_fixed(sqeq_ctx* ctx, int64_t n, const float* q, float* phi, float* force, int want_energy)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    const sqeq_nlist* nl = ctx->fixed.nl;
+    bool alive = false;
+    for (const sqeq_nlist* l : ctx->lists) alive = alive || (l == nl && l->serial == ctx->fixed.serial);
+    if (!nl || !alive || ctx->geom_serial != ctx->fixed.geom_serial)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_fixed: no geometry set (sqeq_geometry_set), its list was freed, or "
+                                           "another evaluation has replaced it");
+    if (n != ctx->fixed.n || !q || (!phi && !force))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_fixed: n differs from the geometry, q is NULL, or no output asked for");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    SQEQ_TRY(prep_charges(ctx, nl, q, nullptr, ctx->stream));
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, ctx->fixed.box, ctx->fixed.rc, ctx->fixed.alpha, phi, force, want_energy != 0, false,
+                          GEOM_FIXED));
     ctx->energy_pending = want_energy != 0;
     return SQEQ_OK;
 }

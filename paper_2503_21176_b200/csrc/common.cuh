@@ -28,6 +28,17 @@ struct TimerRec {
     cudaEvent_t a, b;
 };
 
+// NEXT-1 geometry cache of the real-space sum (realspace.cu): per row of the list, the entries with r < rc and
+// their t = erfc(alpha r)/r (and g), valid for (list, positions of the last prep_atoms, rc, alpha)
+enum { GEOM_NEW = 0, GEOM_FIXED = 1 };
+struct GeomCache {
+    bool valid = false;
+    const sqeq_nlist* nl = nullptr;
+    uint64_t serial = 0;
+    double rc = 0, alpha = 0;
+    DevBuf idx, t, len;
+};
+
 struct sqeq_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -81,6 +92,11 @@ struct sqeq_ctx {
     DevBuf vec_f[6];  // float  [n] scratch charge / potential vectors
     DevBuf vec_d[6];  // double [n] scratch
     DevBuf vec_f3[2]; // float  [n][3] scratch forces
+    GeomCache gc;
+    // sqeq_geometry_set / sqeq_coulomb_fixed session
+    uint64_t geom_serial = 0;             // counts prep_atoms calls: which positions xq/frac/base hold
+    struct { const sqeq_nlist* nl = nullptr; uint64_t serial = 0, geom_serial = 0; int64_t n = 0; double box[3] = {0, 0, 0}; double rc = 0, alpha = 0; } fixed;
+    uint64_t nl_serial = 0;               // build counter: tells a list from a later one at the same address
     DevBuf stage[4];  // device staging for sqeq_coulomb_host: pos, q, phi, force
     // sqeq_coulomb_host_submit / _wait: two slots, copies on their own streams beside the evaluation stream
     DevBuf slot_buf[2][5];                // pos, q, phi, force, energy (one double)
@@ -123,6 +139,7 @@ struct sqeq_nlist {
     longlong2* grp_slice = nullptr;  // [cell groups] (first slot, slots used) of the group's reserved slice of nbr
     void*     nbr = nullptr;         // [>= n_slots] entries: fmt 0: uint32 j (27 bits) | image code << 27;
                                      //                          fmt 1: uint16 local index in the group's neighbourhood
+    uint64_t  serial = 0;            // ctx->nl_serial at build time
     int       fmt = 0;
     int       max_pop = 0;           // fmt 1: largest neighbourhood population of a group
     int       lshift = 0;            // fmt 1: entries are local index << lshift (4: byte offsets of float4 slots)
@@ -202,7 +219,7 @@ int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const floa
 int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const double* q_d,
                  cudaStream_t st);
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
-                  cudaStream_t st);
+                  cudaStream_t st, int geom = GEOM_NEW, bool want_phi = true);
 int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3], int order);
 // nl supplies the cell-major atom runs the shared-memory tiles are built on (NULL: global kernels)
 int pme_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,
@@ -211,8 +228,11 @@ int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, 
                  bool want_energy, bool field_mode, cudaStream_t st);
 // Full evaluation on prepared geometry (used by coulomb, qeq and md drivers).
 // field_mode: `force` receives the per-unit-charge field f_i (F_i = q_i f_i) instead of F_i.
+// geom = GEOM_FIXED: the caller evaluates several charge vectors on the positions of the last prep_atoms; the
+// first such evaluation writes the geometry cache, later ones read it (phi may then be NULL: field only).
 int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc,
-                 double alpha, float* phi, float* force, bool want_energy, bool field_mode = false);
+                 double alpha, float* phi, float* force, bool want_energy, bool field_mode = false,
+                 int geom = GEOM_NEW);
 
 // Generic restarted/unrestarted GMRES on device fp64 vectors (qeq.cu); x_out points into ctx->kry_w.
 int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double*, double*)>& apply,

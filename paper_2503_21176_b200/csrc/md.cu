@@ -232,7 +232,8 @@ static int md_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* 
     SQEQ_TRY(pme_setup(ctx, box, p->alpha, p->grid, p->order));
     SQEQ_TRY(prep_atoms(ctx, nl, pos, chi, ctx->K, st));            // geometry; charge slot set below
     SQEQ_TRY(prep_charges(ctx, nl, nullptr, nv, st));
-    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, phi, f_n, false, true));
+    // all 2 + m evaluations of this time level share the geometry: the first one writes the cache (t and g)
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, phi, f_n, false, true, GEOM_FIXED));
     {
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
         CUDA_TRY(ctx, cudaMemsetAsync(scal + S_T, 0, sizeof(double) * 7, st));
@@ -242,7 +243,7 @@ static int md_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* 
         KERNEL_CHECK(ctx);
     }
     SQEQ_TRY(prep_charges(ctx, nl, nullptr, res, st));
-    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, phi_w, f_d, false, true));
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, nullptr, f_d, false, true, GEOM_FIXED));     // field only
     {
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
         k_md_forces<<<nb, 256, 0, st>>>(n, q, nv, f_n, f_d, p->ke, force);
@@ -267,7 +268,7 @@ static int md_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* 
         };
         auto apply = [&](const double* w, double* out) {
             SQEQ_TRY(prep_charges(ctx, nl, nullptr, w, st));
-            SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, phi_w, nullptr, false));
+            SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, phi_w, nullptr, false, false, GEOM_FIXED));
             StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
             CUDA_TRY(ctx, cudaMemsetAsync(scal + S_JAC, 0, sizeof(double), st));
             k_md_jac_reduce<<<nb, 256, 0, st>>>(n, u, phi_w, p->ke, scal);

@@ -773,6 +773,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     const int64_t ncells = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
     sqeq_nlist* nl = new sqeq_nlist();
     nl->ctx = ctx;
+    nl->serial = ++ctx->nl_serial;
     nl->n = n;
     nl->cutoff = cutoff;
     for (int d = 0; d < 3; ++d) { nl->box[d] = box[d]; nl->ncell[d] = g.nc[d]; }
@@ -805,6 +806,8 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
     NL_TRY(pool_alloc(ctx, (void**)&nl->row_len, sizeof(int) * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->pos0, sizeof(float) * 3 * n));
     NL_TRY(pool_alloc(ctx, (void**)&nl->grp_slice, sizeof(longlong2) * (size_t)nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2]));
+    ctx->gc.valid = false;             // the build reuses ctx->xq: any prepared geometry is gone
+    ctx->geom_serial++;
     NL_TRY(sqeq_reserve(ctx, ctx->xq, sizeof(float4) * (n + 32)));     // 32 padding entries: see k_pairs
     float4* xq = (float4*)ctx->xq.p;
     NL_CUDA(cudaMemsetAsync(xq + n, 0x7f, sizeof(float4) * 32, st));    // 3.4e38: far from everything

@@ -298,7 +298,8 @@ static int qeq_apply(const QeqOp& op, const double* v, double* w)
     cudaStream_t st = ctx->stream;
     const int64_t n = op.n;
     SQEQ_TRY(prep_charges(ctx, op.nl, nullptr, v, st));
-    SQEQ_TRY(coulomb_eval(ctx, op.nl, n, op.box, op.rc, op.alpha, op.phi, nullptr, false));
+    // fixed geometry: the first mat-vec writes the geometry cache, the others are sparse products over it
+    SQEQ_TRY(coulomb_eval(ctx, op.nl, n, op.box, op.rc, op.alpha, op.phi, nullptr, false, false, GEOM_FIXED));
     StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
     CUDA_TRY(ctx, cudaMemsetAsync(w + n, 0, sizeof(double), st));
     k_qeq_matvec<<<ceil_div(n, 256), 256, 0, st>>>(n, v, op.J, op.phi, op.ke, w);

@@ -25,7 +25,7 @@ __global__ void k_prep(int64_t n, const float* __restrict__ pos, const float* __
     const int o = perm[s];
     const char4 w = wrapc[s];
     const int wd[3] = {w.x, w.y, w.z};
-    const float qi = q[o];
+    const float qi = q ? q[o] : 0.f;
     float xw[3], fw[3];
     int f[3];
 #pragma unroll
@@ -73,6 +73,8 @@ int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const floa
     SQEQ_TRY(sqeq_reserve(ctx, ctx->base, sizeof(int4) * n));
     PrepGeom g;
     for (int d = 0; d < 3; ++d) { g.L[d] = nl->box[d]; g.K[d] = K ? K[d] : 0; }
+    ctx->gc.valid = false;                      // new positions: the geometry cache is stale
+    ctx->geom_serial++;
     StageTimer tm(ctx, SQEQ_T_PREP, st);
     k_prep<<<ceil_div(n, 256), 256, 0, st>>>(n, pos, q, nl->perm, nl->wrapc, g, (float4*)ctx->xq.p,
                                               (float4*)ctx->frac.p, (int4*)ctx->base.p);
@@ -201,6 +203,12 @@ k_real(int64_t n, const float4* __restrict__ xq, const int64_t* __restrict__ row
 #ifndef REAL_BPS_P
 #define REAL_BPS_P 4        // ... potential-only kernel
 #endif
+#ifndef REAL_BPS_C
+#define REAL_BPS_C 3        // ... cache-writing variants
+#endif
+#ifndef REAL_BATCH_C
+#define REAL_BATCH_C 4      // entry loads in flight, cache-writing variants
+#endif
 __device__ __forceinline__ float4 lds128(unsigned addr)
 {
     float4 v;
@@ -212,21 +220,32 @@ __device__ __forceinline__ float4 lds128(unsigned addr)
 // LEAN: 32 registers (four blocks per SM would fit) and 4 loads in flight -- the variant launched as a
 // PERSISTENT grid of a few blocks per SM beside the PME kernels (SQEQ_OVERLAP=1), each block walking over
 // cell groups, so that the register file and shared memory have room for both.
-template <bool FORCE, bool SCALED, bool LEAN = false>
-__global__ void __launch_bounds__(REAL_NT, LEAN ? 4 : (FORCE ? REAL_BPS_F : REAL_BPS_P))
+// CACHE (geometry cache): also write, per row, the COMPACT list of the entries with
+// r < rc (same 16-bit entry, same row offset) and their t = erfc(alpha r)/r.  Later evaluations on the same
+// geometry (Krylov iterations, the second force evaluation of an MD step) use that list: potentials are a sparse
+// product over t (k_real_cached: no MUFU, no skin entries), forces run this kernel over the compact rows.
+struct RealCache {
+    uint16_t* idx;     // [n_slots] compact rows, padded to whole warps with the dummy entry
+    float*    t;       // [n_slots]
+    int*      len;     // [n] entries of the compact row
+};
+
+template <bool FORCE, bool SCALED, bool LEAN = false, int CACHE = 0>
+__global__ void __launch_bounds__(REAL_NT, CACHE ? REAL_BPS_C : (LEAN ? 4 : (FORCE ? REAL_BPS_F : REAL_BPS_P)))
 k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
               const int64_t* __restrict__ row_start, const int* __restrict__ row_len,
               const uint16_t* __restrict__ nbr, const longlong2* __restrict__ grp_slice, RealParams p,
-              int ngroups, float4* __restrict__ out)
+              int ngroups, float4* __restrict__ out, RealCache rcache)
 {
     extern __shared__ __align__(16) float4 xs[];               // [neighbourhood population + 1]
     __shared__ GroupPiece pieces[GRP_MAXPIECE];
     __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
     for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
     if (grp != (int)blockIdx.x) __syncthreads();               // the previous group's shared state is still being read
-    {
+    if (grp_slice) {
         // the group's rows sit in one contiguous slice of the list (k_pairs reserves it per group): ask for it
-        // in L2 now, so that the entry loads below meet L2 latency instead of DRAM latency
+        // in L2 now, so that the entry loads below meet L2 latency instead of DRAM latency (not for the compact
+        // rows of the geometry cache, which fill only a part of each row's slots)
         const longlong2 sl = grp_slice[grp];
         const char* base = (const char*)(nbr + sl.x);
         const long long bytes = sl.y * (long long)sizeof(uint16_t);
@@ -274,15 +293,21 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
         const float4 xi = __ldg(xq + s);
         // rows are padded to whole 32-entry steps (the padding points at the dummy slot), so the loop is
         // uniform over the warp
-        const uint16_t* __restrict__ row = nbr + row_start[s] + lane;
+        const int64_t r0 = row_start[s];
+        const uint16_t* __restrict__ row = nbr + r0 + lane;
         const int nst = (row_len[s] + 31) >> 5;
         const unsigned xs_addr = (unsigned)__cvta_generic_to_shared(xs);
         float phi = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+        unsigned ccnt = 0;                                         // CACHE: entries of the compact row so far
+        const unsigned lt = (1u << lane) - 1u;
+        uint16_t* __restrict__ crow_i = CACHE ? rcache.idx + r0 : nullptr;
+        float* __restrict__ crow_t = CACHE ? rcache.t + r0 : nullptr;
         auto pair = [&](unsigned e) {
             const float4 xj = SCALED ? lds128(xs_addr + e) : xs[e];
             const float dx = xi.x - xj.x, dy = xi.y - xj.y, dz = xi.z - xj.z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            const float qj = r2 < p.rc2 ? xj.w : 0.f;
+            const bool inr = r2 < p.rc2;
+            const float qj = inr ? xj.w : 0.f;
             const float rinv = mufu_rsqrt(r2);
             const float ex = mufu_ex2(p.na2l2e * r2);             // exp(-alpha^2 r^2)
             const float t = erfc_from_exp(r2 * rinv, p.pa, ex) * rinv;   // erfc(alpha r)/r
@@ -293,12 +318,21 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
                 fy = fmaf(gq, dy, fy);
                 fz = fmaf(gq, dz, fz);
             }
+            if (CACHE) {
+                const unsigned m = __ballot_sync(0xffffffffu, inr);
+                if (inr) {
+                    const unsigned d = ccnt + __popc(m & lt);
+                    crow_i[d] = (uint16_t)e;
+                    crow_t[d] = t;
+                }
+                ccnt += __popc(m);
+            }
         };
         // four entry loads in flight ahead of the four pair evaluations that use them
         // the entry loads of B steps are issued together ahead of the B pair evaluations that use them
         // (B = 16/8/4 while the row lasts): the potential-only kernel has registers for 16 in flight, the
         // force kernel for 4
-        constexpr int BMAX = LEAN ? 4 : (FORCE ? REAL_BATCH_F : REAL_BATCH_P);
+        constexpr int BMAX = CACHE ? REAL_BATCH_C : (LEAN ? 4 : (FORCE ? REAL_BATCH_F : REAL_BATCH_P));
         int it = 0;
         if (BMAX >= 16)
             for (; it + 16 <= nst; it += 16) {
@@ -327,6 +361,15 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
             it += 2;
         }
         if (it < nst) pair(__ldg(row + 32 * it));
+        if (CACHE) {
+            // pad the compact row to whole warps with the dummy entry (charge 0, t = g = 0)
+            const unsigned padn = (ccnt + 31u) & ~31u;
+            if (ccnt + lane < padn) {
+                crow_i[ccnt + lane] = (uint16_t)(SCALED ? gi.pop << 4 : gi.pop);
+                crow_t[ccnt + lane] = 0.f;
+            }
+            if (lane == 0) rcache.len[s] = (int)ccnt;
+        }
         if (FORCE) {
             const float v = warp_reduce4(fx, fy, fz, phi, lane);        // lanes 0 / 8 / 16 / 24: fx / fy / fz / phi
             if ((lane & 7) == 0) ((float*)(out + s))[lane >> 3] = v;
@@ -339,8 +382,152 @@ k_real_staged(const float4* __restrict__ xq, const int* __restrict__ cell_start,
     }   // groups
 }
 
+// The same sums over the geometry cache a CACHE pass of k_real_staged left behind (NEXT-1): per row the compact
+// list of in-range entries with t = erfc(alpha r)/r (MODE 0: potential, phi_i = sum_j q_j t_ij -- a sparse
+// matrix-vector product, 6 B per entry, no MUFU, the block stages only the neighbourhood's CHARGES) or
+// g (MODE 1: per-unit-charge field, f_i = sum_j q_j g_ij (r_i - r_j), staged float4 as above).  HBM-bound: the
+// loads of 8 steps are issued ahead of their use.
+template <int MODE, bool SCALED>
+__global__ void __launch_bounds__(REAL_NT, MODE == 2 ? 2 : 3)
+k_real_cached(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
+              const int64_t* __restrict__ row_start, RealParams p, int ngroups, float4* __restrict__ out,
+              RealCache rcache)
+{
+    extern __shared__ __align__(16) float4 xs[];               // MODE 1: float4 [pop + 1]; MODE 0: float [pop + 1]
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    float* qs = (float*)xs;
+    const int grp = blockIdx.x;
+    const GroupInfo gi = group_layout(gg, cell_start, grp, pieces, &s_scratch);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int r = 0; r < GRP_G * GRP_G; ++r) {
+            s_rpre[r] = acc;
+            const int ix = r / GRP_G, iy = r % GRP_G;
+            if (ix < gi.ge[0] && iy < gi.ge[1]) {
+                const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+                const int beg = cell_start[colw];
+                s_roff[r] = beg - acc;
+                acc += cell_start[colw + gi.ge[2]] - beg;
+            } else {
+                s_roff[r] = 0;
+            }
+        }
+        s_rpre[GRP_G * GRP_G] = acc;
+        if (MODE == 0) qs[gi.pop] = 0.f; else xs[gi.pop] = make_float4(1e15f, 1e15f, 1e15f, 0.f);
+    }
+    const int np = gi.ncol * 3;
+    for (int ip = wid; ip < np; ip += REAL_NT / 32) {
+        const GroupPiece pc = pieces[ip];
+        if (pc.len == 0) continue;
+        if (MODE == 0) {
+            for (int k = lane; k < pc.len; k += 32) qs[pc.lbase + k] = __ldg(&xq[pc.gbeg + k].w);
+        } else {
+            const float sx = (pc.code / 9 - 1) * p.Lx, sy = ((pc.code / 3) % 3 - 1) * p.Ly, sz = (pc.code % 3 - 1) * p.Lz;
+            for (int k = lane; k < pc.len; k += 32) {
+                float4 v = __ldg(xq + pc.gbeg + k);
+                v.x += sx; v.y += sy; v.z += sz;
+                xs[pc.lbase + k] = v;
+            }
+        }
+    }
+    __syncthreads();
+    const int natoms = s_rpre[GRP_G * GRP_G];
+    const int p1 = s_rpre[1], p2 = s_rpre[2], p3 = s_rpre[3];
+    const unsigned xs_addr = (unsigned)__cvta_generic_to_shared(xs);
+    static_assert(MODE == 0, "only the potential is taken from the cache; forces run k_real_staged over the compact rows");
+    const float* __restrict__ cval = rcache.t;
+    constexpr int NW = REAL_NT / 32;
+    for (int base = 0; base < natoms; base += NW * 32) {
+    // lane l fetches the row offset and length of the l-th row this warp will take: one round trip for all of
+    // them instead of one per row
+    int my_s = 0, my_len = 0;
+    int64_t my_r0 = 0;
+    {
+        const int ia = base + wid + NW * lane;
+        if (ia < natoms) {
+            my_s = ia + s_roff[(ia >= p1) + (ia >= p2) + (ia >= p3)];
+            my_r0 = row_start[my_s];
+            my_len = rcache.len[my_s];
+        }
+    }
+    for (int l = 0; l < 32; ++l) {
+        const int ia = base + wid + NW * l;
+        if (ia >= natoms) break;
+        const int s = __shfl_sync(0xffffffffu, my_s, l);
+        const int len_s = __shfl_sync(0xffffffffu, my_len, l);
+        // A lane takes FOUR consecutive entries of every 128-entry chunk of the row: one 8-byte load of the
+        // entries and one 16-byte load of their values per lane and chunk (rows start on multiples of 32
+        // entries, so both are aligned; a quad is either wholly inside the padded row or wholly outside).  The
+        // loads of up to four chunks -- a whole typical row of ~300 in-range entries -- are issued before the
+        // first use: the kernel is a stream from HBM.
+        const int64_t r0 = __shfl_sync(0xffffffffu, my_r0, l) + 4 * lane;
+        const uint2* __restrict__ ri = (const uint2*)(rcache.idx + r0);
+        const float4* __restrict__ rv = (const float4*)(cval + r0);
+        const float4* __restrict__ rt = (const float4*)(rcache.t + r0);
+        const int padlen = (len_s + 31) & ~31;
+        float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (MODE != 0) xi = __ldg(xq + s);
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+        auto term = [&](unsigned e, float v, float vt) {          // e: 16-bit entry in the low half
+            if (MODE == 0) {
+                float qj;
+                const unsigned a = xs_addr + (SCALED ? e >> 2 : e << 2);
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(qj) : "r"(a));
+                a3 = fmaf(qj, v, a3);
+            } else {
+                const float4 xj = SCALED ? lds128(xs_addr + e) : xs[e];
+                const float gq = xj.w * v;
+                a0 = fmaf(gq, xi.x - xj.x, a0);
+                a1 = fmaf(gq, xi.y - xj.y, a1);
+                a2 = fmaf(gq, xi.z - xj.z, a2);
+                if (MODE == 2) a3 = fmaf(xj.w, vt, a3);
+            }
+        };
+        constexpr int B = MODE == 2 ? 2 : 4;                       // chunks in flight
+        for (int c0 = 0; c0 < padlen; c0 += 128 * B) {
+            uint2 e[B];
+            float4 v[B], vt[B];
+#pragma unroll
+            for (int k = 0; k < B; ++k) {
+                const bool on = c0 + 128 * k + 4 * lane < padlen;
+                e[k] = make_uint2(0u, 0u);                          // entry 0 with value 0: contributes nothing
+                v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                vt[k] = v[k];
+                if (on) {
+                    e[k] = __ldg(ri + ((c0 + 128 * k) >> 2));
+                    v[k] = __ldg(rv + ((c0 + 128 * k) >> 2));
+                    if (MODE == 2) vt[k] = __ldg(rt + ((c0 + 128 * k) >> 2));
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < B; ++k) {
+                if (c0 + 128 * k < padlen) {                        // uniform over the warp
+                    term(e[k].x & 0xffffu, v[k].x, vt[k].x);
+                    term(e[k].x >> 16, v[k].y, vt[k].y);
+                    term(e[k].y & 0xffffu, v[k].z, vt[k].z);
+                    term(e[k].y >> 16, v[k].w, vt[k].w);
+                }
+            }
+        }
+        if (MODE == 0) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a3 += __shfl_xor_sync(0xffffffffu, a3, o);
+            if (lane == 0) out[s] = make_float4(0.f, 0.f, 0.f, a3);
+        } else {
+            const float v = warp_reduce4(a0, a1, a2, a3, lane);
+            if ((lane & 7) == 0) ((float*)(out + s))[lane >> 3] = v;
+        }
+    }
+    }   // row batches
+}
+
+// geom: GEOM_NEW = plain evaluation; GEOM_BUILD = plain evaluation that also writes the geometry cache (t, and g
+// when want_force); GEOM_REUSE_PHI / GEOM_REUSE_FIELD = potential / field from the cache.  The cache belongs to
+// (list, positions of the last prep_atoms, rc, alpha); the drivers that keep the geometry fixed ask for it.
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
-                  cudaStream_t st)
+                  cudaStream_t st, int geom, bool want_phi)
 {
     const int64_t n = nl->n;
     SQEQ_TRY(sqeq_reserve(ctx, ctx->real_out, sizeof(float4) * n));
@@ -355,19 +542,52 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     if (nl->fmt == 1) {
         const size_t smem = sizeof(float4) * ((size_t)nl->max_pop + 1);
         const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
+        const bool lean = ctx->overlap && !ctx->profiling;
+        GeomCache& gc = ctx->gc;
+        RealCache rcache = {(uint16_t*)gc.idx.p, (float*)gc.t.p, (int*)gc.len.p};
+        const bool fixed = geom != GEOM_NEW && !lean;
+        const bool hit = fixed && gc.valid && gc.nl == nl && gc.serial == nl->serial && gc.rc == rc && gc.alpha == alpha;
+        const uint16_t* list = (const uint16_t*)nl->nbr;
+        const int* lens = nl->row_len;
+        if (hit && !want_force) {
+            // NEXT-1: the potential as a sparse product over the cached t
+            const size_t sm = sizeof(float) * ((size_t)nl->max_pop + 1);
+            auto kern = nl->lshift ? k_real_cached<0, true> : k_real_cached<0, false>;
+            CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+            kern<<<ngroups, REAL_NT, sm, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, p, ngroups,
+                                               (float4*)ctx->real_out.p, rcache);
+            KERNEL_CHECK(ctx);
+            return SQEQ_OK;
+        }
+        if (hit) {
+            // forces on a cached geometry: the plain kernel over the compact rows (no skin entries)
+            list = (const uint16_t*)gc.idx.p;
+            lens = (const int*)gc.len.p;
+        }
+        const bool build = fixed && !hit;
+        if (build) {
+            // first evaluation on this geometry: also write the compact in-range rows and their t
+            SQEQ_TRY(sqeq_reserve(ctx, gc.idx, sizeof(uint16_t) * (size_t)nl->n_slots));
+            SQEQ_TRY(sqeq_reserve(ctx, gc.t, sizeof(float) * (size_t)nl->n_slots));
+            SQEQ_TRY(sqeq_reserve(ctx, gc.len, sizeof(int) * (size_t)n));
+            rcache = {(uint16_t*)gc.idx.p, (float*)gc.t.p, (int*)gc.len.p};
+            gc.valid = true; gc.nl = nl; gc.serial = nl->serial; gc.rc = rc; gc.alpha = alpha;
+        }
         // beside the PME side stream: a persistent grid of two lean blocks per SM leaves registers and shared
         // memory for one PME block per SM; otherwise one block per group
-        const bool lean = ctx->overlap && !ctx->profiling;
         auto kern = nl->lshift ? (want_force ? k_real_staged<true, true, false> : k_real_staged<false, true, false>)
                                : (want_force ? k_real_staged<true, false, false> : k_real_staged<false, false, false>);
         if (lean)
             kern = nl->lshift ? (want_force ? k_real_staged<true, true, true> : k_real_staged<false, true, true>)
                               : (want_force ? k_real_staged<true, false, true> : k_real_staged<false, false, true>);
+        if (build)
+            kern = nl->lshift ? (want_force ? k_real_staged<true, true, false, 1> : k_real_staged<false, true, false, 1>)
+                              : (want_force ? k_real_staged<true, false, false, 1> : k_real_staged<false, false, false, 1>);
         const int lean_bps = ctx->real_lean_blocks;
         const int nblocks = lean ? (ngroups < lean_bps * ctx->sm_count ? ngroups : lean_bps * ctx->sm_count) : ngroups;
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<nblocks, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, nl->row_len,
-                                         (const uint16_t*)nl->nbr, nl->grp_slice, p, ngroups, (float4*)ctx->real_out.p);
+        kern<<<nblocks, REAL_NT, smem, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, lens,
+                                         list, hit ? nullptr : nl->grp_slice, p, ngroups, (float4*)ctx->real_out.p, rcache);
     } else if (want_force)
         k_real<true><<<nb, 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->row_start, nl->row_len, (const uint32_t*)nl->nbr, p,
                                           (float4*)ctx->real_out.p);

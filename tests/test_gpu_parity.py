@@ -444,6 +444,55 @@ def test_shadow_md_steps_config2_geometry(ctx):
     nl.free()
 
 
+@pytest.mark.parametrize("k", [2, 4])
+def test_fixed_geometry_cache(ctx, k):
+    """NEXT-1: sqeq_geometry_set + sqeq_coulomb_fixed -- several charge vectors on one geometry.
+    The first evaluation writes the geometry cache (compact in-range rows with erfc(alpha r)/r and the field
+    factor), the others are sparse products over it; every one must meet the bar of a plain evaluation.  List
+    with a skin and perturbed positions, so that skin entries are in the list and dropped from the cache.
+    cfg 2 on all atoms, cfg 4 at full size on sampled atoms."""
+    from paper_2503_21176_b200.binding import SqeqError
+    c = W.CONFIGS[k]
+    pos, q = inputs(k)
+    n = len(q)
+    rng = np.random.default_rng(40 + k)
+    nl = ctx.nl_build(dev(pos), c.box, c.rc + 1.0)
+    p = W.perturb(pos, 0, 0.02, cfg_index=3)
+    rows = None if k == 2 else np.sort(rng.choice(n, 192, replace=False))
+    sel = slice(None) if rows is None else rows
+    vecs = [q, rng.normal(size=n).astype(np.float32), (q * rng.uniform(0.5, 1.5, n)).astype(np.float32),
+            rng.normal(size=n).astype(np.float32)]
+    #        (phi, force) asked for: force first (cache with g), potential-only, both from the cache, field only
+    asks = [(True, True), (True, False), (True, True), (False, True)]
+    for order_of_calls in (asks, [(True, False), (True, True), (True, False), (False, True)]):
+        ctx.geometry_set(nl, dev(p), c.box, c.rc, c.alpha, c.grid, c.order)
+        for v, (want_phi, want_f) in zip(vecs, order_of_calls):
+            phi = torch.empty(n, device="cuda") if want_phi else None
+            F = torch.empty((n, 3), device="cuda") if want_f else None
+            ctx.coulomb_fixed(dev(v), phi, F, want_energy=want_phi)
+            op, oF, oE, _ = oracle.coulomb_pme(p, v, c.box, c.rc, c.alpha, c.grid, c.order, rows=rows)
+            if want_phi:
+                e_phi = relrms(phi.cpu().numpy()[sel], op)
+                assert e_phi < TOL, e_phi
+                E = ctx.energy_fetch()
+                if rows is None:           # E = 1/2 sum q phi cancels for a random vector: scale by sum |q phi|/2
+                    assert abs(E - oE) < TOL * 0.5 * float(np.abs(v.astype(np.float64) * op).sum())
+            if want_f:
+                e_F = relrms(F.cpu().numpy()[sel], oF)
+                assert e_F < TOL, e_F
+    record(f"fixed_geometry_cfg{k}", relrms_phi_last=e_phi, relrms_F_last=e_F)
+    # a plain evaluation or a build replaces the prepared geometry: coulomb_fixed must refuse, not reuse stale data
+    ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+    with pytest.raises(SqeqError):
+        ctx.coulomb_fixed(dev(q), torch.empty(n, device="cuda"))
+    ctx.geometry_set(nl, dev(p), c.box, c.rc, c.alpha, c.grid, c.order)
+    nl2 = ctx.nl_build(dev(pos), c.box, c.rc + 1.0)
+    with pytest.raises(SqeqError):
+        ctx.coulomb_fixed(dev(q), torch.empty(n, device="cuda"))
+    nl2.free()
+    nl.free()
+
+
 def test_pme_tile_window_fallbacks(ctx, monkeypatch):
     """The shared-memory spread/gather tiles assume an atom stays within one grid spacing of the cell
     it was binned into; beyond that the atom takes the global-memory path inside the same kernels,
