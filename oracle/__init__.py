@@ -384,6 +384,43 @@ def harmonic_water(pos, k_oh, r_oh, k_hh, r_hh):
     return V, F
 
 
+def oo_repulsion(pos, box, k_rep, r0):
+    """Second part of the V_short stand-in: a soft-sphere repulsion between the oxygens
+    (atoms 3m) of different molecules, V = 1/2 k_rep (r0 - r)^2 for minimum-image r < r0 < L/2, else 0 --
+    the role the O-O Lennard-Jones term plays in three-site water models: it keeps unshielded point charges
+    from collapsing into each other.  Brute force over all O-O pairs.  Returns V, F (on all atoms)."""
+    pos = _f64(pos, (-1, 3)); box = _box(box)
+    F = np.zeros_like(pos)
+    xo = pos[0::3]
+    V = 0.0
+    no = xo.shape[0]
+    for a in range(no - 1):
+        d = xo[a + 1:] - xo[a]
+        d -= np.rint(d / box) * box
+        r = np.sqrt((d * d).sum(axis=1))
+        m = r < r0
+        if not m.any():
+            continue
+        rr = r[m]
+        V += 0.5 * k_rep * float(((r0 - rr) ** 2).sum())
+        f = (k_rep * (r0 - rr) / rr)[:, None] * d[m]          # pushes b away from a
+        idx = np.nonzero(m)[0] + a + 1
+        np.add.at(F, 3 * idx, f)
+        F[3 * a] -= f.sum(axis=0)
+    return V, F
+
+
+def standin_eval(pos, box, standin):
+    """V_short stand-in: harmonic intramolecular terms (standin[0:4]) and, if given, the O-O repulsion
+    (standin[4:6] = k_rep, r0)."""
+    V, F = harmonic_water(pos, *standin[:4])
+    if len(standin) >= 6 and standin[4] != 0.0:
+        Vr, Fr = oo_repulsion(pos, box, standin[4], standin[5])
+        V += Vr
+        F = F + Fr
+    return V, F
+
+
 def shadow_eval(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin=None):
     """Shadow potential, charges and forces at fixed n (Eqs. 20-22).
 
@@ -402,7 +439,7 @@ def shadow_eval(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin=N
     Fd = coulomb_pme(pos, q - n, box, rc, alpha, grid, order)[1]
     F = ke * (Fq - Fd)
     if standin is not None:
-        Vs, Fs = harmonic_water(pos, *standin)
+        Vs, Fs = standin_eval(pos, box, standin)
         U += Vs
         F = F + Fs
     return dict(U=U, q=q, lam=lam, v=v, F=F, res=q - n)
@@ -443,15 +480,128 @@ def gmres_fixed(apply, b, m):
     return sum(y[i] * V[i] for i in range(k))
 
 
+def gmres_tol(apply, b, tol, max_iter, x0=None, diag=None):
+    """GMRES (unrestarted, modified Gram-Schmidt) to a relative residual ||b - A x||/||b|| <= tol
+    (the paper's convergence measure), at most max_iter Krylov vectors.
+    x0: initial guess (its residual costs one more operator application).
+    diag: right Jacobi preconditioner ("Jacobi preconditioner is used for regular MD runs as the
+    diagonal entries of the matrix are not equal to one"): solves A D^-1 y = b, x = D^-1 y.
+    Returns x, operator applications, relative residual (of the least-squares problem)."""
+    b = _f64(b)
+    bnorm = float(np.linalg.norm(b))
+    n_apply = 0
+    x_start = np.zeros_like(b) if x0 is None else _f64(x0).copy()
+    r0 = b.copy()
+    if x0 is not None:
+        r0 = b - apply(x_start)
+        n_apply += 1
+    beta = float(np.linalg.norm(r0))
+    if bnorm == 0.0 or beta / bnorm <= tol:
+        return x_start, n_apply, (beta / bnorm if bnorm > 0 else 0.0)
+    dinv = None if diag is None else 1.0 / _f64(diag)
+    V = [r0 / beta]
+    H = np.zeros((max_iter + 1, max_iter))
+    relres = beta / bnorm
+    k = 0
+    y = np.zeros(0)
+    for j in range(max_iter):
+        w = apply(V[j] if dinv is None else dinv * V[j])
+        n_apply += 1
+        for i in range(j + 1):
+            H[i, j] = float(np.dot(V[i], w))
+            w = w - H[i, j] * V[i]
+        H[j + 1, j] = float(np.linalg.norm(w))
+        k = j + 1
+        e1 = np.zeros(k + 1); e1[0] = beta
+        y, res, *_ = np.linalg.lstsq(H[:k + 1, :k], e1, rcond=None)
+        relres = float(np.linalg.norm(H[:k + 1, :k] @ y - e1)) / bnorm
+        if relres <= tol or H[j + 1, j] == 0.0:
+            break
+        V.append(w / H[j + 1, j])
+    dx = sum(y[i] * V[i] for i in range(k))
+    if dinv is not None:
+        dx = dinv * dx
+    return x_start + dx, n_apply, relres
+
+
+def ewald_self_diagonal(box, alpha, tol=1e-17):
+    """A_ii of the Ewald matrix (phi[e_i]_i with the uniform background omitted, G11) for r_c < L/2, where
+    no image of the atom itself is inside the real-space cutoff: the reciprocal-space self term
+    (1/(pi V)) sum_{m != 0} exp(-pi^2 |m/L|^2/alpha^2)/|m/L|^2 minus 2 alpha/sqrt(pi) (Eqs. 4-5)."""
+    box = _box(box)
+    V = float(np.prod(box))
+    mmax = [int(math.ceil(math.sqrt(-math.log(tol)) * alpha * L / math.pi)) for L in box]
+    m = np.stack(np.meshgrid(*[np.arange(-k, k + 1) for k in mmax], indexing="ij"), -1).reshape(-1, 3)
+    m = m[(m != 0).any(axis=1)]
+    mt2 = ((m / box) ** 2).sum(axis=1)
+    return float(np.sum(np.exp(-math.pi ** 2 * mt2 / alpha ** 2) / mt2) / (math.pi * V)) - 2.0 * alpha / math.sqrt(math.pi)
+
+
+def bo_eval(pos, chi, u, ke, qtot, box, rc, alpha, grid, order, standin, tol, max_iter, q_guess=None,
+            lam_guess=0.0, jacobi=True):
+    """Regular Born-Oppenheimer evaluation (Eqs. 13-19): q_min from Eq. 18 by GMRES to `tol`
+    (right Jacobi preconditioner diag(u_i + ke A_ii) on the charge rows, 1 on the constraint row; initial guess
+    [q_guess; lam_guess], whose residual costs one operator application), then the forces at FIXED q = q_min,
+    F = ke F_Coul[q] + stand-in (Eq. 19: the gradient of U_BO; dq/dR drops out only for converged q -- the
+    reason regular MD needs tight tolerances), and U_BO of Eq. 28.
+    Coulomb evaluations: GMRES operator applications + 1 (the force evaluation)."""
+    chi = _f64(chi); u = _f64(u)
+    n = chi.size
+
+    def apply(x):
+        phi = coulomb_pme(pos, x[:n], box, rc, alpha, grid, order)[0]
+        return np.concatenate([u * x[:n] + ke * phi + x[n], [x[:n].sum()]])
+
+    b = np.concatenate([-chi, [float(qtot)]])
+    diag = None
+    if jacobi:
+        diag = np.concatenate([u + ke * ewald_self_diagonal(box, alpha), [1.0]])
+    x0 = None
+    if q_guess is not None:
+        x0 = np.concatenate([_f64(q_guess), [float(lam_guess)]])
+    x, n_apply, relres = gmres_tol(apply, b, tol, max_iter, x0=x0, diag=diag)
+    q = x[:n]
+    phi, Fc, Ec, _ = coulomb_pme(pos, q, box, rc, alpha, grid, order)
+    U = float(np.dot(q, chi) + 0.5 * np.dot(q * q, u) + ke * Ec)
+    F = ke * Fc
+    if standin is not None:
+        Vs, Fs = standin_eval(pos, box, standin)
+        U += Vs
+        F = F + Fs
+    return dict(q=q, lam=float(x[n]), F=F, U=U, evals=n_apply + 1, relres=relres)
+
+
+def bo_md_step(state, vel, mass, dt, chi, u, ke, qtot, box, rc, alpha, grid, order, standin, tol, max_iter,
+               jacobi=True, warm_start=True):
+    """One velocity-Verlet step of regular BOMD ("leapfrog velocity Verlet"); the charges of the
+    previous step are the solver's initial guess when warm_start."""
+    mass = _f64(mass); vel = _f64(vel, (-1, 3))
+    vel = vel + 0.5 * dt * ACC_CONV * state["F"] / mass[:, None]
+    pos = state["pos"] + dt * vel
+    ev = bo_eval(pos, chi, u, ke, qtot, box, rc, alpha, grid, order, standin, tol, max_iter,
+                 q_guess=state["q"] if warm_start else None, lam_guess=state.get("lam", 0.0), jacobi=jacobi)
+    vel = vel + 0.5 * dt * ACC_CONV * ev["F"] / mass[:, None]
+    ekin = 0.5 * float(np.sum(mass[:, None] * vel * vel)) / ACC_CONV
+    ev["pos"] = pos
+    return ev, vel, ekin
+
+
 def shadow_md_force_and_ndd(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin,
-                            kappa, krylov_rank):
+                            kappa, krylov_rank, krylov_tol=0.0):
     """Everything the integrator needs at one time level: shadow forces (Eq. 25) and
     dt^2 * ndd from Eq. 27, J (dt^2 ndd) = -kappa (q[n]-n), kappa = dt^2 omega^2, solved by
     `krylov_rank` GMRES steps from zero (the paper's low-rank Krylov approximation of K = J^-1,
     PAPER.md:244-246).  Coulomb evaluations: 1 (v) + 2 (forces) + krylov_rank."""
     ev = shadow_eval(pos, n, chi, u, ke, qtot, box, rc, alpha, grid, order, standin)
     apply = lambda w: kernel_jacobian_apply(pos, w, u, ke, box, rc, alpha, grid, order)
-    ev["ndd_dt2"] = gmres_fixed(apply, -kappa * ev["res"], krylov_rank)
+    if krylov_tol > 0.0:      # Table 1's "Sol. Tol." (PAPER.md:260-275): stop at the relative residual, rank <= krylov_rank
+        ev["ndd_dt2"], it, _ = gmres_tol(apply, -kappa * ev["res"], krylov_tol, krylov_rank)
+    else:
+        ev["ndd_dt2"] = gmres_fixed(apply, -kappa * ev["res"], krylov_rank)
+        it = krylov_rank
+    # Coulomb evaluations of the METHOD at this time level (reading G16): potential + field of n, field of q - n,
+    # one per Krylov vector (this oracle itself spends one more, computing F_Coul[q] and F_Coul[q-n] separately)
+    ev["evals"] = 2 + it
     return ev
 
 
@@ -468,18 +618,18 @@ def xl_n_update(nh, ndd_dt2, alpha_diss, c):
 
 
 def shadow_md_init(pos, n0, chi, u, ke, qtot, box, rc, alpha, grid, order, standin, kappa,
-                   krylov_rank):
+                   krylov_rank, krylov_tol=0.0):
     """History rows 0..5 = n0 (PAPER.md is silent on the start: DESIGN.md R-MD), row 6 = dt^2 ndd."""
     n0 = _f64(n0)
     ev = shadow_md_force_and_ndd(pos, n0, chi, u, ke, qtot, box, rc, alpha, grid, order, standin,
-                                 kappa, krylov_rank)
+                                 kappa, krylov_rank, krylov_tol)
     nhist = np.vstack([np.tile(n0, (6, 1)), ev["ndd_dt2"][None, :]])
     return dict(pos=_f64(pos, (-1, 3)).copy(), nhist=nhist, F=ev["F"], U=ev["U"], q=ev["q"],
                 res=ev["res"])
 
 
 def shadow_md_step(state, vel, mass, dt, chi, u, ke, qtot, box, rc, alpha, grid, order, standin,
-                   kappa, alpha_diss, c, krylov_rank):
+                   kappa, alpha_diss, c, krylov_rank, krylov_tol=0.0):
     """One velocity-Verlet step for R and one Verlet step with dissipation for n
     (R-MD):  n(t+dt) = 2 n(t) - n(t-dt) + dt^2 ndd(t) + alpha_diss * sum_k c_k n(t - k dt).
     Returns the new state, new velocities and the kinetic energy (eV)."""
@@ -490,10 +640,10 @@ def shadow_md_step(state, vel, mass, dt, chi, u, ke, qtot, box, rc, alpha, grid,
     pos = pos + dt * vel
     n_new = xl_n_update(nh[0:6], nh[6], alpha_diss, c)
     ev = shadow_md_force_and_ndd(pos, n_new, chi, u, ke, qtot, box, rc, alpha, grid, order,
-                                 standin, kappa, krylov_rank)
+                                 standin, kappa, krylov_rank, krylov_tol)
     nhist = np.vstack([n_new[None, :], nh[0:5], ev["ndd_dt2"][None, :]])
     a = ACC_CONV * ev["F"] / mass[:, None]
     vel = vel + 0.5 * dt * a
     ekin = 0.5 * float(np.sum(mass[:, None] * vel * vel)) / ACC_CONV
-    new = dict(pos=pos, nhist=nhist, F=ev["F"], U=ev["U"], q=ev["q"], res=ev["res"])
+    new = dict(pos=pos, nhist=nhist, F=ev["F"], U=ev["U"], q=ev["q"], res=ev["res"], evals=ev["evals"])
     return new, vel, ekin

@@ -194,3 +194,104 @@ def test_xl_recursion_is_stable_and_damped():
     assert err[-1] < 1e-4 * err[0]
     rate = (err[100:120].max() / err[40:60].max()) ** (1.0 / 60.0)
     assert abs(rate - rho) < 0.02, (rate, rho)
+
+
+# ---- regular BOMD ingredients (NEXT-2) ----------------------------------------
+def test_oo_repulsion_forces_are_minus_gradient_and_compact():
+    pos, *_ , geo = small_water(3)
+    box = geo["box"]
+    V, F = oracle.oo_repulsion(pos, box, 10.0, 3.3)
+    assert V > 0.0
+    assert np.abs(F[1::3]).max() == 0.0 and np.abs(F[2::3]).max() == 0.0        # oxygens only
+    assert np.abs(F.sum(axis=0)).max() < 1e-12
+    for i, k in ((0, 0), (3, 1), (12, 2)):
+        h = 1e-6
+        p = pos.copy(); p[i, k] += h; Vp = oracle.oo_repulsion(p, box, 10.0, 3.3)[0]
+        p[i, k] -= 2 * h; Vm = oracle.oo_repulsion(p, box, 10.0, 3.3)[0]
+        assert abs(-(Vp - Vm) / (2 * h) - F[i, k]) < 1e-6 * max(1.0, abs(F[i, k]))
+    # translation by a box vector of one molecule changes nothing (minimum image); r0 below the closest O-O: zero
+    p = pos.copy(); p[3:6] += np.array(box) * np.array([1, -2, 0])
+    assert abs(oracle.oo_repulsion(p, box, 10.0, 3.3)[0] - V) < 1e-12
+    do = pos[0::3][:, None, :] - pos[0::3][None, :, :]
+    do -= np.rint(do / np.array(box)) * np.array(box)
+    rmin = np.sqrt((do ** 2).sum(-1))[np.triu_indices(len(pos) // 3, 1)].min()
+    assert oracle.oo_repulsion(pos, box, 10.0, 0.99 * rmin)[0] == 0.0
+
+
+def test_gmres_tol_matches_scipy_with_jacobi_and_initial_guess():
+    rng = np.random.default_rng(3)
+    N = 40
+    B = rng.normal(size=(N, N)); A = B @ B.T / N + np.diag(rng.uniform(1, 30, N))
+    b = rng.normal(size=N)
+    x0 = rng.normal(size=N) * 0.1
+    d = np.diag(A).copy()
+    ap = lambda v: A @ v
+    for tol in (1e-2, 1e-6):
+        x, it, rel = oracle.gmres_tol(ap, b, tol, N, x0=x0, diag=d)
+        assert np.linalg.norm(b - A @ x) / np.linalg.norm(b) <= tol * 1.0001
+        assert abs(rel - np.linalg.norm(b - A @ x) / np.linalg.norm(b)) < 1e-10
+        # scipy's GMRES on the right-preconditioned operator with the same start builds the same Krylov space:
+        # after the same number of vectors the iterates agree
+        nk = it - 1                                                 # one application went into the guess's residual
+        Ar = LinearOperator((N, N), matvec=lambda y: A @ (y / d))
+        ys, _ = gmres(Ar, b - A @ x0, x0=np.zeros(N), restart=nk, maxiter=1, rtol=1e-30, atol=0.0)
+        assert np.abs(x - (x0 + ys / d)).max() < 1e-9
+    # the preconditioner pays: fewer vectors than without it on this badly scaled matrix
+    assert oracle.gmres_tol(ap, b, 1e-6, N, diag=d)[1] < oracle.gmres_tol(ap, b, 1e-6, N)[1]
+
+
+def test_ewald_self_diagonal_is_the_diagonal_of_the_coulomb_matrix():
+    # cubic box: xi/L + pi/(V alpha^2) with xi = -2.8372974795 (the pin of test_oracle_pins), any alpha with
+    # erfc(alpha L) negligible; and equal to the diagonal of the direct-Ewald matrix for a non-cubic box
+    L, a = 9.0, 0.9
+    assert abs(oracle.ewald_self_diagonal([L] * 3, a) - (-2.8372974795 / L + np.pi / (L ** 3 * a * a))) < 1e-9
+    box = [8.0, 9.5, 11.0]
+    phi, _, _ = oracle.ewald_direct(np.array([[1.0, 2.0, 3.0]]), np.array([1.0]), box, 1.1)
+    assert abs(oracle.ewald_self_diagonal(box, 1.1) - phi[0]) < 1e-9
+
+
+def test_bo_forces_are_minus_gradient_of_u_bo_and_match_shadow_at_qmin():
+    pos, q0, chi, u, geo = small_water(2)
+    st6 = STANDIN + (10.0, 3.3)
+    ev = oracle.bo_eval(pos, chi, u, KE, 0.0, standin=st6, tol=1e-13, max_iter=30, **geo)
+    assert ev["relres"] <= 1e-13 and abs(ev["q"].sum()) < 1e-12
+    A = oracle.coulomb_matrix_pme(pos, **geo)
+    qd, lamd = oracle.qeq_dense_solve(A, chi, u, KE, 0.0)
+    assert np.abs(ev["q"] - qd).max() < 1e-10 and abs(ev["lam"] - lamd) < 1e-9
+    for i, k in ((0, 0), (7, 1), (13, 2)):
+        h = 1e-5
+        p = pos.copy(); p[i, k] += h
+        Up = oracle.bo_eval(p, chi, u, KE, 0.0, standin=st6, tol=1e-13, max_iter=30, **geo)["U"]
+        p[i, k] -= 2 * h
+        Um = oracle.bo_eval(p, chi, u, KE, 0.0, standin=st6, tol=1e-13, max_iter=30, **geo)["U"]
+        fd = -(Up - Um) / (2 * h)
+        assert abs(fd - ev["F"][i, k]) < 2e-6 * max(1.0, abs(fd)), (fd, ev["F"][i, k])
+    sh = oracle.shadow_eval(pos, ev["q"], chi, u, KE, 0.0, standin=st6, **geo)
+    assert np.abs(sh["F"] - ev["F"]).max() < 1e-8 and abs(sh["U"] - ev["U"]) < 1e-8
+    # a warm start from the solution needs one application (its residual) and no Krylov vector
+    ev2 = oracle.bo_eval(pos, chi, u, KE, 0.0, standin=st6, tol=1e-8, max_iter=30, q_guess=ev["q"],
+                         lam_guess=ev["lam"], **geo)
+    assert ev2["evals"] == 2
+
+
+def test_bo_md_conserves_energy_when_converged_and_drifts_when_loose():
+    """The paper's Table 1 in miniature: regular BOMD conserves energy with a tight solver and
+    not with a loose one, at more Coulomb evaluations per step than shadow MD needs."""
+    pos, chi, u, geo = aligned_water(2)
+    st6 = STANDIN + (10.0, 2.9)
+    mass = W.masses_water(len(pos)).astype(float)
+    out = {}
+    for tol in (1e-8, 1e-2):
+        ev = oracle.bo_eval(pos, chi, u, KE, 0.0, standin=st6, tol=1e-10, max_iter=40, **geo)
+        st = dict(pos=pos.copy(), F=ev["F"], q=ev["q"], lam=ev["lam"])
+        vel = W.velocities(mass).astype(float)
+        e, evals, k = [], [], []
+        for _ in range(25):
+            st, vel, ekin = oracle.bo_md_step(st, vel, mass, 0.5, chi, u, KE, 0.0, standin=st6, tol=tol, max_iter=40, **geo)
+            e.append(st["U"] + ekin); evals.append(st["evals"]); k.append(ekin)
+        out[tol] = (np.std(e), np.mean(evals), np.ptp(k))
+    # converged charges: the total energy holds to the Verlet error of the stiff bonds (1 % of the kinetic/potential
+    # exchange at 0.5 fs); tol 1e-2: the warm-started solver updates the charges only now and then, the forces are
+    # not the gradient of any potential and the energy wanders by tens of times more -- at a quarter of the cost
+    assert out[1e-8][0] < 0.02 * out[1e-8][2] and out[1e-8][1] > 3 * out[1e-2][1]
+    assert out[1e-2][0] > 10 * out[1e-8][0]
