@@ -183,6 +183,14 @@ int  sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float*
                     double ke, const float* chi, const float* J, double total_charge,
                     double tol, int max_iter, int restart,
                     float* q_out, double* lambda_out, int* iters_out, double* relres_out);
+/* The same solve with the options the paper's regular-MD runs use: jacobi != 0 applies the right
+ * Jacobi preconditioner diag(J_i + ke A_ii) (A_ii: the Ewald self-image diagonal; 1 on the constraint row);
+ * q0 != NULL (device fp32 [n]) and lambda0 give the initial guess (its residual costs one evaluation). */
+int  sqeq_qeq_solve_pc(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                       const double box[3], double rc, double alpha, const int grid[3], int order,
+                       double ke, const float* chi, const float* J, double total_charge,
+                       double tol, int max_iter, int restart, int jacobi, const float* q0, double lambda0,
+                       float* q_out, double* lambda_out, int* iters_out, double* relres_out);
 
 /* ---- shadow XL-BOMD step: PAPER.md:196-246 (Eqs. 19-27); DESIGN.md R-MD -------------------------
  * State arrays are caller-owned device memory, updated in place:
@@ -218,6 +226,13 @@ typedef struct sqeq_md_params {
     double kappa;         /* dt^2 omega^2 */
     double alpha_diss;    /* dissipation strength */
     double c[7];          /* dissipation coefficients c_0..c_5 (c[6] unused) */
+    double krylov_tol;    /* > 0: solve Eq. 27 to this relative residual (Table 1's "Sol. Tol.")
+                             with at most krylov_rank vectors (one host synchronisation per vector); 0: exactly
+                             krylov_rank vectors, no synchronisation */
+    double k_rep, r_rep;  /* V_short stand-in, second part: soft-sphere repulsion 1/2 k_rep (r_rep - r)^2 between the
+                             oxygens (atoms 3m) of different molecules for r < r_rep (eV/Angstrom^2, Angstrom); it
+                             plays the part of the O-O Lennard-Jones term of three-site water models.  k_rep = 0
+                             disables it.  Needs r_rep + (list cutoff - rc) <= the list's cell edge (>= cutoff/2). */
 } sqeq_md_params;
 
 int  sqeq_shadow_md_init(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
@@ -228,6 +243,25 @@ int  sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* 
                          const float* mass, const double box[3], const sqeq_md_params* p,
                          const float* chi, const float* u, double* nhist, float* force,
                          double* energies);
+
+/* ---- regular Born-Oppenheimer MD: PAPER.md:155-200 (Eqs. 13-19), the method shadow MD is compared with
+ * (Table 1, 321-323) -------------------------------------------------------------------
+ * Every step solves Eq. 18 for q_min by GMRES to the relative residual `tol` (at most max_iter Coulomb
+ * evaluations; jacobi != 0: right Jacobi preconditioner diag(u_i + ke A_ii); warm_start != 0: the
+ * previous step's charges and lambda are the initial guess, whose residual costs one evaluation), then
+ * evaluates F = ke F_Coul[q_min] + stand-in at FIXED charges (Eq. 19) and U_BO (Eq. 28).
+ * State, caller-owned device memory: pos, vel [n][3] fp32; q fp64 [n] (charges, in and out); force [n][3] fp32;
+ * lambda: host double, in and out.  p->krylov_rank, kappa, alpha_diss, c are not used.
+ * energies: host double[4] out = {U_BO, kinetic energy (0 from init), relative residual reached, Coulomb
+ * evaluations = solver evaluations + 1}.  Both calls synchronise.  SQEQ_ENOTCONV if tol is not reached
+ * (state and energies are still written). */
+int  sqeq_bomd_init(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
+                    const sqeq_md_params* p, const float* chi, const float* u, double tol, int max_iter,
+                    int jacobi, double* q, double* lambda, float* force, double* energies);
+int  sqeq_bomd_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* pos, float* vel, const float* mass,
+                    const double box[3], const sqeq_md_params* p, const float* chi, const float* u, double tol,
+                    int max_iter, int jacobi, int warm_start, double* q, double* lambda, float* force,
+                    double* energies);
 
 /* ---- per-stage device timing (CUDA events on the context's stream) ----------------------------
  * Stages: see SQEQ_T_*.  Enable, run, then read: total milliseconds and number of launches per

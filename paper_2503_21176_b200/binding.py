@@ -33,7 +33,8 @@ class MdParams(ctypes.Structure):
                 ("k_oh", ctypes.c_double), ("r_oh", ctypes.c_double),
                 ("k_hh", ctypes.c_double), ("r_hh", ctypes.c_double),
                 ("kappa", ctypes.c_double), ("alpha_diss", ctypes.c_double),
-                ("c", ctypes.c_double * 7)]
+                ("c", ctypes.c_double * 7),
+                ("krylov_tol", ctypes.c_double), ("k_rep", ctypes.c_double), ("r_rep", ctypes.c_double)]
 
 
 def load():
@@ -73,6 +74,12 @@ def load():
     L.sqeq_pme_grid.argtypes = [vp, cint, vp]
     L.sqeq_qeq_solve.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint, dbl, vp, vp, dbl, dbl, cint,
                                  cint, vp, dp, ip, dp]
+    L.sqeq_qeq_solve_pc.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint, dbl, vp, vp, dbl, dbl, cint,
+                                    cint, cint, vp, dbl, vp, dp, ip, dp]
+    L.sqeq_bomd_init.argtypes = [vp, vp, i64, vp, dp, ctypes.POINTER(MdParams), vp, vp, dbl, cint, cint,
+                                 vp, dp, vp, dp]
+    L.sqeq_bomd_step.argtypes = [vp, vp, i64, vp, vp, vp, dp, ctypes.POINTER(MdParams), vp, vp, dbl, cint, cint,
+                                 cint, vp, dp, vp, dp]
     L.sqeq_shadow_md_init.argtypes = [vp, vp, i64, vp, dp, ctypes.POINTER(MdParams), vp, vp, dbl, cint,
                                       vp, vp, dp]
     L.sqeq_shadow_md_step.argtypes = [vp, vp, i64, vp, vp, vp, dp, ctypes.POINTER(MdParams), vp, vp,
@@ -312,6 +319,49 @@ class Context:
                         allow=() if raise_on_notconv else (ENOTCONV,))
         return q, lam.value, it.value, rel.value, r == OK
 
+    def qeq_solve_pc(self, nl, pos, box, rc, alpha, grid, order, ke, chi, J, total_charge, tol=1e-6,
+                     max_iter=100, restart=0, jacobi=True, q0=None, lambda0=0.0):
+        """sqeq_qeq_solve_pc: right Jacobi preconditioner and/or an initial guess (q0, lambda0)."""
+        n = pos.shape[0]
+        q = torch.empty(n, dtype=torch.float32, device=self.device)
+        lam, rel = ctypes.c_double(), ctypes.c_double()
+        it = ctypes.c_int()
+        r = self._check(load().sqeq_qeq_solve_pc(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                                 _box(box), float(rc), float(alpha), _grid(grid), int(order),
+                                                 float(ke), _ptr(chi, torch.float32, n), _ptr(J, torch.float32, n),
+                                                 float(total_charge), float(tol), int(max_iter), int(restart),
+                                                 int(bool(jacobi)), _ptr(q0, torch.float32, n) if q0 is not None else None,
+                                                 float(lambda0), _ptr(q, torch.float32, n), ctypes.byref(lam),
+                                                 ctypes.byref(it), ctypes.byref(rel)), allow=(ENOTCONV,))
+        return q, lam.value, it.value, rel.value, r == OK
+
+    # ---- regular Born-Oppenheimer MD
+    def bomd_init(self, nl, pos, box, params, chi, u, tol=1e-6, max_iter=100, jacobi=True):
+        """Returns the state (q fp64 [n], lambda), the force and [U_BO, 0, relres, evaluations]."""
+        n = pos.shape[0]
+        q = torch.zeros(n, dtype=torch.float64, device=self.device)
+        force = torch.empty((n, 3), dtype=torch.float32, device=self.device)
+        lam = ctypes.c_double(0.0)
+        en = (ctypes.c_double * 4)()
+        r = self._check(load().sqeq_bomd_init(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n), _box(box),
+                                              ctypes.byref(params), _ptr(chi, torch.float32, n), _ptr(u, torch.float32, n),
+                                              float(tol), int(max_iter), int(bool(jacobi)), ctypes.c_void_p(q.data_ptr()),
+                                              ctypes.byref(lam), _ptr(force, torch.float32), en), allow=(ENOTCONV,))
+        return dict(q=q, lam=lam, converged=r == OK), force, list(en)
+
+    def bomd_step(self, nl, pos, vel, mass, box, params, chi, u, state, force, tol=1e-6, max_iter=100, jacobi=True,
+                  warm_start=True):
+        n = pos.shape[0]
+        en = (ctypes.c_double * 4)()
+        r = self._check(load().sqeq_bomd_step(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                              _ptr(vel, torch.float32, 3 * n), _ptr(mass, torch.float32, n), _box(box),
+                                              ctypes.byref(params), _ptr(chi, torch.float32, n), _ptr(u, torch.float32, n),
+                                              float(tol), int(max_iter), int(bool(jacobi)), int(bool(warm_start)),
+                                              ctypes.c_void_p(state["q"].data_ptr()), ctypes.byref(state["lam"]),
+                                              _ptr(force, torch.float32, 3 * n), en), allow=(ENOTCONV,))
+        state["converged"] = r == OK
+        return list(en)
+
     # ---- shadow XL-BOMD
     def shadow_md_init(self, nl, pos, box, params, chi, u, tol=1e-8, max_iter=200, n0=None):
         """n0 given (numpy/torch fp64 [n]) with max_iter=0: start the history from n0 instead of q_min."""
@@ -361,7 +411,7 @@ class Context:
 
 
 def md_params(cfg, dt=0.5, ke=14.3996454784255, total_charge=0.0, krylov_rank=4,
-              k_oh=48.0, r_oh=0.9572, k_hh=10.0, r_hh=1.5139):
+              k_oh=48.0, r_oh=0.9572, k_hh=10.0, r_hh=1.5139, krylov_tol=0.0, k_rep=0.0, r_rep=0.0):
     """sqeq_md_params for a workloads.Config with the XL-BOMD constants of DESIGN.md R-MD."""
     p = MdParams()
     p.dt, p.ke, p.total_charge = dt, ke, total_charge
@@ -371,4 +421,5 @@ def md_params(cfg, dt=0.5, ke=14.3996454784255, total_charge=0.0, krylov_rank=4,
     p.k_oh, p.r_oh, p.k_hh, p.r_hh = k_oh, r_oh, k_hh, r_hh
     p.kappa, p.alpha_diss = 1.82, 0.018
     p.c[:] = [-6.0, 14.0, -8.0, -3.0, 4.0, -1.0, 0.0]
+    p.krylov_tol, p.k_rep, p.r_rep = krylov_tol, k_rep, r_rep
     return p

@@ -237,6 +237,12 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
 // Generic restarted/unrestarted GMRES on device fp64 vectors (qeq.cu); x_out points into ctx->kry_w.
 int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double*, double*)>& apply,
                 const std::function<int(double*)>& load_rhs, double tol, int max_iter, int restart,
-                double** x_out, int* iters_out, double* relres_out, bool* converged_out);
+                double** x_out, int* iters_out, double* relres_out, bool* converged_out,
+                const double* x0 = nullptr, const double* dinv = nullptr);
+int qeq_solve_prepared(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc, double alpha,
+                       double ke, const float* chi, const float* J, double total_charge, double tol, int max_iter,
+                       int restart, bool jacobi, bool warm, double* q_io, double* lambda_io, int* iters_out,
+                       double* relres_out, bool* converged_out);
+double ewald_self_diag(const double box[3], double alpha);
 int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3],
                           double rc, double alpha, const int grid[3], int order, const char* who);

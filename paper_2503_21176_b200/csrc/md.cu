@@ -20,7 +20,7 @@
 #define ACC_CONV 0.00964853321   // (eV/Angstrom)/amu -> Angstrom/fs^2
 
 // scal[] slots used here (0 and 1 belong to assemble / influence)
-enum { S_T = 2, S_INVU = 3, S_U = 4, S_RES2 = 5, S_JAC = 6, S_EKIN = 7, S_VSTAND = 8 };
+enum { S_T = 2, S_INVU = 3, S_U = 4, S_RES2 = 5, S_JAC = 6, S_EKIN = 7, S_VSTAND = 8 };   // 12: max drift (nlist.cu)
 
 __device__ __forceinline__ void block_sum_to(double v, double* dst)
 {
@@ -170,6 +170,93 @@ k_md_standin(int64_t nmol, const float* __restrict__ pos, double k_oh, double r_
     if (vsum) block_sum_to(V, vsum);
 }
 
+// V_short stand-in, second part: soft-sphere repulsion 1/2 k (r0 - r)^2 between oxygens (caller index 3m) of
+// different molecules, r < r0.  One warp per atom of the list's cell-major order (non-oxygens leave at once); the
+// warp sweeps the 27 cells around the atom's build-time cell -- r0 + skin <= cell edge, so every partner is there
+// although the cells are those of the last build -- with the periodic image of each cell applied; each pair is
+// seen from both sides, so only atom i is written (no atomics) and the energy is halved.
+struct RepGeom {
+    int nc[3];
+    float L[3];
+    float k, r0;
+};
+__global__ void __launch_bounds__(256)
+k_md_oo_repulsion(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_of,
+                  const int* __restrict__ cell_start, const int* __restrict__ perm, RepGeom g,
+                  float* __restrict__ force, double* __restrict__ vsum)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    double V = 0.0;
+    if (s < n) {
+        const int oi = perm[s];
+        if (oi % 3 == 0) {
+            const float4 xi = xq[s];
+            const int c = cell_of[s];
+            const int cx = c & 1023, cy = (c >> 10) & 1023, cz = c >> 20;
+            float fx = 0.f, fy = 0.f, fz = 0.f, v = 0.f;
+            for (int dx = -1; dx <= 1; ++dx)
+                for (int dy = -1; dy <= 1; ++dy)
+                    for (int dz = -1; dz <= 1; ++dz) {
+                        int ux = cx + dx, uy = cy + dy, uz = cz + dz;
+                        float sx = 0.f, sy = 0.f, sz = 0.f;
+                        if (ux < 0) { ux += g.nc[0]; sx = -g.L[0]; } else if (ux >= g.nc[0]) { ux -= g.nc[0]; sx = g.L[0]; }
+                        if (uy < 0) { uy += g.nc[1]; sy = -g.L[1]; } else if (uy >= g.nc[1]) { uy -= g.nc[1]; sy = g.L[1]; }
+                        if (uz < 0) { uz += g.nc[2]; sz = -g.L[2]; } else if (uz >= g.nc[2]) { uz -= g.nc[2]; sz = g.L[2]; }
+                        const int cell = (ux * g.nc[1] + uy) * g.nc[2] + uz;
+                        const int beg = cell_start[cell], end = cell_start[cell + 1];
+                        for (int t = beg + lane; t < end; t += 32) {
+                            if (perm[t] % 3 != 0) continue;
+                            const float4 xj = xq[t];
+                            const float ddx = xi.x - (xj.x + sx), ddy = xi.y - (xj.y + sy), ddz = xi.z - (xj.z + sz);
+                            const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                            if (r2 < g.r0 * g.r0 && r2 > 0.f) {               // r2 = 0: the atom itself (zero image)
+                                const float r = sqrtf(r2);
+                                const float f = g.k * (g.r0 - r) / r;
+                                fx += f * ddx; fy += f * ddy; fz += f * ddz;
+                                v += 0.25f * g.k * (g.r0 - r) * (g.r0 - r);    // half of the pair energy
+                            }
+                        }
+                    }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                fx += __shfl_xor_sync(0xffffffffu, fx, o);
+                fy += __shfl_xor_sync(0xffffffffu, fy, o);
+                fz += __shfl_xor_sync(0xffffffffu, fz, o);
+                v += __shfl_xor_sync(0xffffffffu, v, o);
+            }
+            if (lane == 0) {
+                force[3 * (int64_t)oi + 0] += fx;
+                force[3 * (int64_t)oi + 1] += fy;
+                force[3 * (int64_t)oi + 2] += fz;
+                V = (double)v;
+            }
+        }
+    }
+    if (vsum) block_sum_to(V, vsum);
+}
+
+// both parts of the stand-in, added to `force`; V into scal[S_VSTAND]
+static int standin_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const sqeq_md_params* p,
+                       float* force, cudaStream_t st)
+{
+    double* scal = (double*)ctx->scal.p;
+    if (p->k_oh != 0.0 || p->k_hh != 0.0) {
+        k_md_standin<<<ceil_div(n / 3, 256), 256, 0, st>>>(n / 3, pos, p->k_oh, p->r_oh, p->k_hh, p->r_hh, force,
+                                                            scal + S_VSTAND);
+        KERNEL_CHECK(ctx);
+    }
+    if (p->k_rep != 0.0) {
+        RepGeom g;
+        for (int d = 0; d < 3; ++d) { g.nc[d] = nl->ncell[d]; g.L[d] = (float)nl->box[d]; }
+        g.k = (float)p->k_rep; g.r0 = (float)p->r_rep;
+        k_md_oo_repulsion<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
+                                                                 nl->perm, g, force, scal + S_VSTAND);
+        KERNEL_CHECK(ctx);
+    }
+    return SQEQ_OK;
+}
+
 // Eq. 24 applied to Eq. 22: (J w)_i = -w_i - (ke phi[w]_i + dlambda)/u_i, dlambda from sum(Jw + w) = 0
 __global__ void __launch_bounds__(256)
 k_md_jac_reduce(int64_t n, const float* __restrict__ u, const float* __restrict__ phi, double ke,
@@ -205,8 +292,16 @@ static int check_md_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const d
     SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, p->rc, p->alpha, p->grid, p->order, who));
     if (!(p->dt > 0.0) || !(p->ke > 0.0) || p->krylov_rank < 0 || p->krylov_rank > 64)
         return sqeq_fail(ctx, SQEQ_EINVAL, "%s: need dt > 0, ke > 0, 0 <= krylov_rank <= 64", who);
-    if ((p->k_oh != 0.0 || p->k_hh != 0.0) && n % 3 != 0)
+    if ((p->k_oh != 0.0 || p->k_hh != 0.0 || p->k_rep != 0.0) && n % 3 != 0)
         return sqeq_fail(ctx, SQEQ_EINVAL, "%s: the O,H,H stand-in needs n divisible by 3", who);
+    if (!(p->krylov_tol >= 0.0)) return sqeq_fail(ctx, SQEQ_EINVAL, "%s: krylov_tol must be >= 0", who);
+    if (p->k_rep != 0.0) {
+        double edge = 1e300;
+        for (int d = 0; d < 3; ++d) edge = fmin(edge, nl->box[d] / nl->ncell[d]);
+        if (!(p->r_rep > 0.0) || p->r_rep + (nl->cutoff - p->rc) > edge)
+            return sqeq_fail(ctx, SQEQ_EINVAL, "%s: r_rep = %g plus the skin %g must not exceed the list's cell edge %g",
+                             who, p->r_rep, nl->cutoff - p->rc, edge);
+    }
     return SQEQ_OK;
 }
 
@@ -248,11 +343,7 @@ static int md_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* 
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
         k_md_forces<<<nb, 256, 0, st>>>(n, q, nv, f_n, f_d, p->ke, force);
         KERNEL_CHECK(ctx);
-        if (p->k_oh != 0.0 || p->k_hh != 0.0) {
-            k_md_standin<<<ceil_div(n / 3, 256), 256, 0, st>>>(n / 3, pos, p->k_oh, p->r_oh, p->k_hh,
-                                                                p->r_hh, force, scal + S_VSTAND);
-            KERNEL_CHECK(ctx);
-        }
+        SQEQ_TRY(standin_run(ctx, nl, n, pos, p, force, st));
     }
     int iters = 0;
     double* ndd = nhist + 6 * n;
@@ -278,7 +369,7 @@ static int md_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* 
             return (int)SQEQ_OK;
         };
         double* x = nullptr;
-        SQEQ_TRY(gmres_solve(ctx, n, apply, load_rhs, 0.0, p->krylov_rank, 0, &x, &iters, nullptr, nullptr));
+        SQEQ_TRY(gmres_solve(ctx, n, apply, load_rhs, p->krylov_tol, p->krylov_rank, 0, &x, &iters, nullptr, nullptr));
         CUDA_TRY(ctx, cudaMemcpyAsync(ndd, x, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
     }
     if (evals) *evals = 2 + iters;
@@ -356,4 +447,108 @@ extern "C" int sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t 
         KERNEL_CHECK(ctx);
     }
     return md_read_energies(ctx, energies, evals);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Regular Born-Oppenheimer MD (NEXT-2): q_min by GMRES on Eq. 18, forces at fixed q_min.
+__global__ void __launch_bounds__(256)
+k_bomd_energy(int64_t n, const double* __restrict__ q, const float* __restrict__ chi, const float* __restrict__ u,
+              double* __restrict__ out)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    double e = 0.0;
+    if (i < n) e = q[i] * (double)chi[i] + 0.5 * q[i] * q[i] * (double)u[i];
+    block_sum_to(e, out);
+}
+
+__global__ void k_bomd_scale_force(int64_t n3, float ke, float* __restrict__ f)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n3) f[i] *= ke;
+}
+
+static int bomd_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
+                     const sqeq_md_params* p, const float* chi, const float* u, double tol, int max_iter, bool jacobi,
+                     bool warm, double* q, double* lambda, float* force, double* energies, double ekin_scalar_ready)
+{
+    (void)ekin_scalar_ready;
+    cudaStream_t st = ctx->stream;
+    const int nb = ceil_div(n, 256);
+    double* scal = (double*)ctx->scal.p;
+    SQEQ_TRY(pme_setup(ctx, box, p->alpha, p->grid, p->order));
+    SQEQ_TRY(prep_atoms(ctx, nl, pos, nullptr, ctx->K, st));
+    int iters = 0;
+    double relres = 1.0;
+    bool converged = false;
+    SQEQ_TRY(qeq_solve_prepared(ctx, nl, n, box, p->rc, p->alpha, p->ke, chi, u, p->total_charge, tol, max_iter, 0,
+                                jacobi, warm, q, lambda, &iters, &relres, &converged));
+    // forces at fixed q = q_min (Eq. 19) and E_Coul[q] on the same geometry (the cache the solve left behind)
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_f[1], sizeof(float) * n));
+    SQEQ_TRY(prep_charges(ctx, nl, nullptr, q, st));
+    SQEQ_TRY(coulomb_eval(ctx, nl, n, box, p->rc, p->alpha, (float*)ctx->vec_f[1].p, force, true, false, GEOM_FIXED));
+    {
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        CUDA_TRY(ctx, cudaMemsetAsync(scal + S_U, 0, sizeof(double), st));
+        CUDA_TRY(ctx, cudaMemsetAsync(scal + S_VSTAND, 0, sizeof(double), st));
+        k_bomd_energy<<<nb, 256, 0, st>>>(n, q, chi, u, scal + S_U);
+        KERNEL_CHECK(ctx);
+        k_bomd_scale_force<<<ceil_div(3 * n, 256), 256, 0, st>>>(3 * n, (float)p->ke, force);
+        KERNEL_CHECK(ctx);
+        SQEQ_TRY(standin_run(ctx, nl, n, pos, p, force, st));
+    }
+    if (energies) { energies[2] = relres; energies[3] = (double)(iters + 1); }
+    return converged ? SQEQ_OK : SQEQ_ENOTCONV;
+}
+
+static int bomd_read(sqeq_ctx* ctx, const sqeq_md_params* p, double* energies)
+{
+    cudaStream_t st = ctx->stream;
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal.p, sizeof(double) * 9, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    if (energies) {
+        energies[0] = ctx->h_scal[S_U] + p->ke * ctx->h_scal[0] + ctx->h_scal[S_VSTAND];    // scal[0]: E_Coul (k_e = 1)
+        energies[1] = ctx->h_scal[S_EKIN];
+    }
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_bomd_init(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
+                              const sqeq_md_params* p, const float* chi, const float* u, double tol, int max_iter,
+                              int jacobi, double* q, double* lambda, float* force, double* energies)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(check_md_args(ctx, nl, n, box, p, "sqeq_bomd_init"));
+    if (!pos || !chi || !u || !q || !lambda || !force || max_iter < 1 || !(tol >= 0.0))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_bomd_init: NULL argument, max_iter < 1 or tol < 0");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    CUDA_TRY(ctx, cudaMemsetAsync((double*)ctx->scal.p + S_EKIN, 0, sizeof(double), ctx->stream));
+    const int r = bomd_eval(ctx, nl, n, pos, box, p, chi, u, tol, max_iter, jacobi != 0, false, q, lambda, force, energies, 0);
+    if (r != SQEQ_OK && r != SQEQ_ENOTCONV) return r;
+    SQEQ_TRY(bomd_read(ctx, p, energies));
+    if (r == SQEQ_ENOTCONV) return sqeq_fail(ctx, SQEQ_ENOTCONV, "sqeq_bomd_init: tol %.3e not reached in %d evaluations", tol, max_iter);
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_bomd_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* pos, float* vel, const float* mass,
+                              const double box[3], const sqeq_md_params* p, const float* chi, const float* u, double tol,
+                              int max_iter, int jacobi, int warm_start, double* q, double* lambda, float* force,
+                              double* energies)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(check_md_args(ctx, nl, n, box, p, "sqeq_bomd_step"));
+    if (!pos || !vel || !mass || !chi || !u || !q || !lambda || !force || max_iter < 1 || !(tol >= 0.0))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_bomd_step: NULL argument, max_iter < 1 or tol < 0");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const int nb = ceil_div(n, 256);
+    k_md_kick<<<nb, 256, 0, st>>>(n, pos, vel, force, mass, p->dt, 1, nullptr);
+    KERNEL_CHECK(ctx);
+    const int r = bomd_eval(ctx, nl, n, pos, box, p, chi, u, tol, max_iter, jacobi != 0, warm_start != 0, q, lambda, force, energies, 0);
+    if (r != SQEQ_OK && r != SQEQ_ENOTCONV) return r;
+    CUDA_TRY(ctx, cudaMemsetAsync((double*)ctx->scal.p + S_EKIN, 0, sizeof(double), st));
+    k_md_kick<<<nb, 256, 0, st>>>(n, pos, vel, force, mass, p->dt, 0, (double*)ctx->scal.p + S_EKIN);
+    KERNEL_CHECK(ctx);
+    SQEQ_TRY(bomd_read(ctx, p, energies));
+    if (r == SQEQ_ENOTCONV) return sqeq_fail(ctx, SQEQ_ENOTCONV, "sqeq_bomd_step: tol %.3e not reached in %d evaluations", tol, max_iter);
+    return SQEQ_OK;
 }

@@ -111,36 +111,82 @@ __global__ void k_axpby(int64_t len, double a, const double* __restrict__ x, dou
     if (i < len) y[i] = a * x[i] + b * y[i];
 }
 
+// z = x o d (right Jacobi preconditioner: d holds the inverse diagonal)
+__global__ void k_hadamard(int64_t len, const double* __restrict__ x, const double* __restrict__ d, double* __restrict__ z)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < len) z[i] = x[i] * d[i];
+}
+
+// x += d o sum_k y[k] V_k
+__global__ void k_add_combo_scaled(int64_t len, int64_t ld, int nv, const double* __restrict__ V,
+                                   const double* __restrict__ y, const double* __restrict__ d, double* __restrict__ x)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i >= len) return;
+    double acc = 0.0;
+    for (int k = 0; k < nv; ++k) acc += y[k] * V[(int64_t)k * ld + i];
+    x[i] += d[i] * acc;
+}
+
+// inverse diagonal of Eq. 18's matrix: 1/(J_i + ke A_ii) on the charge rows, 1 on the constraint row
+__global__ void k_qeq_jacobi(int64_t n, const float* __restrict__ J, double keAii, double* __restrict__ dinv)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) dinv[i] = 1.0 / ((double)J[i] + keAii);
+    else if (i == n) dinv[n] = 1.0;
+}
+
+// x0 = [q0 ; lambda0]
+__global__ void k_qeq_guess(int64_t n, const double* __restrict__ q0, double lam0, double* __restrict__ x)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) x[i] = q0[i];
+    else if (i == n) x[n] = lam0;
+}
+
 __global__ void k_d2f(int64_t n, const double* __restrict__ x, float* __restrict__ y)
 {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i < n) y[i] = (float)x[i];
 }
 
+__global__ void k_f2d(int64_t n, const float* __restrict__ x, double* __restrict__ y)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (i < n) y[i] = (double)x[i];
+}
+
 // ------------------------------------------------------------------------------------------------
 // Generic GMRES on device fp64 vectors of length `len` (leading dimension ld).  Zero initial guess.
 //   apply(v, w): w = A v        load_rhs(w): w = b
 // On return x (ctx->kry_w + ld) holds the iterate.  Host side: Givens-rotated Hessenberg.
+// x0 (device, may be NULL): initial guess; its residual b - A x0 costs one operator application.
+// dinv (device, may be NULL): right Jacobi preconditioner, the solve runs on A D^-1 y = b with x = D^-1 y
+// ("Jacobi preconditioner is used for regular MD runs").
 int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double*, double*)>& apply,
                 const std::function<int(double*)>& load_rhs, double tol, int max_iter, int restart,
-                double** x_out, int* iters_out, double* relres_out, bool* converged_out)
+                double** x_out, int* iters_out, double* relres_out, bool* converged_out,
+                const double* x0, const double* dinv)
 {
     cudaStream_t st = ctx->stream;
     const int m = restart > 0 ? (restart < max_iter ? restart : max_iter) : max_iter;
     const int64_t ld = (len + 31) & ~(int64_t)31;
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_V, sizeof(double) * (size_t)ld * (m + 1)));
-    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_w, sizeof(double) * (size_t)ld * 2));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_w, sizeof(double) * (size_t)ld * 3));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_h, sizeof(double) * (size_t)(2 * (m + 2) + 2)));
     double* V = (double*)ctx->kry_V.p;
     double* w = (double*)ctx->kry_w.p;
     double* x = w + ld;
+    double* z = w + 2 * ld;                      // D^-1 v_j
     double* h = (double*)ctx->kry_h.p;          // [m+2] first-pass coefficients
     double* h2 = h + (m + 2);                    // second pass
     double* nrm2 = h2 + (m + 2);
     std::vector<double> hh((size_t)2 * (m + 2) + 2);
     const int nbl = ceil_div(len, 256);
     const int nchunk = ceil_div(len, DOT_CHUNK);
-    CUDA_TRY(ctx, cudaMemsetAsync(x, 0, sizeof(double) * ld, st));
+    if (x0) CUDA_TRY(ctx, cudaMemcpyAsync(x, x0, sizeof(double) * len, cudaMemcpyDeviceToDevice, st));
+    else CUDA_TRY(ctx, cudaMemsetAsync(x, 0, sizeof(double) * ld, st));
     *x_out = x;
 
     // |b|
@@ -159,7 +205,7 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
     double relres = 1.0;
     bool converged = false;
     if (bnorm == 0.0) { converged = true; relres = 0.0; }
-    bool first_cycle = true;
+    bool first_cycle = x0 == nullptr;       // with a guess the first cycle starts from r = b - A x0, like a restart
     std::vector<double> H((size_t)(m + 1) * m), cs(m), sn(m), gvec(m + 1), y(m);
     // Column j of the Hessenberg matrix from the coefficients of iteration j (hc), its Givens rotation and the
     // residual estimate; true when the cycle ends at this column (converged or exact breakdown).
@@ -226,7 +272,13 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
         gvec[0] = beta;
         int j = 0;
         for (; j < m && iters < max_iter; ++j) {
-            SQEQ_TRY(apply(V + (int64_t)j * ld, w));
+            if (dinv) {
+                k_hadamard<<<nbl, 256, 0, st>>>(len, V + (int64_t)j * ld, dinv, z);
+                KERNEL_CHECK(ctx);
+                SQEQ_TRY(apply(z, w));
+            } else {
+                SQEQ_TRY(apply(V + (int64_t)j * ld, w));
+            }
             ++iters;
             {
                 StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
@@ -269,7 +321,8 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
         if (k > 0) {
             StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
             CUDA_TRY(ctx, cudaMemcpyAsync(h, y.data(), sizeof(double) * k, cudaMemcpyHostToDevice, st));
-            k_add_combo<<<nbl, 256, 0, st>>>(len, ld, k, V, h, x);
+            if (dinv) k_add_combo_scaled<<<nbl, 256, 0, st>>>(len, ld, k, V, h, dinv, x);
+            else k_add_combo<<<nbl, 256, 0, st>>>(len, ld, k, V, h, x);
             KERNEL_CHECK(ctx);
             CUDA_TRY(ctx, cudaStreamSynchronize(st));   // y is a host vector reused next cycle
         }
@@ -307,26 +360,35 @@ static int qeq_apply(const QeqOp& op, const double* v, double* w)
     return SQEQ_OK;
 }
 
-extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
-                              const double box[3], double rc, double alpha, const int grid[3], int order,
-                              double ke, const float* chi, const float* J, double total_charge,
-                              double tol, int max_iter, int restart, float* q_out, double* lambda_out,
-                              int* iters_out, double* relres_out)
+// A_ii of the Ewald matrix for r_c < L/2 (no image of an atom inside its own cutoff): the reciprocal-space self
+// term (1/(pi V)) sum_{m != 0} exp(-pi^2 |m/L|^2/alpha^2)/|m/L|^2 minus 2 alpha/sqrt(pi) (Eqs. 4-5)
+double ewald_self_diag(const double box[3], double alpha)
 {
-    if (!ctx) return SQEQ_EINVAL;
-    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_qeq_solve"));
-    if (!pos || !chi || !J || !q_out) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: NULL argument");
-    if (max_iter < 1 || restart < 0 || !(tol >= 0.0))
-        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_qeq_solve: need max_iter >= 1, restart >= 0, tol >= 0");
-    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    const double V = box[0] * box[1] * box[2];
+    int mmax[3];
+    for (int d = 0; d < 3; ++d) mmax[d] = (int)ceil(6.3 * alpha * box[d] / M_PI);     // exp(-39.7) ~ 6e-18
+    double s = 0.0;
+    for (int a = -mmax[0]; a <= mmax[0]; ++a)
+        for (int b = -mmax[1]; b <= mmax[1]; ++b)
+            for (int c = -mmax[2]; c <= mmax[2]; ++c) {
+                if (!(a | b | c)) continue;
+                const double m2 = (a / box[0]) * (a / box[0]) + (b / box[1]) * (b / box[1]) + (c / box[2]) * (c / box[2]);
+                s += exp(-M_PI * M_PI * m2 / (alpha * alpha)) / m2;
+            }
+    return s / (M_PI * V) - 2.0 * alpha / sqrt(M_PI);
+}
+
+// Eq. 18 on prepared geometry: q (fp64 device [n], out; also the initial guess when warm != 0) and lambda.
+int qeq_solve_prepared(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], double rc, double alpha,
+                       double ke, const float* chi, const float* J, double total_charge, double tol, int max_iter,
+                       int restart, bool jacobi, bool warm, double* q_io, double* lambda_io, int* iters_out,
+                       double* relres_out, bool* converged_out)
+{
     cudaStream_t st = ctx->stream;
     const int64_t len = n + 1;
-    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    const int nbl = ceil_div(len, 256);
     SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_f[0], sizeof(float) * n));
     QeqOp op{ctx, nl, n, box, rc, alpha, ke, J, (float*)ctx->vec_f[0].p};
-    // geometry once; the charge slot is refreshed per mat-vec (q = chi is only a placeholder here)
-    SQEQ_TRY(prep_atoms(ctx, nl, pos, chi, ctx->K, st));
-    const int nbl = ceil_div(len, 256);
     auto apply = [&](const double* v, double* w) { return qeq_apply(op, v, w); };
     auto load_rhs = [&](double* w) {
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
@@ -334,23 +396,90 @@ extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, co
         KERNEL_CHECK(ctx);
         return (int)SQEQ_OK;
     };
+    double* dinv = nullptr;
+    double* x0 = nullptr;
+    if (jacobi || warm) {
+        SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_d[4], sizeof(double) * len));
+        SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_d[5], sizeof(double) * len));
+    }
+    if (jacobi) {
+        dinv = (double*)ctx->vec_d[4].p;
+        k_qeq_jacobi<<<nbl, 256, 0, st>>>(n, J, ke * ewald_self_diag(box, alpha), dinv);
+        KERNEL_CHECK(ctx);
+    }
+    if (warm) {
+        x0 = (double*)ctx->vec_d[5].p;
+        k_qeq_guess<<<nbl, 256, 0, st>>>(n, q_io, *lambda_io, x0);
+        KERNEL_CHECK(ctx);
+    }
     double* x = nullptr;
+    SQEQ_TRY(gmres_solve(ctx, len, apply, load_rhs, tol, max_iter, restart, &x, iters_out, relres_out, converged_out, x0, dinv));
+    CUDA_TRY(ctx, cudaMemcpyAsync(q_io, x, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 5, x + n, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    *lambda_io = ctx->h_scal[5];
+    return SQEQ_OK;
+}
+
+static int qeq_solve_common(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
+                            double rc, double alpha, const int grid[3], int order, double ke, const float* chi,
+                            const float* J, double total_charge, double tol, int max_iter, int restart, bool jacobi,
+                            const float* q0, double lambda0, float* q_out, double* lambda_out, int* iters_out,
+                            double* relres_out, const char* who)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, who));
+    if (!pos || !chi || !J || !q_out) return sqeq_fail(ctx, SQEQ_EINVAL, "%s: NULL argument", who);
+    if (max_iter < 1 || restart < 0 || !(tol >= 0.0))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: need max_iter >= 1, restart >= 0, tol >= 0", who);
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
+    // geometry once; the charge slot is refreshed per mat-vec
+    SQEQ_TRY(prep_atoms(ctx, nl, pos, nullptr, ctx->K, st));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->vec_d[3], sizeof(double) * (n + 1)));
+    double* qd = (double*)ctx->vec_d[3].p;
+    double lam = lambda0;
+    if (q0) {
+        k_f2d<<<ceil_div(n, 256), 256, 0, st>>>(n, q0, qd);
+        KERNEL_CHECK(ctx);
+    }
     int iters = 0;
     double relres = 1.0;
     bool converged = false;
-    SQEQ_TRY(gmres_solve(ctx, len, apply, load_rhs, tol, max_iter, restart, &x, &iters, &relres, &converged));
+    SQEQ_TRY(qeq_solve_prepared(ctx, nl, n, box, rc, alpha, ke, chi, J, total_charge, tol, max_iter, restart, jacobi,
+                                q0 != nullptr, qd, &lam, &iters, &relres, &converged));
     {
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
-        k_d2f<<<ceil_div(n, 256), 256, 0, st>>>(n, x, q_out);
+        k_d2f<<<ceil_div(n, 256), 256, 0, st>>>(n, qd, q_out);
         KERNEL_CHECK(ctx);
-        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 5, x + n, sizeof(double), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(ctx, cudaStreamSynchronize(st));
     }
-    if (lambda_out) *lambda_out = ctx->h_scal[5];
+    if (lambda_out) *lambda_out = lam;
     if (iters_out) *iters_out = iters;
     if (relres_out) *relres_out = relres;
     if (!converged)
-        return sqeq_fail(ctx, SQEQ_ENOTCONV, "sqeq_qeq_solve: relative residual %.3e > tol %.3e after %d Coulomb evaluations",
-                         relres, tol, iters);
+        return sqeq_fail(ctx, SQEQ_ENOTCONV, "%s: relative residual %.3e > tol %.3e after %d Coulomb evaluations",
+                         who, relres, tol, iters);
     return SQEQ_OK;
+}
+
+extern "C" int sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                              const double box[3], double rc, double alpha, const int grid[3], int order,
+                              double ke, const float* chi, const float* J, double total_charge,
+                              double tol, int max_iter, int restart, float* q_out, double* lambda_out,
+                              int* iters_out, double* relres_out)
+{
+    return qeq_solve_common(ctx, nl, n, pos, box, rc, alpha, grid, order, ke, chi, J, total_charge, tol, max_iter,
+                            restart, false, nullptr, 0.0, q_out, lambda_out, iters_out, relres_out, "sqeq_qeq_solve");
+}
+
+extern "C" int sqeq_qeq_solve_pc(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                                 const double box[3], double rc, double alpha, const int grid[3], int order,
+                                 double ke, const float* chi, const float* J, double total_charge,
+                                 double tol, int max_iter, int restart, int jacobi, const float* q0, double lambda0,
+                                 float* q_out, double* lambda_out, int* iters_out, double* relres_out)
+{
+    return qeq_solve_common(ctx, nl, n, pos, box, rc, alpha, grid, order, ke, chi, J, total_charge, tol, max_iter,
+                            restart, jacobi != 0, q0, lambda0, q_out, lambda_out, iters_out, relres_out, "sqeq_qeq_solve_pc");
 }

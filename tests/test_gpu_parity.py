@@ -444,6 +444,63 @@ def test_shadow_md_steps_config2_geometry(ctx):
     nl.free()
 
 
+def test_regular_bomd_against_oracle(ctx):
+    """NEXT-2: Jacobi-preconditioned, warm-started GMRES on Eq. 18 and one
+    regular BOMD step -- forces at fixed q_min, U_BO, the O-O repulsion of the stand-in -- against the oracle, on
+    648 waters-like atoms of the cfg-0 box with the positive-definite per-element parameters."""
+    from paper_2503_21176_b200 import binding
+    c = W.CONFIGS[0]
+    pos, _ = inputs(0)
+    n = len(pos)
+    chi, u = W.qeq_params_water_pd(n)
+    mass = W.masses_water(n)
+    vel = W.velocities(mass)
+    geo = dict(box=c.box, rc=c.rc, alpha=c.alpha, grid=c.grid, order=c.order)
+    p = binding.md_params(c, dt=0.25, k_rep=10.0, r_rep=2.9)
+    standin = (p.k_oh, p.r_oh, p.k_hh, p.r_hh, p.k_rep, p.r_rep)
+    nl = ctx.nl_build(dev(pos), c.box, c.r_list)
+    # the solver alone: with and without the preconditioner, cold and warm, vs the oracle's counts and charges
+    ref = oracle.bo_eval(pos, chi, u, W.KE_EV_A, 0.0, standin=standin, tol=1e-6, max_iter=60, **geo)
+    q, lam, it, rel, ok = ctx.qeq_solve_pc(nl, dev(pos), c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, dev(chi), dev(u),
+                                           0.0, tol=1e-6, max_iter=60, jacobi=True)
+    assert ok and abs(it - (ref["evals"] - 1)) <= 1
+    assert relrms(q.cpu().numpy(), ref["q"]) < 1e-5 and abs(lam - ref["lam"]) < 1e-4 * abs(ref["lam"])
+    q2, lam2, it2, rel2, ok2 = ctx.qeq_solve_pc(nl, dev(pos), c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, dev(chi),
+                                                dev(u), 0.0, tol=1e-6, max_iter=60, jacobi=True, q0=q, lambda0=lam)
+    assert ok2 and it2 <= 2                       # the residual of the guess, at most one vector
+    # the J ~ U(5,10) system of cfg 0: the Jacobi diagonal is not uniform there and must not hurt
+    chi0, J0 = W.qeq_params(n)
+    qa, _, ita, _, oka = ctx.qeq_solve_pc(nl, dev(pos), c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, dev(chi0), dev(J0),
+                                          0.0, tol=1e-3, max_iter=649, jacobi=False)
+    qb, _, itb, _, okb = ctx.qeq_solve_pc(nl, dev(pos), c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, dev(chi0), dev(J0),
+                                          0.0, tol=1e-3, max_iter=649, jacobi=True)
+    print(f"cfg0 indefinite system to 1e-3: {ita} evaluations plain, {itb} with Jacobi")
+    record("qeq_cfg0_jacobi", iters_plain=ita, iters_jacobi=itb)
+    assert oka and okb and relrms(qa.cpu().numpy(), qb.cpu().numpy()) < 2e-2
+    # one BOMD step from the same state
+    state, F, en = ctx.bomd_init(nl, dev(pos), c.box, p, dev(chi), dev(u), tol=1e-7, max_iter=80)
+    ref0 = oracle.bo_eval(pos, chi, u, W.KE_EV_A, 0.0, standin=standin, tol=1e-9, max_iter=80, **geo)
+    eF0, eU0 = relrms(F.cpu().numpy(), ref0["F"]), abs(en[0] / ref0["U"] - 1)
+    print(f"bomd init: F {eF0:.2e} U {eU0:.2e} q {relrms(state['q'].cpu().numpy(), ref0['q']):.2e} evals {en[3]}")
+    assert state["converged"] and eF0 < TOL and eU0 < 1e-6
+    x, v = dev(pos), dev(vel)
+    st = dict(pos=pos.astype(np.float64), F=F.cpu().numpy().astype(np.float64), q=state["q"].cpu().numpy().copy(),
+              lam=state["lam"].value)
+    st, ov, ekin = oracle.bo_md_step(st, vel.astype(np.float64), mass, 0.25, chi, u, W.KE_EV_A, 0.0, standin=standin,
+                                     tol=1e-9, max_iter=80, **geo)
+    en = ctx.bomd_step(nl, x, v, dev(mass), c.box, p, dev(chi), dev(u), state, F, tol=1e-7, max_iter=80)
+    same = oracle.bo_eval(x.cpu().numpy(), chi, u, W.KE_EV_A, 0.0, standin=standin, tol=1e-9, max_iter=80, **geo)
+    eF, eU = relrms(F.cpu().numpy(), same["F"]), abs(en[0] / same["U"] - 1)
+    eq = relrms(state["q"].cpu().numpy(), same["q"])
+    print(f"bomd step: x {np.abs(x.cpu().numpy() - st['pos']).max():.2e} | same state: F {eF:.2e} U {eU:.2e} q {eq:.2e} "
+          f"evals {en[3]} (oracle {st['evals']})")
+    record("bomd_cfg0_box", F_same_state=eF, U_same_state=eU, q_same_state=eq)
+    assert np.abs(x.cpu().numpy() - st["pos"]).max() < 0.51 * 2.0 ** -19       # half an ulp below 16 A... (18.6 A box: 2^-19*2)
+    assert state["converged"] and eF < TOL and eU < 1e-6 and eq < 1e-5
+    assert abs(en[1] - ekin) < 1e-4 * ekin
+    nl.free()
+
+
 @pytest.mark.parametrize("k", [2, 4])
 def test_fixed_geometry_cache(ctx, k):
     """NEXT-1: sqeq_geometry_set + sqeq_coulomb_fixed -- several charge vectors on one geometry.
