@@ -33,6 +33,7 @@ from paper_2503_21176_b200 import workloads as W  # noqa: E402
 METRIC = "PME Coulomb potential+force evals/s at 331,776 atoms"
 REBUILD_EVERY = 10
 N_POSSETS = 10
+E2E_REPS = 3
 
 
 def measured_peaks():
@@ -196,6 +197,18 @@ def run_reference(args, cfg):
 
 
 # ------------------------------------------------------------------------------------------------
+def oracle_full_evaluation(cfg, pos, q):
+    """ONE full oracle evaluation of `cfg`, actually timed (no scaling): brute-force neighbour search, O(N^2)
+    real-space sum, PME with naive line DFTs."""
+    import oracle
+    t0 = time.perf_counter(); oi, oj, os_ = oracle.neighbour_list(pos, cfg.box, cfg.r_list); t_nl = time.perf_counter() - t0
+    t0 = time.perf_counter(); oracle.realspace(pos, q, cfg.box, cfg.rc, cfg.alpha); t_real = time.perf_counter() - t0
+    t0 = time.perf_counter(); oracle.pme_recip(pos, q, cfg.box, cfg.grid, cfg.order, cfg.alpha); t_pme = time.perf_counter() - t0
+    return {"kind": "measured", "t_nl_s": round(t_nl, 4), "t_real_s": round(t_real, 4), "t_pme_s": round(t_pme, 4),
+            "evals_per_s": 1.0 / (t_real + t_pme), "evals_per_s_with_rebuild_every_10": 1.0 / (t_real + t_pme + t_nl / REBUILD_EVERY),
+            "pairs_in_list": int(len(oi)), "cores": oracle.num_threads()}
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
@@ -211,152 +224,200 @@ def run_ours(args, cfg):
     ctx = binding.Context(local)
     hbm_peak, peak_src, _ = measured_peaks()
 
-    pos0, q = W.make(cfg.index)
-    n = len(q)
-    possets = [torch.as_tensor(W.perturb(pos0, k, 0.02, cfg.index)).to(dev) for k in range(N_POSSETS)]
-    # cumulative drift would exceed skin/2 after many steps; the sets are independent perturbations of
-    # pos0 (sigma 0.02 A, max ~0.1 A << skin/2), so a list built on any set is valid for all of them
-    qd = torch.as_tensor(q).to(dev)
-    phi = torch.empty(n, dtype=torch.float32, device=dev)
-    force = torch.empty((n, 3), dtype=torch.float32, device=dev)
-    box, rc, alpha, grid, order, rl = cfg.box, cfg.rc, cfg.alpha, cfg.grid, cfg.order, cfg.r_list
-    state = {"nl": None}
-
-    def step(k, host=None):
-        if k % REBUILD_EVERY == 0:
-            if state["nl"] is not None:
-                state["nl"].free()
-            state["nl"] = ctx.nl_build(possets[k % N_POSSETS], box, rl)
-            state["nl_set"] = k % N_POSSETS
-        if host is None:
-            # potential, force and the fp64 energy reduction, all enqueued; the energy of the last
-            # step is read back once at the end of the timed region (sqeq_energy_fetch)
-            return ctx.coulomb_enqueue(state["nl"], possets[k % N_POSSETS], qd, box, rc, alpha, grid, order,
-                                       phi, force, want_energy=True)
-        hp, hq, hphi, hf = host
-        return ctx.coulomb_host(state["nl"], hp[k % N_POSSETS], hq, box, rc, alpha, grid, order, hphi, hf)
-
     def barrier():
         torch.cuda.synchronize()
         replicas.barrier()
         torch.cuda.synchronize()
 
-    def timed(nsteps, host=None, k0=0):
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(ctx.stream)
-        for k in range(nsteps):
-            step(k0 + k, host)
-        if host is None:
-            state["energy"] = ctx.energy_fetch()
-        e1.record(ctx.stream)
-        barrier()
-        return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+    def eval_loop(c, nsteps, warmup, rebuild_every, perturbed, with_e2e=False):
+        """The evaluation workload of one config: nsteps potential+force+energy evaluations, positions perturbed by
+        sigma 0.02 A per step (or fixed), the list (rc + skin) rebuilt every `rebuild_every` steps inside the timed
+        region (None: built once, outside).  Returns the device-timed value, the per-stage profile and, for the
+        headline config, the host-buffer legs."""
+        pos0, q = W.make(c.index)
+        n = len(q)
+        nsets = N_POSSETS if perturbed else 1
+        # the sets are independent perturbations of pos0 (sigma 0.02 A, max ~0.1 A << skin/2), so a list built on any
+        # set is valid for all of them
+        possets = [torch.as_tensor(W.perturb(pos0, k, 0.02, c.index) if perturbed else pos0).to(dev) for k in range(nsets)]
+        qd = torch.as_tensor(q).to(dev)
+        phi = torch.empty(n, dtype=torch.float32, device=dev)
+        force = torch.empty((n, 3), dtype=torch.float32, device=dev)
+        box, rc, alpha, grid, order, rl = c.box, c.rc, c.alpha, c.grid, c.order, c.r_list
+        state = {"nl": None}
 
-    # ---- device-resident leg: the reported value (no stage events), clocks sampled during it ------
-    for k in range(max(args.warmup, 3)):
-        step(k)
-    ctx.launch_count(reset=True)
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ms_value = timed(args.steps)
-    launches = ctx.launch_count()
-    clocks = sampler.stop() if rank == 0 else {}
-    value = world * 1e3 * args.steps / ms_value
-    ms_step = ms_value / args.steps
-
-    # ---- same loop again with a CUDA-event pair around every stage (per-kernel durations) ---------
-    ctx.profile_enable(True)
-    ctx.profile_reset()
-    ms = timed(args.steps)
-    prof = ctx.profile_read()
-    ctx.profile_enable(False)
-
-    # ---- end-to-end leg: C-ABI call with HOST buffers, copies inside the timed region -----------
-    hp = [p.cpu().pin_memory() for p in possets]
-    hq = qd.cpu().pin_memory()
-    hphi = torch.empty(n, dtype=torch.float32).pin_memory()
-    hf = torch.empty((n, 3), dtype=torch.float32).pin_memory()
-    host = (hp, hq, hphi, hf)
-    for k in range(3):
-        step(k, host)
-    # the host-side legs are timed three times each and the median repetition is reported (all three are in the
-    # JSON line): the first repetition still pays first-use costs of the host path (pinned position sets touched
-    # for the first time, slot buffers), which the three warm-up steps do not cover
-    E2E_REPS = 3
-    reps_sync = [timed(args.steps, host) for _ in range(E2E_REPS)]    # one synchronous sqeq_coulomb_host call per step
-    ms_e2e_sync = sorted(reps_sync)[E2E_REPS // 2]
-    # the same steps through the pipelined entry (sqeq_coulomb_host_submit / _wait, two slots): the evaluations
-    # are independent, so the inputs of step k+1 and the results of step k-1 cross PCIe while step k computes;
-    # every step still copies its 16 B/atom in and 16 B/atom + 8 B out inside the timed region
-    hphi2 = [hphi, torch.empty(n, dtype=torch.float32).pin_memory()]
-    hf2 = [hf, torch.empty((n, 3), dtype=torch.float32).pin_memory()]
-
-    def timed_pipelined(nsteps):
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(ctx.stream)
-        for k in range(nsteps):
-            s = k & 1
-            if k >= 2:
-                state["energy_e2e"] = ctx.coulomb_host_wait(s)
-            if k % REBUILD_EVERY == 0:
+        def rebuild(k):
+            if state["nl"] is not None:
                 state["nl"].free()
-                state["nl"] = ctx.nl_build(possets[k % N_POSSETS], box, rl)
-                state["nl_set"] = k % N_POSSETS
-            ctx.coulomb_host_submit(s, state["nl"], hp[k % N_POSSETS], hq, box, rc, alpha, grid, order,
-                                    hphi2[s], hf2[s])
-        for k in range(max(0, nsteps - 2), nsteps):
-            state["energy_e2e"] = ctx.coulomb_host_wait(k & 1)
-        e1.record(ctx.stream)
-        barrier()
-        return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+            state["nl"] = ctx.nl_build(possets[k % nsets], box, rl)
+            state["nl_set"] = k % nsets
 
-    timed_pipelined(4)
-    reps_pipe = [timed_pipelined(args.steps) for _ in range(E2E_REPS)]
+        def step(k, host=None):
+            if rebuild_every and k % rebuild_every == 0:
+                rebuild(k)
+            if host is None:
+                # potential, force and the fp64 energy reduction, all enqueued; the energy of the last
+                # step is read back once at the end of the timed region (sqeq_energy_fetch)
+                return ctx.coulomb_enqueue(state["nl"], possets[k % nsets], qd, box, rc, alpha, grid, order,
+                                           phi, force, want_energy=True)
+            hp, hq, hphi, hf = host
+            return ctx.coulomb_host(state["nl"], hp[k % nsets], hq, box, rc, alpha, grid, order, hphi, hf)
+
+        def timed(ns, host=None):
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(ctx.stream)
+            for k in range(ns):
+                step(k, host)
+            if host is None:
+                state["energy"] = ctx.energy_fetch()
+            e1.record(ctx.stream)
+            barrier()
+            return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+
+        res = {"n": n, "state": state, "possets": possets, "qd": qd}
+        if not rebuild_every:
+            # build timed on its own (median of 5), then kept
+            tb = []
+            for _ in range(5):
+                torch.cuda.synchronize(); t0 = time.perf_counter(); rebuild(0); torch.cuda.synchronize()
+                tb.append((time.perf_counter() - t0) * 1e3)
+            res["nl_build_ms"] = sorted(tb)[2]
+        for k in range(max(warmup, 3)):
+            step(k)
+        ctx.launch_count(reset=True)
+        sampler = ClockSampler(local)
+        if rank == 0 and with_e2e:
+            sampler.start()
+        ms_value = timed(nsteps)
+        res["launches"] = ctx.launch_count()
+        res["clocks"] = sampler.stop() if (rank == 0 and with_e2e) else {}
+        res["ms_value"] = ms_value
+        # same loop again with a CUDA-event pair around every stage (per-kernel durations)
+        ctx.profile_enable(True)
+        ctx.profile_reset()
+        res["ms_profiled"] = timed(nsteps)
+        res["prof"] = ctx.profile_read()
+        ctx.profile_enable(False)
+        if with_e2e:
+            # end-to-end legs: C-ABI calls with HOST buffers, copies inside the timed region
+            hp = [p.cpu().pin_memory() for p in possets]
+            hq = qd.cpu().pin_memory()
+            hphi = torch.empty(n, dtype=torch.float32).pin_memory()
+            hf = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+            host = (hp, hq, hphi, hf)
+            for k in range(3):
+                step(k, host)
+            # the host-side legs are timed three times each and the median repetition is reported (all three are in
+            # the JSON line): the first repetition still pays first-use costs of the host path
+            res["reps_sync"] = [timed(nsteps, host) for _ in range(E2E_REPS)]
+            # the same steps through the pipelined entry (sqeq_coulomb_host_submit / _wait, two slots): the inputs of
+            # step k+1 and the results of step k-1 cross PCIe while step k computes; every step still copies its
+            # 16 B/atom in and 16 B/atom + 8 B out inside the timed region
+            hphi2 = [hphi, torch.empty(n, dtype=torch.float32).pin_memory()]
+            hf2 = [hf, torch.empty((n, 3), dtype=torch.float32).pin_memory()]
+
+            def timed_pipelined(ns):
+                barrier()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(ctx.stream)
+                for k in range(ns):
+                    s = k & 1
+                    if k >= 2:
+                        state["energy_e2e"] = ctx.coulomb_host_wait(s)
+                    if rebuild_every and k % rebuild_every == 0:
+                        rebuild(k)
+                    ctx.coulomb_host_submit(s, state["nl"], hp[k % nsets], hq, box, rc, alpha, grid, order, hphi2[s], hf2[s])
+                for k in range(max(0, ns - 2), ns):
+                    state["energy_e2e"] = ctx.coulomb_host_wait(k & 1)
+                e1.record(ctx.stream)
+                barrier()
+                return replicas.max_over_ranks(e0.elapsed_time(e1), dev)
+
+            timed_pipelined(4)
+            res["reps_pipe"] = [timed_pipelined(nsteps) for _ in range(E2E_REPS)]
+        return res
+
+    def kernel_table(c, res, nsteps):
+        """Per-stage durations (CUDA events on the launching stream) against each kernel's algorithmic bytes."""
+        n, grid = res["n"], c.grid
+        info = res["state"]["nl"].info()
+        P, EB = info["n_directed"], info["entry_bytes"]
+        G3, S3 = grid ** 3, grid * grid * (grid // 2 + 1)
+        alg_bytes = {  # algorithmic bytes per launch (DESIGN.md section 7)
+            "real": EB * P + 32 * n, "spread": 16 * n + 4 * G3, "fft_fwd": 4 * G3 + 8 * S3, "influence": 16 * S3,
+            "fft_inv": 4 * G3 + 8 * S3, "gather": 32 * n + 4 * G3, "prep": 64 * n, "assemble": 64 * n,
+            "nl_pairs": EB * P + 32 * n, "nl_bin": 52 * n}
+        kernels = {}
+        ms_step = res["ms_profiled"] / nsteps
+        for name, (tot, cnt) in res["prof"].items():
+            if cnt == 0:
+                continue
+            avg = tot / cnt
+            b = alg_bytes.get(name)
+            kernels[name] = {"ms_avg": round(avg, 5), "launches": cnt, "share_of_step": round(tot / (nsteps * ms_step), 4),
+                             "alg_MB": round(b / 1e6, 2) if b else None, "GBps": round(b / avg / 1e6, 1) if b else None,
+                             "hbm_frac": round(b / avg / 1e6 / hbm_peak, 4) if b else None}
+        return kernels, alg_bytes, info
+
+    def pairs_within_rc(c, res):
+        """unique pairs with r < rc (the list also holds the skin pairs), from the exported list."""
+        st = res["state"]
+        gi, gj, gs = st["nl"].export()
+        pb = res["possets"][st["nl_set"]]
+        boxv = torch.tensor(c.box, dtype=torch.float32, device=dev)
+        n_in, CH = 0, 1 << 24
+        for a in range(0, gi.numel(), CH):
+            sl = slice(a, min(a + CH, gi.numel()))
+            d = pb[gj[sl].long()] + gs[sl].float() * boxv - pb[gi[sl].long()]
+            n_in += int(((d * d).sum(1) < c.rc * c.rc).sum())
+        return n_in, int(gi.numel())
+
+    def config_summary(c, res, nsteps, world=1):
+        kernels, alg_bytes, info = kernel_table(c, res, nsteps)
+        n_in, n_list = pairs_within_rc(c, res)
+        out = {"workload": c.workload, "atoms": res["n"], "grid": c.grid,
+               "evals_per_s": world * 1e3 * nsteps / res["ms_value"], "ms_per_eval": res["ms_value"] / nsteps,
+               "launches_per_eval": round(res["launches"] / nsteps, 1),
+               "unique_pairs_within_rc": n_in, "unique_pairs_in_list": n_list, "list_entry_bytes": info["entry_bytes"]}
+        if "nl_build_ms" in res:
+            out["nl_build_ms"] = round(res["nl_build_ms"], 4)
+        if "real" in kernels:
+            out["pair_interactions_per_s"] = n_in / (kernels["real"]["ms_avg"] * 1e-3)
+            out["real_kernel_hbm_frac"] = kernels["real"]["hbm_frac"]
+        pme_ms = sum(kernels[k]["ms_avg"] for k in ("spread", "fft_fwd", "influence", "fft_inv", "gather") if k in kernels)
+        if pme_ms > 0:
+            out["grid_points_per_s"] = c.grid ** 3 / (pme_ms * 1e-3)
+            out["cufft_ms"] = round(sum(kernels[k]["ms_avg"] for k in ("fft_fwd", "fft_inv") if k in kernels), 5)
+        dom = max((k for k in kernels if k not in ("nl_pairs", "nl_bin")), key=lambda k: res["prof"][k][0])
+        out["dominant_kernel"] = dom
+        out["dominant_kernel_share"] = kernels[dom]["share_of_step"]
+        out["dominant_kernel_hbm_frac"] = kernels[dom]["hbm_frac"]
+        out["stage_ms"] = {k: v["ms_avg"] for k, v in kernels.items()}
+        return out, kernels, alg_bytes, info
+
+    # ---- headline: configs[4] (or --config), device-resident value + stage profile + host-buffer legs -----
+    res = eval_loop(cfg, args.steps, args.warmup, REBUILD_EVERY, True, with_e2e=True)
+    n = res["n"]
+    clocks, launches = res["clocks"], res["launches"]
+    value = world * 1e3 * args.steps / res["ms_value"]
+    ms_step = res["ms_value"] / args.steps
+    reps_sync, reps_pipe = res["reps_sync"], res["reps_pipe"]
     ms_e2e = sorted(reps_pipe)[E2E_REPS // 2]
     e2e_val = world * 1e3 * args.steps / ms_e2e
-    e2e_sync_val = world * 1e3 * args.steps / ms_e2e_sync
-
-    # ---- per-kernel roofline (stage events on the launching streams, over the timed region) -----
-    info = state["nl"].info()
-    P = info["n_directed"]
-    EB = info["entry_bytes"]       # 2: 16-bit local list (staged real-space kernel), 4: atom index | image
-    G3 = grid ** 3
-    S3 = grid * grid * (grid // 2 + 1)
-    alg_bytes = {  # algorithmic bytes per launch
-        "real": EB * P + 32 * n,
-        "spread": 16 * n + 4 * G3,
-        "fft_fwd": 4 * G3 + 8 * S3,
-        "influence": 16 * S3,
-        "fft_inv": 4 * G3 + 8 * S3,
-        "gather": 32 * n + 4 * G3,
-        "prep": 16 * n + 16 * n + 16 * n + 16 * n,
-        "assemble": 48 * n + 16 * n,
-        "nl_pairs": EB * P + 2 * 16 * n,
-        "nl_bin": 12 * n * 2 + 16 * n + 12 * n,
-    }
-    kernels = {}
-    for name, (tot, cnt) in prof.items():
-        if cnt == 0:
-            continue
-        avg = tot / cnt
-        b = alg_bytes.get(name)
-        kernels[name] = {"ms_avg": round(avg, 5), "launches": cnt,
-                         "share_of_step": round(tot / (args.steps * (ms / args.steps)), 4),
-                         "alg_MB": round(b / 1e6, 2) if b else None,
-                         "GBps": round(b / avg / 1e6, 1) if b else None,
-                         "hbm_frac": round(b / avg / 1e6 / hbm_peak, 4) if b else None}
-    dom = max((k for k in kernels if k not in ("nl_pairs", "nl_bin")), key=lambda k: prof[k][0])
-    traffic = None
+    e2e_sync_val = world * 1e3 * args.steps / sorted(reps_sync)[E2E_REPS // 2]
+    summ, kernels, alg_bytes, info = config_summary(cfg, res, args.steps, world)
+    P, EB = info["n_directed"], info["entry_bytes"]
+    dom = summ["dominant_kernel"]
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(dom)
+        tj = json.load(open(tpath))
+        traffic, traffic_src = tj.get(dom), tj.get("_source")
     roofline = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["GBps"], "peak": hbm_peak,
                 "unit": "GB/s", "frac": kernels[dom]["hbm_frac"], "traffic": traffic,
-                "peak_source": peak_src,
-                "alg_bytes_per_launch": alg_bytes[dom],
+                "traffic_source": traffic_src or "ncu --set full capture recorded in profiles/traffic.json (not measured in this run)",
+                "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes[dom],
                 "note": "%d B x directed list entries + 32 B x atoms for the real-space kernel; ms_avg from CUDA "
                         "events on the launching stream over the timed region; the kernel is instruction-issue "
                         "bound (DESIGN.md section 7), see roofline_alu" % EB}
@@ -368,42 +429,44 @@ def run_ours(args, cfg):
                     "peak": round(fp32_peak, 1), "unit": "TFLOP/s",
                     "frac": round(flops / (kernels[dom]["ms_avg"] * 1e-3) / 1e12 / fp32_peak, 4)} if dom == "real" else None
 
-    extra = {"kernels": kernels,
-             "pair_interactions_per_s": None, "grid_points_per_s": None,
-             "n_directed_list_entries": P, "ms_per_step_with_stage_events": round(ms / args.steps, 4)}
+    extra = {"kernels": kernels, "pair_interactions_per_s": summ.get("pair_interactions_per_s"),
+             "grid_points_per_s": summ.get("grid_points_per_s"), "n_directed_list_entries": P,
+             "ms_per_step_with_stage_events": round(res["ms_profiled"] / args.steps, 4),
+             "unique_pairs_within_rc": summ["unique_pairs_within_rc"], "unique_pairs_in_list": summ["unique_pairs_in_list"]}
     if "real" in kernels:
-        # unique pairs with r < rc per second of the real-space kernel; counted here from
-        # the exported list (the list itself also holds the skin pairs between rc and r_list)
-        gi, gj, gs = state["nl"].export()
-        pb = possets[state["nl_set"]]
-        boxv = torch.tensor(box, dtype=torch.float32, device=dev)
-        n_in = 0
-        CH = 1 << 24
-        for a in range(0, gi.numel(), CH):
-            sl = slice(a, min(a + CH, gi.numel()))
-            d = pb[gj[sl].long()] + gs[sl].float() * boxv - pb[gi[sl].long()]
-            n_in += int(((d * d).sum(1) < rc * rc).sum())
-        del gi, gj, gs
-        extra["unique_pairs_within_rc"] = n_in
-        extra["unique_pairs_in_list"] = P // 2
-        extra["pair_interactions_per_s"] = n_in / (kernels["real"]["ms_avg"] * 1e-3)
         extra["list_pairs_per_s"] = (P / 2) / (kernels["real"]["ms_avg"] * 1e-3)
-    pme_ms = sum(kernels[k]["ms_avg"] for k in ("spread", "fft_fwd", "influence", "fft_inv", "gather") if k in kernels)
-    if pme_ms > 0:
-        extra["grid_points_per_s"] = G3 / (pme_ms * 1e-3)
+    res["state"]["nl"].free()
+    pos_md = res["possets"][0]
+    del res
 
-    # ---- a-10 / a-11 legs: QEq Krylov iterations and shadow XL-BOMD steps ------------------------
+    # ---- every config's own workload ------------------------------------------
+    per_config = {}
+    if rank == 0 and not args.no_per_config:
+        per_config[str(cfg.index)] = {k: v for k, v in summ.items()}
+        for k in range(4):
+            try:
+                per_config[str(k)] = run_config_workload(ctx, k, dev, eval_loop, config_summary, args)
+            except Exception as ex:  # report, never hide
+                per_config[str(k)] = {"error": str(ex)}
+    extra["per_config"] = per_config
+
+    # ---- a-10 / a-11 / NEXT-2 legs: QEq Krylov iterations, shadow XL-BOMD and regular BOMD steps ----------
     if not args.no_md and rank == 0:
         try:
-            extra.update(run_md_legs(ctx, cfg, possets[0], n, dev, args))
+            extra.update(run_md_legs(ctx, cfg, pos_md, n, dev, args))
         except Exception as ex:  # report, never hide
             extra["md_error"] = str(ex)
+        if not args.no_per_config:
+            try:
+                extra["table1_shaped"] = run_table1(ctx, dev, args)
+            except Exception as ex:
+                extra["table1_error"] = str(ex)
 
     out = {"metric": METRIC, "value": value, "unit": "evals/s", "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": f"configs[{cfg.index}] {cfg.name}: {n} atoms, L {cfg.L} A, rc {cfg.rc} A "
-                                  f"(+{cfg.skin} A skin), alpha {cfg.alpha}, PME {grid}^3 order {order}; one "
+                                  f"(+{cfg.skin} A skin), alpha {cfg.alpha}, PME {cfg.grid}^3 order {cfg.order}; one "
                                   f"potential+force+energy evaluation per step, positions perturbed (sigma 0.02 A) "
                                   f"each step, neighbour rebuild every {REBUILD_EVERY} steps inside the timed region",
                       "l2": "inputs larger than L2: the %.0f MB neighbour list is streamed every step; no flush" % (EB * P / 1e6),
@@ -421,14 +484,129 @@ def run_ours(args, cfg):
 
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
+            pos0, q = W.make(cfg.index)
             m = OracleSampler(cfg, q).sample(pos0, args.cpu_budget)
-            out["cpu_baseline"] = {"value": 1.0 / m["t_eval"], "unit": "evals/s", "cores": m["cores"],
-                                   "kind": "oracle", "sample": m["sample"],
-                                   "seconds_scaled": {k: round(m[k], 3) for k in
-                                                      ("t_real", "t_spread", "t_dft", "t_gather", "t_nl")}}
+            cb = {"value": 1.0 / m["t_eval"], "unit": "evals/s", "cores": m["cores"], "kind": "oracle",
+                  "how": "extrapolated: bounded sample of configs[%d] scaled linearly (a full oracle evaluation there is "
+                         "over a minute); configs 0-3 below are full evaluations, actually timed" % cfg.index,
+                  "sample": m["sample"],
+                  "seconds_scaled": {k: round(m[k], 3) for k in ("t_real", "t_spread", "t_dft", "t_gather", "t_nl")},
+                  "per_config_measured": {}}
+            for k in range(4):
+                c = W.CONFIGS[k]
+                p_, q_ = W.make(k)
+                cb["per_config_measured"][str(k)] = oracle_full_evaluation(c, p_, q_)
+            # check of the scaling on the largest fully timed config: the sampler's estimate beside the measurement
+            c3 = W.CONFIGS[3]
+            p3, q3 = W.make(3)
+            m3 = OracleSampler(c3, q3).sample(p3, 3.0)
+            cb["extrapolation_check_cfg3"] = {"extrapolated_evals_per_s": 1.0 / m3["t_eval"],
+                                              "measured_evals_per_s": cb["per_config_measured"]["3"]["evals_per_s_with_rebuild_every_10"]}
+            out["cpu_baseline"] = cb
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_config_workload(ctx, k, dev, eval_loop, config_summary, args):
+    """configs[0..3], each its own workload."""
+    import torch
+    c = W.CONFIGS[k]
+    if k == 3:      # evaluations with sigma 0.02 A perturbations and a rebuild every 10
+        res = eval_loop(c, 50, 10, REBUILD_EVERY, True)
+        out, _, _, _ = config_summary(c, res, 50)
+        res["state"]["nl"].free()
+        return out
+    res = eval_loop(c, 50, 10, None, False)        # cfg 0, 1, 2: one build (timed on its own), evaluations on it
+    out, _, _, _ = config_summary(c, res, 50)
+    nl, n = res["state"]["nl"], res["n"]
+    pos, qd = res["possets"][0], res["qd"]
+    if k in (0, 2):
+        chi, J = W.qeq_params(n)
+        chi_d, J_d = torch.as_tensor(chi).to(dev), torch.as_tensor(J).to(dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if k == 0:      # one qeq_solve, unrestarted GMRES (the system is symmetric indefinite, cond ~5e3)
+            kw = dict(tol=1e-5, max_iter=649, restart=0)
+        else:           # 50 Krylov iterations, each one PME Coulomb evaluation
+            kw = dict(tol=0.0, max_iter=50, restart=0)
+        ctx.qeq_solve(nl, pos, c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, chi_d, J_d, 0.0, **kw)
+        ctx.launch_count(reset=True)
+        torch.cuda.synchronize()
+        e0.record(ctx.stream)
+        q, lam, it, rel, ok = ctx.qeq_solve(nl, pos, c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, chi_d, J_d, 0.0, **kw)
+        e1.record(ctx.stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        out["qeq"] = {"krylov_iterations": it, "ms": round(ms, 3), "iterations_per_s": it / (ms * 1e-3),
+                      "relres_estimate": rel, "converged": ok, "launches_per_iteration": round(ctx.launch_count() / max(it, 1), 1)}
+    if k == 0:
+        # latency regime: potential-only evaluations of one charge vector after another on the fixed geometry
+        # (sqeq_geometry_set / sqeq_coulomb_fixed), back to back with no synchronisation
+        phi = torch.empty(n, dtype=torch.float32, device=dev)
+        ctx.geometry_set(nl, pos, c.box, c.rc, c.alpha, c.grid, c.order)
+        for _ in range(20):
+            ctx.coulomb_fixed(qd, phi)
+        ctx.launch_count(reset=True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(ctx.stream)
+        for _ in range(500):
+            ctx.coulomb_fixed(qd, phi)
+        e1.record(ctx.stream)
+        torch.cuda.synchronize()
+        out["fixed_geometry_potential_eval"] = {"us_per_eval": round(e0.elapsed_time(e1) * 1e3 / 500, 2),
+                                                "launches_per_eval": round(ctx.launch_count() / 500, 1)}
+    nl.free()
+    return out
+
+
+def md_loop(ctx, cfg, pos, n, dev, nsteps, mode, p, chi_d, u_d, tol=1e-6, skin_slack=0.02, dt=0.5, record_energy=False):
+    """nsteps of shadow XL-BOMD (mode 'shadow') or regular BOMD ('bomd') with the list rebuilt BEFORE a step whenever
+    the displacement since the build, one position update ahead, reaches skin/2 minus a slack."""
+    import torch
+    mass_h = W.masses_water(n)
+    mass = torch.as_tensor(mass_h).to(dev)
+    vel = torch.as_tensor(W.velocities(mass_h)).to(dev)
+    x = pos.clone()
+    box, rl = cfg.box, cfg.r_list
+    half_skin = 0.5 * (rl - cfg.rc)
+    nl = ctx.nl_build(x, box, rl)
+    if mode == "shadow":
+        nhist, force, en0 = ctx.shadow_md_init(nl, x, box, p, chi_d, u_d, tol=1e-6, max_iter=200)
+    else:
+        state, force, en0 = ctx.bomd_init(nl, x, box, p, chi_d, u_d, tol=min(tol, 1e-6), max_iter=300)
+    step = (lambda want: ctx.shadow_md_step(nl_ref[0], x, vel, mass, box, p, chi_d, u_d, nhist, force, want_energies=want)) \
+        if mode == "shadow" else \
+        (lambda want: ctx.bomd_step(nl_ref[0], x, vel, mass, box, p, chi_d, u_d, state, force, tol=tol, max_iter=300))
+    nl_ref = [nl]
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(ctx.stream)
+    rebuilds, evals, worst, energies = 0, 0.0, 0.0, []
+    for s in range(nsteps):
+        ahead = nl_ref[0].max_drift_ahead(x, vel, dt)
+        if ahead >= half_skin - skin_slack:
+            nl_ref[0].free()
+            nl_ref[0] = ctx.nl_build(x, box, rl)
+            rebuilds += 1
+        en = step(record_energy or s == nsteps - 1)
+        if record_energy or mode == "bomd":
+            evals += en[3]
+            energies.append(en[0] + en[1])
+        if s % 5 == 4 or s == nsteps - 1:
+            worst = max(worst, nl_ref[0].max_drift(x))       # the drift the evaluation of this step ran with
+    e1.record(ctx.stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    nl_ref[0].free()
+    out = {"steps": nsteps, "ms_per_step": ms / nsteps, "atom_steps_per_s": n * nsteps / (ms * 1e-3), "rebuilds": rebuilds,
+           "max_drift_seen_A": worst, "half_skin_A": half_skin,
+           "coulomb_evals_per_step": (evals / nsteps) if (record_energy or mode == "bomd") else (en[3] if en else None)}
+    if energies:
+        e = np.array(energies)
+        out["energy_std_eV"] = float(e.std())
+        out["energy_drift_eV"] = float(e[-1] - e[0])
+    return out
 
 
 def run_md_legs(ctx, cfg, pos, n, dev, args):
@@ -454,40 +632,47 @@ def run_md_legs(ctx, cfg, pos, n, dev, args):
     msq = e0.elapsed_time(e1)
     res["qeq_krylov_iters_per_s"] = it / (msq * 1e-3)
     res["qeq_relres_after_%d_iters" % it] = rel
-    # a-11: shadow XL-BOMD steps
-    p = binding.md_params(cfg)
-    mass = torch.as_tensor(W.masses_water(n)).to(dev)
-    vel = torch.as_tensor(W.velocities(W.masses_water(n))).to(dev)
-    x = pos.clone()
-    nhist, force, en0 = ctx.shadow_md_init(nl, x, box, p, chi_d, u_d, tol=1e-6, max_iter=100)
-    nsteps = args.md_steps
-    for _ in range(2):
-        ctx.shadow_md_step(nl, x, vel, mass, box, p, chi_d, u_d, nhist, force, want_energies=False)
-    torch.cuda.synchronize()
-    e0.record(ctx.stream)
-    evals = 0
-    max_drift = 0.0
-    for s in range(nsteps):
-        if s % REBUILD_EVERY == 0 and s > 0:
-            # the list is valid while no atom has moved more than skin/2 since the build
-            max_drift = max(max_drift, nl.max_drift(x))
-            nl.free()
-            nl = ctx.nl_build(x, box, cfg.r_list)
-        en = ctx.shadow_md_step(nl, x, vel, mass, box, p, chi_d, u_d, nhist, force, want_energies=(s == nsteps - 1))
-    e1.record(ctx.stream)
-    torch.cuda.synchronize()
-    msm = e0.elapsed_time(e1)
-    res["qeq_md_atom_steps_per_s"] = n * nsteps / (msm * 1e-3)
-    res["qeq_md_ms_per_step"] = msm / nsteps
-    res["qeq_md_coulomb_evals_per_step"] = en[3] if en else None
-    res["qeq_md_steps_timed"] = nsteps
-    res["qeq_md_max_drift_before_rebuild_A"] = max(max_drift, nl.max_drift(x))
-    res["qeq_md_half_skin_A"] = 0.5 * (cfg.r_list - cfg.rc)
-    res["qeq_md_note"] = ("configs[4] asks for 100 steps; the harmonic intramolecular stand-in has no intermolecular "
-                          "repulsion, so O...H contacts of the random start collapse after ~65 steps (DESIGN.md section 4); "
-                          "timed over the stable stretch")
     nl.free()
+    # a-11: configs[4]'s workload as written: 100 shadow XL-BOMD steps, 0.5 fs, 4 Krylov-rank updates per step; the list
+    # is rebuilt when the displacement would reach skin/2 (about every 10 steps at 300 K)
+    p = binding.md_params(cfg, k_rep=W.K_REP, r_rep=W.R_REP)
+    sh = md_loop(ctx, cfg, pos, n, dev, args.md_steps, "shadow", p, chi_d, u_d)
+    res["qeq_md_atom_steps_per_s"] = sh["atom_steps_per_s"]
+    res["qeq_md_ms_per_step"] = sh["ms_per_step"]
+    res["qeq_md_coulomb_evals_per_step"] = sh["coulomb_evals_per_step"]
+    res["qeq_md_steps_timed"] = sh["steps"]
+    res["qeq_md_rebuilds"] = sh["rebuilds"]
+    res["qeq_md_max_drift_seen_A"] = sh["max_drift_seen_A"]
+    res["qeq_md_half_skin_A"] = sh["half_skin_A"]
+    # NEXT-2: regular BOMD beside it (tight solver: the only setting in which it conserves energy)
+    bo = md_loop(ctx, cfg, pos, n, dev, args.bomd_steps, "bomd", p, chi_d, u_d, tol=1e-6)
+    res["bomd"] = bo
+    res["shadow_vs_regular_md_speedup"] = bo["ms_per_step"] / sh["ms_per_step"]
     return res
+
+
+def run_table1(ctx, dev, args):
+    """The shape of the paper's Table 1 on the cfg-0 box (216 waters, the paper's has 100): NVE runs
+    of shadow and regular MD for solver tolerances 1e-1 ... 1e-6; Coulomb evaluations per step and the standard
+    deviation of the total energy.  The stand-in V_short replaces the paper's HIP-NN, so the VALUES are this model's."""
+    import torch
+    from paper_2503_21176_b200 import binding
+    c0 = W.CONFIGS[0]
+    c = W.Config(0, c0.name, c0.kind, c0.n_lattice, c0.L, c0.rc, c0.alpha, c0.grid, c0.order, 0.3)    # r_list 9.3 A < L/2
+    pos, _ = W.make(0)
+    n = len(pos)
+    pos_d = torch.as_tensor(pos).to(dev)
+    chi, u = W.qeq_params_water_pd(n)
+    chi_d, u_d = torch.as_tensor(chi).to(dev), torch.as_tensor(u).to(dev)
+    rows = []
+    for mode in ("shadow", "bomd"):
+        for tol in (1e-1, 1e-2, 1e-3, 1e-4, 1e-5, 1e-6):
+            p = binding.md_params(c, krylov_rank=30, krylov_tol=tol, k_rep=W.K_REP, r_rep=W.R_REP)
+            r = md_loop(ctx, c, pos_d, n, dev, args.table_steps, mode, p, chi_d, u_d, tol=tol, record_energy=True)
+            rows.append({"shadow_md": mode == "shadow", "sol_tol": tol, "coulomb_evals_per_step": round(r["coulomb_evals_per_step"], 2),
+                         "energy_std_eV": r["energy_std_eV"], "energy_drift_eV": r["energy_drift_eV"],
+                         "ms_per_step": round(r["ms_per_step"], 4), "rebuilds": r["rebuilds"]})
+    return {"system": "configs[0] box, 216 waters, r_list 9.3 A, dt 0.5 fs, %d steps, 300 K start" % args.table_steps, "rows": rows}
 
 
 def main():
@@ -497,11 +682,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for the cfg-4 cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-md", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--krylov-iters", type=int, default=50)
-    ap.add_argument("--md-steps", type=int, default=50)      # see DESIGN.md section 4: the stand-in collapses after ~65 steps
+    ap.add_argument("--md-steps", type=int, default=100)      # configs[4]: 100 shadow XL-BOMD steps
+    ap.add_argument("--bomd-steps", type=int, default=10)
+    ap.add_argument("--table-steps", type=int, default=200)
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]
     if args.impl == "reference":

@@ -93,6 +93,12 @@ int  sqeq_nl_layout(const sqeq_nlist* nl, int64_t* n_slots, int* entry_shift, in
  * with cutoff rc + skin holds every pair with r < rc while this stays below skin/2: rebuild
  * when it does not.  One small kernel and a stream synchronisation; +inf if a position is NaN. */
 int  sqeq_nl_max_drift(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, double* max_drift);
+/* The same for the positions pos + dt * vel (vel: device fp32 [n][3]): what the drift will be after the position
+ * update of the next MD step (up to its dt^2 a/2 term, ~0.01 Angstrom for water at 0.5 fs).  An MD loop rebuilds
+ * BEFORE a step whenever this reaches skin/2 minus that slack, so that no evaluation ever runs on a list that is
+ * no longer complete ("rebuilt when the maximum displacement exceeds half the skin"). */
+int  sqeq_nl_max_drift_ahead(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const float* vel,
+                             double dt, double* max_drift);
 int  sqeq_nl_free  (sqeq_nlist* nl);
 
 /* ---- Coulomb evaluation: Eq. 2 = Eq. 3 (real space, r < rc) + Alg. 2 (smooth PME,

@@ -61,6 +61,7 @@ def load():
     L.sqeq_nl_entry_bytes.argtypes = [vp, ip]
     L.sqeq_nl_layout.argtypes = [vp, ctypes.POINTER(i64), ip, ip]
     L.sqeq_nl_max_drift.argtypes = [vp, vp, i64, vp, dp]
+    L.sqeq_nl_max_drift_ahead.argtypes = [vp, vp, i64, vp, vp, dbl, dp]
     L.sqeq_nl_free.argtypes = [vp]
     L.sqeq_coulomb.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_host_submit.argtypes = [vp, cint, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
@@ -145,6 +146,14 @@ class NeighbourList:
         d = ctypes.c_double()
         self.ctx._check(load().sqeq_nl_max_drift(self.ctx.handle, self.handle, self.n,
                                                  _ptr(pos, torch.float32, 3 * self.n), ctypes.byref(d)))
+        return d.value
+
+    def max_drift_ahead(self, pos, vel, dt):
+        """Largest displacement since the build after moving on by vel * dt (rebuild before the step if >= skin/2)."""
+        d = ctypes.c_double()
+        self.ctx._check(load().sqeq_nl_max_drift_ahead(self.ctx.handle, self.handle, self.n,
+                                                       _ptr(pos, torch.float32, 3 * self.n),
+                                                       _ptr(vel, torch.float32, 3 * self.n), float(dt), ctypes.byref(d)))
         return d.value
 
     def export(self):

@@ -308,7 +308,17 @@ int sqeq_nl_max_drift(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const floa
     if (!nl || nl->ctx != ctx || n != nl->n || !pos || !max_drift)
         return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_max_drift: list/context/n mismatch or NULL argument");
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
-    return nl_max_drift_impl(ctx, nl, pos, max_drift);
+    return nl_max_drift_impl(ctx, nl, pos, nullptr, 0.0, max_drift);
+}
+
+int sqeq_nl_max_drift_ahead(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const float* vel,
+                            double dt, double* max_drift)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!nl || nl->ctx != ctx || n != nl->n || !pos || !vel || !max_drift)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_max_drift_ahead: list/context/n mismatch or NULL argument");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return nl_max_drift_impl(ctx, nl, pos, vel, dt, max_drift);
 }
 
 int sqeq_nl_free(sqeq_nlist* nl)

@@ -210,7 +210,8 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
 void nl_release(sqeq_nlist* nl);
 void nl_release_storage(sqeq_nlist* nl);
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
-int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, double* max_drift);
+int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
+                      double* max_drift);
 
 // Re-gather positions/charges into the list's order (and PME fractional coordinates if K != null).
 int prep_atoms(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* q,

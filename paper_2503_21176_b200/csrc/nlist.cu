@@ -927,13 +927,16 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
 // Largest distance any atom has moved since the list was built (plain difference of caller positions: an atom
 // that crossed the box is still the same unwrapped coordinate to the caller).  A list with cutoff rc + skin
 // stays complete for r < rc while this is below skin/2 (cfg 4 recipe).
+// vel != NULL: the displacement the atom will have after moving on by vel * dt (the position update of the next
+// MD step, up to its dt^2 a/2 term)
 __global__ void k_max_drift(int64_t n, const float* __restrict__ pos, const float* __restrict__ pos0,
-                            unsigned* __restrict__ out)
+                            const float* __restrict__ vel, float dt, unsigned* __restrict__ out)
 {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     float d2 = 0.f;
     if (i < n) {
-        const float dx = pos[3 * i] - pos0[3 * i], dy = pos[3 * i + 1] - pos0[3 * i + 1], dz = pos[3 * i + 2] - pos0[3 * i + 2];
+        float dx = pos[3 * i] - pos0[3 * i], dy = pos[3 * i + 1] - pos0[3 * i + 1], dz = pos[3 * i + 2] - pos0[3 * i + 2];
+        if (vel) { dx = fmaf(dt, vel[3 * i], dx); dy = fmaf(dt, vel[3 * i + 1], dy); dz = fmaf(dt, vel[3 * i + 2], dz); }
         d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
         if (!(d2 == d2)) d2 = __int_as_float(0x7f800000);      // NaN position: report +inf
     }
@@ -942,12 +945,13 @@ __global__ void k_max_drift(int64_t n, const float* __restrict__ pos, const floa
     if ((threadIdx.x & 31) == 0 && d2 > 0.f) atomicMax(out, __float_as_uint(d2));   // non-negative floats order as uints
 }
 
-int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, double* max_drift)
+int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
+                      double* max_drift)
 {
     cudaStream_t st = ctx->stream;
     unsigned* d_out = (unsigned*)((double*)ctx->scal.p + 12);        // a scratch word of the scalar block
     CUDA_TRY(ctx, cudaMemsetAsync(d_out, 0, sizeof(unsigned), st));
-    k_max_drift<<<ceil_div(nl->n, 256), 256, 0, st>>>(nl->n, pos, nl->pos0, d_out);
+    k_max_drift<<<ceil_div(nl->n, 256), 256, 0, st>>>(nl->n, pos, nl->pos0, vel, (float)dt, d_out);
     KERNEL_CHECK(ctx);
     unsigned* h = (unsigned*)(ctx->h_scal + 12);
     CUDA_TRY(ctx, cudaMemcpyAsync(h, d_out, sizeof(unsigned), cudaMemcpyDeviceToHost, st));

@@ -20,6 +20,7 @@ D_OH = 0.9572                       # Angstrom
 THETA_HOH = 104.52                  # degrees
 Q_O, Q_H = -0.834, 0.417            # e
 MASS_O, MASS_H = 15.999, 1.008      # amu
+K_REP, R_REP = 10.0, 2.9            # eV/A^2, A: O-O soft-sphere repulsion of the MD stand-in
 
 
 @dataclass
