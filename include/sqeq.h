@@ -250,6 +250,19 @@ int  sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* 
                          const float* chi, const float* u, double* nhist, float* force,
                          double* energies);
 
+/* nsteps shadow-MD steps in one call, the neighbour list kept valid by the library: it is rebuilt (cutoff
+ * list_cutoff = rc + skin, which must be the cutoff of *nl_io) before a step whenever the largest displacement since
+ * the build would reach skin/2 - slack, judged WITHOUT waiting for the GPU each step: the test looks
+ * two steps ahead from a number the device reduced two steps ago (the first steps after a build are checked
+ * synchronously).  slack (Angstrom) covers the 2 dt^2 a of that extrapolation: 0.05 for water at 0.5 fs.
+ * *nl_io: in, a list built for the current positions; out, the list in use at the end (the caller frees it; lists
+ * replaced on the way are freed by the call).  stats: host double[8] out = {U, kinetic energy, |q[n]-n|, Coulomb
+ * evaluations of the last step, rebuilds, largest look-ahead displacement accepted, displacement at the end,
+ * skin/2}; may be NULL.  Synchronises at the end (and at every rebuild). */
+int  sqeq_shadow_md_run(sqeq_ctx* ctx, sqeq_nlist** nl_io, int64_t n, float* pos, float* vel, const float* mass,
+                        const double box[3], const sqeq_md_params* p, const float* chi, const float* u,
+                        double* nhist, float* force, int nsteps, double list_cutoff, double slack, double* stats);
+
 /* ---- regular Born-Oppenheimer MD: PAPER.md:155-200 (Eqs. 13-19), the method shadow MD is compared with
  * (Table 1, 321-323) -------------------------------------------------------------------
  * Every step solves Eq. 18 for q_min by GMRES to the relative residual `tol` (at most max_iter Coulomb
@@ -289,6 +302,17 @@ enum {
 int  sqeq_profile_enable(sqeq_ctx* ctx, int on);
 int  sqeq_profile_reset (sqeq_ctx* ctx);
 int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* launches);
+/* Switches (also read from the environment by sqeq_create, as SQEQ_<NAME IN CAPITALS>=0/1):
+ *   "graphs"           1  replay launch-bound sequences (sqeq_coulomb_fixed on a cached geometry, the steps of
+ *                         sqeq_shadow_md_run) as CUDA graphs; needs a context stream other than the legacy default
+ *   "overlap"          0  PME on an internal side stream beside a persistent real-space grid
+ *   "real_lean_blocks" 2  blocks per SM of that persistent grid
+ *   "pme_tiles"        1  shared-memory tiles for spreading and gathering (0: global-memory kernels)
+ *   "spread_float"     0  fp32 compare-and-swap accumulation in the spreading tile instead of fixed point
+ *   "real_staged"      1  16-bit list + shared-memory-staged real-space kernel (0: 32-bit list, global gather;
+ *                         takes effect at the next sqeq_nl_build)
+ * Synchronises the stream.  SQEQ_EINVAL for an unknown name. */
+int  sqeq_set_option(sqeq_ctx* ctx, const char* name, int value);
 /* Number of the library's own kernel launches (cuFFT's excluded) since sqeq_create / last reset. */
 int  sqeq_launch_count  (sqeq_ctx* ctx, int64_t* launches, int reset);
 

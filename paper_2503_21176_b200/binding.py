@@ -85,9 +85,12 @@ def load():
                                       vp, vp, dp]
     L.sqeq_shadow_md_step.argtypes = [vp, vp, i64, vp, vp, vp, dp, ctypes.POINTER(MdParams), vp, vp,
                                       vp, vp, dp]
+    L.sqeq_shadow_md_run.argtypes = [vp, ctypes.POINTER(vp), i64, vp, vp, vp, dp, ctypes.POINTER(MdParams), vp, vp,
+                                     vp, vp, cint, dbl, dbl, dp]
     L.sqeq_profile_enable.argtypes = [vp, cint]
     L.sqeq_profile_reset.argtypes = [vp]
     L.sqeq_profile_read.argtypes = [vp, cint, dp, ctypes.POINTER(i64)]
+    L.sqeq_set_option.argtypes = [vp, ctypes.c_char_p, cint]
     L.sqeq_launch_count.argtypes = [vp, ctypes.POINTER(i64), cint]
     _lib = L
     return L
@@ -398,6 +401,23 @@ class Context:
                                                en if want_energies else None))
         return list(en) if want_energies else None
 
+    def shadow_md_run(self, nl, pos, vel, mass, box, params, chi, u, nhist, force, nsteps, slack=0.05):
+        """sqeq_shadow_md_run: nsteps steps, the list rebuilt by the library when the drift would reach skin/2 - slack.
+        `nl` is updated in place (its handle may be replaced).  Returns the stats dict."""
+        n = pos.shape[0]
+        st = (ctypes.c_double * 8)()
+        h = ctypes.c_void_p(nl.handle.value)
+        try:
+            self._check(load().sqeq_shadow_md_run(self.handle, ctypes.byref(h), n, _ptr(pos, torch.float32, 3 * n),
+                                                  _ptr(vel, torch.float32, 3 * n), _ptr(mass, torch.float32, n), _box(box),
+                                                  ctypes.byref(params), _ptr(chi, torch.float32, n), _ptr(u, torch.float32, n),
+                                                  ctypes.c_void_p(nhist.data_ptr()), _ptr(force, torch.float32, 3 * n),
+                                                  int(nsteps), float(nl.cutoff), float(slack), st))
+        finally:
+            nl.handle = h
+        keys = ["U", "ekin", "resnorm", "evals_last_step", "rebuilds", "max_ahead_accepted", "drift_end", "half_skin"]
+        return dict(zip(keys, list(st)))
+
     # ---- timing
     def profile_enable(self, on=True):
         self._check(load().sqeq_profile_enable(self.handle, int(on)))
@@ -412,6 +432,9 @@ class Context:
             self._check(load().sqeq_profile_read(self.handle, k, ctypes.byref(ms), ctypes.byref(cnt)))
             out[name] = (ms.value, cnt.value)
         return out
+
+    def set_option(self, name, value):
+        self._check(load().sqeq_set_option(self.handle, name.encode(), int(value)))
 
     def launch_count(self, reset=False):
         c = ctypes.c_int64()

@@ -39,6 +39,45 @@ int sqeq_reserve(sqeq_ctx* ctx, DevBuf& b, size_t bytes)
     return SQEQ_OK;
 }
 
+int graph_run(sqeq_ctx* ctx, int slot, uint64_t key, const std::function<int()>& body)
+{
+    cudaStream_t st = ctx->stream;
+    if (!ctx->graphs || ctx->profiling || st == nullptr || st == cudaStreamLegacy) return body();
+    auto& g = ctx->gslot[slot];
+    if (!(g.exec && g.key == key)) {
+        const int64_t l0 = ctx->launches;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+            cudaGetLastError();
+            return body();
+        }
+        const int r = body();
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(st, &graph);
+        const int64_t nl = ctx->launches - l0;
+        ctx->launches = l0;
+        if (r != SQEQ_OK || e != cudaSuccess || !graph) {
+            cudaGetLastError();
+            if (graph) cudaGraphDestroy(graph);
+            if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+            return body();                      // plain run; it also brings workspaces to size for the next capture
+        }
+        bool ok = false;
+        if (g.exec) {
+            cudaGraphExecUpdateResultInfo info;
+            ok = cudaGraphExecUpdate(g.exec, graph, &info) == cudaSuccess;
+            if (!ok) { cudaGetLastError(); cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+        }
+        if (!ok) ok = cudaGraphInstantiate(&g.exec, graph, 0) == cudaSuccess;
+        cudaGraphDestroy(graph);
+        if (!ok) { cudaGetLastError(); g.exec = nullptr; return body(); }
+        g.key = key;
+        g.nlaunch = nl;
+    }
+    CUDA_TRY(ctx, cudaGraphLaunch(g.exec, st));
+    ctx->launches += g.nlaunch;
+    return SQEQ_OK;
+}
+
 StageTimer::StageTimer(sqeq_ctx* c, int stage, cudaStream_t s) : ctx(c), st(s ? s : c->stream)
 {
     if (!ctx->profiling) return;
@@ -123,6 +162,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->real_lean_blocks = env && atoi(env) > 0 ? atoi(env) : 2;
     env = getenv("SQEQ_REAL_STAGED");
     ctx->real_staged_off = env && env[0] == '0';
+    env = getenv("SQEQ_GRAPHS");
+    ctx->graphs = !(env && env[0] == '0');
     *out = ctx;
     return SQEQ_OK;
 }
@@ -158,6 +199,10 @@ int sqeq_destroy(sqeq_ctx* ctx)
     if (ctx->h_nl) cudaFreeHost(ctx->h_nl);
     if (ctx->h_kry) cudaFreeHost(ctx->h_kry);
     if (ctx->h_slot_e) cudaFreeHost(ctx->h_slot_e);
+    if (ctx->h_ring) cudaFreeHost(ctx->h_ring);
+    if (ctx->d_ring) cudaFree(ctx->d_ring);
+    for (auto& e : ctx->ring_ev) if (e) cudaEventDestroy(e);
+    for (auto& g : ctx->gslot) if (g.exec) cudaGraphExecDestroy(g.exec);
     for (int k = 0; k < 2; ++k) {
         if (ctx->slot_in[k]) cudaEventDestroy(ctx->slot_in[k]);
         if (ctx->slot_done[k]) cudaEventDestroy(ctx->slot_done[k]);
@@ -220,6 +265,21 @@ int sqeq_profile_read(sqeq_ctx* ctx, int stage, double* total_ms, int64_t* launc
     SQEQ_TRY(drain_timers(ctx));
     if (total_ms) *total_ms = ctx->t_total[stage];
     if (launches) *launches = ctx->t_count[stage];
+    return SQEQ_OK;
+}
+
+int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
+{
+    if (!ctx || !name) return SQEQ_EINVAL;
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    if (!strcmp(name, "graphs")) ctx->graphs = value != 0;
+    else if (!strcmp(name, "overlap")) ctx->overlap = value != 0;
+    else if (!strcmp(name, "pme_tiles")) { ctx->pme_tiles_off = value == 0; ctx->tile_plan.valid = false; }
+    else if (!strcmp(name, "spread_float")) ctx->spread_float = value != 0;
+    else if (!strcmp(name, "real_staged")) ctx->real_staged_off = value == 0;
+    else if (!strcmp(name, "real_lean_blocks")) { if (value < 1) return sqeq_fail(ctx, SQEQ_EINVAL, "real_lean_blocks must be >= 1"); ctx->real_lean_blocks = value; }
+    else return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_set_option: unknown option '%s'", name);
+    for (auto& g : ctx->gslot) if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
     return SQEQ_OK;
 }
 
@@ -429,9 +489,22 @@ extern "C" int sqeq_coulomb_fixed(sqeq_ctx* ctx, int64_t n, const float* q, floa
     if (n != ctx->fixed.n || !q || (!phi && !force))
         return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_fixed: n differs from the geometry, q is NULL, or no output asked for");
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
-    SQEQ_TRY(prep_charges(ctx, nl, q, nullptr, ctx->stream));
-    SQEQ_TRY(coulomb_eval(ctx, nl, n, ctx->fixed.box, ctx->fixed.rc, ctx->fixed.alpha, phi, force, want_energy != 0, false,
-                          GEOM_FIXED));
+    auto body = [&]() -> int {
+        SQEQ_TRY(prep_charges(ctx, nl, q, nullptr, ctx->stream));
+        return coulomb_eval(ctx, nl, n, ctx->fixed.box, ctx->fixed.rc, ctx->fixed.alpha, phi, force, want_energy != 0, false,
+                            GEOM_FIXED);
+    };
+    // once the geometry cache exists every evaluation is the same sequence of launches: replay it as a CUDA graph
+    // (the launch-latency regime of small systems: 648 atoms are ~12 kernels of a few microseconds each)
+    const bool warm = ctx->gc.valid && ctx->gc.nl == nl && ctx->gc.serial == nl->serial && nl->fmt == 1;
+    if (warm) {
+        uint64_t key = hash_mix(0x51, ctx->geom_serial);
+        for (uint64_t v : {(uint64_t)(uintptr_t)q, (uint64_t)(uintptr_t)phi, (uint64_t)(uintptr_t)force, (uint64_t)(want_energy != 0)})
+            key = hash_mix(key, v);
+        SQEQ_TRY(graph_run(ctx, 0, key, body));
+    } else {
+        SQEQ_TRY(body());
+    }
     ctx->energy_pending = want_energy != 0;
     return SQEQ_OK;
 }

@@ -93,6 +93,8 @@ struct sqeq_ctx {
     DevBuf vec_d[6];  // double [n] scratch
     DevBuf vec_f3[2]; // float  [n][3] scratch forces
     GeomCache gc;
+    struct { bool valid = false, tiles = false; int order = 0, nt = 0, K[3] = {0, 0, 0}, nc[3] = {0, 0, 0}; size_t bytes = 0;
+             alignas(8) unsigned char blob[128]; } tile_plan;     // cached TileGeom of the PME tile kernels (pme.cu)
     // sqeq_geometry_set / sqeq_coulomb_fixed session
     uint64_t geom_serial = 0;             // counts prep_atoms calls: which positions xq/frac/base hold
     struct { const sqeq_nlist* nl = nullptr; uint64_t serial = 0, geom_serial = 0; int64_t n = 0; double box[3] = {0, 0, 0}; double rc = 0, alpha = 0; } fixed;
@@ -105,6 +107,10 @@ struct sqeq_ctx {
     bool slot_busy[2] = {false, false};
     bool slot_energy[2] = {false, false};
     double* h_slot_e = nullptr;           // pinned [2]
+    // sqeq_shadow_md_run: ring of lagged drift checks (device words, pinned mirror, one event each)
+    unsigned* d_ring = nullptr;
+    unsigned* h_ring = nullptr;
+    cudaEvent_t ring_ev[4] = {nullptr, nullptr, nullptr, nullptr};
 
     // ---- timing ----
     bool profiling = false;
@@ -113,6 +119,10 @@ struct sqeq_ctx {
     double t_total[SQEQ_T_COUNT] = {0};
     int64_t t_count[SQEQ_T_COUNT] = {0};
     int64_t launches = 0;
+
+    // CUDA graphs of launch-bound sequences (sqeq_coulomb_fixed, the shadow-MD step): slot 0 / 1
+    struct GraphSlot { uint64_t key = 0; cudaGraphExec_t exec = nullptr; int64_t nlaunch = 0; } gslot[2];
+    bool graphs = true;                   // SQEQ_GRAPHS=0 / sqeq_set_option("graphs", 0): always launch kernel by kernel
 
     // live neighbour lists of this context: sqeq_destroy releases their device storage and detaches them, so a
     // handle freed after its context is only deleted (no use of a dead stream or pool)
@@ -148,6 +158,12 @@ struct sqeq_nlist {
 
 // ---------------------------------------------------------------------------------------------
 int sqeq_fail(sqeq_ctx* ctx, int code, const char* fmt, ...);
+// Runs `body` (a sequence of launches on ctx->stream with no synchronisation) through a CUDA graph kept in slot
+// `slot`: replayed when `key` is unchanged, re-captured (and the executable graph updated in place) when it is not.
+// Falls back to running body() directly when graphs are off, stage timing is on, the stream cannot be captured
+// (legacy default stream) or the capture fails (e.g. a workspace had to grow: the next call captures).
+int graph_run(sqeq_ctx* ctx, int slot, uint64_t key, const std::function<int()>& body);
+static inline uint64_t hash_mix(uint64_t h, uint64_t v) { h ^= v + 0x9e3779b97f4a7c15ull + (h << 6) + (h >> 2); return h; }
 int sqeq_reserve(sqeq_ctx* ctx, DevBuf& b, size_t bytes);
 
 #define CUDA_TRY(ctx, expr)                                                              \
@@ -210,6 +226,8 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
 void nl_release(sqeq_nlist* nl);
 void nl_release_storage(sqeq_nlist* nl);
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
+int nl_max_drift_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
+                         unsigned* d_out);
 int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
                       double* max_drift);
 

@@ -14,6 +14,7 @@
 //   n(t+dt) = 2 n(t) - n(t-dt) + dt^2 ndd(t) + alpha_diss sum_k c_k n(t-k dt).
 // All per-atom work runs in the kernels below; fp64 for n, q and every reduction.
 #include <math.h>
+#include <string.h>
 
 #include "common.cuh"
 
@@ -417,16 +418,11 @@ extern "C" int sqeq_shadow_md_init(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t 
     return md_read_energies(ctx, energies, evals + solve_iters);
 }
 
-extern "C" int sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* pos, float* vel,
-                                   const float* mass, const double box[3], const sqeq_md_params* p,
-                                   const float* chi, const float* u, double* nhist, float* force,
-                                   double* energies)
+// one step, enqueued: half kick + drift, n update, md_eval at the new time level, second half kick
+static int md_step_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* pos, float* vel, const float* mass,
+                           const double box[3], const sqeq_md_params* p, const float* chi, const float* u,
+                           double* nhist, float* force, int* evals)
 {
-    if (!ctx) return SQEQ_EINVAL;
-    SQEQ_TRY(check_md_args(ctx, nl, n, box, p, "sqeq_shadow_md_step"));
-    if (!pos || !vel || !mass || !chi || !u || !nhist || !force)
-        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_shadow_md_step: NULL argument");
-    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     const int nb = ceil_div(n, 256);
     {
@@ -439,14 +435,109 @@ extern "C" int sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t 
         k_md_n_update<<<nb, 256, 0, st>>>(n, nhist, k);
         KERNEL_CHECK(ctx);
     }
-    int evals = 0;
-    SQEQ_TRY(md_eval(ctx, nl, n, pos, box, p, chi, u, nhist, force, &evals));
+    SQEQ_TRY(md_eval(ctx, nl, n, pos, box, p, chi, u, nhist, force, evals));
     {
         StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
         k_md_kick<<<nb, 256, 0, st>>>(n, pos, vel, force, mass, p->dt, 0, (double*)ctx->scal.p + S_EKIN);
         KERNEL_CHECK(ctx);
     }
+    return SQEQ_OK;
+}
+
+extern "C" int sqeq_shadow_md_step(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, float* pos, float* vel,
+                                   const float* mass, const double box[3], const sqeq_md_params* p,
+                                   const float* chi, const float* u, double* nhist, float* force,
+                                   double* energies)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    SQEQ_TRY(check_md_args(ctx, nl, n, box, p, "sqeq_shadow_md_step"));
+    if (!pos || !vel || !mass || !chi || !u || !nhist || !force)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_shadow_md_step: NULL argument");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    int evals = 0;
+    SQEQ_TRY(md_step_enqueue(ctx, nl, n, pos, vel, mass, box, p, chi, u, nhist, force, &evals));
     return md_read_energies(ctx, energies, evals);
+}
+
+// nsteps steps with the neighbour list kept valid by the library (rebuilt when the largest displacement
+// since the build exceeds half the skin).  The host must not wait for the GPU every step, so the test runs two steps
+// behind: after step s the displacement the atoms will have two position updates later, |x + 2 dt v - x0|, is
+// reduced on the device and copied to pinned memory; before step s + 2 the host looks at that number (the GPU is
+// long past it) and rebuilds if it reaches skin/2 - slack (slack covers the 2 dt^2 a the extrapolation leaves out).
+// The first two steps after a (re)build, for which no such number exists yet, are checked synchronously.
+extern "C" int sqeq_shadow_md_run(sqeq_ctx* ctx, sqeq_nlist** nl_io, int64_t n, float* pos, float* vel,
+                                  const float* mass, const double box[3], const sqeq_md_params* p, const float* chi,
+                                  const float* u, double* nhist, float* force, int nsteps, double list_cutoff,
+                                  double slack, double* stats)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!nl_io || !*nl_io) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_shadow_md_run: needs a list built for the current positions");
+    SQEQ_TRY(check_md_args(ctx, *nl_io, n, box, p, "sqeq_shadow_md_run"));
+    if (!pos || !vel || !mass || !chi || !u || !nhist || !force || nsteps < 1)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_shadow_md_run: NULL argument or nsteps < 1");
+    const double half_skin = 0.5 * (list_cutoff - p->rc);
+    if (!(list_cutoff == (*nl_io)->cutoff) || !(slack >= 0.0) || !(half_skin - slack > 0.0))
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_shadow_md_run: list_cutoff must be the list's cutoff and skin/2 > slack >= 0");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    if (!ctx->d_ring) {
+        CUDA_TRY(ctx, cudaMalloc((void**)&ctx->d_ring, 4 * sizeof(unsigned)));
+        CUDA_TRY(ctx, cudaMallocHost((void**)&ctx->h_ring, 4 * sizeof(unsigned)));
+        for (auto& e : ctx->ring_ev) CUDA_TRY(ctx, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    uint64_t ring_serial[4] = {0, 0, 0, 0};
+    int rebuilds = 0, evals = 0;
+    double worst_ahead = 0.0;
+    auto rebuild = [&]() -> int {
+        sqeq_nlist* fresh = nullptr;
+        SQEQ_TRY(nl_build_impl(ctx, n, pos, box, list_cutoff, &fresh));
+        nl_release(*nl_io);
+        *nl_io = fresh;
+        ++rebuilds;
+        return SQEQ_OK;
+    };
+    for (int s = 0; s < nsteps; ++s) {
+        sqeq_nlist* nl = *nl_io;
+        double ahead = -1.0;
+        if (s >= 2 && ring_serial[(s - 2) & 3] == nl->serial) {
+            CUDA_TRY(ctx, cudaEventSynchronize(ctx->ring_ev[(s - 2) & 3]));
+            float d2;
+            memcpy(&d2, &ctx->h_ring[(s - 2) & 3], sizeof(float));
+            ahead = sqrt((double)d2);
+        } else {
+            SQEQ_TRY(nl_max_drift_impl(ctx, nl, pos, vel, p->dt, &ahead));      // synchronous, one update ahead
+        }
+        if (ahead > worst_ahead && ahead < half_skin - slack) worst_ahead = ahead;
+        if (!(ahead < half_skin - slack)) SQEQ_TRY(rebuild());
+        nl = *nl_io;
+        {
+            // every step on one list is the same ~120 launches: a CUDA graph, re-captured (and updated in place)
+            // after a rebuild
+            uint64_t key = hash_mix(0x3d, nl->serial);
+            for (uint64_t v : {(uint64_t)(uintptr_t)pos, (uint64_t)(uintptr_t)vel, (uint64_t)(uintptr_t)mass, (uint64_t)(uintptr_t)chi,
+                               (uint64_t)(uintptr_t)u, (uint64_t)(uintptr_t)nhist, (uint64_t)(uintptr_t)force, (uint64_t)n})
+                key = hash_mix(key, v);
+            const unsigned char* pb = (const unsigned char*)p;
+            for (size_t k = 0; k < sizeof(sqeq_md_params); ++k) key = hash_mix(key, pb[k]);
+            SQEQ_TRY(graph_run(ctx, 1, key, [&]() { return md_step_enqueue(ctx, nl, n, pos, vel, mass, box, p, chi, u, nhist, force, &evals); }));
+            ctx->gc.valid = false;          // replays move the atoms without passing through prep_atoms on the host
+            ctx->geom_serial++;
+        }
+        unsigned* d = ctx->d_ring + (s & 3);
+        SQEQ_TRY(nl_max_drift_enqueue(ctx, nl, pos, vel, 2.0 * p->dt, d));
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_ring + (s & 3), d, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaEventRecord(ctx->ring_ev[s & 3], st));
+        ring_serial[s & 3] = nl->serial;
+    }
+    double en[4] = {0, 0, 0, 0};
+    SQEQ_TRY(md_read_energies(ctx, en, evals));
+    double drift_now = 0.0;
+    SQEQ_TRY(nl_max_drift_impl(ctx, *nl_io, pos, nullptr, 0.0, &drift_now));
+    if (stats) {
+        stats[0] = en[0]; stats[1] = en[1]; stats[2] = en[2]; stats[3] = en[3];
+        stats[4] = (double)rebuilds; stats[5] = worst_ahead; stats[6] = drift_now; stats[7] = half_skin;
+    }
+    return SQEQ_OK;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -945,6 +945,17 @@ __global__ void k_max_drift(int64_t n, const float* __restrict__ pos, const floa
     if ((threadIdx.x & 31) == 0 && d2 > 0.f) atomicMax(out, __float_as_uint(d2));   // non-negative floats order as uints
 }
 
+// enqueue only: *d_out (device word, zeroed here) <- bits of the largest squared displacement
+int nl_max_drift_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
+                         unsigned* d_out)
+{
+    cudaStream_t st = ctx->stream;
+    CUDA_TRY(ctx, cudaMemsetAsync(d_out, 0, sizeof(unsigned), st));
+    k_max_drift<<<ceil_div(nl->n, 256), 256, 0, st>>>(nl->n, pos, nl->pos0, vel, (float)dt, d_out);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
 int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
                       double* max_drift)
 {

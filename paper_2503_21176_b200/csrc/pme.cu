@@ -749,10 +749,28 @@ template <int P>
 static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,
                      bool want_energy, cudaStream_t st)
 {
+    // the tile plan depends only on (cells of the list, grid, order): searched once, then reused
+    static_assert(sizeof(TileGeom) <= sizeof(ctx->tile_plan.blob), "tile plan cache too small");
     TileGeom tg;
     size_t tile_bytes = 0;
     int nt = 256;
-    const bool tiles = plan_tiles(ctx, nl, P, tg, tile_bytes, nt);
+    bool tiles;
+    {
+        auto& tp = ctx->tile_plan;
+        const bool same = tp.valid && nl && tp.order == P && tp.K[0] == ctx->K[0] && tp.K[1] == ctx->K[1] && tp.K[2] == ctx->K[2] &&
+                          tp.nc[0] == nl->ncell[0] && tp.nc[1] == nl->ncell[1] && tp.nc[2] == nl->ncell[2];
+        if (same) {
+            memcpy(&tg, tp.blob, sizeof(TileGeom));
+            tile_bytes = tp.bytes; nt = tp.nt; tiles = tp.tiles;
+        } else {
+            tiles = plan_tiles(ctx, nl, P, tg, tile_bytes, nt);
+            if (nl) {
+                memcpy(tp.blob, &tg, sizeof(TileGeom));
+                tp.bytes = tile_bytes; tp.nt = nt; tp.tiles = tiles; tp.order = P; tp.valid = true;
+                for (int d = 0; d < 3; ++d) { tp.K[d] = ctx->K[d]; tp.nc[d] = nl->ncell[d]; }
+            }
+        }
+    }
     const int ngroups = tiles ? tg.ng[0] * tg.ng[1] * tg.ng[2] : 0;
     const int K0 = ctx->K[0], K1 = ctx->K[1], K2 = ctx->K[2], K2h = K2 / 2 + 1;
     const size_t G3 = (size_t)K0 * K1 * K2;

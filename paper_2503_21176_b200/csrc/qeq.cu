@@ -161,6 +161,129 @@ __global__ void k_f2d(int64_t n, const float* __restrict__ x, double* __restrict
 // Generic GMRES on device fp64 vectors of length `len` (leading dimension ld).  Zero initial guess.
 //   apply(v, w): w = A v        load_rhs(w): w = b
 // On return x (ctx->kry_w + ld) holds the iterate.  Host side: Givens-rotated Hessenberg.
+// Least-squares problem of a finished GMRES cycle, on the device (one thread: m <= 64 columns of a few numbers):
+// Hessenberg columns from the CGS2 coefficients of each iteration (hcols[j]: first pass [m+2], second pass [m+2],
+// |w|^2), Givens rotations, back substitution.  y[0..m) <- the combination coefficients (0 beyond an exact
+// breakdown), *relres <- the residual estimate |g_k| / |b|.  scratch: (m+1) m + 3 m + 1 doubles.
+__global__ void k_gmres_lsq(int m, const double* __restrict__ hcols, const double* __restrict__ bn2,
+                            double* __restrict__ scratch, double* __restrict__ y, double* __restrict__ relres)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int HL = 2 * (m + 2) + 1;
+    double* H = scratch;
+    double* cs = H + (size_t)(m + 1) * m;
+    double* sn = cs + m;
+    double* g = sn + m;
+    const double bnorm = sqrt(*bn2);
+    for (int k = 0; k <= m; ++k) g[k] = 0.0;
+    g[0] = bnorm;
+    int kd = m;
+    for (int j = 0; j < m; ++j) {
+        const double* hc = hcols + (size_t)j * HL;
+        double* Hj = H + (size_t)j * (m + 1);
+        for (int k = 0; k <= j; ++k) Hj[k] = hc[k] + hc[(m + 2) + k];
+        Hj[j + 1] = sqrt(hc[2 * (m + 2)]);
+        for (int k = 0; k < j; ++k) {
+            const double t = cs[k] * Hj[k] + sn[k] * Hj[k + 1];
+            Hj[k + 1] = -sn[k] * Hj[k] + cs[k] * Hj[k + 1];
+            Hj[k] = t;
+        }
+        const double a = Hj[j], b = Hj[j + 1], rr = hypot(a, b);
+        cs[j] = rr > 0 ? a / rr : 1.0;
+        sn[j] = rr > 0 ? b / rr : 0.0;
+        Hj[j] = rr;
+        Hj[j + 1] = 0.0;
+        g[j + 1] = -sn[j] * g[j];
+        g[j] = cs[j] * g[j];
+        if (b == 0.0) { kd = j + 1; break; }
+    }
+    for (int i = 0; i < m; ++i) y[i] = 0.0;
+    for (int i = kd - 1; i >= 0; --i) {
+        double sacc = g[i];
+        for (int l = i + 1; l < kd; ++l) sacc -= H[(size_t)l * (m + 1) + i] * y[l];
+        const double d = H[(size_t)i * (m + 1) + i];
+        y[i] = d != 0.0 ? sacc / d : 0.0;
+    }
+    *relres = bnorm > 0.0 ? fabs(g[kd]) / bnorm : 0.0;
+}
+
+// m GMRES iterations from a zero initial guess with NO host synchronisation (the rank-m updates of Eq. 27, timed
+// Krylov loops): coefficients stay on the device, k_gmres_lsq solves the small problem there.  relres_host may be
+// NULL (then the call returns with everything merely enqueued -- a whole MD step can be captured in a CUDA graph).
+static int gmres_fixed_async(sqeq_ctx* ctx, int64_t len, const std::function<int(const double*, double*)>& apply,
+                             const std::function<int(double*)>& load_rhs, int m, double** x_out, double* relres_host,
+                             const double* dinv)
+{
+    cudaStream_t st = ctx->stream;
+    const int64_t ld = (len + 31) & ~(int64_t)31;
+    const size_t HL = (size_t)2 * (m + 2) + 1;
+    const size_t nh = HL * m + 1 + m + 1 + (size_t)(m + 1) * m + 3 * m + 1;
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_V, sizeof(double) * (size_t)ld * (m + 1)));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_w, sizeof(double) * (size_t)ld * 3));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_h, sizeof(double) * nh));
+    double* V = (double*)ctx->kry_V.p;
+    double* w = (double*)ctx->kry_w.p;
+    double* x = w + ld;
+    double* z = w + 2 * ld;
+    double* hcols = (double*)ctx->kry_h.p;
+    double* bn2 = hcols + HL * m;
+    double* y = bn2 + 1;
+    double* relres = y + m;
+    double* scratch = relres + 1;
+    const int nbl = ceil_div(len, 256);
+    const int nchunk = ceil_div(len, DOT_CHUNK);
+    *x_out = x;
+    SQEQ_TRY(load_rhs(w));
+    {
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        CUDA_TRY(ctx, cudaMemsetAsync(hcols, 0, sizeof(double) * (HL * m + 1), st));       // all coefficients and |b|^2
+        CUDA_TRY(ctx, cudaMemsetAsync(x, 0, sizeof(double) * ld, st));
+        k_dots<<<dim3(nchunk, 1), 256, 0, st>>>(len, ld, w, w, bn2);
+        KERNEL_CHECK(ctx);
+        k_normalise<<<nbl, 256, 0, st>>>(len, w, bn2, V);
+        KERNEL_CHECK(ctx);
+    }
+    for (int j = 0; j < m; ++j) {
+        if (dinv) {
+            k_hadamard<<<nbl, 256, 0, st>>>(len, V + (int64_t)j * ld, dinv, z);
+            KERNEL_CHECK(ctx);
+            SQEQ_TRY(apply(z, w));
+        } else {
+            SQEQ_TRY(apply(V + (int64_t)j * ld, w));
+        }
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        double* h = hcols + HL * j;
+        double* h2 = h + (m + 2);
+        double* nrm2 = h2 + (m + 2);
+        k_dots<<<dim3(nchunk, j + 1), 256, 0, st>>>(len, ld, V, w, h);
+        KERNEL_CHECK(ctx);
+        k_sub_combo<<<nbl, 256, 0, st>>>(len, ld, j + 1, V, h, w);
+        KERNEL_CHECK(ctx);
+        k_dots<<<dim3(nchunk, j + 1), 256, 0, st>>>(len, ld, V, w, h2);
+        KERNEL_CHECK(ctx);
+        k_sub_combo<<<nbl, 256, 0, st>>>(len, ld, j + 1, V, h2, w);
+        KERNEL_CHECK(ctx);
+        k_dots<<<dim3(nchunk, 1), 256, 0, st>>>(len, ld, w, w, nrm2);
+        KERNEL_CHECK(ctx);
+        k_normalise<<<nbl, 256, 0, st>>>(len, w, nrm2, V + (int64_t)(j + 1) * ld);
+        KERNEL_CHECK(ctx);
+    }
+    {
+        StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
+        k_gmres_lsq<<<1, 32, 0, st>>>(m, hcols, bn2, scratch, y, relres);
+        KERNEL_CHECK(ctx);
+        if (dinv) k_add_combo_scaled<<<nbl, 256, 0, st>>>(len, ld, m, V, y, dinv, x);
+        else k_add_combo<<<nbl, 256, 0, st>>>(len, ld, m, V, y, x);
+        KERNEL_CHECK(ctx);
+    }
+    if (relres_host) {
+        CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal + 4, relres, sizeof(double), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        *relres_host = ctx->h_scal[4];
+    }
+    return SQEQ_OK;
+}
+
 // x0 (device, may be NULL): initial guess; its residual b - A x0 costs one operator application.
 // dinv (device, may be NULL): right Jacobi preconditioner, the solve runs on A D^-1 y = b with x = D^-1 y
 // ("Jacobi preconditioner is used for regular MD runs").
@@ -171,6 +294,12 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
 {
     cudaStream_t st = ctx->stream;
     const int m = restart > 0 ? (restart < max_iter ? restart : max_iter) : max_iter;
+    if (tol <= 0.0 && !x0 && m == max_iter && m <= 64) {
+        // a fixed number of iterations in one cycle: nothing for the host to decide, nothing to wait for
+        if (iters_out) *iters_out = m;
+        if (converged_out) *converged_out = false;
+        return gmres_fixed_async(ctx, len, apply, load_rhs, m, x_out, relres_out, dinv);
+    }
     const int64_t ld = (len + 31) & ~(int64_t)31;
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_V, sizeof(double) * (size_t)ld * (m + 1)));
     SQEQ_TRY(sqeq_reserve(ctx, ctx->kry_w, sizeof(double) * (size_t)ld * 3));

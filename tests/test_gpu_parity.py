@@ -444,6 +444,105 @@ def test_shadow_md_steps_config2_geometry(ctx):
     nl.free()
 
 
+def test_cuda_graph_replay_matches_plain_launches():
+    """On a context with its own stream sqeq_coulomb_fixed replays a cached geometry as a CUDA graph, and
+    sqeq_shadow_md_run replays the MD step: same numbers as kernel-by-kernel launches ("graphs" = 0), the launch
+    counter keeps counting, a changed charge pointer or a new geometry re-captures."""
+    from paper_2503_21176_b200 import binding
+    c = W.CONFIGS[0]
+    pos, q = inputs(0)
+    n = len(q)
+    res = {}
+    for graphs in (1, 0):
+        stream = torch.cuda.Stream()
+        cx = binding.Context(0, stream=stream)
+        cx.set_option("graphs", graphs)
+        try:
+            x, qa, qb = dev(pos), dev(q), dev(q[::-1].copy())
+            torch.cuda.synchronize()
+            nl = cx.nl_build(x, c.box, c.r_list)
+            cx.geometry_set(nl, x, c.box, c.rc, c.alpha, c.grid, c.order)
+            phi, F = torch.empty(n, device="cuda"), torch.empty((n, 3), device="cuda")
+            outs = []
+            cx.launch_count(reset=True)
+            for v in (qa, qa, qa, qb, qb, qa):
+                cx.coulomb_fixed(v, phi, None)
+                torch.cuda.synchronize()
+                outs.append(phi.cpu().numpy().copy())
+            per_eval = cx.launch_count() / 6
+            cx.coulomb_fixed(qa, phi, F, want_energy=True)
+            cx.coulomb_fixed(qa, phi, F, want_energy=True)
+            E = cx.energy_fetch()
+            outs.append(F.cpu().numpy().copy())
+            # new positions: the graph of the old geometry must not be replayed
+            x2 = dev(W.perturb(pos, 0, 0.02, 0))
+            torch.cuda.synchronize()
+            cx.geometry_set(nl, x2, c.box, c.rc, c.alpha, c.grid, c.order)
+            for _ in range(3):
+                cx.coulomb_fixed(qa, phi, None)
+            torch.cuda.synchronize()
+            outs.append(phi.cpu().numpy().copy())
+            res[graphs] = (outs, per_eval, E)
+            nl.free()
+        finally:
+            cx.close()
+    assert res[1][1] == res[0][1] and res[1][1] >= 5           # same launches counted with and without replay
+    for a, b in zip(res[1][0], res[0][0]):
+        assert relrms(a, b) < 2e-6                              # only the order of atomic tile flushes differs
+    assert abs(res[1][2] / res[0][2] - 1) < 1e-6
+    op, _, _, _ = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order)
+    assert relrms(res[1][0][2], op) < TOL and relrms(res[1][0][0], op) < TOL
+
+
+@pytest.mark.parametrize("own_stream", [False, True])
+def test_shadow_md_run_keeps_the_list_valid(ctx, own_stream):
+    """sqeq_shadow_md_run: N steps in one call with rebuilds decided two steps behind the GPU.  Against a loop of
+    single steps that rebuilds before EVERY step (always a valid list): same trajectory up to fp32 summation order,
+    rebuilds did happen (thin skin), and no look-ahead displacement above skin/2 - slack was ever accepted."""
+    from paper_2503_21176_b200 import binding
+    c2 = W.CONFIGS[2]
+    pos, _ = inputs(2)
+    n = len(pos)
+    chi, u = W.qeq_params_water_pd(n)
+    mass = W.masses_water(n)
+    vel = W.velocities(mass)
+    skin = 0.4
+    cfg = W.Config(9, "md_run", "water", c2.n_lattice, c2.L, c2.rc, c2.alpha, c2.grid, c2.order, skin)
+    p = binding.md_params(cfg, dt=0.5, k_rep=W.K_REP, r_rep=W.R_REP)
+    n0 = np.tile([-0.5, 0.25, 0.25], n // 3)
+    nsteps = 14
+    out = []
+    if own_stream:          # with its own stream the steps are replayed as a CUDA graph (re-captured at every rebuild)
+        ctx = binding.Context(0, stream=torch.cuda.Stream())
+    for mode in ("run", "steps"):
+        x, v = dev(pos), dev(vel)
+        torch.cuda.synchronize()
+        nl = ctx.nl_build(x, cfg.box, cfg.r_list)
+        nh, F, en = ctx.shadow_md_init(nl, x, cfg.box, p, dev(chi), dev(u), max_iter=0, n0=n0)
+        if mode == "run":
+            st = ctx.shadow_md_run(nl, x, v, dev(mass), cfg.box, p, dev(chi), dev(u), nh, F, nsteps, slack=0.05)
+            print("md_run stats", st)
+            assert st["rebuilds"] >= 2 and st["max_ahead_accepted"] < 0.5 * skin - 0.05 and st["drift_end"] < 0.5 * skin
+            assert st["evals_last_step"] == 6
+        else:
+            worst = 0.0
+            for s_ in range(nsteps):
+                nl.free()
+                nl = ctx.nl_build(x, cfg.box, cfg.r_list)
+                en = ctx.shadow_md_step(nl, x, v, dev(mass), cfg.box, p, dev(chi), dev(u), nh, F)
+                worst = max(worst, nl.max_drift(x))
+            assert worst < 0.5 * skin                    # one step never outruns this skin: the reference is valid
+        out.append((x.cpu().numpy().copy(), v.cpu().numpy().copy(), nh[0].cpu().numpy().copy(), F.cpu().numpy().copy(),
+                    st["U"] if mode == "run" else en[0]))
+        nl.free()
+    (xa, va, na, Fa, Ua), (xb, vb, nb, Fb, Ub) = out
+    print(f"md_run vs stepwise: x {np.abs(xa - xb).max():.2e} v {relrms(va, vb):.2e} n {relrms(na, nb):.2e} F {relrms(Fa, Fb):.2e}")
+    assert np.abs(xa - xb).max() < 2e-5 and relrms(va, vb) < 1e-4 and relrms(na, nb) < 1e-5 and relrms(Fa, Fb) < 1e-4
+    assert abs(Ua / Ub - 1) < 1e-6
+    if own_stream:
+        ctx.close()
+
+
 def test_regular_bomd_against_oracle(ctx):
     """NEXT-2: Jacobi-preconditioned, warm-started GMRES on Eq. 18 and one
     regular BOMD step -- forces at fixed q_min, U_BO, the O-O repulsion of the stand-in -- against the oracle, on
