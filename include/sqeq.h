@@ -151,6 +151,22 @@ int  sqeq_coulomb_host_submit(sqeq_ctx* ctx, int slot, const sqeq_nlist* nl, int
                               float* phi_host, float* force_host, int want_energy);
 int  sqeq_coulomb_host_wait(sqeq_ctx* ctx, int slot, double* energy);
 
+/* ---- regular Ewald summation: PAPER.md:98-132 (section 3.2, Eqs. 6-12); SURVEY.md 8(f) NEXT-3 ---------------
+ * The same evaluation with the reciprocal part summed directly over the k-vectors k = 2 pi (m_x/L_x, m_y/L_y,
+ * m_z/L_z), m != 0, |m_d| <= kmax[d] (host int[3], each in [1, 128]) instead of on a mesh: the structure
+ * factors S(k) = sum_i q_i e^{i k.r_i} (Eqs. 7-9), then Eqs. 10-11 per atom, the phase matrix of Eq. 9 formed
+ * block by block on the fly and never stored.  O(N * number of k-vectors): the faster method below about 5,000
+ * atoms.  Real-space part, self term, arguments and outputs as for sqeq_coulomb.  A non-NULL
+ * energy synchronises. */
+int  sqeq_coulomb_ewald(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const float* q,
+                        const double box[3], double rc, double alpha, const int kmax[3], float* phi,
+                        float* force, double* energy);
+/* Parameters from an accuracy delta by the heuristics the paper takes from OpenMM (the formulas
+ * are that library's, recalled -- DESIGN.md reading G17): alpha = sqrt(-ln 2 delta)/rc; kmax[d] for
+ * sqeq_coulomb_ewald; grid[d] = ceil(2 alpha L_d/(3 delta^(1/5))) rounded up to an even 2^a 3^b 5^c for
+ * sqeq_coulomb.  Host outputs, any may be NULL.  No context needed. */
+int  sqeq_ewald_params(const double box[3], double rc, double delta, double* alpha, int kmax[3], int grid[3]);
+
 /* ---- fixed geometry, many charge vectors ("Each iteration involves
  * calculating a Coulomb-like potential") ------------------------------------------------------
  * Every Krylov iteration of a QEq solve and all 2 + m evaluations of a shadow-MD step repeat the evaluation on

@@ -199,6 +199,23 @@ def ewald_direct(pos, q, box, alpha, tol=1e-16, background=False):
     return phi, F, float(E[0])
 
 
+def ewald_truncated(pos, q, box, rc, alpha, kmax):
+    """Regular Ewald with the cutoffs of a production run: real space over minimum-image pairs
+    with r < rc (rc < L/2), reciprocal space over all m != 0 with |m_d| <= kmax[d], self term.  The same routine as
+    ewald_direct with those cutoffs given instead of derived from a tolerance.  Returns phi, F, E."""
+    pos = _f64(pos, (-1, 3)); q = _f64(q); box = _box(box)
+    n = pos.shape[0]
+    # the C routine visits images -1, 0, +1 of the positions it is given: hand it the positions wrapped into the box
+    # (nothing changes physically: the real-space sum is over images, the phases are periodic)
+    pos = pos - np.floor(pos / box) * box
+    nimg = np.ones(3, dtype=np.intc)
+    mmax = np.ascontiguousarray(np.asarray(kmax, dtype=np.intc).reshape(3))
+    phi = np.zeros(n); F = np.zeros((n, 3)); E = np.zeros(1)
+    lib().orc_ewald_direct(n, _dp(pos), _dp(q), _dp(box), float(alpha), float(rc), _ip(nimg), _ip(mmax), 0,
+                           _dp(phi), _dp(F), _dp(E))
+    return phi, F, float(E[0])
+
+
 # --------------------------------------------------------------------------
 # c-PME  smooth PME, Alg. 2 (PAPER.md:140-151)
 # --------------------------------------------------------------------------

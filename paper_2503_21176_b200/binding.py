@@ -68,6 +68,8 @@ def load():
     L.sqeq_coulomb_host_wait.argtypes = [vp, cint, dp]
     L.sqeq_coulomb_enqueue.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, cint]
     L.sqeq_energy_fetch.argtypes = [vp, dp]
+    L.sqeq_coulomb_ewald.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, vp, vp, dp]
+    L.sqeq_ewald_params.argtypes = [dp, dbl, dbl, dp, ip, ip]
     L.sqeq_geometry_set.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint]
     L.sqeq_coulomb_fixed.argtypes = [vp, i64, vp, vp, vp, cint]
     L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
@@ -239,6 +241,18 @@ class Context:
                                         _ptr(force, torch.float32, 3 * n) if want_force else None,
                                         ctypes.byref(e) if want_energy else None))
         return phi, (force if want_force else None), (e.value if want_energy else None)
+
+    def coulomb_ewald(self, nl, pos, q, box, rc, alpha, kmax, want_force=True, want_energy=True):
+        """sqeq_coulomb_ewald: regular Ewald, reciprocal part summed over |m_d| <= kmax[d]."""
+        n = pos.shape[0]
+        phi = torch.empty(n, dtype=torch.float32, device=self.device)
+        force = torch.empty((n, 3), dtype=torch.float32, device=self.device) if want_force else None
+        e = ctypes.c_double()
+        self._check(load().sqeq_coulomb_ewald(self.handle, nl.handle, n, _ptr(pos, torch.float32, 3 * n),
+                                              _ptr(q, torch.float32, n), _box(box), float(rc), float(alpha), _grid(kmax),
+                                              _ptr(phi, torch.float32, n), _ptr(force, torch.float32, 3 * n) if want_force else None,
+                                              ctypes.byref(e) if want_energy else None))
+        return phi, force, (e.value if want_energy else None)
 
     def coulomb_enqueue(self, nl, pos, q, box, rc, alpha, grid, order, phi, force, want_energy=True):
         """sqeq_coulomb_enqueue: no synchronisation; read the energy later with energy_fetch()."""
@@ -440,6 +454,16 @@ class Context:
         c = ctypes.c_int64()
         self._check(load().sqeq_launch_count(self.handle, ctypes.byref(c), int(reset)))
         return c.value
+
+
+def ewald_params(box, rc, delta):
+    """sqeq_ewald_params: (alpha, kmax[3], grid[3]) for an Ewald accuracy delta (OpenMM's heuristics)."""
+    a = ctypes.c_double()
+    km, gr = (ctypes.c_int * 3)(), (ctypes.c_int * 3)()
+    rc_ = load().sqeq_ewald_params(_box(box), float(rc), float(delta), ctypes.byref(a), km, gr)
+    if rc_ != OK:
+        raise SqeqError(rc_, "sqeq_ewald_params: bad argument")
+    return a.value, list(km), list(gr)
 
 
 def md_params(cfg, dt=0.5, ke=14.3996454784255, total_charge=0.0, krylov_rank=4,

@@ -185,7 +185,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
         cufftDestroy(ctx->plan_r2c);
         cufftDestroy(ctx->plan_c2r);
     }
-    DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len,
+    DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len, &ctx->ew_tab, &ctx->ew_sf,
                       &ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
                       &ctx->base, &ctx->real_out, &ctx->rec_out, &ctx->scal, &ctx->kry_V,
                       &ctx->kry_w, &ctx->kry_h};

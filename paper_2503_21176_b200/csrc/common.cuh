@@ -70,6 +70,8 @@ struct sqeq_ctx {
     DevBuf grid;      // float  [K0][K1][K2]        charge grid Q, then potential grid Phi
     DevBuf gridQ;     // float  copy of Q kept for sqeq_pme_grid (diagnostics only when enabled)
     DevBuf spec;      // float2 [K0][K1][K2/2+1]
+    DevBuf ew_tab;    // float2 [ntab][n]  per-atom phase tables of the regular-Ewald kernels (ewald.cu)
+    DevBuf ew_sf;     // float2 [nk]       structure factors / coefficients
     DevBuf tabs;      // float  per-axis tables: |b|^2, gaussian, mtilde^2  (3 x (K0+K1+K2))
 
     // ---- per-evaluation atom workspaces (sorted = cell-major order of the list) ----

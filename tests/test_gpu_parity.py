@@ -543,6 +543,46 @@ def test_shadow_md_run_keeps_the_list_valid(ctx, own_stream):
         ctx.close()
 
 
+def test_regular_ewald_against_oracle(ctx):
+    """NEXT-3 (Eqs. 6-12): sqeq_coulomb_ewald -- reciprocal part summed directly over
+    |m_d| <= kmax -- against the oracle's direct Ewald with the same cutoffs, at the sizes the paper says the method
+    is for (below ~5,000 atoms): cfg 0 (648 atoms) and a 3,000-atom non-cubic box with unwrapped positions; and the
+    parameter helper against the formulas it implements."""
+    from paper_2503_21176_b200 import binding
+    c = W.CONFIGS[0]
+    pos, q = inputs(0)
+    nl = ctx.nl_build(dev(pos), c.box, c.r_list)
+    alpha, kmax, grid = binding.ewald_params(c.box, c.rc, 5e-4)       # the paper's Ewald accuracy (PAPER.md:297)
+    assert abs(alpha - math.sqrt(-math.log(1e-3)) / c.rc) < 1e-12
+    k = kmax[0]
+    err = lambda kk: kk * math.sqrt(c.L * alpha) / 20 * math.exp(-(math.pi * kk / (c.L * alpha)) ** 2)
+    assert err(k) < 5e-4 <= err(k - 1) and grid[0] % 2 == 0 and grid[0] >= 2 * alpha * c.L / (3 * 5e-4 ** 0.2)
+    for a, km in ((c.alpha, [9, 9, 9]), (alpha, kmax)):
+        phi, F, E = ctx.coulomb_ewald(nl, dev(pos), dev(q), c.box, c.rc, a, km)
+        op, oF, oE = oracle.ewald_truncated(pos, q, c.box, c.rc, a, km)
+        e_phi, e_F = relrms(phi.cpu().numpy(), op), relrms(F.cpu().numpy(), oF)
+        print(f"regular Ewald cfg0 alpha {a:.3f} kmax {km}: phi {e_phi:.2e} F {e_F:.2e} E {abs(E / oE - 1):.2e}")
+        assert e_phi < TOL and e_F < TOL and abs(E / oE - 1) < TOL
+    record("regular_ewald_cfg0", relrms_phi=e_phi, relrms_F=e_F)
+    # converged regular Ewald and PME agree to the method error of the mesh (1e-5 ... 1e-4 at this grid)
+    phi_p, F_p, E_p = ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+    phi_e, F_e, E_e = ctx.coulomb_ewald(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, [9, 9, 9])
+    assert relrms(phi_p.cpu().numpy(), phi_e.cpu().numpy()) < 2e-4 and abs(E_p / E_e - 1) < 1e-4
+    nl.free()
+    rng = np.random.default_rng(33)
+    n = 3000
+    box = np.array([30.0, 33.0, 36.0])
+    p = (rng.uniform(0, 1, (n, 3)) * box + rng.integers(-2, 3, (n, 3)) * box).astype(np.float32)
+    qq = rng.normal(size=n).astype(np.float32)
+    nl = ctx.nl_build(dev(p), box, 9.0)
+    phi, F, E = ctx.coulomb_ewald(nl, dev(p), dev(qq), box, 9.0, 0.35, [12, 13, 14])
+    op, oF, oE = oracle.ewald_truncated(p, qq, box, 9.0, 0.35, [12, 13, 14])
+    assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL
+    phi2, _, _ = ctx.coulomb_ewald(nl, dev(p), dev(qq), box, 9.0, 0.35, [12, 13, 14], want_force=False, want_energy=False)
+    assert relrms(phi2.cpu().numpy(), op) < TOL
+    nl.free()
+
+
 def test_regular_bomd_against_oracle(ctx):
     """NEXT-2: Jacobi-preconditioned, warm-started GMRES on Eq. 18 and one
     regular BOMD step -- forces at fixed q_min, U_BO, the O-O repulsion of the stand-in -- against the oracle, on

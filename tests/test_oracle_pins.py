@@ -250,6 +250,21 @@ def test_neighbour_rows_are_the_symmetric_closure():
         assert np.array_equal(sr[jr < a], -s[j == a])
 
 
+def test_ewald_truncated_is_direct_ewald_with_given_cutoffs():
+    """ewald_truncated = the pinned ewald_direct routine with production cutoffs: it equals the converged sum
+    when the cutoffs are generous, and the real-space part alone equals realspace() for kmax -> nothing."""
+    rng = np.random.default_rng(2)
+    box = [11.0, 12.0, 13.0]
+    pos = rng.uniform(0, 1, (40, 3)) * box
+    q = rng.normal(size=40); q -= q.mean()
+    phi, F, E = oracle.ewald_direct(pos, q, box, 0.9)
+    p2, F2, E2 = oracle.ewald_truncated(pos, q, box, 5.4, 0.9, [22, 24, 26])
+    assert np.abs(p2 - phi).max() < 1e-8 and np.abs(F2 - F).max() < 1e-8 and abs(E2 - E) < 1e-8
+    # wrapped or unwrapped positions: the same (minimum image in real space, periodic phases in reciprocal space)
+    p3, F3, E3 = oracle.ewald_truncated(pos + np.array(box) * rng.integers(-2, 3, (40, 3)), q, box, 5.4, 0.9, [22, 24, 26])
+    assert np.abs(p3 - p2).max() < 1e-9
+
+
 def test_neighbour_rows_upper_is_a_slice_of_the_list():
     """The chunked walk used by the full-size GPU list tests returns exactly rows i0..i1 of the list
     (also when the first capacity guess is too small)."""
