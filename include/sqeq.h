@@ -76,6 +76,16 @@ int  sqeq_nl_count (const sqeq_nlist* nl, int64_t* n_pairs_unique);
  * build time) is the in-range vector.  i, j: device int32 [n_pairs_unique]; shift3: device int8
  * [n_pairs_unique][3]; caller-owned.  Synchronises the stream. */
 int  sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
+/* The paper's two output formats, DIRECTED rows in the caller's numbering, neighbours of an atom in
+ * ascending order, shift = image shift of the ordered pair (i, j) on the raw caller positions at build time:
+ *   ELLPACK: nbr device int32 [n][K], row i = the neighbours of atom i padded with -1; shift3 device int8 [n][K][3];
+ *            counts device int32 [n] (may be NULL) = neighbours per atom.  K >= the longest row (sqeq_nl_info), else
+ *            SQEQ_ECAPACITY.
+ *   COO:     i, j device int32 [2 * n_pairs_unique], shift3 device int8 [..][3]: every pair in both directions,
+ *            sorted by (i, j).
+ * Both synchronise the stream. */
+int  sqeq_nl_export_ellpack(sqeq_ctx* ctx, const sqeq_nlist* nl, int K, int32_t* nbr, int8_t* shift3, int32_t* counts);
+int  sqeq_nl_export_coo(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
 /* List introspection (host outputs, any may be NULL): cells per axis, directed entries, max row. */
 int  sqeq_nl_info  (const sqeq_nlist* nl, int ncell[3], int64_t* n_directed, int* max_row);
 /* Bytes per stored list entry: 2 (16-bit index into the cell group's neighbourhood, the format of the

@@ -57,6 +57,8 @@ def load():
     L.sqeq_nl_build.argtypes = [vp, i64, vp, dp, dbl, ctypes.POINTER(vp)]
     L.sqeq_nl_count.argtypes = [vp, ctypes.POINTER(i64)]
     L.sqeq_nl_export.argtypes = [vp, vp, vp, vp, vp]
+    L.sqeq_nl_export_ellpack.argtypes = [vp, vp, cint, vp, vp, vp]
+    L.sqeq_nl_export_coo.argtypes = [vp, vp, vp, vp, vp]
     L.sqeq_nl_info.argtypes = [vp, ip, ctypes.POINTER(i64), ip]
     L.sqeq_nl_entry_bytes.argtypes = [vp, ip]
     L.sqeq_nl_layout.argtypes = [vp, ctypes.POINTER(i64), ip, ip]
@@ -171,6 +173,29 @@ class NeighbourList:
         self.ctx._check(load().sqeq_nl_export(self.ctx.handle, self.handle,
                                               ctypes.c_void_p(i.data_ptr()), ctypes.c_void_p(j.data_ptr()),
                                               ctypes.c_void_p(s.data_ptr())))
+        return i, j, s
+
+    def export_ellpack(self, K=None):
+        """ELLPACK rows [n][K] (padded with -1), shifts [n][K][3], counts [n] on the device."""
+        K = self.info()["max_row"] if K is None else K
+        K = max(int(K), 1)
+        dev = self.ctx.device
+        nbr = torch.empty((self.n, K), dtype=torch.int32, device=dev)
+        sh = torch.empty((self.n, K, 3), dtype=torch.int8, device=dev)
+        cnt = torch.empty(self.n, dtype=torch.int32, device=dev)
+        self.ctx._check(load().sqeq_nl_export_ellpack(self.ctx.handle, self.handle, K, ctypes.c_void_p(nbr.data_ptr()),
+                                                      ctypes.c_void_p(sh.data_ptr()), ctypes.c_void_p(cnt.data_ptr())))
+        return nbr, sh, cnt
+
+    def export_coo(self):
+        """Directed COO (every pair both ways) sorted by (i, j) on the device."""
+        m = 2 * self.count()
+        dev = self.ctx.device
+        i = torch.empty(m, dtype=torch.int32, device=dev)
+        j = torch.empty(m, dtype=torch.int32, device=dev)
+        s = torch.empty((m, 3), dtype=torch.int8, device=dev)
+        self.ctx._check(load().sqeq_nl_export_coo(self.ctx.handle, self.handle, ctypes.c_void_p(i.data_ptr()),
+                                                  ctypes.c_void_p(j.data_ptr()), ctypes.c_void_p(s.data_ptr())))
         return i, j, s
 
     def free(self):

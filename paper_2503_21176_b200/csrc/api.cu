@@ -346,6 +346,27 @@ int sqeq_nl_export(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, 
     return nl_export_impl(ctx, nl, i, j, shift3);
 }
 
+int sqeq_nl_export_ellpack(sqeq_ctx* ctx, const sqeq_nlist* nl, int K, int32_t* nbr, int8_t* shift3, int32_t* counts)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!nl || nl->ctx != ctx) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_export_ellpack: list does not belong to this context");
+    if (!nbr || !shift3 || K < 1) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_export_ellpack: NULL output or K < 1");
+    if (K < nl->max_row)
+        return sqeq_fail(ctx, SQEQ_ECAPACITY, "sqeq_nl_export_ellpack: K = %d but the longest row has %d neighbours", K, nl->max_row);
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return nl_export_rows_impl(ctx, nl, 0, K, nullptr, nbr, shift3, counts);
+}
+
+int sqeq_nl_export_coo(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    if (!nl || nl->ctx != ctx) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_export_coo: list does not belong to this context");
+    if (nl->n_directed > 0 && (!i || !j || !shift3)) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_nl_export_coo: NULL output");
+    if (nl->n_directed == 0) return SQEQ_OK;
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return nl_export_rows_impl(ctx, nl, 1, 0, i, j, shift3, nullptr);
+}
+
 int sqeq_nl_entry_bytes(const sqeq_nlist* nl, int* bytes)
 {
     if (!nl || !bytes) return SQEQ_EINVAL;

@@ -228,6 +228,8 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
 void nl_release(sqeq_nlist* nl);
 void nl_release_storage(sqeq_nlist* nl);
 int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* i, int32_t* j, int8_t* shift3);
+int nl_export_rows_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int mode, int K, int32_t* oi, int32_t* oj, int8_t* shift3,
+                        int32_t* counts);
 int nl_max_drift_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,
                          unsigned* d_out);
 int nl_max_drift_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* pos, const float* vel, double dt,

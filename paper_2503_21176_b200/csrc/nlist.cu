@@ -664,6 +664,72 @@ k_export_fill(int64_t n, const int64_t* __restrict__ row_start, const int* __res
     }
 }
 
+// Directed rows in the caller's numbering (the paper's two output formats):
+// one block per sorted atom collects ALL its neighbours, sorts them by caller index and writes either row oi of an
+// ELLPACK matrix [n][K] (padded with -1) or its stretch of a directed COO list (offsets from a scan of the row
+// lengths in caller order).  shift = image shift of the ordered pair (oi, oj) on the raw caller positions.
+#define EXPORT_ROW_CAP 8192
+__global__ void __launch_bounds__(256)
+k_export_rows(const int64_t* __restrict__ row_start, const int* __restrict__ row_len, const uint32_t* __restrict__ nbr,
+              const int* __restrict__ perm, const char4* __restrict__ wrapc, int K, const int64_t* __restrict__ off_orig,
+              int32_t* __restrict__ out_i, int32_t* __restrict__ out_j, int8_t* __restrict__ out_s, int32_t* __restrict__ counts)
+{
+    extern __shared__ int sh_rows[];
+    int* key = sh_rows;
+    int* val = sh_rows + EXPORT_ROW_CAP;
+    const int64_t s = blockIdx.x;
+    const int oi = perm[s];
+    const int64_t beg = row_start[s];
+    const int m = row_len[s];
+    if (counts && threadIdx.x == 0) counts[oi] = m;
+    int p2 = 1;
+    while (p2 < m) p2 <<= 1;
+    for (int t = threadIdx.x; t < p2; t += blockDim.x) {
+        key[t] = t < m ? perm[nbr[beg + t] & 0x07ffffffu] : 0x7fffffff;
+        val[t] = t;
+    }
+    __syncthreads();
+    for (int k = 2; k <= p2; k <<= 1)
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < p2; t += blockDim.x) {
+                const int x = t ^ j;
+                if (x > t) {
+                    const int a = key[t], b = key[x];
+                    const bool up = (t & k) == 0;
+                    if ((a > b) == up) {
+                        key[t] = b; key[x] = a;
+                        const int va = val[t]; val[t] = val[x]; val[x] = va;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    const char4 wi = wrapc[s];
+    const int64_t o0 = off_orig ? off_orig[oi] : (int64_t)oi * K;
+    for (int t = threadIdx.x; t < m; t += blockDim.x) {
+        const uint32_t e = nbr[beg + val[t]];
+        int tj, ox, oy, oz;
+        decode_img(e, tj, ox, oy, oz);
+        const char4 wj = wrapc[tj];
+        if (out_i) out_i[o0 + t] = oi;
+        out_j[o0 + t] = key[t];
+        out_s[3 * (o0 + t) + 0] = (int8_t)(ox - wj.x + wi.x);
+        out_s[3 * (o0 + t) + 1] = (int8_t)(oy - wj.y + wi.y);
+        out_s[3 * (o0 + t) + 2] = (int8_t)(oz - wj.z + wi.z);
+    }
+    if (!off_orig)
+        for (int t = m + threadIdx.x; t < K; t += blockDim.x) {
+            out_j[o0 + t] = -1;
+            out_s[3 * (o0 + t) + 0] = 0; out_s[3 * (o0 + t) + 1] = 0; out_s[3 * (o0 + t) + 2] = 0;
+        }
+}
+
+__global__ void k_row_len_orig(int64_t n, const int* __restrict__ row_len, const int* __restrict__ perm, int* __restrict__ cnt)
+{
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s < n) cnt[perm[s]] = row_len[s];
+}
+
 // ------------------------------------------------------------------------------------------ host
 static void fill_geom(NLGeom& g, const double box[3], double cutoff, int64_t n)
 {
@@ -1022,5 +1088,49 @@ int nl_export_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int32_t* oi, int32_t* oj
     if (total * 2 != nl->n_directed)
         return sqeq_fail(ctx, SQEQ_ECUDA, "sqeq_nl_export: list is not symmetric (%lld upper entries, %lld directed)",
                          (long long)total, (long long)nl->n_directed);
+    return SQEQ_OK;
+}
+
+// mode 0: ELLPACK rows [n][K]; mode 1: directed COO of n_directed entries sorted by (i, j)
+int nl_export_rows_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int mode, int K, int32_t* oi, int32_t* oj, int8_t* shift3,
+                        int32_t* counts)
+{
+    cudaStream_t st = ctx->stream;
+    const int64_t n = nl->n;
+    if (nl->max_row > EXPORT_ROW_CAP)
+        return sqeq_fail(ctx, SQEQ_ECAPACITY, "neighbour export: a row has %d neighbours, more than %d", nl->max_row, EXPORT_ROW_CAP);
+    uint32_t* expanded = nullptr;
+    int* cnt = nullptr;
+    int64_t* off = nullptr;
+    auto body = [&]() -> int {
+        const uint32_t* nbr32 = (const uint32_t*)nl->nbr;
+        if (nl->fmt == 1 && nl->n_slots > 0) {
+            SQEQ_TRY(pool_alloc(ctx, (void**)&expanded, sizeof(uint32_t) * (size_t)nl->n_slots));
+            k_local_to_global<<<nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2], 256, 0, st>>>(
+                nl->cell_start, nl->gg, nl->row_start, nl->row_len, (const uint16_t*)nl->nbr, nl->lshift, expanded);
+            KERNEL_CHECK(ctx);
+            nbr32 = expanded;
+        }
+        if (mode == 1) {
+            SQEQ_TRY(pool_alloc(ctx, (void**)&cnt, sizeof(int) * (n + 1)));
+            SQEQ_TRY(pool_alloc(ctx, (void**)&off, sizeof(int64_t) * (n + 1)));
+            CUDA_TRY(ctx, cudaMemsetAsync(cnt, 0, sizeof(int) * (n + 1), st));
+            k_row_len_orig<<<ceil_div(n, 256), 256, 0, st>>>(n, nl->row_len, nl->perm, cnt);
+            KERNEL_CHECK(ctx);
+            SQEQ_TRY(exclusive_scan<int>(ctx, n + 1, cnt, off, st));
+        }
+        const size_t sm = sizeof(int) * 2 * EXPORT_ROW_CAP;
+        CUDA_TRY(ctx, cudaFuncSetAttribute(k_export_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        k_export_rows<<<(unsigned)n, 256, sm, st>>>(nl->row_start, nl->row_len, nbr32, nl->perm, nl->wrapc, K, off,
+                                                     mode == 1 ? oi : nullptr, oj, shift3, counts);
+        KERNEL_CHECK(ctx);
+        return SQEQ_OK;
+    };
+    const int r = body();
+    cudaError_t e = cudaStreamSynchronize(st);
+    for (void* p : {(void*)expanded, (void*)cnt, (void*)off})
+        if (p) cudaFreeAsync(p, st);
+    if (r != SQEQ_OK) return r;
+    if (e != cudaSuccess) return sqeq_fail(ctx, SQEQ_ECUDA, "neighbour export: %s", cudaGetErrorString(e));
     return SQEQ_OK;
 }

@@ -543,6 +543,38 @@ def test_shadow_md_run_keeps_the_list_valid(ctx, own_stream):
         ctx.close()
 
 
+def test_ellpack_and_coo_exports(ctx):
+    """NEXT-4: the ELLPACK [n][K] and directed-COO output formats against the oracle's list (its
+    symmetric closure, written out here): bit-exact rows, -1 padding, K too small is an error."""
+    from paper_2503_21176_b200.binding import SqeqError, ECAPACITY
+    rng = np.random.default_rng(8)
+    cases = [(inputs(0)[0], W.CONFIGS[0].box, W.CONFIGS[0].r_list), (inputs(1)[0], W.CONFIGS[1].box, W.CONFIGS[1].r_list)]
+    boxn = np.array([17.0, 19.5, 23.0])
+    cases.append(((rng.uniform(0, 1, (700, 3)) * boxn + rng.integers(-3, 4, (700, 3)) * boxn).astype(np.float32), boxn, 8.4))
+    cases.append((np.array([[0.5, 5.0, 5.0], [9.5, 5.0, 5.0], [4.5, 5.0, 5.0]], dtype=np.float32), [10.0, 12.0, 14.0], 4.0))
+    for pos, box, rl in cases:
+        n = len(pos)
+        nl = ctx.nl_build(dev(pos), box, rl)
+        oi, oj, os_ = oracle.neighbour_list(pos, box, rl)
+        di = np.concatenate([oi, oj]); dj = np.concatenate([oj, oi]); ds = np.concatenate([os_, -os_])
+        o = np.lexsort((dj, di))
+        di, dj, ds = di[o], dj[o], ds[o]
+        ci, cj, cs = [t.cpu().numpy() for t in nl.export_coo()]
+        assert np.array_equal(ci, di) and np.array_equal(cj, dj) and np.array_equal(cs, ds)
+        K = nl.info()["max_row"] + 3
+        nbr, sh, cnt = [t.cpu().numpy() for t in nl.export_ellpack(K)]
+        counts = np.bincount(di, minlength=n)
+        assert np.array_equal(cnt, counts) and counts.max() == K - 3
+        mask = np.arange(K)[None, :] < counts[:, None]
+        assert np.array_equal(nbr[mask], dj) and np.array_equal(sh[mask], ds)
+        assert (nbr[~mask] == -1).all() and (sh[~mask] == 0).all()
+        if K > 4:
+            with pytest.raises(SqeqError) as e:
+                nl.export_ellpack(K - 4)
+            assert e.value.code == ECAPACITY
+        nl.free()
+
+
 def test_regular_ewald_against_oracle(ctx):
     """NEXT-3 (Eqs. 6-12): sqeq_coulomb_ewald -- reciprocal part summed directly over
     |m_d| <= kmax -- against the oracle's direct Ewald with the same cutoffs, at the sizes the paper says the method
