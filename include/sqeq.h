@@ -333,6 +333,9 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *                         sqeq_shadow_md_run) as CUDA graphs; needs a context stream other than the legacy default
  *   "overlap"          0  PME on an internal side stream beside a persistent real-space grid
  *   "real_lean_blocks" 2  blocks per SM of that persistent grid
+ *   "fft_fused"        1  x-axis transforms fused with the influence multiply in one own kernel between batched 2-D
+ *                         cuFFT transforms (0, or a grid whose x size has a prime factor above 5: 3-D cuFFT transforms
+ *                         and a separate influence kernel)
  *   "pme_tiles"        1  shared-memory tiles for spreading and gathering (0: global-memory kernels)
  *   "spread_float"     0  fp32 compare-and-swap accumulation in the spreading tile instead of fixed point
  *   "real_staged"      1  16-bit list + shared-memory-staged real-space kernel (0: 32-bit list, global gather;

@@ -162,6 +162,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->real_lean_blocks = env && atoi(env) > 0 ? atoi(env) : 2;
     env = getenv("SQEQ_REAL_STAGED");
     ctx->real_staged_off = env && env[0] == '0';
+    env = getenv("SQEQ_FFT_FUSED");
+    ctx->fft_fused_off = env && env[0] == '0';
     env = getenv("SQEQ_GRAPHS");
     ctx->graphs = !(env && env[0] == '0');
     *out = ctx;
@@ -185,7 +187,11 @@ int sqeq_destroy(sqeq_ctx* ctx)
         cufftDestroy(ctx->plan_r2c);
         cufftDestroy(ctx->plan_c2r);
     }
-    DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len, &ctx->ew_tab, &ctx->ew_sf,
+    if (ctx->xf_ok) {
+        cufftDestroy(ctx->plan2_r2c);
+        cufftDestroy(ctx->plan2_c2r);
+    }
+    DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len, &ctx->ew_tab, &ctx->ew_sf, &ctx->xf_tw,
                       &ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
                       &ctx->base, &ctx->real_out, &ctx->rec_out, &ctx->scal, &ctx->kry_V,
                       &ctx->kry_w, &ctx->kry_h};
@@ -274,6 +280,7 @@ int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
     CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
     if (!strcmp(name, "graphs")) ctx->graphs = value != 0;
     else if (!strcmp(name, "overlap")) ctx->overlap = value != 0;
+    else if (!strcmp(name, "fft_fused")) ctx->fft_fused_off = value == 0;
     else if (!strcmp(name, "pme_tiles")) { ctx->pme_tiles_off = value == 0; ctx->tile_plan.valid = false; }
     else if (!strcmp(name, "spread_float")) ctx->spread_float = value != 0;
     else if (!strcmp(name, "real_staged")) ctx->real_staged_off = value == 0;

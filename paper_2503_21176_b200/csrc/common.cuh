@@ -66,6 +66,12 @@ struct sqeq_ctx {
     double tab_alpha = 0;
     cufftHandle plan_r2c = 0, plan_c2r = 0;
     bool plans_ok = false;
+    // fused x-axis pass (pme.cu, k_xline_influence): batched 2-D plans over (y,z), twiddles, radix schedule
+    cufftHandle plan2_r2c = 0, plan2_c2r = 0;
+    bool xf_ok = false;
+    bool fft_fused_off = false;           // SQEQ_FFT_FUSED=0: 3-D cuFFT transforms + separate influence kernel
+    int xf_npass = 0, xf_radix[12] = {0};
+    DevBuf xf_tw;
     bool pme_tiles_off = false;           // SQEQ_PME_TILES=0: global-memory spread/gather only (testing)
     DevBuf grid;      // float  [K0][K1][K2]        charge grid Q, then potential grid Phi
     DevBuf gridQ;     // float  copy of Q kept for sqeq_pme_grid (diagnostics only when enabled)

@@ -153,6 +153,166 @@ k_influence(int K0, int K1, int K2h, int K2, const float* __restrict__ tab, floa
     }
 }
 
+// -------------------------------------------------------------------------------------- fused x-axis pass
+// north_star: "the influence-function convolution fused into the FFT pre- and post-passes".  The 3-D transforms
+// are split as  [cuFFT 2-D R2C over (y,z), batched over x]  ->  THIS KERNEL  ->  [cuFFT 2-D C2R, batched over x]:
+// for a tile of XF_TJ neighbouring (m1, m2) lines the block holds the whole x-extent in shared memory, runs the
+// forward 1-D transform along x (Stockham autosort, radices 2/3/4/5), multiplies by G(m) and accumulates
+// E_rec = 1/2 sum w G |Qhat|^2, runs the inverse transform along x and writes the lines back: the spectrum is read
+// and written ONCE where cuFFT's two x-passes and a separate influence kernel touched it three times.
+#define XF_TJ 16
+#define XF_NT 320
+#define XF_MAXPASS 12
+struct XfPlan {
+    int N;                      // K0
+    int npass;
+    int radix[XF_MAXPASS];
+};
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
+// one Stockham pass of radix R over all XF_TJ lines: in[x][tj] -> out[x][tj].  INV: conjugate twiddles.
+template <int R, bool INV>
+__device__ __forceinline__ void xf_pass(const float2* __restrict__ in, float2* __restrict__ out, const float2* __restrict__ W,
+                                        int N, int Ns)
+{
+    const int nb = N / R;                                   // butterflies per line
+    const int tstep = N / (Ns * R);                         // twiddle index step: angle = -2 pi t k / (Ns R)
+    const float inv_ns = 1.f / (float)Ns;
+    for (int task = threadIdx.x; task < nb * XF_TJ; task += XF_NT) {
+        const int j = task / XF_TJ, tj = task - j * XF_TJ;
+        const int jq = __float2int_rd(((float)j + 0.5f) * inv_ns);     // j / Ns, exact for j < 2^20
+        const int k = j - jq * Ns;
+        float2 v[R];
+#pragma unroll
+        for (int t = 0; t < R; ++t) {
+            v[t] = in[(j + t * nb) * XF_TJ + tj];
+            if (t > 0) {
+                float2 w = W[t * k * tstep];                   // t k < R Ns, so the index stays below N
+                if (INV) w.y = -w.y;
+                v[t] = cmul(v[t], w);
+            }
+        }
+        const float sg = INV ? 1.f : -1.f;                  // forward: e^{-i...}
+        if (R == 2) {
+            const float2 a = v[0], b = v[1];
+            v[0] = make_float2(a.x + b.x, a.y + b.y);
+            v[1] = make_float2(a.x - b.x, a.y - b.y);
+        } else if (R == 4) {
+            const float2 a = make_float2(v[0].x + v[2].x, v[0].y + v[2].y), b = make_float2(v[0].x - v[2].x, v[0].y - v[2].y);
+            const float2 c = make_float2(v[1].x + v[3].x, v[1].y + v[3].y), d = make_float2(v[1].x - v[3].x, v[1].y - v[3].y);
+            const float2 id = make_float2(-sg * d.y, sg * d.x);   // (sg i) d : forward -i d
+            v[0] = make_float2(a.x + c.x, a.y + c.y);
+            v[2] = make_float2(a.x - c.x, a.y - c.y);
+            v[1] = make_float2(b.x + id.x, b.y + id.y);
+            v[3] = make_float2(b.x - id.x, b.y - id.y);
+        } else if (R == 3) {
+            const float c3 = -0.5f, s3 = sg * 0.86602540378443865f;
+            const float2 s = make_float2(v[1].x + v[2].x, v[1].y + v[2].y), d = make_float2(v[1].x - v[2].x, v[1].y - v[2].y);
+            const float2 m = make_float2(v[0].x + c3 * s.x, v[0].y + c3 * s.y);
+            const float2 id = make_float2(-s3 * d.y, s3 * d.x);   // i s3 d
+            v[0] = make_float2(v[0].x + s.x, v[0].y + s.y);
+            v[1] = make_float2(m.x + id.x, m.y + id.y);
+            v[2] = make_float2(m.x - id.x, m.y - id.y);
+        } else if (R == 5) {
+            const float c1 = 0.30901699437494742f, c2 = -0.80901699437494742f;
+            const float s1 = sg * 0.95105651629515357f, s2 = sg * 0.58778525229247313f;
+            const float2 a1 = make_float2(v[1].x + v[4].x, v[1].y + v[4].y), b1 = make_float2(v[1].x - v[4].x, v[1].y - v[4].y);
+            const float2 a2 = make_float2(v[2].x + v[3].x, v[2].y + v[3].y), b2 = make_float2(v[2].x - v[3].x, v[2].y - v[3].y);
+            const float2 m1 = make_float2(v[0].x + c1 * a1.x + c2 * a2.x, v[0].y + c1 * a1.y + c2 * a2.y);
+            const float2 m2 = make_float2(v[0].x + c2 * a1.x + c1 * a2.x, v[0].y + c2 * a1.y + c1 * a2.y);
+            const float2 n1 = make_float2(s1 * b1.x + s2 * b2.x, s1 * b1.y + s2 * b2.y);
+            const float2 n2 = make_float2(s2 * b1.x - s1 * b2.x, s2 * b1.y - s1 * b2.y);
+            v[0] = make_float2(v[0].x + a1.x + a2.x, v[0].y + a1.y + a2.y);
+            v[1] = make_float2(m1.x - n1.y, m1.y + n1.x);          // m1 + i n1
+            v[4] = make_float2(m1.x + n1.y, m1.y - n1.x);
+            v[2] = make_float2(m2.x - n2.y, m2.y + n2.x);
+            v[3] = make_float2(m2.x + n2.y, m2.y - n2.x);
+        }
+        const int j0 = jq * Ns * R + k;
+#pragma unroll
+        for (int t = 0; t < R; ++t) out[(j0 + t * Ns) * XF_TJ + tj] = v[t];
+    }
+}
+
+template <bool INV>
+__device__ __forceinline__ float2* xf_transform(float2* a, float2* b, const float2* W, const XfPlan& pl)
+{
+    int Ns = 1;
+    for (int p = 0; p < pl.npass; ++p) {
+        const int R = pl.radix[p];
+        if (R == 4) xf_pass<4, INV>(a, b, W, pl.N, Ns);
+        else if (R == 2) xf_pass<2, INV>(a, b, W, pl.N, Ns);
+        else if (R == 3) xf_pass<3, INV>(a, b, W, pl.N, Ns);
+        else xf_pass<5, INV>(a, b, W, pl.N, Ns);
+        Ns *= R;
+        __syncthreads();
+        float2* t = a; a = b; b = t;
+    }
+    return a;                                               // where the result is
+}
+
+__global__ void __launch_bounds__(XF_NT)
+k_xline_influence(XfPlan pl, int K1, int K2h, int K2, const float* __restrict__ tab, float inv_piV,
+                  const float2* __restrict__ Wg, float2* __restrict__ spec, double* __restrict__ e_out)
+{
+    extern __shared__ __align__(16) float2 xf_sh[];         // W[N] | buf A [N][TJ] | buf B [N][TJ]
+    const int N = pl.N;
+    float2* W = xf_sh;
+    float2* A = W + N;
+    float2* B = A + N * XF_TJ;
+    const int nline = K1 * K2h;
+    const int j0 = blockIdx.x * XF_TJ;
+    for (int i = threadIdx.x; i < N; i += XF_NT) W[i] = Wg[i];
+    for (int e = threadIdx.x; e < N * XF_TJ; e += XF_NT) {
+        const int x = e / XF_TJ, tj = e - x * XF_TJ;
+        A[e] = j0 + tj < nline ? spec[(size_t)x * nline + j0 + tj] : make_float2(0.f, 0.f);
+    }
+    __syncthreads();
+    float2* F = xf_transform<false>(A, B, W, pl);
+    float2* O = F == A ? B : A;
+    // influence multiply (Alg. 2 step 3) and the energy, as in k_influence
+    const float* Bg0 = tab;       const float* s0 = Bg0 + N;
+    const float* Bg1 = s0 + N;    const float* s1 = Bg1 + K1;
+    const float* Bg2 = s1 + K1;   const float* s2 = Bg2 + K2;
+    float er = 0.f;
+    static_assert(XF_NT % XF_TJ == 0, "a thread keeps its line");
+    // a thread always meets the same line tj (XF_NT is a multiple of XF_TJ): its (m1, m2) factors once
+    const int tj_ = threadIdx.x % XF_TJ, jl = j0 + tj_;
+    const bool line_on = jl < nline;
+    const int m1 = line_on ? jl / K2h : 0, m2 = line_on ? jl - m1 * K2h : 0;
+    const float bg12 = Bg1[m1] * Bg2[m2] * inv_piV, s12 = s1[m1] + s2[m2];
+    const float w = !line_on ? 0.f : ((m2 == 0 || 2 * m2 == K2) ? 0.5f : 1.0f);
+    for (int e = threadIdx.x; e < N * XF_TJ; e += XF_NT) {
+        const int m0 = e / XF_TJ;
+        float G = 0.f;
+        if (line_on && (m0 | jl)) G = __fdividef(Bg0[m0] * bg12, s0[m0] + s12);
+        float2 z = F[e];
+        er = fmaf(w * G, fmaf(z.x, z.x, z.y * z.y), er);
+        z.x *= G; z.y *= G;
+        F[e] = z;
+    }
+    __syncthreads();
+    float2* R = xf_transform<true>(F, O, W, pl);
+    for (int e = threadIdx.x; e < N * XF_TJ; e += XF_NT) {
+        const int x = e / XF_TJ, tj = e - x * XF_TJ;
+        if (j0 + tj < nline) spec[(size_t)x * nline + j0 + tj] = R[e];
+    }
+    if (e_out) {
+        double e = (double)er;
+        __shared__ double red[XF_NT / 32];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = e;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int k = 0; k < XF_NT / 32; ++k) t += red[k];
+            atomicAdd(e_out, t);
+        }
+    }
+}
+
 // -------------------------------------------------------------------------------------- gather
 // a-8, Alg. 2 step 5: phi_i = sum W Phi;  F_i,x = -q_i (K_x/L_x) sum dW_x Phi.
 // One warp per atom, one (x,y) ROW of P z-contiguous points per lane: per row the z sums
@@ -638,6 +798,37 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
             return sqeq_fail(ctx, SQEQ_ECUFFT, "cufftPlan3d(C2R) failed: %d", (int)r);
         }
         ctx->plans_ok = true;
+        // fused x-axis pass: needs K0 = 2^a 3^b 5^c; then the 3-D transforms become batched 2-D cuFFT transforms over
+        // (y,z) around k_xline_influence
+        if (ctx->xf_ok) { cufftDestroy(ctx->plan2_r2c); cufftDestroy(ctx->plan2_c2r); ctx->xf_ok = false; }
+        {
+            int r = grid[0], np = 0;
+            int radix[XF_MAXPASS];
+            while (r % 4 == 0 && np < XF_MAXPASS) { radix[np++] = 4; r /= 4; }
+            for (int pfac : {2, 3, 5}) while (r % pfac == 0 && np < XF_MAXPASS) { radix[np++] = pfac; r /= pfac; }
+            const size_t sm = sizeof(float2) * ((size_t)grid[0] * (2 * XF_TJ + 1));
+            if (r == 1 && sm <= 200 * 1024) {
+                int nn[2] = {grid[1], grid[2]};
+                const int K2h = grid[2] / 2 + 1;
+                cufftResult r1 = cufftPlanMany(&ctx->plan2_r2c, 2, nn, nullptr, 1, grid[1] * grid[2], nullptr, 1, grid[1] * K2h,
+                                               CUFFT_R2C, grid[0]);
+                cufftResult r2 = r1 == CUFFT_SUCCESS ? cufftPlanMany(&ctx->plan2_c2r, 2, nn, nullptr, 1, grid[1] * K2h, nullptr, 1,
+                                                                     grid[1] * grid[2], CUFFT_C2R, grid[0]) : r1;
+                if (r1 == CUFFT_SUCCESS && r2 != CUFFT_SUCCESS) cufftDestroy(ctx->plan2_r2c);
+                if (r1 == CUFFT_SUCCESS && r2 == CUFFT_SUCCESS) {
+                    ctx->xf_ok = true;
+                    ctx->xf_npass = np;
+                    for (int k = 0; k < np; ++k) ctx->xf_radix[k] = radix[k];
+                    std::vector<float2> W(grid[0]);
+                    for (int m = 0; m < grid[0]; ++m) {
+                        const double a = -2.0 * M_PI * (double)m / (double)grid[0];
+                        W[m] = make_float2((float)cos(a), (float)sin(a));
+                    }
+                    SQEQ_TRY(sqeq_reserve(ctx, ctx->xf_tw, sizeof(float2) * W.size()));
+                    CUDA_TRY(ctx, cudaMemcpy(ctx->xf_tw.p, W.data(), sizeof(float2) * W.size(), cudaMemcpyHostToDevice));
+                }
+            }
+        }
         for (int d = 0; d < 3; ++d) ctx->K[d] = grid[d];
         const size_t G3 = (size_t)grid[0] * grid[1] * grid[2];
         const size_t S3 = (size_t)grid[0] * grid[1] * (grid[2] / 2 + 1);
@@ -795,10 +986,12 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     }
     if (ctx->gridQ.p) SQEQ_TRY(sqeq_reserve(ctx, ctx->gridQ, sizeof(float) * G3));    // the grid may have grown since the capture was enabled
     if (ctx->gridQ.p) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->gridQ.p, grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, st));
+    const bool fused = ctx->xf_ok && !ctx->fft_fused_off;
     {
         StageTimer tm(ctx, SQEQ_T_FFT_FWD, st);
-        cufftSetStream(ctx->plan_r2c, st);
-        cufftResult r = cufftExecR2C(ctx->plan_r2c, grid, (cufftComplex*)spec);
+        cufftHandle plan = fused ? ctx->plan2_r2c : ctx->plan_r2c;
+        cufftSetStream(plan, st);
+        cufftResult r = cufftExecR2C(plan, grid, (cufftComplex*)spec);
         if (r != CUFFT_SUCCESS) return sqeq_fail(ctx, SQEQ_ECUFFT, "cufftExecR2C failed: %d", (int)r);
     }
     {
@@ -806,15 +999,27 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         double* e_out = (double*)ctx->scal.p + 1;
         CUDA_TRY(ctx, cudaMemsetAsync(e_out, 0, sizeof(double), st));
         const float inv_piV = (float)(1.0 / (M_PI * box[0] * box[1] * box[2]));
-        int nb = ceil_div((int64_t)K0 * K1, 8);
-        if (nb > ctx->sm_count * 8) nb = ctx->sm_count * 8;
-        k_influence<<<nb, 256, 0, st>>>(K0, K1, K2h, K2, (const float*)ctx->tabs.p, inv_piV, spec, e_out);
+        if (fused) {
+            // forward x-transform, influence multiply + energy, inverse x-transform: one pass over the spectrum
+            XfPlan pl;
+            pl.N = K0; pl.npass = ctx->xf_npass;
+            for (int k = 0; k < pl.npass; ++k) pl.radix[k] = ctx->xf_radix[k];
+            const size_t sm = sizeof(float2) * ((size_t)K0 * (2 * XF_TJ + 1));
+            CUDA_TRY(ctx, cudaFuncSetAttribute(k_xline_influence, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+            k_xline_influence<<<ceil_div((int64_t)K1 * K2h, XF_TJ), XF_NT, sm, st>>>(pl, K1, K2h, K2, (const float*)ctx->tabs.p, inv_piV,
+                                                                                    (const float2*)ctx->xf_tw.p, spec, e_out);
+        } else {
+            int nb = ceil_div((int64_t)K0 * K1, 8);
+            if (nb > ctx->sm_count * 8) nb = ctx->sm_count * 8;
+            k_influence<<<nb, 256, 0, st>>>(K0, K1, K2h, K2, (const float*)ctx->tabs.p, inv_piV, spec, e_out);
+        }
         KERNEL_CHECK(ctx);
     }
     {
         StageTimer tm(ctx, SQEQ_T_FFT_INV, st);
-        cufftSetStream(ctx->plan_c2r, st);
-        cufftResult r = cufftExecC2R(ctx->plan_c2r, (cufftComplex*)spec, grid);
+        cufftHandle plan = fused ? ctx->plan2_c2r : ctx->plan_c2r;
+        cufftSetStream(plan, st);
+        cufftResult r = cufftExecC2R(plan, (cufftComplex*)spec, grid);
         if (r != CUFFT_SUCCESS) return sqeq_fail(ctx, SQEQ_ECUFFT, "cufftExecC2R failed: %d", (int)r);
     }
     {
