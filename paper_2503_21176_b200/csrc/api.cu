@@ -157,7 +157,7 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     env = getenv("SQEQ_SPREAD_FLOAT");
     ctx->spread_float = env && env[0] == '1';
     env = getenv("SQEQ_OVERLAP");
-    ctx->overlap = env && env[0] == '1';
+    ctx->overlap = env ? atoi(env) : 1;
     env = getenv("SQEQ_REAL_LEAN_BLOCKS");          // persistent real-space blocks per SM beside the side stream
     ctx->real_lean_blocks = env && atoi(env) > 0 ? atoi(env) : 2;
     env = getenv("SQEQ_REAL_STAGED");
@@ -279,7 +279,7 @@ int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
     if (!ctx || !name) return SQEQ_EINVAL;
     CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
     if (!strcmp(name, "graphs")) ctx->graphs = value != 0;
-    else if (!strcmp(name, "overlap")) ctx->overlap = value != 0;
+    else if (!strcmp(name, "overlap")) ctx->overlap = value;
     else if (!strcmp(name, "fft_fused")) ctx->fft_fused_off = value == 0;
     else if (!strcmp(name, "pme_tiles")) { ctx->pme_tiles_off = value == 0; ctx->tile_plan.valid = false; }
     else if (!strcmp(name, "spread_float")) ctx->spread_float = value != 0;
@@ -456,7 +456,10 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
     // them: at cfg 4 the device-side step goes from 0.624 to 0.587 ms, but a single synchronous evaluation
     // (sqeq_coulomb_host) gets slower (0.94 -> 1.02 ms), so it stays an option.  Never
     // with stage timing on, where every event pair brackets one kernel running alone.
-    if (ctx->profiling || !ctx->overlap) {
+    const bool overlap = !ctx->profiling && geom == GEOM_NEW && nl->fmt == 1 &&
+                         (ctx->overlap >= 2 || (ctx->overlap == 1 && ctx->throughput_call));
+    ctx->overlap_now = overlap;
+    if (!overlap) {
         SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream));
         SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, ctx->stream, geom, want_phi));
     } else {
@@ -473,11 +476,26 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
     return SQEQ_OK;
 }
 
+static int coulomb_enqueue_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                                const float* q, const double box[3], double rc, double alpha,
+                                const int grid[3], int order, float* phi, float* force, int want_energy, bool throughput);
+
 extern "C" int sqeq_coulomb_enqueue(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
                                     const float* q, const double box[3], double rc, double alpha,
                                     const int grid[3], int order, float* phi, float* force, int want_energy)
 {
+    return coulomb_enqueue_impl(ctx, nl, n, pos, q, box, rc, alpha, grid, order, phi, force, want_energy, true);
+}
+
+// throughput: the caller does not wait for this evaluation (enqueue / pipelined entries): PME may run on the side
+// stream beside a persistent real-space grid ("overlap" = 1).  A caller that waits (energy returned, host buffers)
+// gets the one-stream schedule, which finishes a single evaluation sooner.
+static int coulomb_enqueue_impl(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
+                                const float* q, const double box[3], double rc, double alpha,
+                                const int grid[3], int order, float* phi, float* force, int want_energy, bool throughput)
+{
     if (!ctx) return SQEQ_EINVAL;
+    ctx->throughput_call = throughput;
     SQEQ_TRY(validate_coulomb_args(ctx, nl, n, box, rc, alpha, grid, order, "sqeq_coulomb"));
     if (!pos || !q) return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb: pos or q is NULL");
     CUDA_TRY(ctx, cudaSetDevice(ctx->device));
@@ -553,7 +571,7 @@ extern "C" int sqeq_coulomb(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, cons
                  const double box[3], double rc, double alpha, const int grid[3], int order,
                  float* phi, float* force, double* energy)
 {
-    SQEQ_TRY(sqeq_coulomb_enqueue(ctx, nl, n, pos, q, box, rc, alpha, grid, order, phi, force, energy != nullptr));
+    SQEQ_TRY(coulomb_enqueue_impl(ctx, nl, n, pos, q, box, rc, alpha, grid, order, phi, force, energy != nullptr, energy == nullptr));
     if (energy) SQEQ_TRY(sqeq_energy_fetch(ctx, energy));
     return SQEQ_OK;
 }
@@ -580,6 +598,7 @@ extern "C" int sqeq_coulomb_host(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n,
     CUDA_TRY(ctx, cudaMemcpyAsync(d_q, q_host, sizeof(float) * n, cudaMemcpyHostToDevice, st));
     SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
     SQEQ_TRY(prep_atoms(ctx, nl, d_pos, d_q, ctx->K, st));
+    ctx->throughput_call = false;
     SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, d_phi, d_f, energy != nullptr));
     if (phi_host) CUDA_TRY(ctx, cudaMemcpyAsync(phi_host, d_phi, sizeof(float) * n, cudaMemcpyDeviceToHost, st));
     if (force_host) CUDA_TRY(ctx, cudaMemcpyAsync(force_host, d_f, sizeof(float) * 3 * n, cudaMemcpyDeviceToHost, st));
@@ -642,6 +661,7 @@ extern "C" int sqeq_coulomb_host_submit(sqeq_ctx* ctx, int slot, const sqeq_nlis
     CUDA_TRY(ctx, cudaStreamWaitEvent(st, ctx->slot_in[slot], 0));
     SQEQ_TRY(pme_setup(ctx, box, alpha, grid, order));
     SQEQ_TRY(prep_atoms(ctx, nl, d_pos, d_q, ctx->K, st));
+    ctx->throughput_call = true;
     SQEQ_TRY(coulomb_eval(ctx, nl, n, box, rc, alpha, d_phi, d_f, want_energy != 0));
     if (want_energy)
         CUDA_TRY(ctx, cudaMemcpyAsync(b[4].p, ctx->scal.p, sizeof(double), cudaMemcpyDeviceToDevice, st));

@@ -55,7 +55,10 @@ struct sqeq_ctx {
     int nl_last_max_pop = 0;
     int64_t nl_last_pairs = 0;
     bool spread_float = false;            // SQEQ_SPREAD_FLOAT=1: fp32 (CAS) instead of fixed-point shared accumulation
-    bool overlap = false;                 // SQEQ_OVERLAP=1: PME on the side stream beside the real-space kernel
+    int overlap = 1;                      // "overlap": 0 never, 1 (default) evaluations nobody waits for, 2 always: PME on
+                                          // the side stream beside a persistent real-space grid
+    bool throughput_call = false;         // set by the entry point: the caller does not wait for this evaluation
+    bool overlap_now = false;             // decision of the evaluation being enqueued (coulomb_eval)
     int real_lean_blocks = 2;             // SQEQ_REAL_LEAN_BLOCKS: persistent real-space blocks per SM with SQEQ_OVERLAP=1
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
 

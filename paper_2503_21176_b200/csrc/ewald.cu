@@ -258,6 +258,7 @@ extern "C" int sqeq_coulomb_ewald(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n
     const bool want_force = force != nullptr;
     SQEQ_TRY(prep_atoms(ctx, nl, pos, q, nullptr, st));
     SQEQ_TRY(ewald_recip_run(ctx, nl, n, pos, box, alpha, kmax, want_force, st));
+    ctx->overlap_now = false;
     SQEQ_TRY(realspace_run(ctx, nl, rc, alpha, want_force, st));
     SQEQ_TRY(assemble_run(ctx, nl, alpha, phi, force, energy != nullptr, false, st));
     ctx->last_had_force = want_force;

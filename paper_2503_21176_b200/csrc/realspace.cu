@@ -542,7 +542,7 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
     if (nl->fmt == 1) {
         const size_t smem = sizeof(float4) * ((size_t)nl->max_pop + 1);
         const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
-        const bool lean = ctx->overlap && !ctx->profiling;
+        const bool lean = ctx->overlap_now;
         GeomCache& gc = ctx->gc;
         RealCache rcache = {(uint16_t*)gc.idx.p, (float*)gc.t.p, (int*)gc.len.p};
         const bool fixed = geom != GEOM_NEW && !lean;

@@ -793,10 +793,10 @@ def test_neighbour_build_resizes_for_clustered_systems(ctx):
 def test_global_list_format_and_side_stream(ctx, monkeypatch):
     """SQEQ_REAL_STAGED=0 keeps the 32-bit (atom | image code) list and the global-gather real-space
     kernel (the path taken when a cell group's neighbourhood does not fit 16 bits / shared memory);
-    SQEQ_OVERLAP=1 runs PME on the side stream.  Same bars as the default path."""
+    SQEQ_OVERLAP=2 runs PME on the side stream for every evaluation.  Same bars as the default path."""
     from paper_2503_21176_b200 import binding
     monkeypatch.setenv("SQEQ_REAL_STAGED", "0")
-    monkeypatch.setenv("SQEQ_OVERLAP", "1")
+    monkeypatch.setenv("SQEQ_OVERLAP", "2")
     c2 = binding.Context(0)
     try:
         for k in (0, 1):
@@ -850,10 +850,11 @@ def test_local_list_layouts(ctx):
 
 @pytest.mark.gpu
 def test_side_stream_with_persistent_real_space(monkeypatch):
-    """SQEQ_OVERLAP=1 with the default 16-bit list: PME runs on the side stream beside a persistent grid of
+    """SQEQ_OVERLAP=2 (every evaluation; the default 1 overlaps only evaluations nobody waits for, which this test
+    covers through coulomb_enqueue below) with the default 16-bit list: PME runs on the side stream beside a persistent grid of
     lean real-space blocks (here one per SM), each walking over several cell groups.  Same bars as the default."""
     from paper_2503_21176_b200 import binding
-    monkeypatch.setenv("SQEQ_OVERLAP", "1")
+    monkeypatch.setenv("SQEQ_OVERLAP", "2")
     monkeypatch.setenv("SQEQ_REAL_LEAN_BLOCKS", "1")      # 148 blocks: at cfg 2 (216 cell groups) some take two
     c2 = binding.Context(0)
     try:
