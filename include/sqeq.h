@@ -339,6 +339,8 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *   "fft_fused"        1  x-axis transforms fused with the influence multiply in one own kernel between batched 2-D
  *                         cuFFT transforms (0, or a grid whose x size has a prime factor above 5: 3-D cuFFT transforms
  *                         and a separate influence kernel)
+ *   "pme_atom_threads" 1  one thread per atom in the tile kernels (a third of the instructions of the lane-group
+ *                         mapping): 0 never, 1 when the grid has at least two tiles per SM, 2 always
  *   "pme_tiles"        1  shared-memory tiles for spreading and gathering (0: global-memory kernels)
  *   "spread_float"     0  fp32 compare-and-swap accumulation in the spreading tile instead of fixed point
  *   "real_staged"      1  16-bit list + shared-memory-staged real-space kernel (0: 32-bit list, global gather;

@@ -162,6 +162,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->real_lean_blocks = env && atoi(env) > 0 ? atoi(env) : 2;
     env = getenv("SQEQ_REAL_STAGED");
     ctx->real_staged_off = env && env[0] == '0';
+    env = getenv("SQEQ_PME_ATOM_THREADS");
+    ctx->pme_atom_threads = env ? atoi(env) : 1;
     env = getenv("SQEQ_FFT_FUSED");
     ctx->fft_fused_off = env && env[0] == '0';
     env = getenv("SQEQ_GRAPHS");
@@ -281,8 +283,9 @@ int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
     if (!strcmp(name, "graphs")) ctx->graphs = value != 0;
     else if (!strcmp(name, "overlap")) ctx->overlap = value;
     else if (!strcmp(name, "fft_fused")) ctx->fft_fused_off = value == 0;
+    else if (!strcmp(name, "pme_atom_threads")) ctx->pme_atom_threads = value;
     else if (!strcmp(name, "pme_tiles")) { ctx->pme_tiles_off = value == 0; ctx->tile_plan.valid = false; }
-    else if (!strcmp(name, "spread_float")) ctx->spread_float = value != 0;
+    else if (!strcmp(name, "spread_float")) { ctx->spread_float = value != 0; ctx->tile_plan.valid = false; }
     else if (!strcmp(name, "real_staged")) ctx->real_staged_off = value == 0;
     else if (!strcmp(name, "real_lean_blocks")) { if (value < 1) return sqeq_fail(ctx, SQEQ_EINVAL, "real_lean_blocks must be >= 1"); ctx->real_lean_blocks = value; }
     else return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_set_option: unknown option '%s'", name);

@@ -75,6 +75,8 @@ struct sqeq_ctx {
     bool fft_fused_off = false;           // SQEQ_FFT_FUSED=0: 3-D cuFFT transforms + separate influence kernel
     int xf_npass = 0, xf_radix[12] = {0};
     DevBuf xf_tw;
+    int pme_atom_threads = 1;             // "pme_atom_threads": one thread per atom in the tile kernels: 0 never (lane
+                                          // groups), 1 when there are at least two tiles per SM, 2 always
     bool pme_tiles_off = false;           // SQEQ_PME_TILES=0: global-memory spread/gather only (testing)
     DevBuf grid;      // float  [K0][K1][K2]        charge grid Q, then potential grid Phi
     DevBuf gridQ;     // float  copy of Q kept for sqeq_pme_grid (diagnostics only when enabled)

@@ -412,6 +412,9 @@ struct TileGeom {
     unsigned nvz_magic;  // ceil(2^32 / (T[2]/4)): i / (T[2]/4) = umulhi(i, nvz_magic) for i < T[0] T[1] T[2]/4
 };
 #define TILE_MAXRANGES 16
+#ifndef PME_ATOM_NT
+#define PME_ATOM_NT 384       // threads per block of the one-thread-per-atom tile kernels
+#endif
 #define TILE_CHUNK(NT) ((NT) / 4)
 // per-atom record (floats): theta_z[8] | dtheta_z[8] | theta_x[P] | theta_y[P] | dtheta_x[P] | dtheta_y[P]
 #define REC_Z 0
@@ -769,6 +772,159 @@ k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
     }
 }
 
+// -------------------------------------------------------------------------------------- one thread per atom
+// The same tiles with ONE THREAD PER ATOM: the thread evaluates its atom's 3 x P spline weights into registers and
+// walks all P^3 points itself.  No per-chunk weight records in shared memory, no barriers between chunks, no idle
+// lanes, no shuffles: a third of the instructions of the lane-group mappings above (216 shared-memory accesses
+// and as many FMAs or atomics per atom are what is left), at the price of fewer threads per block with work.
+template <int P, bool FORCE, int NT>
+__global__ void __launch_bounds__(NT, 2)
+k_gather_atom(const float4* __restrict__ frac, const int4* __restrict__ base, const int* __restrict__ cell_start,
+              TileGeom tg, const float* __restrict__ grid, float sx, float sy, float sz, float4* __restrict__ out)
+{
+    extern __shared__ __align__(16) float tile[];
+    __shared__ int rbeg[TILE_MAXRANGES], rpre[TILE_MAXRANGES + 1];
+    const TileBlock tb = tile_block_setup(tg, cell_start, P, rbeg, rpre);
+    if (tb.natoms == 0) return;
+    tile_move<false>(tile, const_cast<float*>(grid), tb, tg);
+    __syncthreads();
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
+    for (int i = threadIdx.x; i < tb.natoms; i += NT) {
+        const int s = tile_atom(i, rbeg, rpre);
+        const float4 fw = frac[s];
+        const int4 f = base[s];
+        float thx[P], thy[P], thz[P], dx[P], dy[P], dz[P];
+        bspline_weights<P>(fw.x, thx, dx);
+        bspline_weights<P>(fw.y, thy, dy);
+        bspline_weights<P>(fw.z, thz, dz);
+        const int tx = wrap1(f.x - tb.o[0], K0), ty = wrap1(f.y - tb.o[1], K1), tz = wrap1(f.z - tb.o[2], K2);
+        const bool in = tx >= P - 1 && tx < tg.T[0] && ty >= P - 1 && ty < tg.T[1] && tz >= P - 1 && tz < tg.T[2];
+        float ph = 0.f, gx = 0.f, gy = 0.f, gz = 0.f;
+        if (in) {
+            const float* p0 = tile + (tx * tg.XS + ty * tg.ZS + tz);
+#pragma unroll
+            for (int a = 0; a < P; ++a) {
+                float pa = 0.f, gya = 0.f, gza = 0.f;
+#pragma unroll
+                for (int b = 0; b < P; ++b) {
+                    const float* rowp = p0 - a * tg.XS - b * tg.ZS;
+                    float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+                    for (int c = 0; c < P; ++c) {
+                        const float v = rowp[-c];
+                        s0 = fmaf(thz[c], v, s0);
+                        if (FORCE) s1 = fmaf(dz[c], v, s1);
+                    }
+                    pa = fmaf(thy[b], s0, pa);
+                    if (FORCE) { gya = fmaf(dy[b], s0, gya); gza = fmaf(thy[b], s1, gza); }
+                }
+                ph = fmaf(thx[a], pa, ph);
+                if (FORCE) { gx = fmaf(dx[a], pa, gx); gy = fmaf(thx[a], gya, gy); gz = fmaf(thx[a], gza, gz); }
+            }
+        } else {                                            // footprint outside the window: global grid
+            for (int a = 0; a < P; ++a) {
+                int gxi = f.x - a; gxi += gxi < 0 ? K0 : 0;
+                float pa = 0.f, gya = 0.f, gza = 0.f;
+                for (int b = 0; b < P; ++b) {
+                    int gyi = f.y - b; gyi += gyi < 0 ? K1 : 0;
+                    const float* rowp = grid + ((size_t)gxi * K1 + gyi) * K2;
+                    float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+                    for (int c = 0; c < P; ++c) {
+                        int gzi = f.z - c; gzi += gzi < 0 ? K2 : 0;
+                        const float v = __ldg(rowp + gzi);
+                        s0 = fmaf(thz[c], v, s0);
+                        if (FORCE) s1 = fmaf(dz[c], v, s1);
+                    }
+                    pa = fmaf(thy[b], s0, pa);
+                    if (FORCE) { gya = fmaf(dy[b], s0, gya); gza = fmaf(thy[b], s1, gza); }
+                }
+                ph = fmaf(thx[a], pa, ph);
+                if (FORCE) { gx = fmaf(dx[a], pa, gx); gy = fmaf(thx[a], gya, gy); gz = fmaf(thx[a], gza, gz); }
+            }
+        }
+        out[s] = make_float4(-sx * gx, -sy * gy, -sz * gz, ph);         // per unit charge; a-9 applies q_i
+    }
+}
+
+template <int P, int NT>
+__global__ void __launch_bounds__(NT, 2)
+k_spread_atom(const float4* __restrict__ frac, const int4* __restrict__ base, const int* __restrict__ cell_start,
+              TileGeom tg, float* __restrict__ grid)
+{
+    extern __shared__ __align__(16) float tile[];
+    __shared__ int rbeg[TILE_MAXRANGES], rpre[TILE_MAXRANGES + 1];
+    __shared__ float s_part[NT / 32];
+    const TileBlock tb = tile_block_setup(tg, cell_start, P, rbeg, rpre);
+    if (tb.natoms == 0) return;
+    const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
+    const int tsize = tg.XS * tg.T[0];
+    for (int e = threadIdx.x; e < (tsize >> 2); e += NT) ((float4*)tile)[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (threadIdx.x < (tsize & 3)) tile[(tsize & ~3) + threadIdx.x] = 0.f;
+    // fixed-point scale of the block (see k_spread_tile): |tile point| <= (2/3)^3 sum |q|
+    float aq = 0.f;
+    for (int i = threadIdx.x; i < tb.natoms; i += NT) aq += fabsf(frac[tile_atom(i, rbeg, rpre)].w);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) aq += __shfl_xor_sync(0xffffffffu, aq, o);
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = aq;
+    __syncthreads();
+    aq = 0.f;
+#pragma unroll
+    for (int k = 0; k < NT / 32; ++k) aq += s_part[k];
+    const float scale = aq > 0.f ? 1073741824.f / (0.2962963f * aq * 1.0001f) : 1.f;
+    const float inv_scale = 1.f / scale;
+    for (int i = threadIdx.x; i < tb.natoms; i += NT) {
+        const int s = tile_atom(i, rbeg, rpre);
+        const float4 fw = frac[s];
+        const int4 f = base[s];
+        float thx[P], thy[P], thz[P], dd[P];
+        bspline_weights<P>(fw.x, thx, dd);
+        bspline_weights<P>(fw.y, thy, dd);
+        bspline_weights<P>(fw.z, thz, dd);
+        const float qs = fw.w * scale;
+#pragma unroll
+        for (int a = 0; a < P; ++a) thx[a] *= qs;
+        const int tx = wrap1(f.x - tb.o[0], K0), ty = wrap1(f.y - tb.o[1], K1), tz = wrap1(f.z - tb.o[2], K2);
+        const bool in = tx >= P - 1 && tx < tg.T[0] && ty >= P - 1 && ty < tg.T[1] && tz >= P - 1 && tz < tg.T[2];
+        if (in) {
+            int* p0 = (int*)tile + (tx * tg.XS + ty * tg.ZS + tz);
+#pragma unroll
+            for (int a = 0; a < P; ++a)
+#pragma unroll
+                for (int b = 0; b < P; ++b) {
+                    int* rowp = p0 - a * tg.XS - b * tg.ZS;
+                    const float w2 = thx[a] * thy[b];
+                    // error feedback along z: the row's points are the differences of the ROUNDED running sum
+                    float run = 0.f;
+                    int kprev = 0;
+#pragma unroll
+                    for (int c = 0; c < P; ++c) {
+                        run = fmaf(w2, thz[c], run);
+                        const int k = __float2int_rn(run);
+                        atomicAdd(rowp - c, k - kprev);
+                        kprev = k;
+                    }
+                }
+        } else {
+            for (int a = 0; a < P; ++a) {
+                int gxi = f.x - a; gxi += gxi < 0 ? K0 : 0;
+                for (int b = 0; b < P; ++b) {
+                    int gyi = f.y - b; gyi += gyi < 0 ? K1 : 0;
+                    float* rowp = grid + ((size_t)gxi * K1 + gyi) * K2;
+                    const float w2g = thx[a] * thy[b] * inv_scale;
+#pragma unroll
+                    for (int c = 0; c < P; ++c) {
+                        int gzi = f.z - c; gzi += gzi < 0 ? K2 : 0;
+                        atomicAdd(rowp + gzi, w2g * thz[c]);
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    tile_move<true, true>(tile, grid, tb, tg, inv_scale);
+}
+
 // -------------------------------------------------------------------------------------- host side
 static double host_bspline(int n, double u)
 {
@@ -963,6 +1119,9 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         }
     }
     const int ngroups = tiles ? tg.ng[0] * tg.ng[1] * tg.ng[2] : 0;
+    // one thread per atom needs many blocks to hide its long serial chains (measured: faster from cfg 3's 343 tiles
+    // on, slower at cfg 1/2's 64 and 125): lane groups below two tiles per SM
+    const bool atom_threads = ctx->pme_atom_threads == 2 || (ctx->pme_atom_threads == 1 && ngroups >= 2 * ctx->sm_count);
     const int K0 = ctx->K[0], K1 = ctx->K[1], K2 = ctx->K[2], K2h = K2 / 2 + 1;
     const size_t G3 = (size_t)K0 * K1 * K2;
     float* grid = (float*)ctx->grid.p;
@@ -974,7 +1133,11 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     {
         StageTimer tm(ctx, SQEQ_T_SPREAD, st);
         CUDA_TRY(ctx, cudaMemsetAsync(grid, 0, sizeof(float) * G3, st));
-        if (tiles) {
+        if (tiles && atom_threads && !ctx->spread_float) {
+            auto kern = k_spread_atom<P, PME_ATOM_NT>;
+            CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+            kern<<<ngroups, PME_ATOM_NT, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid);
+        } else if (tiles) {
             auto kern = ctx->spread_float ? (nt == 256 ? k_spread_tile<P, 256, false> : k_spread_tile<P, 512, false>)
                                           : (nt == 256 ? k_spread_tile<P, 256, true> : k_spread_tile<P, 512, true>);
             CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
@@ -1026,7 +1189,11 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         StageTimer tm(ctx, SQEQ_T_GATHER, st);
         const float sx = (float)(K0 / box[0]), sy = (float)(K1 / box[1]), sz = (float)(K2 / box[2]);
         float4* rec = (float4*)ctx->rec_out.p;
-        if (tiles) {
+        if (tiles && atom_threads) {
+            auto kern = want_force ? k_gather_atom<P, true, PME_ATOM_NT> : k_gather_atom<P, false, PME_ATOM_NT>;
+            CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
+            kern<<<ngroups, PME_ATOM_NT, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
+        } else if (tiles) {
             auto kern = want_force ? (nt == 256 ? k_gather_tile<P, true, 256> : k_gather_tile<P, true, 512>)
                                    : (nt == 256 ? k_gather_tile<P, false, 256> : k_gather_tile<P, false, 512>);
             CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));

@@ -721,6 +721,44 @@ def test_fixed_geometry_cache(ctx, k):
     nl.free()
 
 
+def test_pme_thread_per_atom_kernels(ctx):
+    """The one-thread-per-atom tile kernels (default from two tiles per SM on, i.e. cfg 3 and cfg 4) forced on for the
+    small configs too, all three spline orders, atoms that left their window, potential-only mode."""
+    from paper_2503_21176_b200 import binding
+    c2 = binding.Context(0)
+    c2.set_option("pme_atom_threads", 2)
+    try:
+        for k in (0, 2):
+            c = W.CONFIGS[k]
+            pos, q = inputs(k)
+            nl = c2.nl_build(dev(pos), c.box, c.r_list)
+            check_coulomb(c2, nl, pos, q, c)
+            nl.free()
+        c = W.CONFIGS[2]
+        pos, q = inputs(2)
+        h = c.L / c.grid
+        nl = c2.nl_build(dev(pos), c.box, c.r_list)
+        moved = (pos.astype(np.float64) + np.array([2.7 * h, -1.6 * h, 0.4 * h])).astype(np.float32)
+        rows = np.sort(np.random.default_rng(3).choice(len(q), 256, replace=False))
+        op, oF, _, _ = oracle.coulomb_pme(moved, q, c.box, c.rc, c.alpha, c.grid, c.order, rows=rows)
+        phi, F, E = c2.coulomb(nl, dev(moved), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
+        assert relrms(phi.cpu().numpy()[rows], op) < TOL and relrms(F.cpu().numpy()[rows], oF) < TOL
+        nl.free()
+        rng = np.random.default_rng(12)
+        n = 4000
+        boxn = np.array([34.0, 39.0, 46.0])
+        p = (rng.uniform(0, 1, (n, 3)) * boxn).astype(np.float32)
+        qq = rng.normal(size=n).astype(np.float32)
+        nl = c2.nl_build(dev(p), boxn, 8.4)
+        for order, grid in ((4, [64, 72, 80]), (8, [48, 56, 64])):
+            phi, F, E = c2.coulomb(nl, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
+            op, oF, oE, _ = oracle.coulomb_pme(p, qq, boxn, 8.0, 0.4, grid, order)
+            assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL
+        nl.free()
+    finally:
+        c2.close()
+
+
 def test_pme_tile_window_fallbacks(ctx, monkeypatch):
     """The shared-memory spread/gather tiles assume an atom stays within one grid spacing of the cell
     it was binned into; beyond that the atom takes the global-memory path inside the same kernels,
