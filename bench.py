@@ -727,6 +727,15 @@ def main():
     ap.add_argument("--table-steps", type=int, default=200)
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]
+    if args.gpus > 1 and "RANK" not in os.environ:
+        # started without a launcher: start the N ranks ourselves (one replica per GPU)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

@@ -65,8 +65,9 @@ const char* sqeq_version(void);
  * Internally: atoms are wrapped, binned into cells of edge >= cutoff/2, reordered cell-major; the
  * list is directed rows over the reordered atoms, entries either 16-bit indices into the neighbourhood
  * of the atom's 2x2x2 cell group or 32-bit (atom index | 27-valued image code).  Synchronises the
- * stream (the pair count sizes the list allocation).  SQEQ_ECAPACITY if an atom has more than 6528
- * neighbours. */
+ * stream (the pair count sizes the list allocation).  SQEQ_ECAPACITY if an atom has more neighbours
+ * than the per-warp staging rows in shared memory hold (about 12,700 in the 16-bit format, 6,300 in the 32-bit
+ * one). */
 int  sqeq_nl_build (sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3],
                     double cutoff, sqeq_nlist** out);
 /* Number of unique (i<j) pairs in the list.  host int64 out. */
