@@ -340,6 +340,9 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *   "fft_fused"        1  x-axis transforms fused with the influence multiply in one own kernel between batched 2-D
  *                         cuFFT transforms (0, or a grid whose x size has a prime factor above 5: 3-D cuFFT transforms
  *                         and a separate influence kernel)
+ *   "real_tma"         0  geometry-cache rows streamed into shared memory by the bulk-copy engine (cp.async.bulk +
+ *                         mbarrier, two rows in flight per warp) instead of per-lane vector loads; 4 % slower at
+ *                         331,776 atoms (0.151 vs 0.145 ms), kept as the measured alternative
  *   "pme_atom_threads" 1  one thread per atom in the tile kernels (a third of the instructions of the lane-group
  *                         mapping): 0 never, 1 when the grid has at least two tiles per SM, 2 always
  *   "pme_tiles"        1  shared-memory tiles for spreading and gathering (0: global-memory kernels)

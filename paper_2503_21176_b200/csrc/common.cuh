@@ -60,6 +60,8 @@ struct sqeq_ctx {
     bool throughput_call = false;         // set by the entry point: the caller does not wait for this evaluation
     bool overlap_now = false;             // decision of the evaluation being enqueued (coulomb_eval)
     int real_lean_blocks = 2;             // SQEQ_REAL_LEAN_BLOCKS: persistent real-space blocks per SM with SQEQ_OVERLAP=1
+    bool real_tma = false;                // "real_tma": geometry-cache rows streamed with cp.async.bulk + mbarrier (measured
+                                          // 4 % slower than per-lane vector loads at cfg 4: an option)
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
 
     // ---- PME state (cached by grid/order/box/alpha) ----

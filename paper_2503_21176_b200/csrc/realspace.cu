@@ -523,6 +523,156 @@ k_real_cached(const float4* __restrict__ xq, const int* __restrict__ cell_start,
     }   // row batches
 }
 
+// The same sparse product with the rows STREAMED BY THE BULK-COPY ENGINE (TMA 1-D, cp.async.bulk + mbarrier): one
+// lane of a warp asks for a whole row -- its compact entries and their t, two contiguous 16-byte-aligned stretches of
+// the cache -- to be copied into the warp's shared-memory buffer, and the copy of the NEXT row is in flight while the
+// warp sums the current one (two buffers and two mbarriers per warp).  The lanes then read entries and values from
+// shared memory with conflict-free vector loads: no per-lane global loads, predicates or address arithmetic, and the
+// bytes in flight do not depend on registers.  Rows longer than the buffer (RCAP entries) take the kernel above.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned phase)
+{
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(phase) : "memory");
+    } while (!ok);
+}
+
+template <bool SCALED, int RCAP>
+__global__ void __launch_bounds__(REAL_NT, 2)
+k_real_cached_tma(const float4* __restrict__ xq, const int* __restrict__ cell_start, GroupGeom gg,
+                  const int64_t* __restrict__ row_start, RealParams p, int ngroups, float4* __restrict__ out,
+                  RealCache rcache)
+{
+    constexpr int NW = REAL_NT / 32;
+    constexpr int BUFB = RCAP * 6;                              // t [RCAP] fp32, then entries [RCAP] u16
+    extern __shared__ __align__(128) unsigned char smem_tma[];  // NW x 2 buffers | charges [pop + 1]
+    __shared__ __align__(8) unsigned long long bars[NW][2];
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    float* qs = (float*)(smem_tma + (size_t)NW * 2 * BUFB);
+    const int grp = blockIdx.x;
+    const GroupInfo gi = group_layout(gg, cell_start, grp, pieces, &s_scratch);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int r = 0; r < GRP_G * GRP_G; ++r) {
+            s_rpre[r] = acc;
+            const int ix = r / GRP_G, iy = r % GRP_G;
+            if (ix < gi.ge[0] && iy < gi.ge[1]) {
+                const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+                const int beg = cell_start[colw];
+                s_roff[r] = beg - acc;
+                acc += cell_start[colw + gi.ge[2]] - beg;
+            } else {
+                s_roff[r] = 0;
+            }
+        }
+        s_rpre[GRP_G * GRP_G] = acc;
+        qs[gi.pop] = 0.f;
+    }
+    if (lane == 0) {
+        mbar_init(smem_u32(&bars[wid][0]), 1);
+        mbar_init(smem_u32(&bars[wid][1]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    const int np = gi.ncol * 3;
+    for (int ip = wid; ip < np; ip += NW) {
+        const GroupPiece pc = pieces[ip];
+        for (int k = lane; k < pc.len; k += 32) qs[pc.lbase + k] = __ldg(&xq[pc.gbeg + k].w);
+    }
+    __syncthreads();
+    const int natoms = s_rpre[GRP_G * GRP_G];
+    const int p1 = s_rpre[1], p2 = s_rpre[2], p3 = s_rpre[3];
+    const unsigned qs_addr = smem_u32(qs);
+    unsigned char* mybuf = smem_tma + (size_t)wid * 2 * BUFB;
+    unsigned phase0 = 0, phase1 = 0;
+    for (int base = 0; base < natoms; base += NW * 32) {
+        // lane l holds the row offset and length of the l-th row this warp will take
+        int my_s = 0, my_len = 0;
+        int64_t my_r0 = 0;
+        {
+            const int ia = base + wid + NW * lane;
+            if (ia < natoms) {
+                my_s = ia + s_roff[(ia >= p1) + (ia >= p2) + (ia >= p3)];
+                my_r0 = row_start[my_s];
+                my_len = rcache.len[my_s];
+            }
+        }
+        int nrows = (natoms - base - wid + NW - 1) / NW;
+        nrows = nrows < 0 ? 0 : (nrows > 32 ? 32 : nrows);
+        auto issue = [&](int l) {                               // all lanes call; lane 0 issues
+            const int64_t r0 = __shfl_sync(0xffffffffu, my_r0, l);
+            const int pl = (__shfl_sync(0xffffffffu, my_len, l) + 31) & ~31;
+            if (lane == 0 && pl > 0 && pl <= RCAP) {
+                const unsigned bar = smem_u32(&bars[wid][l & 1]);
+                const unsigned dst = smem_u32(mybuf + (size_t)(l & 1) * BUFB);
+                mbar_expect_tx(bar, (unsigned)pl * 6u);
+                bulk_g2s(dst, rcache.t + r0, (unsigned)pl * 4u, bar);
+                bulk_g2s(dst + RCAP * 4, rcache.idx + r0, (unsigned)pl * 2u, bar);
+            }
+        };
+        if (nrows > 0) issue(0);
+        for (int l = 0; l < nrows; ++l) {
+            if (l + 1 < nrows) issue(l + 1);
+            const int s = __shfl_sync(0xffffffffu, my_s, l);
+            const int len_s = __shfl_sync(0xffffffffu, my_len, l);
+            const int padlen = (len_s + 31) & ~31;
+            float a3 = 0.f;
+            auto term = [&](unsigned e, float v) {
+                float qj;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(qj) : "r"(qs_addr + (SCALED ? e >> 2 : e << 2)));
+                a3 = fmaf(qj, v, a3);
+            };
+            if (padlen > 0 && padlen <= RCAP) {
+                const unsigned bar = smem_u32(&bars[wid][l & 1]);
+                mbar_wait(bar, (l & 1) ? phase1 : phase0);
+                if (l & 1) phase1 ^= 1; else phase0 ^= 1;
+                const float4* tv = (const float4*)(mybuf + (size_t)(l & 1) * BUFB);
+                const uint2* ev = (const uint2*)(mybuf + (size_t)(l & 1) * BUFB + RCAP * 4);
+                for (int c = 4 * lane; c < padlen; c += 128) {
+                    const float4 v = tv[c >> 2];
+                    const uint2 e = ev[c >> 2];
+                    term(e.x & 0xffffu, v.x);
+                    term(e.x >> 16, v.y);
+                    term(e.y & 0xffffu, v.z);
+                    term(e.y >> 16, v.w);
+                }
+                // the buffer is written again by the copy engine two rows on: order these reads before it
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+            } else if (padlen > 0) {                            // a row longer than the buffer: straight from global
+                const int64_t r0 = __shfl_sync(0xffffffffu, my_r0, l);
+                for (int c = 4 * lane; c < padlen; c += 128) {
+                    const float4 v = __ldg((const float4*)(rcache.t + r0 + c));
+                    const uint2 e = __ldg((const uint2*)(rcache.idx + r0 + c));
+                    term(e.x & 0xffffu, v.x);
+                    term(e.x >> 16, v.y);
+                    term(e.y & 0xffffu, v.z);
+                    term(e.y >> 16, v.w);
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a3 += __shfl_xor_sync(0xffffffffu, a3, o);
+            if (lane == 0) out[s] = make_float4(0.f, 0.f, 0.f, a3);
+        }
+    }
+}
+
 // geom: GEOM_NEW = plain evaluation; GEOM_BUILD = plain evaluation that also writes the geometry cache (t, and g
 // when want_force); GEOM_REUSE_PHI / GEOM_REUSE_FIELD = potential / field from the cache.  The cache belongs to
 // (list, positions of the last prep_atoms, rc, alpha); the drivers that keep the geometry fixed ask for it.
@@ -552,6 +702,17 @@ int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, 
         if (hit && !want_force) {
             // NEXT-1: the potential as a sparse product over the cached t
             const size_t sm = sizeof(float) * ((size_t)nl->max_pop + 1);
+            constexpr int RCAP = 512;
+            const size_t sm_tma = (size_t)(REAL_NT / 32) * 2 * RCAP * 6 + sm + 128;
+            if (ctx->real_tma && nl->max_row <= RCAP && sm_tma <= 113 * 1024) {
+                // rows streamed by the bulk-copy engine (two 111 KB blocks per SM)
+                auto kern = nl->lshift ? k_real_cached_tma<true, RCAP> : k_real_cached_tma<false, RCAP>;
+                CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_tma));
+                kern<<<ngroups, REAL_NT, sm_tma, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, p, ngroups,
+                                                       (float4*)ctx->real_out.p, rcache);
+                KERNEL_CHECK(ctx);
+                return SQEQ_OK;
+            }
             auto kern = nl->lshift ? k_real_cached<0, true> : k_real_cached<0, false>;
             CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
             kern<<<ngroups, REAL_NT, sm, st>>>((const float4*)ctx->xq.p, nl->cell_start, nl->gg, nl->row_start, p, ngroups,

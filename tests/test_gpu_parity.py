@@ -709,6 +709,17 @@ def test_fixed_geometry_cache(ctx, k):
                 e_F = relrms(F.cpu().numpy()[sel], oF)
                 assert e_F < TOL, e_F
     record(f"fixed_geometry_cfg{k}", relrms_phi_last=e_phi, relrms_F_last=e_F)
+    # the same potentials with the cache rows streamed by the bulk-copy engine ("real_tma"): identical sums
+    ctx.geometry_set(nl, dev(p), c.box, c.rc, c.alpha, c.grid, c.order)
+    pa, pb = torch.empty(n, device="cuda"), torch.empty(n, device="cuda")
+    ctx.coulomb_fixed(dev(vecs[1]), pa)
+    ctx.coulomb_fixed(dev(vecs[1]), pa)
+    ctx.set_option("real_tma", 1)
+    try:
+        ctx.coulomb_fixed(dev(vecs[1]), pb)
+    finally:
+        ctx.set_option("real_tma", 0)
+    assert relrms(pb.cpu().numpy(), pa.cpu().numpy()) < 1e-6
     # a plain evaluation or a build replaces the prepared geometry: coulomb_fixed must refuse, not reuse stale data
     ctx.coulomb(nl, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
     with pytest.raises(SqeqError):
