@@ -136,7 +136,8 @@ struct sqeq_ctx {
     int64_t launches = 0;
 
     // CUDA graphs of launch-bound sequences (sqeq_coulomb_fixed, the shadow-MD step): slot 0 / 1
-    struct GraphSlot { uint64_t key = 0; cudaGraphExec_t exec = nullptr; int64_t nlaunch = 0; } gslot[2];
+    struct GraphSlot { uint64_t key = 0; cudaGraphExec_t exec = nullptr; int64_t nlaunch = 0; uint64_t used = 0; } gslot[2 + 12];
+    uint64_t gclock = 0;                  // slots 2..13: plain evaluations of small systems, least recently used replaced
     bool graphs = true;                   // SQEQ_GRAPHS=0 / sqeq_set_option("graphs", 0): always launch kernel by kernel
 
     // live neighbour lists of this context: sqeq_destroy releases their device storage and detaches them, so a

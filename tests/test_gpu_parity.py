@@ -482,6 +482,20 @@ def test_cuda_graph_replay_matches_plain_launches():
                 cx.coulomb_fixed(qa, phi, None)
             torch.cuda.synchronize()
             outs.append(phi.cpu().numpy().copy())
+            # plain evaluations of a small system are graphs too: same arrays, updated in place between calls
+            phi2, F2 = torch.empty(n, device="cuda"), torch.empty((n, 3), device="cuda")
+            xs = dev(pos)
+            torch.cuda.synchronize()
+            for rep in range(4):
+                cx.coulomb_enqueue(nl, xs, qa, c.box, c.rc, c.alpha, c.grid, c.order, phi2, F2, want_energy=True)
+                E2 = cx.energy_fetch()
+                if rep == 1:
+                    outs.append(phi2.cpu().numpy().copy())
+                    outs.append(F2.cpu().numpy().copy())
+                    xs.copy_(x2)                      # move the atoms: later replays must see the new positions
+                    torch.cuda.synchronize()
+            outs.append(phi2.cpu().numpy().copy())
+            outs.append(np.array([E2]))
             res[graphs] = (outs, per_eval, E)
             nl.free()
         finally:
@@ -490,8 +504,11 @@ def test_cuda_graph_replay_matches_plain_launches():
     for a, b in zip(res[1][0], res[0][0]):
         assert relrms(a, b) < 2e-6                              # only the order of atomic tile flushes differs
     assert abs(res[1][2] / res[0][2] - 1) < 1e-6
-    op, _, _, _ = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order)
+    op, oF, _, _ = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order)
     assert relrms(res[1][0][2], op) < TOL and relrms(res[1][0][0], op) < TOL
+    assert relrms(res[1][0][-4], op) < TOL and relrms(res[1][0][-3], oF) < TOL         # replayed plain evaluation
+    op2, _, oE2, _ = oracle.coulomb_pme(W.perturb(pos, 0, 0.02, 0), q, c.box, c.rc, c.alpha, c.grid, c.order)
+    assert relrms(res[1][0][-2], op2) < TOL and abs(res[1][0][-1][0] / oE2 - 1) < TOL  # ... after the atoms moved
 
 
 @pytest.mark.parametrize("own_stream", [False, True])
