@@ -265,6 +265,35 @@ def test_ewald_truncated_is_direct_ewald_with_given_cutoffs():
     assert np.abs(p3 - p2).max() < 1e-9
 
 
+def test_cpu_method_baseline_matches_the_oracle():
+    """bench.py's second CPU baseline (oracle/cpu_method: cell list + list sums + FFT PME) is a restatement of the
+    method, not the oracle: pin it AGAINST the oracle -- same pair set, same potentials and forces to fp64 rounding,
+    also on a stale list with a skin."""
+    from oracle.cpu_method import CpuMethod
+    c = W.CONFIGS[1]
+    pos, q = W.make(1)
+    cm = CpuMethod(c.box, c.rc, c.alpha, c.grid, c.order, c.rc + 1.0)
+    npairs = cm.build_list(pos)
+    oi, oj, os_ = oracle.neighbour_list(pos, c.box, c.rc + 1.0)
+    gi, gj, gs = cm.pairs()
+    assert npairs == len(oi) and np.array_equal(gi, oi) and np.array_equal(gj, oj) and np.array_equal(gs, os_)
+    moved = W.perturb(pos, 0, 0.02, 1)
+    phi, F, E = cm.coulomb(moved, q)
+    op, oF, oE, _ = oracle.coulomb_pme(moved, q, c.box, c.rc, c.alpha, c.grid, c.order)
+    assert np.abs(phi - op).max() < 1e-10 * np.abs(op).max() and np.abs(F - oF).max() < 1e-9 * np.abs(oF).max()
+    assert abs(E / oE - 1) < 1e-11
+    # unwrapped positions, non-cubic box, another order
+    rng = np.random.default_rng(4)
+    box = np.array([31.0, 34.0, 38.0])
+    p = rng.uniform(0, 1, (900, 3)) * box + rng.integers(-2, 3, (900, 3)) * box
+    qq = rng.normal(size=900)
+    cm = CpuMethod(box, 8.0, 0.4, [32, 36, 40], 4, 8.5)
+    cm.build_list(p)
+    phi, F, E = cm.coulomb(p, qq)
+    op, oF, oE, _ = oracle.coulomb_pme(p, qq, box, 8.0, 0.4, [32, 36, 40], 4)
+    assert np.abs(phi - op).max() < 1e-10 * np.abs(op).max() and np.abs(F - oF).max() < 1e-9 * np.abs(oF).max()
+
+
 def test_neighbour_rows_upper_is_a_slice_of_the_list():
     """The chunked walk used by the full-size GPU list tests returns exactly rows i0..i1 of the list
     (also when the first capacity guess is too small)."""
