@@ -174,6 +174,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->real_staged_off = env && env[0] == '0';
     env = getenv("SQEQ_PME_ATOM_THREADS");
     ctx->pme_atom_threads = env ? atoi(env) : 1;
+    env = getenv("SQEQ_PAIRS_STAGED");
+    ctx->pairs_staged_off = env && env[0] == '0';
     env = getenv("SQEQ_REAL_TMA");
     ctx->real_tma = env && env[0] == '1';
     env = getenv("SQEQ_FFT_FUSED");
@@ -296,6 +298,7 @@ int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
     else if (!strcmp(name, "overlap")) ctx->overlap = value;
     else if (!strcmp(name, "fft_fused")) ctx->fft_fused_off = value == 0;
     else if (!strcmp(name, "real_tma")) ctx->real_tma = value != 0;
+    else if (!strcmp(name, "pairs_staged")) ctx->pairs_staged_off = value == 0;
     else if (!strcmp(name, "pme_atom_threads")) ctx->pme_atom_threads = value;
     else if (!strcmp(name, "pme_tiles")) { ctx->pme_tiles_off = value == 0; ctx->tile_plan.valid = false; }
     else if (!strcmp(name, "spread_float")) { ctx->spread_float = value != 0; ctx->tile_plan.valid = false; }

@@ -62,6 +62,7 @@ struct sqeq_ctx {
     int real_lean_blocks = 2;             // SQEQ_REAL_LEAN_BLOCKS: persistent real-space blocks per SM with SQEQ_OVERLAP=1
     bool real_tma = false;                // "real_tma": geometry-cache rows streamed with cp.async.bulk + mbarrier (measured
                                           // 4 % slower than per-lane vector loads at cfg 4: an option)
+    bool pairs_staged_off = false;        // "pairs_staged" = 0: always the segment-sweep pair kernel (k_pairs)
     bool real_staged_off = false;         // SQEQ_REAL_STAGED=0: 32-bit list + global-gather real-space kernel
 
     // ---- PME state (cached by grid/order/box/alpha) ----

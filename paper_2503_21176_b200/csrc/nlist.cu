@@ -250,6 +250,8 @@ struct NLCounters {
     unsigned long long pairs;      // directed pairs
     int max_row;
     int max_pop;
+    int stage_overflow;            // k_pairs_staged: a neighbourhood did not fit the shared memory it was launched with
+    int pad_;
     NLExact ex;
 };
 
@@ -536,6 +538,214 @@ k_pairs(const float4* __restrict__ xq, const int* __restrict__ cell_of,
     }
 }
 
+// The same enumeration with the group's neighbourhood STAGED IN SHARED MEMORY (as the real-space kernel stages it: every
+// run copied with its image shift added), used once a build of the same system has told how large neighbourhoods get.
+// A warp takes one atom of the group at a time; lanes test which of the neighbourhood's (x,y) COLUMNS can reach the
+// cutoff sphere; the surviving columns of one x-row are neighbours in the staged order, so the warp sweeps at most
+// (g + 2w) contiguous stretches of the staged array, 32 candidates per step, with conflict-free 16-byte shared loads: no
+// per-candidate global load, no segment records, no index arithmetic beyond an add -- half the instructions of k_pairs
+// per candidate step and 15 % more candidates (whole columns instead of chords).  The local index a candidate is
+// stored under IS its position in the staged array.  Everything after the sweep (guard band settled by the exact
+// fp64 predicate, padding, reservation, copy-out) is k_pairs' code.
+#define NLS_WARPS 16
+#ifndef NLS_BPS
+#define NLS_BPS 2
+#endif
+__global__ void __launch_bounds__(NLS_WARPS * 32, NLS_BPS)
+k_pairs_staged(const float4* __restrict__ xq, const int* __restrict__ cell_of, const int* __restrict__ cell_start,
+               const int* __restrict__ perm, const float* __restrict__ pos, NLGeom g, GroupGeom gg, int cap_row, int lshift,
+               int est_row, int stage_cap, unsigned long long capacity, NLCounters* __restrict__ ctr,
+               int64_t* __restrict__ row_start, int* __restrict__ row_len, longlong2* __restrict__ grp_slice,
+               uint16_t* __restrict__ nbr_out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float4* xs = (float4*)smem_raw;                                                   // [stage_cap + 33] (32 of slack)
+    uint16_t* stage_all = (uint16_t*)(xs + stage_cap + 33);                           // [NLS_WARPS][cap_row]
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_colbeg[GRP_MAXCOL + 1];
+    __shared__ int s_scratch, s_rbeg[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    __shared__ unsigned long long s_base, s_pairs;
+    __shared__ int s_used, s_res, s_maxrow;
+    const GroupInfo gi = group_layout(gg, cell_start, blockIdx.x, pieces, &s_scratch);
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int r = 0; r < GRP_G * GRP_G; ++r) {
+            s_rpre[r] = acc;
+            const int ix = r / GRP_G, iy = r % GRP_G;
+            if (ix < gi.ge[0] && iy < gi.ge[1]) {
+                const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+                const int beg = cell_start[colw];
+                s_rbeg[r] = beg;
+                acc += cell_start[colw + gi.ge[2]] - beg;
+            } else {
+                s_rbeg[r] = 0;
+            }
+        }
+        s_rpre[GRP_G * GRP_G] = acc;
+        atomicMax(&ctr->max_pop, gi.pop);
+        if (gi.pop > stage_cap) atomicExch(&ctr->stage_overflow, 1);
+        s_res = gi.pop > stage_cap ? 0 : acc * est_row;
+        s_base = s_res > 0 ? atomicAdd(&ctr->cursor, (unsigned long long)s_res) : 0ull;
+        s_used = 0;
+        s_maxrow = 0;
+        s_pairs = 0ull;
+    }
+    // staged start of every column (its three image runs are consecutive in the staged order)
+    if (threadIdx.x <= gi.ncol) s_colbeg[threadIdx.x] = threadIdx.x < gi.ncol ? pieces[threadIdx.x * 3].lbase : gi.pop;
+    if (gi.pop > stage_cap) {                       // the host re-runs the build with k_pairs
+        if (threadIdx.x == 0) grp_slice[blockIdx.x] = make_longlong2(0, 0);
+        return;
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int np_grp = gi.ncol * 3;
+    for (int ip = wid; ip < np_grp; ip += NLS_WARPS) {
+        const GroupPiece pc = pieces[ip];
+        if (pc.len == 0) continue;
+        const float sx = (pc.code / 9 - 1) * g.Lf[0], sy = ((pc.code / 3) % 3 - 1) * g.Lf[1], sz = (pc.code % 3 - 1) * g.Lf[2];
+        for (int k = lane; k < pc.len; k += 32) {
+            float4 v = __ldg(xq + pc.gbeg + k);
+            v.x += sx; v.y += sy; v.z += sz;
+            xs[pc.lbase + k] = v;
+        }
+    }
+    __syncthreads();
+    const int natoms = s_rpre[GRP_G * GRP_G];
+    uint16_t* stage = stage_all + (size_t)wid * cap_row;
+    const unsigned lt = (1u << lane) - 1u;
+    const float hi_thr = g.rl2f + g.band, lo_thr = g.rl2f - g.band;
+    const unsigned xs_addr = (unsigned)__cvta_generic_to_shared(xs);
+    const int ncolx = gi.ncol / gi.ncoly;
+
+    for (int ia = wid; ia < natoms; ia += NLS_WARPS) {
+        int r = 0;
+#pragma unroll
+        for (int k = 1; k < GRP_G * GRP_G; ++k) r += (ia >= s_rpre[k]);
+        const int s = s_rbeg[r] + (ia - s_rpre[r]);
+        const float4 xi = xq[s];
+        const int c = cell_of[s];
+        const int cx = c & 1023, cy = (c >> 10) & 1023;
+        // the atom's own place in the staged array: its column of the group, zero-image run
+        int self_local;
+        {
+            const int col = (cx - (gi.c0[0] - gg.w[0])) * gi.ncoly + (cy - (gi.c0[1] - gg.w[1]));
+            const GroupPiece pc = pieces[col * 3 + 1];
+            self_local = s + pc.lbase - pc.gbeg;
+        }
+        // lane <-> x-row of columns (<= 6): the y-interval of columns whose rectangle is within reach
+        int rb = 0, re = 0;                       // staged stretch [rb, re) of this lane's x-row
+        if (lane < ncolx) {
+            const int ux = gi.c0[0] - gg.w[0] + lane;
+            float dxm = fmaxf(fmaxf((float)ux * g.a[0] - xi.x, xi.x - (float)(ux + 1) * g.a[0]) - g.marg, 0.f);
+            if (ux == cx) dxm = 0.f;
+            const float rem = hi_thr - dxm * dxm;
+            if (rem > 0.f && abs(ux - cx) <= gg.w[0]) {
+                const float yr = sqrtf(rem) + g.marg;
+                int ylo = (int)floorf((xi.y - yr) * g.inva[1]), yhi = (int)floorf((xi.y + yr) * g.inva[1]);
+                ylo = max(ylo, cy - gg.w[1]); ylo = min(ylo, cy);
+                yhi = min(yhi, cy + gg.w[1]); yhi = max(yhi, cy);
+                const int y0 = gi.c0[1] - gg.w[1];
+                rb = s_colbeg[lane * gi.ncoly + (ylo - y0)];
+                re = s_colbeg[lane * gi.ncoly + (yhi - y0) + 1];
+            }
+        }
+        int count = 0;
+        float r2max = 0.f;                         // largest accepted r2: tells whether anything fell into the guard band
+        const unsigned self_addr = xs_addr + ((unsigned)self_local << 4);
+        for (int xr = 0; xr < ncolx; ++xr) {
+            const int beg = __shfl_sync(0xffffffffu, rb, xr), end = __shfl_sync(0xffffffffu, re, xr);
+            // the lane's candidate by its shared-memory address (one add per step); the staged array has 32 slots of
+            // slack behind it, so the last step of a stretch reads past `end` unclamped and is masked
+            unsigned a = xs_addr + ((unsigned)(beg + lane) << 4);
+            const unsigned a_end = xs_addr + ((unsigned)end << 4);
+#pragma unroll 2
+            for (int k0 = beg; k0 < end; k0 += 32, a += 512u) {
+                float4 v;
+                asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+                const float dx = v.x - xi.x, dy = v.y - xi.y, dz = v.z - xi.z;
+                const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                const bool ok = r2 < hi_thr && a < a_end && a != self_addr;
+                r2max = fmaxf(r2max, ok ? r2 : 0.f);
+                const unsigned m = __ballot_sync(0xffffffffu, ok);
+                const int at = min(count + __popc(m & lt), cap_row - 1);   // an overflowing row is re-run anyway
+                if (ok) stage[at] = (uint16_t)((a - xs_addr) >> 4);
+                count += __popc(m);
+            }
+        }
+        const bool band_seen = r2max >= lo_thr;
+        __syncwarp();
+        // guard band (rare): re-decide the staged candidates inside it with the exact fp64 predicate on the raw
+        // caller positions, and compact the staging row in place
+        if (__any_sync(0xffffffffu, band_seen) && count <= cap_row) {
+            const int oi = perm[s];
+            int kept = 0;
+            for (int k0 = 0; k0 < count; k0 += 32) {
+                const int k = k0 + lane;
+                bool ok = k < count;
+                uint16_t e = 0;
+                if (ok) {
+                    e = stage[k];
+                    const float4 v = xs[e];
+                    const float dx = v.x - xi.x, dy = v.y - xi.y, dz = v.z - xi.z;
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));     // same expression as in the sweep
+                    if (r2 >= lo_thr) {
+                        int lo = 0, hi = np_grp - 1;                          // local index -> run -> atom
+                        while (lo < hi) {
+                            const int mid = (lo + hi + 1) >> 1;
+                            if (pieces[mid].lbase <= (int)e) lo = mid; else hi = mid - 1;
+                        }
+                        const int t = pieces[lo].gbeg + ((int)e - pieces[lo].lbase);
+                        ok = exact_in_range(pos, oi, perm[t], &ctr->ex);
+                    }
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, ok);
+                __syncwarp();
+                if (ok) stage[kept + __popc(m & lt)] = e;
+                __syncwarp();
+                kept += __popc(m);
+            }
+            count = kept;
+        }
+        __syncwarp();
+        // reserve and copy out (as in k_pairs)
+        const int padn = (count + 31) & ~31;
+        unsigned long long off = 0;
+        if (lane == 0) {
+            const int old = atomicAdd(&s_used, padn);
+            off = old + padn <= s_res ? s_base + (unsigned long long)old
+                                      : atomicAdd(&ctr->cursor, (unsigned long long)padn);
+            atomicAdd(&s_pairs, (unsigned long long)count);
+            atomicMax(&s_maxrow, count);
+            row_start[s] = (int64_t)off;
+            row_len[s] = count;
+        }
+        off = __shfl_sync(0xffffffffu, off, 0);
+        if (count <= cap_row && off + (unsigned long long)padn <= capacity) {
+            if (count + lane < padn) stage[count + lane] = (uint16_t)gi.pop;
+            __syncwarp();
+            const uint32_t keep = lshift ? 0x0fff0fffu : 0xffffffffu;
+            const uint2* src = (const uint2*)stage;
+            uint2* dst = (uint2*)(nbr_out + off);
+            for (int k = lane; 4 * k < padn; k += 32) {
+                uint2 w = src[k];
+                w.x = (w.x & keep) << lshift;
+                w.y = (w.y & keep) << lshift;
+                dst[k] = w;
+            }
+        } else if (lane == 0) {
+            row_len[s] = 0;                        // never leave a row that points outside the allocation
+        }
+        __syncwarp();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (natoms > 0) {
+            atomicAdd(&ctr->pairs, s_pairs);
+            atomicMax(&ctr->max_row, s_maxrow);
+        }
+        grp_slice[blockIdx.x] = make_longlong2((long long)s_base, (long long)min(s_used, s_res));
+    }
+}
+
 // Expands a 16-bit local list to 32-bit entries j | image code << 27 with the same row offsets (used by
 // the canonical export only): one block per group, binary search of each entry in the piece table.
 __global__ void __launch_bounds__(256)
@@ -813,10 +1023,21 @@ static size_t pairs_smem(int cap_row, bool local)
 }
 
 static int launch_pairs(sqeq_ctx* ctx, sqeq_nlist* nl, const float* pos, const NLGeom& g, bool local,
-                        int lshift, int est_row, int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st)
+                        int lshift, int est_row, int cap_row, size_t capacity, NLCounters* ctr, cudaStream_t st,
+                        int stage_cap)
 {
     const size_t smem = pairs_smem(cap_row, local);
     const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
+    if (local && stage_cap > 0) {
+        // neighbourhoods of known size: candidates from shared memory
+        const size_t sm = sizeof(float4) * ((size_t)stage_cap + 33) + (size_t)NLS_WARPS * cap_row * sizeof(uint16_t);
+        CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs_staged, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+        k_pairs_staged<<<ngroups, NLS_WARPS * 32, sm, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start, nl->perm, pos, g,
+            nl->gg, cap_row, lshift, est_row, stage_cap, (unsigned long long)capacity, ctr, nl->row_start, nl->row_len, nl->grp_slice,
+            (uint16_t*)nl->nbr);
+        KERNEL_CHECK(ctx);
+        return SQEQ_OK;
+    }
     if (local) {
         CUDA_TRY(ctx, cudaFuncSetAttribute(k_pairs<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         k_pairs<true><<<ngroups, NL_WARPS * 32, smem, st>>>((const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
@@ -930,6 +1151,7 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
         // local entries are stored as byte offsets of the staged float4 slots (index << 4) while the most
         // populous neighbourhood, dummy slot included, stays below 4096 atoms
         int lshift = (ctx->nl_last_n == n && ctx->nl_last_max_pop > 4094) ? 0 : 4;
+        bool use_staged = !ctx->pairs_staged_off;
         for (int attempt = 0;; ++attempt) {
             // the staging rows must fit the 227 KB a block can opt into (minus the kernel's static shared memory)
             const int cap_row_max = (int)(((size_t)232448 - 1024 - pairs_smem(0, local)) / (NL_WARPS * (local ? sizeof(uint16_t) : sizeof(uint32_t)))) & ~31;
@@ -943,13 +1165,22 @@ int nl_build_impl(sqeq_ctx* ctx, int64_t n, const float* pos, const double box[3
             init.ex.rl2 = g.rl2;
             *hinit = init;
             NL_CUDA(cudaMemcpyAsync(ctr, hinit, sizeof(NLCounters), cudaMemcpyHostToDevice, st));
-            NL_TRY(launch_pairs(ctx, nl, pos, g, local, local ? lshift : 0, est_row, cap_row, capacity, ctr, st));
+            // the staged sweep needs the neighbourhood size before the launch: a previous build of this system gives it
+            // (+6 % and 64 atoms of room; a neighbourhood that outgrows it raises stage_overflow and k_pairs runs instead)
+            int stage_cap = 0;
+            if (local && use_staged && ctx->nl_last_n == n && ctx->nl_last_max_pop > 0) {
+                stage_cap = (int)(1.06 * ctx->nl_last_max_pop) + 64;
+                const size_t sm = sizeof(float4) * ((size_t)stage_cap + 33) + (size_t)NLS_WARPS * cap_row * sizeof(uint16_t);
+                if (stage_cap > 65534 || sm > 110 * 1024) stage_cap = 0;      // two 512-thread blocks per SM
+            }
+            NL_TRY(launch_pairs(ctx, nl, pos, g, local, local ? lshift : 0, est_row, cap_row, capacity, ctr, st, stage_cap));
             NL_CUDA(cudaMemcpyAsync(h, ctr, sizeof(NLCounters), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaMemcpyAsync(h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
             NL_CUDA(cudaStreamSynchronize(st));
             if (h_flag[0] & 1)
                 return cleanup(sqeq_fail(ctx, SQEQ_EINVAL,
                                          "sqeq_nl_build: a position is non-finite or more than 127 box lengths away"));
+            if (h->stage_overflow) { use_staged = false; if (attempt < 3) continue; }
             const bool row_ok = h->max_row <= cap_row, cap_ok = h->cursor <= capacity;
             const bool fmt_ok = !local || (h->max_pop <= 65534 && ((size_t)h->max_pop + 1) * sizeof(float4) <= REAL_STAGE_MAX_BYTES);
             const bool shift_ok = !local || !fmt_ok || lshift == 0 || h->max_pop <= 4094;

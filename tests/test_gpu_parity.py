@@ -61,13 +61,28 @@ def inputs(k):
 
 
 def check_nl_exact(ctx, pos, box, rl):
-    nl = ctx.nl_build(dev(pos), box, rl)
-    gi, gj, gs = [t.cpu().numpy() for t in nl.export()]
+    """Two builds: the first of a system sizes its buffers from the mean density and runs the segment-sweep pair kernel
+    (k_pairs); the second knows the sizes and runs the shared-memory-staged one (k_pairs_staged).  Both must be the
+    oracle's set."""
     oi, oj, os_ = oracle.neighbour_list(pos, box, rl)
-    assert nl.count() == len(oi)
-    assert np.array_equal(gi, oi) and np.array_equal(gj, oj)
-    assert np.array_equal(gs, os_)
+    for _ in range(2):
+        nl = ctx.nl_build(dev(pos), box, rl)
+        gi, gj, gs = [t.cpu().numpy() for t in nl.export()]
+        assert nl.count() == len(oi)
+        assert np.array_equal(gi, oi) and np.array_equal(gj, oj)
+        assert np.array_equal(gs, os_)
+        if _ == 0:
+            nl.free()
     return nl, len(oi)
+
+
+def second_build_equals(ctx, pos, c, first):
+    """The same system built again (now by k_pairs_staged): identical export."""
+    nl2 = ctx.nl_build(dev(pos), c.box, c.r_list)
+    second = nl2.export()
+    for a, b in zip(first, second):
+        assert torch.equal(a, b)
+    nl2.free()
 
 
 def check_coulomb(ctx, nl, pos, q, c, rows=None):
@@ -266,11 +281,13 @@ def test_neighbour_list_full_set_config3(ctx):
     pos, q = inputs(3)
     n = len(q)
     nl = ctx.nl_build(dev(pos), c.box, c.r_list)
-    gi, gj, gs = [t.cpu().numpy() for t in nl.export()]
+    first = nl.export()
+    gi, gj, gs = [t.cpu().numpy() for t in first]
     total = compare_list_rows(pos, c, gi, gj, gs, 0, n)
     assert total == len(gi) == nl.count()
     print(f"cfg3 full list: {total} pairs bit-exact")
     nl.free()
+    second_build_equals(ctx, pos, c, first)
 
 
 @pytest.mark.slow
@@ -282,7 +299,8 @@ def test_neighbour_list_full_set_config4(ctx):
     pos, q = inputs(4)
     n = len(q)
     nl = ctx.nl_build(dev(pos), c.box, c.r_list)
-    gi, gj, gs = [t.cpu().numpy() for t in nl.export()]
+    first = nl.export()
+    gi, gj, gs = [t.cpu().numpy() for t in first]
     full = os.environ.get("SQEQ_TEST_FULL_CFG4", "1") == "1"
     i1 = n if full else n // 16
     total = compare_list_rows(pos, c, gi, gj, gs, 0, i1)
@@ -290,6 +308,7 @@ def test_neighbour_list_full_set_config4(ctx):
         assert total == len(gi) == nl.count()
     print(f"cfg4 list rows [0, {i1}): {total} pairs bit-exact (list holds {len(gi)})")
     nl.free()
+    second_build_equals(ctx, pos, c, first)
 
 
 @pytest.mark.parametrize("k", [3, 4])
