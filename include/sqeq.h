@@ -340,6 +340,8 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *   "fft_fused"        1  x-axis transforms fused with the influence multiply in one own kernel between batched 2-D
  *                         cuFFT transforms (0, or a grid whose x size has a prime factor above 5: 3-D cuFFT transforms
  *                         and a separate influence kernel)
+ *   "pairs_staged"     1  pair enumeration with the cell group's neighbourhood staged in shared memory (from the second
+ *                         build of a system on, when the neighbourhood size is known); 0: always the segment sweep
  *   "real_tma"         0  geometry-cache rows streamed into shared memory by the bulk-copy engine (cp.async.bulk +
  *                         mbarrier, two rows in flight per warp) instead of per-lane vector loads; 4 % slower at
  *                         331,776 atoms (0.151 vs 0.145 ms), kept as the measured alternative
