@@ -78,3 +78,43 @@ def test_replicas_aggregate_over_gloo_world_size_2(tmp_path):
                          capture_output=True, text=True, timeout=300)
     assert out.returncode == 0, out.stderr[-2000:]
     assert "AGG_OK 5000.0" in out.stdout
+
+
+def test_ewald_params_deliver_the_requested_accuracy():
+    """sqeq_ewald_params is pure host code (no context): alpha follows its closed form, the mesh is even and
+    2-3-5 smooth, and -- the check that matters -- the ORACLE's truncated Ewald sum with these alpha/kmax is within
+    a small multiple of delta of its converged sum on a small ionic box (PAPER.md:132 'error tolerance delta')."""
+    import numpy as np
+    import oracle
+    from paper_2503_21176_b200 import binding
+    box, rc = (13.0, 11.0, 12.0), 5.0
+    rng = np.random.default_rng(5)
+    m = 6
+    g = np.stack(np.meshgrid(*[np.arange(m)] * 3, indexing="ij"), -1).reshape(-1, 3)
+    pos = (g + 0.5) / m * np.array(box) + rng.uniform(-0.3, 0.3, (m ** 3, 3))
+    q = np.where(g.sum(1) % 2 == 0, 1.0, -1.0) * rng.uniform(0.6, 1.0, m ** 3)
+    q -= q.mean()
+    prev_k = None
+    for delta in (1e-3, 1e-4, 1e-5):
+        alpha, kmax, grid = binding.ewald_params(box, rc, delta)
+        assert abs(alpha - np.sqrt(-np.log(2 * delta)) / rc) < 1e-14
+        for K, L in zip(grid, box):
+            r = K
+            for f in (2, 3, 5):
+                while r % f == 0:
+                    r //= f
+            assert r == 1 and K % 2 == 0 and K >= 2 * alpha * L / (3 * delta ** 0.2)
+        if prev_k is not None:
+            assert all(a >= b for a, b in zip(kmax, prev_k))
+        prev_k = kmax
+        phi, F, _ = oracle.ewald_truncated(pos, q, box, rc, alpha, kmax)
+        phi0, F0, _ = oracle.ewald_direct(pos, q, box, alpha)
+        err = np.sqrt(((F - F0) ** 2).sum() / (F0 ** 2).sum())
+        assert err < 10 * delta, (delta, err)
+        assert err > delta / 200, (delta, err)      # and not wastefully over-converged
+        Fp = oracle.coulomb_pme(pos, q, box, rc, alpha, grid, 6)[1]      # the mesh it proposes, order 6
+        assert np.sqrt(((Fp - F0) ** 2).sum() / (F0 ** 2).sum()) < 10 * delta
+    with pytest.raises(binding.SqeqError):
+        binding.ewald_params(box, rc, 0.7)
+    with pytest.raises(binding.SqeqError):
+        binding.ewald_params((1.0, -1.0, 1.0), rc, 1e-4)
