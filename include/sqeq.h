@@ -340,6 +340,11 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *   "fft_fused"        1  x-axis transforms fused with the influence multiply in one own kernel between batched 2-D
  *                         cuFFT transforms (0, or a grid whose x size has a prime factor above 5: 3-D cuFFT transforms
  *                         and a separate influence kernel)
+ *   "fft_xline2"       1  that kernel in its register-resident form (two small DFTs around one shared-memory exchange
+ *                         per transform) for x sizes 24, 32, 48, 64, 72, 80, 96, 108, 120, 128, 144, 160, 192, 256; 0 or
+ *                         another size: radix-2/3/4/5 passes through shared memory
+ *   "fft_own"          1  the y and z passes by own kernels of the same kind too (no cuFFT call in an evaluation) when all
+ *                         three extents are among those sizes; 0: batched 2-D cuFFT transforms over (y, z)
  *   "pairs_staged"     1  pair enumeration with the cell group's neighbourhood staged in shared memory (from the second
  *                         build of a system on, when the neighbourhood size is known); 0: always the segment sweep
  *   "real_tma"         0  geometry-cache rows streamed into shared memory by the bulk-copy engine (cp.async.bulk +

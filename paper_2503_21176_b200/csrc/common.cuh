@@ -76,6 +76,9 @@ struct sqeq_ctx {
     cufftHandle plan2_r2c = 0, plan2_c2r = 0;
     bool xf_ok = false;
     bool fft_fused_off = false;           // SQEQ_FFT_FUSED=0: 3-D cuFFT transforms + separate influence kernel
+    bool fft3_ok = false;                 // all three grid extents are sizes fftx.cu / fftz.cu are built for
+    bool fft_own_off = false;             // "fft_own" = 0: cuFFT for the y and z axes even then
+    bool fft_xline2_off = false;          // "fft_xline2" = 0: the Stockham x-pass (pme.cu) even where fftx.cu has the size
     int xf_npass = 0, xf_radix[12] = {0};
     DevBuf xf_tw;
     int pme_atom_threads = 1;             // "pme_atom_threads": one thread per atom in the tile kernels: 0 never (lane
@@ -262,6 +265,14 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
 // nl supplies the cell-major atom runs the shared-memory tiles are built on (NULL: global kernels)
 int pme_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,
             bool want_energy, cudaStream_t st);
+// fftx.cu: register-resident two-step version of the fused x-axis pass, for the x extents it is built for
+bool xline2_supported(int K0);
+int xline2_run(sqeq_ctx* ctx, int K0, int K1, int K2h, int K2, const float* tab, float inv_piV, const float2* W,
+               float2* spec, double* e_out, cudaStream_t st);
+int yline_run(sqeq_ctx* ctx, int K0, int K1, int K2h, const float2* W, float2* spec, bool inverse, cudaStream_t st);
+// fftz.cu: z-axis real-to-complex / complex-to-real passes (layouts as cuFFT's R2C/C2R, unnormalised)
+bool zline_supported(int K2);
+int zline_run(sqeq_ctx* ctx, int nlines, int K2, const float2* W, float* grid, float2* spec, bool inverse, cudaStream_t st);
 int assemble_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double alpha, float* phi, float* force,
                  bool want_energy, bool field_mode, cudaStream_t st);
 // Full evaluation on prepared geometry (used by coulomb, qeq and md drivers).

@@ -957,6 +957,7 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
         // fused x-axis pass: needs K0 = 2^a 3^b 5^c; then the 3-D transforms become batched 2-D cuFFT transforms over
         // (y,z) around k_xline_influence
         if (ctx->xf_ok) { cufftDestroy(ctx->plan2_r2c); cufftDestroy(ctx->plan2_c2r); ctx->xf_ok = false; }
+        ctx->fft3_ok = false;
         {
             int r = grid[0], np = 0;
             int radix[XF_MAXPASS];
@@ -975,11 +976,14 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
                     ctx->xf_ok = true;
                     ctx->xf_npass = np;
                     for (int k = 0; k < np; ++k) ctx->xf_radix[k] = radix[k];
-                    std::vector<float2> W(grid[0]);
-                    for (int m = 0; m < grid[0]; ++m) {
-                        const double a = -2.0 * M_PI * (double)m / (double)grid[0];
-                        W[m] = make_float2((float)cos(a), (float)sin(a));
-                    }
+                    // roots of unity e^{-2 pi i m/K} of the three axes, one after the other
+                    std::vector<float2> W;
+                    for (int d = 0; d < 3; ++d)
+                        for (int m = 0; m < grid[d]; ++m) {
+                            const double a = -2.0 * M_PI * (double)m / (double)grid[d];
+                            W.push_back(make_float2((float)cos(a), (float)sin(a)));
+                        }
+                    ctx->fft3_ok = xline2_supported(grid[0]) && xline2_supported(grid[1]) && zline_supported(grid[2]);
                     SQEQ_TRY(sqeq_reserve(ctx, ctx->xf_tw, sizeof(float2) * W.size()));
                     CUDA_TRY(ctx, cudaMemcpy(ctx->xf_tw.p, W.data(), sizeof(float2) * W.size(), cudaMemcpyHostToDevice));
                 }
@@ -1150,7 +1154,17 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     if (ctx->gridQ.p) SQEQ_TRY(sqeq_reserve(ctx, ctx->gridQ, sizeof(float) * G3));    // the grid may have grown since the capture was enabled
     if (ctx->gridQ.p) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->gridQ.p, grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, st));
     const bool fused = ctx->xf_ok && !ctx->fft_fused_off;
-    {
+    // all three axes by the two-step kernels of fftx.cu / fftz.cu (no cuFFT call) where the extents allow
+    const bool own3 = fused && ctx->fft3_ok && !ctx->fft_xline2_off && !ctx->fft_own_off;
+    const float2* Wx = (const float2*)ctx->xf_tw.p;
+    const float2* Wy = Wx + K0;
+    const float2* Wz = Wy + K1;
+    if (own3) {
+        StageTimer tm(ctx, SQEQ_T_FFT_FWD, st);
+        SQEQ_TRY(zline_run(ctx, K0 * K1, K2, Wz, grid, spec, false, st));
+        SQEQ_TRY(yline_run(ctx, K0, K1, K2h, Wy, spec, false, st));
+        KERNEL_CHECK(ctx);
+    } else {
         StageTimer tm(ctx, SQEQ_T_FFT_FWD, st);
         cufftHandle plan = fused ? ctx->plan2_r2c : ctx->plan_r2c;
         cufftSetStream(plan, st);
@@ -1164,6 +1178,10 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         const float inv_piV = (float)(1.0 / (M_PI * box[0] * box[1] * box[2]));
         if (fused) {
             // forward x-transform, influence multiply + energy, inverse x-transform: one pass over the spectrum
+            if (!ctx->fft_xline2_off && xline2_supported(K0)) {
+                SQEQ_TRY(xline2_run(ctx, K0, K1, K2h, K2, (const float*)ctx->tabs.p, inv_piV, (const float2*)ctx->xf_tw.p, spec,
+                                    e_out, st));
+            } else {
             XfPlan pl;
             pl.N = K0; pl.npass = ctx->xf_npass;
             for (int k = 0; k < pl.npass; ++k) pl.radix[k] = ctx->xf_radix[k];
@@ -1171,6 +1189,7 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
             CUDA_TRY(ctx, cudaFuncSetAttribute(k_xline_influence, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
             k_xline_influence<<<ceil_div((int64_t)K1 * K2h, XF_TJ), XF_NT, sm, st>>>(pl, K1, K2h, K2, (const float*)ctx->tabs.p, inv_piV,
                                                                                     (const float2*)ctx->xf_tw.p, spec, e_out);
+            }
         } else {
             int nb = ceil_div((int64_t)K0 * K1, 8);
             if (nb > ctx->sm_count * 8) nb = ctx->sm_count * 8;
@@ -1178,7 +1197,12 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         }
         KERNEL_CHECK(ctx);
     }
-    {
+    if (own3) {
+        StageTimer tm(ctx, SQEQ_T_FFT_INV, st);
+        SQEQ_TRY(yline_run(ctx, K0, K1, K2h, Wy, spec, true, st));
+        SQEQ_TRY(zline_run(ctx, K0 * K1, K2, Wz, grid, spec, true, st));
+        KERNEL_CHECK(ctx);
+    } else {
         StageTimer tm(ctx, SQEQ_T_FFT_INV, st);
         cufftHandle plan = fused ? ctx->plan2_c2r : ctx->plan_c2r;
         cufftSetStream(plan, st);

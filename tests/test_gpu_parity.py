@@ -806,6 +806,52 @@ def test_pme_thread_per_atom_kernels(ctx):
         c2.close()
 
 
+def test_own_transforms_every_size(ctx):
+    """The register-resident two-step transforms (fftx.cu, fftz.cu) replace cuFFT whenever all three grid extents are
+    among their 14 sizes.  Every size on every axis, in non-cubic combinations: against the oracle where its O(K^4)
+    transforms finish in seconds, and against the library's own 3-D cuFFT + separate influence kernel path
+    (fft_fused = 0) for all of them."""
+    from paper_2503_21176_b200 import binding
+    sizes = [24, 32, 48, 64, 72, 80, 96, 108, 120, 128, 144, 160, 192, 256]
+    ref = binding.Context(0)
+    ref.set_option("fft_fused", 0)
+    rng = np.random.default_rng(21)
+    n = 600
+    boxn = np.array([21.0, 24.5, 23.0])
+    p = (rng.uniform(0, 1, (n, 3)) * boxn).astype(np.float32)
+    qq = rng.normal(size=n).astype(np.float32)
+    qq -= qq.mean()
+    worst = 0.0
+    try:
+        nl = ctx.nl_build(dev(p), boxn, 8.4)
+        nlr = ref.nl_build(dev(p), boxn, 8.4)
+        for i, K0 in enumerate(sizes):
+            grid = [K0, sizes[(i + 5) % 14], sizes[(i + 9) % 14]]
+            order = (4, 6, 8)[i % 3]
+            phi, F, E = ctx.coulomb(nl, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
+            phr, Fr, Er = ref.coulomb(nlr, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
+            e_phi, e_F = relrms(phi.cpu().numpy(), phr.cpu().numpy()), relrms(F.cpu().numpy(), Fr.cpu().numpy())
+            worst = max(worst, e_phi, e_F)
+            scale = 0.5 * float(np.abs(qq * phr.cpu().numpy()).sum())      # E = 1/2 sum q phi cancels heavily for random q
+            assert e_phi < 2e-6 and e_F < 2e-6 and abs(E - Er) < 2e-6 * scale, (grid, e_phi, e_F, E, Er)
+            if max(grid) <= 96:
+                op, oF, oE, _ = oracle.coulomb_pme(p, qq, boxn, 8.0, 0.4, grid, order)
+                assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL and abs(E - oE) < TOL * scale, grid
+        # the options in between: own x pass with cuFFT 2-D transforms, and the radix-2/3/4/5 x pass
+        grid = [72, 160, 64]
+        phr, Fr, Er = ref.coulomb(nlr, dev(p), dev(qq), boxn, 8.0, 0.4, grid, 6)
+        for opt in ("fft_own", "fft_xline2"):
+            ctx.set_option(opt, 0)
+            phi, F, E = ctx.coulomb(nl, dev(p), dev(qq), boxn, 8.0, 0.4, grid, 6)
+            assert relrms(phi.cpu().numpy(), phr.cpu().numpy()) < 2e-6 and relrms(F.cpu().numpy(), Fr.cpu().numpy()) < 2e-6
+        nl.free(); nlr.free()
+    finally:
+        ctx.set_option("fft_own", 1)
+        ctx.set_option("fft_xline2", 1)
+        ref.close()
+    record("own_transforms_vs_cufft", worst_relrms=worst)
+
+
 def test_pme_tile_window_fallbacks(ctx, monkeypatch):
     """The shared-memory spread/gather tiles assume an atom stays within one grid spacing of the cell
     it was binned into; beyond that the atom takes the global-memory path inside the same kernels,
