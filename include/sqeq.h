@@ -345,6 +345,9 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *                         another size: radix-2/3/4/5 passes through shared memory
  *   "fft_own"          1  the y and z passes by own kernels of the same kind too (no cuFFT call in an evaluation) when all
  *                         three extents are among those sizes; 0: batched 2-D cuFFT transforms over (y, z)
+ *   "pdl"              1  the transform kernels are launched with programmatic stream serialisation (each starts its
+ *                         prologue while the one before drains and waits, griddepcontrol.wait, before touching data):
+ *                         -2 us per evaluation where the five kernels are not hidden behind the real-space kernel
  *   "pairs_staged"     1  pair enumeration with the cell group's neighbourhood staged in shared memory (from the second
  *                         build of a system on, when the neighbourhood size is known); 0: always the segment sweep
  *   "real_tma"         0  geometry-cache rows streamed into shared memory by the bulk-copy engine (cp.async.bulk +

@@ -180,6 +180,8 @@ int sqeq_create(sqeq_ctx** out, int device, void* cuda_stream)
     ctx->real_tma = env && env[0] == '1';
     env = getenv("SQEQ_FFT_FUSED");
     ctx->fft_fused_off = env && env[0] == '0';
+    env = getenv("SQEQ_PDL");
+    ctx->pdl_off = env && env[0] == '0';
     env = getenv("SQEQ_FFT_OWN");
     ctx->fft_own_off = env && env[0] == '0';
     env = getenv("SQEQ_FFT_XLINE2");
@@ -301,6 +303,7 @@ int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
     if (!strcmp(name, "graphs")) ctx->graphs = value != 0;
     else if (!strcmp(name, "overlap")) ctx->overlap = value;
     else if (!strcmp(name, "fft_fused")) ctx->fft_fused_off = value == 0;
+    else if (!strcmp(name, "pdl")) ctx->pdl_off = value == 0;
     else if (!strcmp(name, "fft_own")) ctx->fft_own_off = value == 0;
     else if (!strcmp(name, "fft_xline2")) ctx->fft_xline2_off = value == 0;
     else if (!strcmp(name, "real_tma")) ctx->real_tma = value != 0;

@@ -76,6 +76,7 @@ struct sqeq_ctx {
     cufftHandle plan2_r2c = 0, plan2_c2r = 0;
     bool xf_ok = false;
     bool fft_fused_off = false;           // SQEQ_FFT_FUSED=0: 3-D cuFFT transforms + separate influence kernel
+    bool pdl_off = false;                 // "pdl" = 0: ordinary stream-ordered launches everywhere
     bool fft3_ok = false;                 // all three grid extents are sizes fftx.cu / fftz.cu are built for
     bool fft_own_off = false;             // "fft_own" = 0: cuFFT for the y and z axes even then
     bool fft_xline2_off = false;          // "fft_xline2" = 0: the Stockham x-pass (pme.cu) even where fftx.cu has the size
@@ -219,6 +220,34 @@ struct StageTimer {
 };
 
 #ifdef __CUDACC__
+// ---- programmatic dependent launch (PTX griddepcontrol; guide: "PDL") --------------------------------------------
+// A kernel launched with launch_pdl may start while the kernel before it in the stream is still draining: its
+// blocks become resident as that kernel's last blocks retire and run their prologue (index arithmetic, constant
+// tables) up to pdl_wait(), which returns when the previous kernel has completed and its writes are visible.  Rules
+// kept throughout: pdl_trigger() is the first statement of every kernel that may be followed by such a launch;
+// pdl_wait() comes before the first access to anything an earlier kernel wrote or still reads; EVERY kernel launched
+// with launch_pdl executes pdl_wait() in all its threads (completion of a kernel then implies completion of all before
+// it).  Both are no-ops in a kernel launched the ordinary way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+static inline cudaError_t launch_pdl(sqeq_ctx* ctx, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                     Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = ctx->pdl_off ? 0 : 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // Sums four per-lane values over the warp with 6 shuffles instead of 20: the first two butterfly steps
 // halve the number of values a lane carries (lanes keep one half of the values and send the other),
 // the last three are an ordinary butterfly.  On return lane 0 holds the sum of a, lane 8 of b, lane 16 of

@@ -47,7 +47,9 @@ k_xline2(int K1, int K2h, int K2, const float* __restrict__ tab, float inv_piV, 
     const int tid = threadIdx.x, tj = tid % TJ, hi = tid / TJ;     // hi = n2 (steps A, A') or k1 (step B)
     const int jl = blockIdx.x * TJ + tj;
     const bool line_on = jl < nline;
+    pdl_trigger();
     for (int i = tid; i < N; i += NT) W[i] = Wg[i];
+    pdl_wait();
 
     // ---- step A: N1-point transforms over n1, straight from global memory
     float2 v[N1];
@@ -140,7 +142,8 @@ int launch(sqeq_ctx* ctx, int K1, int K2h, int K2, const float* tab, float inv_p
     static_assert(C::NT % 32 == 0 && C::NT <= 1024, "whole warps");
     auto kern = k_xline2<N1, N2, TJ>;
     CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-    kern<<<ceil_div((int64_t)K1 * K2h, TJ), C::NT, C::SMEM, st>>>(K1, K2h, K2, tab, inv_piV, W, spec, e_out);
+    CUDA_TRY(ctx, launch_pdl(ctx, kern, dim3(ceil_div((int64_t)K1 * K2h, TJ)), dim3(C::NT), C::SMEM, st, K1, K2h, K2, tab, inv_piV, W, spec,
+                             e_out));
     return SQEQ_OK;
 }
 
@@ -159,7 +162,9 @@ k_yline(int K2h, const float2* __restrict__ Wg, float2* __restrict__ spec)
     const int zc = blockIdx.x * TJ + tj;
     const bool line_on = zc < K2h;
     float2* g = spec + (size_t)blockIdx.y * N * K2h + zc;   // (x, y = 0, zc)
+    pdl_trigger();
     for (int i = tid; i < N; i += NT) W[i] = Wg[i];
+    pdl_wait();
     float2 v[N1];
     const bool actA = hi < N2;
     if (actA) {
@@ -201,11 +206,11 @@ int launch_y(sqeq_ctx* ctx, int K0, int K2h, const float2* W, float2* spec, bool
     if (inverse) {
         auto kern = k_yline<N1, N2, TJ, true>;
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        kern<<<gr, C::NT, C::SMEM, st>>>(K2h, W, spec);
+        CUDA_TRY(ctx, launch_pdl(ctx, kern, gr, dim3(C::NT), C::SMEM, st, K2h, W, spec));
     } else {
         auto kern = k_yline<N1, N2, TJ, false>;
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        kern<<<gr, C::NT, C::SMEM, st>>>(K2h, W, spec);
+        CUDA_TRY(ctx, launch_pdl(ctx, kern, gr, dim3(C::NT), C::SMEM, st, K2h, W, spec));
     }
     return SQEQ_OK;
 }

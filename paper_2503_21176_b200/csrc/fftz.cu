@@ -33,7 +33,9 @@ k_zr2c(int nlines, const float2* __restrict__ Wg, const float* __restrict__ grid
     float2* Zs = S + TJ * N1 * RS;
     float2* W = Zs + TJ * ZS;
     const int tid = threadIdx.x, line0 = blockIdx.x * TJ;
+    pdl_trigger();
     for (int i = tid; i < K2; i += NT) W[i] = Wg[i];
+    pdl_wait();
     float2 v[N1];
     const int tjA = tid / N2, n2 = tid - tjA * N2;
     const bool actA = tid < C::NTA;
@@ -90,7 +92,9 @@ k_zc2r(int nlines, const float2* __restrict__ Wg, const float2* __restrict__ spe
     float2* Xs = S + TJ * N1 * RS;
     float2* W = Xs + TJ * ZS;
     const int tid = threadIdx.x, line0 = blockIdx.x * TJ;
+    pdl_trigger();
     for (int i = tid; i < K2; i += NT) W[i] = Wg[i];
+    pdl_wait();
     const int nin = min(TJ, nlines - line0) * K2h;
     const float2* src = spec + (size_t)line0 * K2h;
     for (int e = tid; e < TJ * K2h; e += NT) {
@@ -146,11 +150,11 @@ int launch_z(sqeq_ctx* ctx, int nlines, const float2* W, float* grid, float2* sp
     if (inverse) {
         auto kern = k_zc2r<N1, N2, TJ>;
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        kern<<<nb, C::NT, C::SMEM, st>>>(nlines, W, spec, grid);
+        CUDA_TRY(ctx, launch_pdl(ctx, kern, dim3(nb), dim3(C::NT), C::SMEM, st, nlines, W, spec, grid));
     } else {
         auto kern = k_zr2c<N1, N2, TJ>;
         CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        kern<<<nb, C::NT, C::SMEM, st>>>(nlines, W, grid, spec);
+        CUDA_TRY(ctx, launch_pdl(ctx, kern, dim3(nb), dim3(C::NT), C::SMEM, st, nlines, W, (const float*)grid, spec));
     }
     return SQEQ_OK;
 }

@@ -1154,6 +1154,9 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     if (ctx->gridQ.p) SQEQ_TRY(sqeq_reserve(ctx, ctx->gridQ, sizeof(float) * G3));    // the grid may have grown since the capture was enabled
     if (ctx->gridQ.p) CUDA_TRY(ctx, cudaMemcpyAsync(ctx->gridQ.p, grid, sizeof(float) * G3, cudaMemcpyDeviceToDevice, st));
     const bool fused = ctx->xf_ok && !ctx->fft_fused_off;
+    // E_rec accumulator: cleared here rather than next to its kernel so that the transform kernels follow one another
+    // in the stream (programmatic dependent launch needs the kernels adjacent)
+    CUDA_TRY(ctx, cudaMemsetAsync((double*)ctx->scal.p + 1, 0, sizeof(double), st));
     // all three axes by the two-step kernels of fftx.cu / fftz.cu (no cuFFT call) where the extents allow
     const bool own3 = fused && ctx->fft3_ok && !ctx->fft_xline2_off && !ctx->fft_own_off;
     const float2* Wx = (const float2*)ctx->xf_tw.p;
@@ -1174,7 +1177,6 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     {
         StageTimer tm(ctx, SQEQ_T_INFLUENCE, st);
         double* e_out = (double*)ctx->scal.p + 1;
-        CUDA_TRY(ctx, cudaMemsetAsync(e_out, 0, sizeof(double), st));
         const float inv_piV = (float)(1.0 / (M_PI * box[0] * box[1] * box[2]));
         if (fused) {
             // forward x-transform, influence multiply + energy, inverse x-transform: one pass over the spectrum
