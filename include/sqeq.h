@@ -333,9 +333,10 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *   "graphs"           1  replay launch-bound sequences (sqeq_coulomb_fixed on a cached geometry, the steps of
  *                         sqeq_shadow_md_run) as CUDA graphs; needs a context stream other than the legacy default
  *   "overlap"          1  PME on an internal side stream beside a persistent real-space grid: 0 never, 1 for
- *                         evaluations the caller does not wait for (sqeq_coulomb_enqueue, sqeq_coulomb with
- *                         energy == NULL, sqeq_coulomb_host_submit: +3-5 % throughput at 331,776 atoms), 2 always
- *                         (a single evaluation that is waited for finishes 12 % LATER that way)
+ *                         force evaluations the caller does not wait for (sqeq_coulomb_enqueue, sqeq_coulomb with
+ *                         energy == NULL, sqeq_coulomb_host_submit: +3 % throughput at 331,776 atoms, +14 % at 98,304),
+ *                         2 always (a single evaluation that is waited for finishes LATER that way, and a potential-
+ *                         only one takes 0.47 instead of 0.40 ms at 331,776 atoms)
  *   "real_lean_blocks" 2  blocks per SM of that persistent grid
  *   "fft_fused"        1  x-axis transforms fused with the influence multiply in one own kernel between batched 2-D
  *                         cuFFT transforms (0, or a grid whose x size has a prime factor above 5: 3-D cuFFT transforms

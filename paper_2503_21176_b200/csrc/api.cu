@@ -484,8 +484,10 @@ int coulomb_eval(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double bo
     // them: at cfg 4 the device-side step goes from 0.624 to 0.587 ms, but a single synchronous evaluation
     // (sqeq_coulomb_host) gets slower (0.94 -> 1.02 ms), so it stays an option.  Never
     // with stage timing on, where every event pair brackets one kernel running alone.
+    // Potential-only evaluations are excluded from the automatic choice: their real-space kernel is list-bandwidth
+    // bound and loses more as two persistent blocks per SM than the overlap returns (cfg 4: 0.472 ms against 0.398).
     const bool overlap = !ctx->profiling && geom == GEOM_NEW && nl->fmt == 1 &&
-                         (ctx->overlap >= 2 || (ctx->overlap == 1 && ctx->throughput_call));
+                         (ctx->overlap >= 2 || (ctx->overlap == 1 && ctx->throughput_call && want_force));
     ctx->overlap_now = overlap;
     if (!overlap) {
         SQEQ_TRY(pme_run(ctx, nl, n, box, want_force, false, ctx->stream));

@@ -227,7 +227,10 @@ struct StageTimer {
 // kept throughout: pdl_trigger() is the first statement of every kernel that may be followed by such a launch;
 // pdl_wait() comes before the first access to anything an earlier kernel wrote or still reads; EVERY kernel launched
 // with launch_pdl executes pdl_wait() in all its threads (completion of a kernel then implies completion of all before
-// it).  Both are no-ops in a kernel launched the ordinary way.
+// it); and NO non-coherent load (const __restrict__ pointer, __ldg: LDG.CONSTANT) of anything the previous kernel
+// wrote -- the block may sit on an SM whose L1 still holds the old lines, and only ordinary loads are made coherent
+// by the wait (measured: a const __restrict__ input gave wrong transforms at cfg 2).  Both are no-ops in a kernel
+// launched the ordinary way.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 

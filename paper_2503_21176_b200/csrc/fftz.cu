@@ -17,20 +17,24 @@ struct ZCfg {
     static constexpr int M = N1 * N2, K2 = 2 * M, K2h = M + 1;
     static constexpr int RS = (N2 % 2 == 0) ? N2 + 1 : N2;          // row of one (line, k1): odd stride, no bank conflicts
     static constexpr int ZS = K2h + ((24 - K2h % 16) % 16);          // a line's spectrum, stride = 8 mod 16 elements
+    static constexpr int TS = N1 * RS + ((24 - (N1 * RS) % 16) % 16);  // a line's block of S, likewise: the N2-wide runs
+                                                                     // of two lines in a half-warp fall on different banks
     static constexpr int NTA = TJ * N2, NTB = TJ * N1;
     static constexpr int NT = (((NTA > NTB ? NTA : NTB) + 31) / 32) * 32;
-    static constexpr size_t SMEM = sizeof(float2) * ((size_t)TJ * N1 * RS + (size_t)TJ * ZS + K2);
+    static constexpr size_t SMEM = sizeof(float2) * ((size_t)TJ * TS + (size_t)TJ * ZS + K2);
 };
 
 template <int N1, int N2, int TJ>
 __global__ void __launch_bounds__(ZCfg<N1, N2, TJ>::NT)
-k_zr2c(int nlines, const float2* __restrict__ Wg, const float* __restrict__ grid, float2* __restrict__ spec)
+k_zr2c(int nlines, const float2* __restrict__ Wg, const float* grid, float2* spec)      // grid: written by the kernel before;
+                                                                                    // no __restrict__, or its loads may be hoisted
+                                                                                    // above pdl_wait() as read-only (ld.global.nc)
 {
     using C = ZCfg<N1, N2, TJ>;
-    constexpr int M = C::M, K2 = C::K2, K2h = C::K2h, RS = C::RS, ZS = C::ZS, NT = C::NT;
+    constexpr int M = C::M, K2 = C::K2, K2h = C::K2h, RS = C::RS, ZS = C::ZS, TS = C::TS, NT = C::NT;
     extern __shared__ __align__(16) float2 z_sh[];                   // S[TJ][N1][RS] | Zs[TJ][ZS] | W[K2]
     float2* S = z_sh;
-    float2* Zs = S + TJ * N1 * RS;
+    float2* Zs = S + TJ * TS;
     float2* W = Zs + TJ * ZS;
     const int tid = threadIdx.x, line0 = blockIdx.x * TJ;
     pdl_trigger();
@@ -54,14 +58,14 @@ k_zr2c(int nlines, const float2* __restrict__ Wg, const float* __restrict__ grid
             constexpr int k1 = decltype(i_)::value;
             float2 z = v[k1];
             if (k1 > 0) z = fx::cmulf(z, W[2 * n2 * k1]);            // W_M^(n2 k1); 2 n2 k1 < K2
-            S[(tjA * N1 + k1) * RS + n2] = z;
+            S[tjA * TS + k1 * RS + n2] = z;
         });
     }
     __syncthreads();
     if (tid < C::NTB) {
         const int tj = tid / N1, k1 = tid - tj * N1;
         float2 u[N2];
-        const float2* row = S + (tj * N1 + k1) * RS;
+        const float2* row = S + tj * TS + k1 * RS;
         fx::sfor<0, N2>([&](auto i_) { constexpr int j = decltype(i_)::value; u[j] = row[j]; });
         fx::Dft<N2, false>::run(u);
         fx::sfor<0, N2>([&](auto i_) { constexpr int k2 = decltype(i_)::value; Zs[tj * ZS + k1 + N1 * k2] = u[k2]; });
@@ -83,33 +87,37 @@ k_zr2c(int nlines, const float2* __restrict__ Wg, const float* __restrict__ grid
 
 template <int N1, int N2, int TJ>
 __global__ void __launch_bounds__(ZCfg<N1, N2, TJ>::NT)
-k_zc2r(int nlines, const float2* __restrict__ Wg, const float2* __restrict__ spec, float* __restrict__ grid)
+k_zc2r(int nlines, const float2* __restrict__ Wg, const float2* spec, float* grid)      // spec: likewise
 {
     using C = ZCfg<N1, N2, TJ>;
-    constexpr int M = C::M, K2 = C::K2, K2h = C::K2h, RS = C::RS, ZS = C::ZS, NT = C::NT;
+    constexpr int M = C::M, K2 = C::K2, K2h = C::K2h, RS = C::RS, ZS = C::ZS, TS = C::TS, NT = C::NT;
     extern __shared__ __align__(16) float2 z_sh[];
     float2* S = z_sh;
-    float2* Xs = S + TJ * N1 * RS;
-    float2* W = Xs + TJ * ZS;
+    float2* W = S + TJ * TS + TJ * ZS;
     const int tid = threadIdx.x, line0 = blockIdx.x * TJ;
     pdl_trigger();
     for (int i = tid; i < K2; i += NT) W[i] = Wg[i];
     pdl_wait();
-    const int nin = min(TJ, nlines - line0) * K2h;
-    const float2* src = spec + (size_t)line0 * K2h;
-    for (int e = tid; e < TJ * K2h; e += NT) {
-        const int tj = e / K2h, k = e - tj * K2h;
-        Xs[tj * ZS + k] = e < nin ? src[e] : make_float2(0.f, 0.f);
-    }
-    __syncthreads();
+    // the even/odd merge needs Qhat[k] and Qhat[M-k]: both straight from global memory (each element is read by two
+    // threads of the block; the second read hits L1)
     const int tjA = tid / N2, j = tid - tjA * N2;
+    const bool actA = tid < C::NTA && line0 + tjA < nlines;
+    float2 xa[N1], xb[N1];
+    if (actA) {
+        const float2* X = spec + (size_t)(line0 + tjA) * K2h;
+        fx::sfor<0, N1>([&](auto i_) {
+            constexpr int i = decltype(i_)::value;
+            xa[i] = X[N2 * i + j];
+            xb[i] = X[M - N2 * i - j];
+        });
+    }
+    __syncthreads();                                                  // W
     if (tid < C::NTA) {
         float2 v[N1];
-        const float2* X = Xs + tjA * ZS;
         fx::sfor<0, N1>([&](auto i_) {
             constexpr int i = decltype(i_)::value;
             const int k = N2 * i + j;
-            const float2 a = X[k], b = X[M - k];
+            const float2 a = actA ? xa[i] : make_float2(0.f, 0.f), b = actA ? xb[i] : make_float2(0.f, 0.f);
             const float sx = a.x + b.x, sy = a.y - b.y;                            // a + conj b
             const float dx = a.x - b.x, dy = a.y + b.y;                            // a - conj b
             const float2 w = W[k];                                                 // conj w below
@@ -125,14 +133,14 @@ k_zc2r(int nlines, const float2* __restrict__ Wg, const float2* __restrict__ spe
                 c.y = -c.y;
                 z = fx::cmulf(z, c);
             }
-            S[(tjA * N1 + k1) * RS + j] = z;
+            S[tjA * TS + k1 * RS + j] = z;
         });
     }
     __syncthreads();
     if (tid < C::NTB) {
         const int tj = tid / N1, k1 = tid - tj * N1;
         float2 u[N2];
-        const float2* row = S + (tj * N1 + k1) * RS;
+        const float2* row = S + tj * TS + k1 * RS;
         fx::sfor<0, N2>([&](auto i_) { constexpr int jj = decltype(i_)::value; u[jj] = row[jj]; });
         fx::Dft<N2, true>::run(u);
         if (line0 + tj < nlines) {

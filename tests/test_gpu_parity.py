@@ -852,6 +852,35 @@ def test_own_transforms_every_size(ctx):
     record("own_transforms_vs_cufft", worst_relrms=worst)
 
 
+def test_dependent_launch_sees_the_previous_kernels_writes():
+    """The transform kernels start before the kernel ahead of them has finished (programmatic dependent launch) and must
+    read its output only after griddepcontrol.wait and only with coherent loads: a const __restrict__ input once read
+    stale lines of the evaluation before (errors of order one).  Alternating charge vectors, reciprocal parts against
+    the same library with ordinary launches ("pdl" = 0); the tolerance covers the order of the floating-point atomics
+    with which the spreading tiles are flushed."""
+    from paper_2503_21176_b200 import binding
+    c = W.CONFIGS[2]
+    pos, q = inputs(2)
+    a, b = binding.Context(0), binding.Context(0)
+    b.set_option("pdl", 0)
+    try:
+        nla, nlb = a.nl_build(dev(pos), c.box, c.r_list), b.nl_build(dev(pos), c.box, c.r_list)
+        rng = np.random.default_rng(8)
+        for it in range(12):
+            qq = (q * rng.uniform(-2, 2)).astype(np.float32) if it % 2 else rng.normal(size=len(q)).astype(np.float32)
+            wf = it % 3 != 2
+            pa, Fa, Ea = a.coulomb(nla, dev(pos), dev(qq), c.box, c.rc, c.alpha, c.grid, c.order, want_force=wf)
+            pb, Fb, Eb = b.coulomb(nlb, dev(pos), dev(qq), c.box, c.rc, c.alpha, c.grid, c.order, want_force=wf)
+            close = lambda u, v: relrms(u.cpu().numpy(), v.cpu().numpy()) < 1e-6
+            assert close(pa, pb) and (not wf or close(Fa, Fb)), it
+            if wf:
+                ga, gb = a.coulomb_parts(nla), b.coulomb_parts(nlb)
+                assert close(ga["phi_rec"], gb["phi_rec"]) and close(ga["F_rec"], gb["F_rec"]), it
+        nla.free(); nlb.free()
+    finally:
+        a.close(); b.close()
+
+
 def test_pme_tile_window_fallbacks(ctx, monkeypatch):
     """The shared-memory spread/gather tiles assume an atom stays within one grid spacing of the cell
     it was binned into; beyond that the atom takes the global-memory path inside the same kernels,
