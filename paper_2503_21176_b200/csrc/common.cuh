@@ -247,7 +247,9 @@ static inline cudaError_t launch_pdl(sqeq_ctx* ctx, void (*kern)(KArgs...), dim3
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
-    cfg.numAttrs = ctx->pdl_off ? 0 : 1;
+    // not beside the persistent real-space grid of the side-stream schedule: blocks that wait for the kernel ahead
+    // would hold the one block slot per SM that grid leaves free (measured: 0.525 instead of 0.517 ms per step)
+    cfg.numAttrs = (ctx->pdl_off || ctx->overlap_now) ? 0 : 1;
     return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
