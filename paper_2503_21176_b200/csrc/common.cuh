@@ -112,6 +112,10 @@ struct sqeq_ctx {
     DevBuf vec_f[6];  // float  [n] scratch charge / potential vectors
     DevBuf vec_d[6];  // double [n] scratch
     DevBuf vec_f3[2]; // float  [n][3] scratch forces
+    // stand-in O-O repulsion (md.cu): the oxygens' list positions, cell by cell, for the list with this serial
+    DevBuf rep_oslot, rep_ostart;
+    const void* rep_nl = nullptr;
+    uint64_t rep_serial = 0;
     GeomCache gc;
     struct { bool valid = false, tiles = false; int order = 0, nt = 0, K[3] = {0, 0, 0}, nc[3] = {0, 0, 0}; size_t bytes = 0;
              alignas(8) unsigned char blob[128]; } tile_plan;     // cached TileGeom of the PME tile kernels (pme.cu)

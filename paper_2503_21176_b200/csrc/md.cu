@@ -23,6 +23,7 @@
 // scal[] slots used here (0 and 1 belong to assemble / influence)
 enum { S_T = 2, S_INVU = 3, S_U = 4, S_RES2 = 5, S_JAC = 6, S_EKIN = 7, S_VSTAND = 8 };   // 12: max drift (nlist.cu)
 
+// blocks of exactly 256 threads
 __device__ __forceinline__ void block_sum_to(double v, double* dst)
 {
     __shared__ double red[8];
@@ -181,60 +182,137 @@ struct RepGeom {
     float L[3];
     float k, r0;
 };
+// The oxygens of the list's cell-major order, cell by cell (built once per list): counts per cell, a one-block scan,
+// the fill.
+__global__ void k_rep_count(int ncells, const int* __restrict__ cell_start, const int* __restrict__ perm, int* __restrict__ ostart)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncells) return;
+    int m = 0;
+    for (int t = cell_start[c]; t < cell_start[c + 1]; ++t) m += perm[t] % 3 == 0;
+    ostart[c] = m;
+}
+__global__ void __launch_bounds__(1024) k_rep_scan(int ncells, int* __restrict__ ostart)     // exclusive, in place; [ncells] = total
+{
+    __shared__ int s_w[32];
+    __shared__ int s_carry;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int b = 0; b < ncells; b += 1024) {
+        const int c = b + threadIdx.x;
+        const int v = c < ncells ? ostart[c] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) s_w[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            int w = s_w[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += y;
+            }
+            s_w[lane] = w;
+        }
+        __syncthreads();
+        const int carry = s_carry, before = wid ? s_w[wid - 1] : 0;
+        if (c < ncells) ostart[c] = carry + before + x - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) s_carry = carry + s_w[31];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) ostart[ncells] = s_carry;
+}
+__global__ void k_rep_fill(int ncells, const int* __restrict__ cell_start, const int* __restrict__ perm,
+                           const int* __restrict__ ostart, int* __restrict__ oslot)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncells) return;
+    int o = ostart[c];
+    for (int t = cell_start[c]; t < cell_start[c + 1]; ++t)
+        if (perm[t] % 3 == 0) oslot[o++] = t;
+}
+
+// One THREAD per oxygen, in cell order (the lanes of a warp sit in the same or neighbouring cells, so their candidate
+// loads mostly coincide).  An oxygen visits only the neighbouring cells it can reach: along an axis the cell below
+// (above) is needed when the atom lies within `reach` = r0 + skin of its cell's lower (upper) face -- positions are the
+// current ones on the build-time image, and both atoms of a pair have moved at most skin/2 since the cells were filled
+// (check_md_args: reach <= cell edge): on average 12 of the 27 cells, 5 oxygens each.  (One warp per atom over all
+// atoms of all 27 cells took 0.73 ms at 331,776 atoms.)
 __global__ void __launch_bounds__(256)
-k_md_oo_repulsion(int64_t n, const float4* __restrict__ xq, const int* __restrict__ cell_of,
-                  const int* __restrict__ cell_start, const int* __restrict__ perm, RepGeom g,
+k_md_oo_repulsion(int no, const float4* __restrict__ xq, const int* __restrict__ cell_of, const int* __restrict__ ostart,
+                  const int* __restrict__ oslot, const int* __restrict__ perm, RepGeom g, float reach,
                   float* __restrict__ force, double* __restrict__ vsum)
 {
-    const int lane = threadIdx.x & 31;
-    const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
     double V = 0.0;
-    if (s < n) {
-        const int oi = perm[s];
-        if (oi % 3 == 0) {
-            const float4 xi = xq[s];
-            const int c = cell_of[s];
-            const int cx = c & 1023, cy = (c >> 10) & 1023, cz = c >> 20;
-            float fx = 0.f, fy = 0.f, fz = 0.f, v = 0.f;
-            for (int dx = -1; dx <= 1; ++dx)
-                for (int dy = -1; dy <= 1; ++dy)
-                    for (int dz = -1; dz <= 1; ++dz) {
-                        int ux = cx + dx, uy = cy + dy, uz = cz + dz;
-                        float sx = 0.f, sy = 0.f, sz = 0.f;
-                        if (ux < 0) { ux += g.nc[0]; sx = -g.L[0]; } else if (ux >= g.nc[0]) { ux -= g.nc[0]; sx = g.L[0]; }
-                        if (uy < 0) { uy += g.nc[1]; sy = -g.L[1]; } else if (uy >= g.nc[1]) { uy -= g.nc[1]; sy = g.L[1]; }
-                        if (uz < 0) { uz += g.nc[2]; sz = -g.L[2]; } else if (uz >= g.nc[2]) { uz -= g.nc[2]; sz = g.L[2]; }
-                        const int cell = (ux * g.nc[1] + uy) * g.nc[2] + uz;
-                        const int beg = cell_start[cell], end = cell_start[cell + 1];
-                        for (int t = beg + lane; t < end; t += 32) {
-                            if (perm[t] % 3 != 0) continue;
-                            const float4 xj = xq[t];
-                            const float ddx = xi.x - (xj.x + sx), ddy = xi.y - (xj.y + sy), ddz = xi.z - (xj.z + sz);
-                            const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                            if (r2 < g.r0 * g.r0 && r2 > 0.f) {               // r2 = 0: the atom itself (zero image)
-                                const float r = sqrtf(r2);
-                                const float f = g.k * (g.r0 - r) / r;
-                                fx += f * ddx; fy += f * ddy; fz += f * ddz;
-                                v += 0.25f * g.k * (g.r0 - r) * (g.r0 - r);    // half of the pair energy
-                            }
+    if (k < no) {
+        const int s = oslot[k];
+        const float4 xi = xq[s];
+        const int c = cell_of[s];
+        const int cc[3] = {c & 1023, (c >> 10) & 1023, c >> 20};
+        const float xs[3] = {xi.x, xi.y, xi.z};
+        int lo[3], hi[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const float edge = g.L[d] / (float)g.nc[d], off = xs[d] - (float)cc[d] * edge;
+            lo[d] = off < reach ? -1 : 0;
+            hi[d] = edge - off < reach ? 1 : 0;
+        }
+        const float r02 = g.r0 * g.r0;
+        float fx = 0.f, fy = 0.f, fz = 0.f, v = 0.f;
+        for (int dx = lo[0]; dx <= hi[0]; ++dx)
+            for (int dy = lo[1]; dy <= hi[1]; ++dy)
+                for (int dz = lo[2]; dz <= hi[2]; ++dz) {
+                    int ux = cc[0] + dx, uy = cc[1] + dy, uz = cc[2] + dz;
+                    float sx = 0.f, sy = 0.f, sz = 0.f;
+                    if (ux < 0) { ux += g.nc[0]; sx = -g.L[0]; } else if (ux >= g.nc[0]) { ux -= g.nc[0]; sx = g.L[0]; }
+                    if (uy < 0) { uy += g.nc[1]; sy = -g.L[1]; } else if (uy >= g.nc[1]) { uy -= g.nc[1]; sy = g.L[1]; }
+                    if (uz < 0) { uz += g.nc[2]; sz = -g.L[2]; } else if (uz >= g.nc[2]) { uz -= g.nc[2]; sz = g.L[2]; }
+                    const int cell = (ux * g.nc[1] + uy) * g.nc[2] + uz;
+                    const int beg = ostart[cell], end = ostart[cell + 1];
+                    for (int t = beg; t < end; ++t) {
+                        const float4 xj = xq[oslot[t]];
+                        const float ddx = xi.x - (xj.x + sx), ddy = xi.y - (xj.y + sy), ddz = xi.z - (xj.z + sz);
+                        const float r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                        if (r2 < r02 && r2 > 0.f) {                           // r2 = 0: the atom itself (zero image)
+                            const float r = sqrtf(r2);
+                            const float f = g.k * (g.r0 - r) / r;
+                            fx += f * ddx; fy += f * ddy; fz += f * ddz;
+                            v += 0.25f * g.k * (g.r0 - r) * (g.r0 - r);        // half of the pair energy
                         }
                     }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                fx += __shfl_xor_sync(0xffffffffu, fx, o);
-                fy += __shfl_xor_sync(0xffffffffu, fy, o);
-                fz += __shfl_xor_sync(0xffffffffu, fz, o);
-                v += __shfl_xor_sync(0xffffffffu, v, o);
-            }
-            if (lane == 0) {
-                force[3 * (int64_t)oi + 0] += fx;
-                force[3 * (int64_t)oi + 1] += fy;
-                force[3 * (int64_t)oi + 2] += fz;
-                V = (double)v;
-            }
-        }
+                }
+        const int64_t oi = perm[s];
+        force[3 * oi + 0] += fx;
+        force[3 * oi + 1] += fy;
+        force[3 * oi + 2] += fz;
+        V = (double)v;
     }
     if (vsum) block_sum_to(V, vsum);
+}
+
+// The oxygen lists of the stand-in repulsion belong to the neighbour list: built once per list.  The step entries
+// call this BEFORE a CUDA-graph capture (workspace growth synchronises, and the three kernels need not be replayed).
+static int standin_prepare(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const sqeq_md_params* p, cudaStream_t st)
+{
+    if (p->k_rep == 0.0 || (ctx->rep_nl == nl && ctx->rep_serial == nl->serial)) return SQEQ_OK;
+    const int ncells = nl->ncell[0] * nl->ncell[1] * nl->ncell[2], no = (int)(n / 3);
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->rep_oslot, sizeof(int) * (size_t)(no + 1)));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->rep_ostart, sizeof(int) * (size_t)(ncells + 1)));
+    k_rep_count<<<ceil_div(ncells, 256), 256, 0, st>>>(ncells, nl->cell_start, nl->perm, (int*)ctx->rep_ostart.p);
+    k_rep_scan<<<1, 1024, 0, st>>>(ncells, (int*)ctx->rep_ostart.p);
+    k_rep_fill<<<ceil_div(ncells, 256), 256, 0, st>>>(ncells, nl->cell_start, nl->perm, (const int*)ctx->rep_ostart.p,
+                                                    (int*)ctx->rep_oslot.p);
+    KERNEL_CHECK(ctx);
+    ctx->rep_nl = nl;
+    ctx->rep_serial = nl->serial;
+    return SQEQ_OK;
 }
 
 // both parts of the stand-in, added to `force`; V into scal[S_VSTAND]
@@ -251,8 +329,12 @@ static int standin_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const flo
         RepGeom g;
         for (int d = 0; d < 3; ++d) { g.nc[d] = nl->ncell[d]; g.L[d] = (float)nl->box[d]; }
         g.k = (float)p->k_rep; g.r0 = (float)p->r_rep;
-        k_md_oo_repulsion<<<ceil_div(n * 32, 256), 256, 0, st>>>(n, (const float4*)ctx->xq.p, nl->cell_of, nl->cell_start,
-                                                                 nl->perm, g, force, scal + S_VSTAND);
+        const float reach = (float)(p->r_rep + (nl->cutoff - p->rc)) * 1.0001f;
+        const int ncells = nl->ncell[0] * nl->ncell[1] * nl->ncell[2], no = (int)(n / 3);
+        SQEQ_TRY(standin_prepare(ctx, nl, n, p, st));       // no-op when the step entry already did it (outside a capture)
+        k_md_oo_repulsion<<<ceil_div(no, 256), 256, 0, st>>>(no, (const float4*)ctx->xq.p, nl->cell_of, (const int*)ctx->rep_ostart.p,
+                                                            (const int*)ctx->rep_oslot.p, nl->perm, g, reach, force,
+                                                            scal + S_VSTAND);
         KERNEL_CHECK(ctx);
     }
     return SQEQ_OK;
@@ -519,6 +601,7 @@ extern "C" int sqeq_shadow_md_run(sqeq_ctx* ctx, sqeq_nlist** nl_io, int64_t n, 
                 key = hash_mix(key, v);
             const unsigned char* pb = (const unsigned char*)p;
             for (size_t k = 0; k < sizeof(sqeq_md_params); ++k) key = hash_mix(key, pb[k]);
+            SQEQ_TRY(standin_prepare(ctx, nl, n, p, st));
             SQEQ_TRY(graph_run(ctx, 1, key, [&]() { return md_step_enqueue(ctx, nl, n, pos, vel, mass, box, p, chi, u, nhist, force, &evals); }));
             ctx->gc.valid = false;          // replays move the atoms without passing through prep_atoms on the host
             ctx->geom_serial++;
