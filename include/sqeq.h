@@ -318,9 +318,9 @@ enum {
     SQEQ_T_PREP,         /* per-evaluation re-gather / fractional coordinates */
     SQEQ_T_REAL,         /* real-space erfc pair sum                  (a-3) */
     SQEQ_T_SPREAD,       /* B-spline spreading incl. grid clear       (a-4) */
-    SQEQ_T_FFT_FWD,      /* cuFFT R2C                                 (a-5) */
+    SQEQ_T_FFT_FWD,      /* forward transforms but the x pass         (a-5) */
     SQEQ_T_INFLUENCE,    /* influence multiply + energy               (a-6) */
-    SQEQ_T_FFT_INV,      /* cuFFT C2R                                 (a-7) */
+    SQEQ_T_FFT_INV,      /* inverse transforms but the x pass         (a-7) */
     SQEQ_T_GATHER,       /* gather                                    (a-8) */
     SQEQ_T_ASSEMBLE,     /* self term, sum, un-permute, energy        (a-9) */
     SQEQ_T_KRYLOV,       /* GMRES / MD vector algebra                 (a-10, a-11) */

@@ -1,8 +1,9 @@
 // fftx.cu -- the fused x-axis pass of the PME reciprocal part, register-resident two-step version.
 //
 // north_star: "the influence-function convolution fused into the FFT pre- and post-passes" (Alg. 2 steps 2-4,
-// PAPER.md:147-149).  The 3-D transforms are split as  [cuFFT 2-D R2C over (y,z), batched over x] -> THIS KERNEL ->
-// [cuFFT 2-D C2R]; this kernel does, for a tile of TJ neighbouring (m1, m2) lines, the forward transform along x, the
+// PAPER.md:147-149).  The 3-D transforms are split as  [z real-to-complex (fftz.cu), y forward (k_yline below); or a
+// batched 2-D cuFFT R2C over (y,z)] -> k_xline2 -> [y inverse, z complex-to-real; or cuFFT 2-D C2R].  k_xline2
+// does, for a tile of TJ neighbouring (m1, m2) lines, the forward transform along x, the
 // multiplication by G(m) with the energy sum, and the inverse transform along x, reading and writing the spectrum
 // once.  K0 = N1 * N2 with N1, N2 <= 16, and each transform is TWO register-resident DFTs (fftx.cuh) around ONE
 // exchange through shared memory:

@@ -309,6 +309,7 @@ static int standin_prepare(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const
     k_rep_scan<<<1, 1024, 0, st>>>(ncells, (int*)ctx->rep_ostart.p);
     k_rep_fill<<<ceil_div(ncells, 256), 256, 0, st>>>(ncells, nl->cell_start, nl->perm, (const int*)ctx->rep_ostart.p,
                                                     (int*)ctx->rep_oslot.p);
+    ctx->launches += 2;
     KERNEL_CHECK(ctx);
     ctx->rep_nl = nl;
     ctx->rep_serial = nl->serial;

@@ -1165,6 +1165,7 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     if (own3) {
         StageTimer tm(ctx, SQEQ_T_FFT_FWD, st);
         SQEQ_TRY(zline_run(ctx, K0 * K1, K2, Wz, grid, spec, false, st));
+        KERNEL_CHECK(ctx);
         SQEQ_TRY(yline_run(ctx, K0, K1, K2h, Wy, spec, false, st));
         KERNEL_CHECK(ctx);
     } else {
@@ -1202,6 +1203,7 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     if (own3) {
         StageTimer tm(ctx, SQEQ_T_FFT_INV, st);
         SQEQ_TRY(yline_run(ctx, K0, K1, K2h, Wy, spec, true, st));
+        KERNEL_CHECK(ctx);
         SQEQ_TRY(zline_run(ctx, K0 * K1, K2, Wz, grid, spec, true, st));
         KERNEL_CHECK(ctx);
     } else {

@@ -155,9 +155,10 @@ k_sub_norm(int64_t len, int64_t ld, int nv, const double* __restrict__ V, const 
 }
 
 // The sweep for column j: h = V^T w, w -= V h, h2 = V^T w, w -= V h2, nrm2 = |w|^2 (h, h2, nrm2 zeroed by the caller).
-static void cgs2_sweep(int64_t len, int64_t ld, int nv, const double* V, double* w, double* h, double* h2, double* nrm2,
-                       cudaStream_t st)
+static void cgs2_sweep(sqeq_ctx* ctx, int64_t len, int64_t ld, int nv, const double* V, double* w, double* h, double* h2,
+                       double* nrm2, cudaStream_t st)
 {
+    ctx->launches += nv <= 8 ? 2 : 4;                       // the caller's KERNEL_CHECK counts the last one
     const int nchunk = ceil_div(len, DOT_CHUNK), nbl = ceil_div(len, 256);
     k_dots<<<dim3(nchunk, nv), 256, 0, st>>>(len, ld, V, w, h);
     if (nv <= 8) {
@@ -346,7 +347,7 @@ static int gmres_fixed_async(sqeq_ctx* ctx, int64_t len, const std::function<int
         double* h = hcols + HL * j;
         double* h2 = h + (m + 2);
         double* nrm2 = h2 + (m + 2);
-        cgs2_sweep(len, ld, j + 1, V, w, h, h2, nrm2, st);
+        cgs2_sweep(ctx, len, ld, j + 1, V, w, h, h2, nrm2, st);
         KERNEL_CHECK(ctx);
         k_normalise<<<nbl, 256, 0, st>>>(len, w, nrm2, V + (int64_t)(j + 1) * ld);
         KERNEL_CHECK(ctx);
@@ -495,7 +496,7 @@ int gmres_solve(sqeq_ctx* ctx, int64_t len, const std::function<int(const double
             {
                 StageTimer tm(ctx, SQEQ_T_KRYLOV, st);
                 CUDA_TRY(ctx, cudaMemsetAsync(h, 0, sizeof(double) * (2 * (m + 2) + 1), st));
-                cgs2_sweep(len, ld, j + 1, V, w, h, h2, nrm2, st);
+                cgs2_sweep(ctx, len, ld, j + 1, V, w, h, h2, nrm2, st);
                 KERNEL_CHECK(ctx);
                 k_normalise<<<nbl, 256, 0, st>>>(len, w, nrm2, V + (int64_t)(j + 1) * ld);
                 KERNEL_CHECK(ctx);
