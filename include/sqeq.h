@@ -346,6 +346,8 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *                         another size: radix-2/3/4/5 passes through shared memory
  *   "fft_own"          1  the y and z passes by own kernels of the same kind too (no cuFFT call in an evaluation) when all
  *                         three extents are among those sizes; 0: batched 2-D cuFFT transforms over (y, z)
+ *   "pme_atom_sched"   1  in those kernels, atoms dealt to lanes by the shared-memory bank their footprint starts on (a warp's
+ *                         lanes then never collide): 0 never, 1 from four tiles per SM on (-8 us at 331,776 atoms), 2 always
  *   "pdl"              1  the transform kernels are launched with programmatic stream serialisation (each starts its
  *                         prologue while the one before drains and waits, griddepcontrol.wait, before touching data):
  *                         -2 us per evaluation where the five kernels are not hidden behind the real-space kernel

@@ -309,6 +309,7 @@ int sqeq_set_option(sqeq_ctx* ctx, const char* name, int value)
     else if (!strcmp(name, "real_tma")) ctx->real_tma = value != 0;
     else if (!strcmp(name, "pairs_staged")) ctx->pairs_staged_off = value == 0;
     else if (!strcmp(name, "pme_atom_threads")) ctx->pme_atom_threads = value;
+    else if (!strcmp(name, "pme_atom_sched")) ctx->pme_atom_sched = value;
     else if (!strcmp(name, "pme_tiles")) { ctx->pme_tiles_off = value == 0; ctx->tile_plan.valid = false; }
     else if (!strcmp(name, "spread_float")) { ctx->spread_float = value != 0; ctx->tile_plan.valid = false; }
     else if (!strcmp(name, "real_staged")) ctx->real_staged_off = value == 0;

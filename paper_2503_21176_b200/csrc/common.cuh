@@ -84,6 +84,8 @@ struct sqeq_ctx {
     DevBuf xf_tw;
     int pme_atom_threads = 1;             // "pme_atom_threads": one thread per atom in the tile kernels: 0 never (lane
                                           // groups), 1 when there are at least two tiles per SM, 2 always
+    int pme_atom_sched = 1;               // "pme_atom_sched": lanes dealt by start bank in those kernels: 0 never, 1 from four
+                                          // tiles per SM on, 2 always
     bool pme_tiles_off = false;           // SQEQ_PME_TILES=0: global-memory spread/gather only (testing)
     DevBuf grid;      // float  [K0][K1][K2]        charge grid Q, then potential grid Phi
     DevBuf gridQ;     // float  copy of Q kept for sqeq_pme_grid (diagnostics only when enabled)

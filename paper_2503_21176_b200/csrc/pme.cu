@@ -777,7 +777,37 @@ k_gather_tile(const float4* __restrict__ frac, const int4* __restrict__ base,
 // walks all P^3 points itself.  No per-chunk weight records in shared memory, no barriers between chunks, no idle
 // lanes, no shuffles: a third of the instructions of the lane-group mappings above (216 shared-memory accesses
 // and as many FMAs or atomics per atom are what is left), at the price of fewer threads per block with work.
-template <int P, bool FORCE, int NT>
+// Which atom of a chunk of up to NT a thread takes, chosen so that the lanes of a warp start on DISTINCT shared-memory
+// banks.  All lanes walk their P^3 points in the same order, so the bank a lane hits at every step is (its atom's
+// first-point address + a common offset) mod 32: with atoms dealt to threads as they come, a warp's 32 start banks are
+// random and a shared access costs about three wavefronts.  Here atoms are bucketed by start bank (`res`, or -1 for a
+// thread without an atom) and the k-th atom of a bucket goes to warp k, lane = bank; atoms beyond the NT/32-th of a
+// bucket fill the slots left empty.  Returns the chunk-local index of the thread's atom or -1.  Every thread of the
+// block calls it (four barriers).
+template <int NT>
+__device__ __forceinline__ int bank_schedule(int res)
+{
+    __shared__ int s_slot[NT], s_free[NT], s_left[NT], s_cnt[32], s_n[2];
+    const int tid = threadIdx.x;
+    s_slot[tid] = -1;
+    if (tid < 32) s_cnt[tid] = 0;
+    if (tid < 2) s_n[tid] = 0;
+    __syncthreads();
+    if (res >= 0) {
+        const int k = atomicAdd(&s_cnt[res], 1);
+        if (k < NT / 32) s_slot[k * 32 + res] = tid;
+        else s_left[atomicAdd(&s_n[0], 1)] = tid;
+    }
+    __syncthreads();
+    const int nleft = s_n[0];
+    if (nleft > 0 && s_slot[tid] < 0) s_free[atomicAdd(&s_n[1], 1)] = tid;
+    __syncthreads();
+    if (tid < nleft) s_slot[s_free[tid]] = s_left[tid];
+    __syncthreads();
+    return s_slot[tid];
+}
+
+template <int P, bool FORCE, int NT, bool SCHED>
 __global__ void __launch_bounds__(NT, 2)
 k_gather_atom(const float4* __restrict__ frac, const int4* __restrict__ base, const int* __restrict__ cell_start,
               TileGeom tg, const float* __restrict__ grid, float sx, float sy, float sz, float4* __restrict__ out)
@@ -789,7 +819,19 @@ k_gather_atom(const float4* __restrict__ frac, const int4* __restrict__ base, co
     tile_move<false>(tile, const_cast<float*>(grid), tb, tg);
     __syncthreads();
     const int K0 = tg.K[0], K1 = tg.K[1], K2 = tg.K[2];
-    for (int i = threadIdx.x; i < tb.natoms; i += NT) {
+    for (int ch = 0; ch < tb.natoms; ch += NT) {
+        int li = ch + (int)threadIdx.x < tb.natoms ? (int)threadIdx.x : -1;
+        if (SCHED) {
+            int res = -1;
+            if (li >= 0) {
+                const int4 f0 = base[tile_atom(ch + li, rbeg, rpre)];
+                const int ux = wrap1(f0.x - tb.o[0], K0), uy = wrap1(f0.y - tb.o[1], K1), uz = wrap1(f0.z - tb.o[2], K2);
+                res = (ux * tg.XS + uy * tg.ZS + uz) & 31;
+            }
+            li = bank_schedule<NT>(res);
+        }
+        if (li < 0) continue;
+        const int i = ch + li;
         const int s = tile_atom(i, rbeg, rpre);
         const float4 fw = frac[s];
         const int4 f = base[s];
@@ -847,7 +889,7 @@ k_gather_atom(const float4* __restrict__ frac, const int4* __restrict__ base, co
     }
 }
 
-template <int P, int NT>
+template <int P, int NT, bool SCHED>
 __global__ void __launch_bounds__(NT, 2)
 k_spread_atom(const float4* __restrict__ frac, const int4* __restrict__ base, const int* __restrict__ cell_start,
               TileGeom tg, float* __restrict__ grid)
@@ -873,7 +915,19 @@ k_spread_atom(const float4* __restrict__ frac, const int4* __restrict__ base, co
     for (int k = 0; k < NT / 32; ++k) aq += s_part[k];
     const float scale = aq > 0.f ? 1073741824.f / (0.2962963f * aq * 1.0001f) : 1.f;
     const float inv_scale = 1.f / scale;
-    for (int i = threadIdx.x; i < tb.natoms; i += NT) {
+    for (int ch = 0; ch < tb.natoms; ch += NT) {
+        int li = ch + (int)threadIdx.x < tb.natoms ? (int)threadIdx.x : -1;
+        if (SCHED) {
+            int res = -1;
+            if (li >= 0) {
+                const int4 f0 = base[tile_atom(ch + li, rbeg, rpre)];
+                const int ux = wrap1(f0.x - tb.o[0], K0), uy = wrap1(f0.y - tb.o[1], K1), uz = wrap1(f0.z - tb.o[2], K2);
+                res = (ux * tg.XS + uy * tg.ZS + uz) & 31;
+            }
+            li = bank_schedule<NT>(res);
+        }
+        if (li < 0) continue;
+        const int i = ch + li;
         const int s = tile_atom(i, rbeg, rpre);
         const float4 fw = frac[s];
         const int4 f = base[s];
@@ -1126,6 +1180,7 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
     // one thread per atom needs many blocks to hide its long serial chains (measured: faster from cfg 3's 343 tiles
     // on, slower at cfg 1/2's 64 and 125): lane groups below two tiles per SM
     const bool atom_threads = ctx->pme_atom_threads == 2 || (ctx->pme_atom_threads == 1 && ngroups >= 2 * ctx->sm_count);
+    const bool atom_sched = ctx->pme_atom_sched == 2 || (ctx->pme_atom_sched == 1 && ngroups >= 4 * ctx->sm_count);
     const int K0 = ctx->K[0], K1 = ctx->K[1], K2 = ctx->K[2], K2h = K2 / 2 + 1;
     const size_t G3 = (size_t)K0 * K1 * K2;
     float* grid = (float*)ctx->grid.p;
@@ -1138,7 +1193,9 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         StageTimer tm(ctx, SQEQ_T_SPREAD, st);
         CUDA_TRY(ctx, cudaMemsetAsync(grid, 0, sizeof(float) * G3, st));
         if (tiles && atom_threads && !ctx->spread_float) {
-            auto kern = k_spread_atom<P, PME_ATOM_NT>;
+            // lanes dealt by start bank where tiles are many (cfg 4: 1000 tiles, -8 us per evaluation; cfg 3: 343 tiles,
+            // +4 us from the four extra barriers)
+            auto kern = atom_sched ? k_spread_atom<P, PME_ATOM_NT, true> : k_spread_atom<P, PME_ATOM_NT, false>;
             CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
             kern<<<ngroups, PME_ATOM_NT, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid);
         } else if (tiles) {
@@ -1218,7 +1275,8 @@ static int pme_run_t(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const doubl
         const float sx = (float)(K0 / box[0]), sy = (float)(K1 / box[1]), sz = (float)(K2 / box[2]);
         float4* rec = (float4*)ctx->rec_out.p;
         if (tiles && atom_threads) {
-            auto kern = want_force ? k_gather_atom<P, true, PME_ATOM_NT> : k_gather_atom<P, false, PME_ATOM_NT>;
+            auto kern = atom_sched ? (want_force ? k_gather_atom<P, true, PME_ATOM_NT, true> : k_gather_atom<P, false, PME_ATOM_NT, true>)
+                                   : (want_force ? k_gather_atom<P, true, PME_ATOM_NT, false> : k_gather_atom<P, false, PME_ATOM_NT, false>);
             CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_bytes));
             kern<<<ngroups, PME_ATOM_NT, tile_bytes, st>>>(frac, base, nl->cell_start, tg, grid, sx, sy, sz, rec);
         } else if (tiles) {
