@@ -114,6 +114,7 @@ struct sqeq_ctx {
     DevBuf vec_f[6];  // float  [n] scratch charge / potential vectors
     DevBuf vec_d[6];  // double [n] scratch
     DevBuf vec_f3[2]; // float  [n][3] scratch forces
+    double diag_box[3] = {0, 0, 0}, diag_alpha = 0, diag_val = 0;     // ewald_self_diag of the last (box, alpha)
     // stand-in O-O repulsion (md.cu): the oxygens' list positions, cell by cell, for the list with this serial
     DevBuf rep_oslot, rep_ostart;
     const void* rep_nl = nullptr;
