@@ -79,9 +79,20 @@ __global__ void k_sub_combo(int64_t len, int64_t ld, int nv, const double* __res
 {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (i >= len) return;
-    double acc = w[i];
-    for (int k = 0; k < nv; ++k) acc -= h[k] * V[(int64_t)k * ld + i];
-    w[i] = acc;
+    // eight loads in flight per thread: with one accumulator the loop runs at the latency of its load (2.4 TB/s at 25
+    // vectors of 331,777 doubles)
+    double a0 = w[i], a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    const double* v = V + i;
+    int k = 0;
+    for (; k + 8 <= nv; k += 8) {
+        double x[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) x[j] = v[(int64_t)(k + j) * ld];
+        a0 -= h[k] * x[0]; a1 -= h[k + 1] * x[1]; a2 -= h[k + 2] * x[2]; a3 -= h[k + 3] * x[3];
+        a0 -= h[k + 4] * x[4]; a1 -= h[k + 5] * x[5]; a2 -= h[k + 6] * x[6]; a3 -= h[k + 7] * x[7];
+    }
+    for (; k < nv; ++k) a0 -= h[k] * v[(int64_t)k * ld];
+    w[i] = (a0 + a1) + (a2 + a3);
 }
 
 // Fused steps of the twice-applied classical Gram-Schmidt sweep.  A dot product is a sum over chunks, and an element of
