@@ -209,7 +209,9 @@ int  sqeq_pme_grid (sqeq_ctx* ctx, int which, float* out);
  *   tol         stop when the GMRES residual estimate ||b-Ax||/||b|| <= tol
  *   max_iter    maximum number of Coulomb evaluations; restart: Krylov dimension (0 = unrestarted,
  *               i.e. up to max_iter vectors)
- *   q_out       device fp32 [n]; lambda_out, iters_out, relres_out: host scalars (may be NULL)
+ *   q_out       device fp32 [n]; lambda_out, iters_out, relres_out: host scalars (may be NULL).  *iters_out counts the
+ *               Coulomb evaluations the returned solution is built from; with tol > 0 the host judges an iteration
+ *               while the next one already runs, so one further evaluation is launched and discarded
  * Returns SQEQ_ENOTCONV if tol was not reached (outputs are still written).  Synchronises. */
 int  sqeq_qeq_solve(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos,
                     const double box[3], double rc, double alpha, const int grid[3], int order,

@@ -226,6 +226,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
     if (ctx->h_scal) cudaFreeHost(ctx->h_scal);
     if (ctx->h_nl) cudaFreeHost(ctx->h_nl);
     if (ctx->h_kry) cudaFreeHost(ctx->h_kry);
+    for (auto& e : ctx->kry_ev) if (e) cudaEventDestroy(e);
     if (ctx->h_slot_e) cudaFreeHost(ctx->h_slot_e);
     if (ctx->h_ring) cudaFreeHost(ctx->h_ring);
     if (ctx->d_ring) cudaFree(ctx->d_ring);

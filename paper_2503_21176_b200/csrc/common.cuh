@@ -49,6 +49,7 @@ struct sqeq_ctx {
     cudaMemPool_t pool = nullptr;         // stream-ordered pool for neighbour-list storage (kept across rebuilds)
     double* h_kry = nullptr;              // pinned: GMRES coefficients of a whole cycle (deferred host pass)
     size_t h_kry_cap = 0;
+    cudaEvent_t kry_ev[4] = {nullptr, nullptr, nullptr, nullptr};   // behind the coefficient copies of the last iterations
     int64_t nl_last_n = 0, nl_last_total = 0;   // sizes of the previous build: next build's estimate
     int nl_last_max_row = 0;
     int nl_last_fmt = 1;
