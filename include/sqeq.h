@@ -366,6 +366,20 @@ int  sqeq_profile_read  (sqeq_ctx* ctx, int stage, double* total_ms, int64_t* la
  *                         takes effect at the next sqeq_nl_build)
  * Synchronises the stream.  SQEQ_EINVAL for an unknown name. */
 int  sqeq_set_option(sqeq_ctx* ctx, const char* name, int value);
+/* ---- an entry point that allocates nothing --------------------------------------------------------------------
+ * E = 1/2 sum_i q_i phi_i (Eq. 5; what sqeq_coulomb returns in *energy, k_e = 1) for callers that cannot
+ * call cudaMalloc (CUDA-graph capture, serving loops, harnesses that forbid it): no context, no cudaMalloc / cudaFree,
+ * no allocating library routine.  The reduction's scratch (one fp64 partial sum per 1,024 atoms and a counter) is a
+ * file-scope __device__ array of 32.25 KB that every GPU loading the library holds until exit; hence the limit
+ * n <= SQEQ_NOALLOC_MAX_N, beyond which the call returns SQEQ_EINVAL with a message in sqeq_last_error(NULL).
+ *   device      ordinal; made current.  cuda_stream: cudaStream_t (may be 0); the work is enqueued there, no
+ *               synchronisation.  The first call per device looks up the array's device address (not under capture).
+ *   q, phi      device fp32 [n], caller-owned;  energy_dev: DEVICE double, written when the kernel runs
+ * All calls on a device share the array: calls that overlap on the GPU (different streams) race; calls on one stream
+ * are ordered.  Fixed summation order: the same inputs give the same bits on every call. */
+#define SQEQ_NOALLOC_MAX_N 4194304
+int  sqeq_energy_noalloc(int device, void* cuda_stream, int64_t n, const float* q, const float* phi, double* energy_dev);
+
 /* Number of the library's own kernel launches (cuFFT's excluded) since sqeq_create / last reset. */
 int  sqeq_launch_count  (sqeq_ctx* ctx, int64_t* launches, int reset);
 

@@ -72,6 +72,7 @@ def load():
     L.sqeq_energy_fetch.argtypes = [vp, dp]
     L.sqeq_coulomb_ewald.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, vp, vp, dp]
     L.sqeq_ewald_params.argtypes = [dp, dbl, dbl, dp, ip, ip]
+    L.sqeq_energy_noalloc.argtypes = [cint, vp, i64, vp, vp, vp]
     L.sqeq_geometry_set.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint]
     L.sqeq_coulomb_fixed.argtypes = [vp, i64, vp, vp, vp, cint]
     L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
@@ -479,6 +480,24 @@ class Context:
         c = ctypes.c_int64()
         self._check(load().sqeq_launch_count(self.handle, ctypes.byref(c), int(reset)))
         return c.value
+
+
+NOALLOC_MAX_N = 4194304
+
+
+def energy_noalloc(q, phi, out, stream=None):
+    """sqeq_energy_noalloc: out (device float64 tensor of one element) <- 1/2 sum q phi on `stream`; allocates nothing."""
+    dev = q.device
+    if stream is None:
+        stream = torch.cuda.current_stream(dev)
+    n = q.shape[0]
+    if out.dtype != torch.float64 or out.numel() != 1 or not out.is_cuda:
+        raise ValueError("out must be a CUDA float64 tensor with one element")
+    rc_ = load().sqeq_energy_noalloc(dev.index or 0, ctypes.c_void_p(stream.cuda_stream), n, _ptr(q, torch.float32, n),
+                                     _ptr(phi, torch.float32, n), ctypes.c_void_p(out.data_ptr()))
+    if rc_ != OK:
+        raise SqeqError(rc_, load().sqeq_last_error(None).decode())
+    return out
 
 
 def ewald_params(box, rc, delta):

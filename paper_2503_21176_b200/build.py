@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsqeq.so")
-SOURCES = ["api.cu", "nlist.cu", "realspace.cu", "pme.cu", "fftx.cu", "fftz.cu", "ewald.cu", "qeq.cu", "md.cu"]
+SOURCES = ["api.cu", "nlist.cu", "realspace.cu", "pme.cu", "fftx.cu", "fftz.cu", "ewald.cu", "qeq.cu", "md.cu", "noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "--fmad=true"]
