@@ -695,6 +695,27 @@ def run_md_legs(ctx, cfg, pos, n, dev, args):
     msq = e0.elapsed_time(e1)
     res["qeq_krylov_iters_per_s"] = it / (msq * 1e-3)
     res["qeq_relres_after_%d_iters" % it] = rel
+    # NEXT-1: potentials of several charge vectors on one geometry: one by one (sqeq_coulomb_fixed) and batched
+    # (sqeq_coulomb_fixed_batch: up to four vectors per pass over the geometry cache)
+    rng = np.random.default_rng(7)
+    qh = q.cpu().numpy()
+    vecs = torch.as_tensor(np.stack([qh * rng.uniform(0.5, 1.5, n) for _ in range(4)]).astype(np.float32)).to(dev)
+    phis = torch.empty((4, n), dtype=torch.float32, device=dev)
+    ctx.geometry_set(nl, pos, box, cfg.rc, cfg.alpha, cfg.grid, cfg.order)
+    ctx.coulomb_fixed(vecs[0], phis[0])
+    def per_vector(f, nv, rep=20):
+        for _ in range(3):
+            f()
+        torch.cuda.synchronize()
+        e0.record(ctx.stream)
+        for _ in range(rep):
+            f()
+        e1.record(ctx.stream)
+        torch.cuda.synchronize()
+        return round(e0.elapsed_time(e1) / (rep * nv), 4)
+    res["fixed_geometry_ms_per_vector"] = {"one_by_one": per_vector(lambda: ctx.coulomb_fixed(vecs[1], phis[1]), 1),
+                                           "batch_2": per_vector(lambda: ctx.coulomb_fixed_batch(vecs[:2], phis[:2]), 2),
+                                           "batch_4": per_vector(lambda: ctx.coulomb_fixed_batch(vecs, phis), 4)}
     nl.free()
     # a-11: configs[4]'s workload as written: 100 shadow XL-BOMD steps, 0.5 fs, 4 Krylov-rank updates per step; the list
     # is rebuilt when the displacement would reach skin/2 (about every 10 steps at 300 K)

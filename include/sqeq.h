@@ -193,6 +193,12 @@ int  sqeq_ewald_params(const double box[3], double rc, double delta, double* alp
 int  sqeq_geometry_set (sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const float* pos, const double box[3],
                         double rc, double alpha, const int grid[3], int order);
 int  sqeq_coulomb_fixed(sqeq_ctx* ctx, int64_t n, const float* q, float* phi, float* force, int want_energy);
+/* The batched form (the other half of NEXT-1): potentials of nvec (1..64) charge vectors q[nvec][n]
+ * (device fp32, row v = vector v) on the geometry of the last sqeq_geometry_set -> phi[nvec][n].  Up to four vectors
+ * share ONE pass over the geometry cache for the real-space part (the cache stream bounds the single-vector kernel:
+ * 0.145 ms for one vector at 331,776 atoms, 0.19 for four); the reciprocal part runs per vector on the shared prepared
+ * geometry.  The first vector on a fresh geometry is evaluated alone (it writes the cache).  No synchronisation. */
+int  sqeq_coulomb_fixed_batch(sqeq_ctx* ctx, int64_t n, int nvec, const float* q, float* phi);
 
 /* Parts of the last sqeq_coulomb call on this context, for diagnostics and stage-wise parity
  * (caller order; device fp32 outputs, any may be NULL): phi_real[n], F_real[n][3], phi_rec[n],

@@ -75,6 +75,7 @@ def load():
     L.sqeq_energy_noalloc.argtypes = [cint, vp, i64, vp, vp, vp]
     L.sqeq_geometry_set.argtypes = [vp, vp, i64, vp, dp, dbl, dbl, ip, cint]
     L.sqeq_coulomb_fixed.argtypes = [vp, i64, vp, vp, vp, cint]
+    L.sqeq_coulomb_fixed_batch.argtypes = [vp, i64, cint, vp, vp]
     L.sqeq_coulomb_host.argtypes = [vp, vp, i64, vp, vp, dp, dbl, dbl, ip, cint, vp, vp, dp]
     L.sqeq_coulomb_parts.argtypes = [vp, vp, i64, vp, vp, vp, vp, dp]
     L.sqeq_pme_grid.argtypes = [vp, cint, vp]
@@ -302,6 +303,15 @@ class Context:
                                               _ptr(phi, torch.float32, n) if phi is not None else None,
                                               _ptr(force, torch.float32, 3 * n) if force is not None else None,
                                               int(want_energy)))
+
+    def coulomb_fixed_batch(self, q, phi=None):
+        """sqeq_coulomb_fixed_batch: potentials of the charge vectors q[nvec][n] on the geometry of geometry_set."""
+        nvec, n = q.shape
+        if phi is None:
+            phi = torch.empty((nvec, n), dtype=torch.float32, device=self.device)
+        self._check(load().sqeq_coulomb_fixed_batch(self.handle, n, nvec, _ptr(q, torch.float32, nvec * n),
+                                                    _ptr(phi, torch.float32, nvec * n)))
+        return phi
 
     def energy_fetch(self):
         e = ctypes.c_double()

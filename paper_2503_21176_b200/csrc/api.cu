@@ -216,7 +216,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
     DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len, &ctx->ew_tab, &ctx->ew_sf, &ctx->xf_tw,
                       &ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
                       &ctx->base, &ctx->real_out, &ctx->rec_out, &ctx->scal, &ctx->kry_V,
-                      &ctx->kry_w, &ctx->kry_h, &ctx->rep_oslot, &ctx->rep_ostart};
+                      &ctx->kry_w, &ctx->kry_h, &ctx->rep_oslot, &ctx->rep_ostart, &ctx->batch_q, &ctx->batch_r};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto& b : ctx->vec_f) if (b.p) cudaFree(b.p);
@@ -604,6 +604,69 @@ extern "C" int sqeq_coulomb_fixed(sqeq_ctx* ctx, int64_t n, const float* q, floa
         SQEQ_TRY(body());
     }
     ctx->energy_pending = want_energy != 0;
+    return SQEQ_OK;
+}
+
+// NEXT-1, the batched half: potentials of nvec charge vectors on the fixed geometry.  The real-space part of up to four
+// vectors is ONE pass over the geometry cache (its 6 B per entry stream is what bounds the single-vector kernel); the
+// reciprocal part runs per vector on the shared prepared geometry (spreading and gathering are bound by their 216
+// shared-memory atomics / loads per atom AND vector, the transforms by their points per vector: nothing there is shared
+// between vectors but the spline weights).
+extern "C" int sqeq_coulomb_fixed_batch(sqeq_ctx* ctx, int64_t n, int nvec, const float* q, float* phi)
+{
+    if (!ctx) return SQEQ_EINVAL;
+    const sqeq_nlist* nl = ctx->fixed.nl;
+    bool alive = false;
+    for (const sqeq_nlist* l : ctx->lists) alive = alive || (l == nl && l->serial == ctx->fixed.serial);
+    if (!nl || !alive || ctx->geom_serial != ctx->fixed.geom_serial)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_fixed_batch: no geometry set (sqeq_geometry_set), its list was freed, or "
+                                           "another evaluation has replaced it");
+    if (n != ctx->fixed.n || !q || !phi || nvec < 1 || nvec > 64)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "sqeq_coulomb_fixed_batch: n differs from the geometry, NULL argument, or nvec outside [1, 64]");
+    CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    auto single = [&](int v) -> int {
+        SQEQ_TRY(prep_charges(ctx, nl, q + (int64_t)v * n, nullptr, st));
+        return coulomb_eval(ctx, nl, n, ctx->fixed.box, ctx->fixed.rc, ctx->fixed.alpha, phi + (int64_t)v * n, nullptr, false, false,
+                            GEOM_FIXED);
+    };
+    int v0 = 0;
+    auto warm = [&]() { return ctx->gc.valid && ctx->gc.nl == nl && ctx->gc.serial == nl->serial && ctx->gc.rc == ctx->fixed.rc &&
+                               ctx->gc.alpha == ctx->fixed.alpha && nl->fmt == 1; };
+    if (!warm()) SQEQ_TRY(single(v0++));                   // the first evaluation on a geometry writes the cache
+    auto rest = [&]() -> int {
+        int v = v0;
+        while (v < nvec) {
+            const int nb = nvec - v < 4 ? nvec - v : 4;
+            if (nb == 1 || !warm()) {
+                SQEQ_TRY(single(v++));
+                continue;
+            }
+            SQEQ_TRY(realspace_cached_multi(ctx, nl, nb, q + (int64_t)v * n, st));
+            for (int k = 0; k < nb; ++k) {
+                SQEQ_TRY(prep_charges(ctx, nl, q + (int64_t)(v + k) * n, nullptr, st));
+                ctx->overlap_now = false;
+                SQEQ_TRY(pme_run(ctx, nl, n, ctx->fixed.box, false, false, st));
+                SQEQ_TRY(realspace_multi_select(ctx, nl, k, st));
+                SQEQ_TRY(assemble_run(ctx, nl, ctx->fixed.alpha, phi + (int64_t)(v + k) * n, nullptr, false, false, st));
+            }
+            v += nb;
+        }
+        return SQEQ_OK;
+    };
+    if (v0 < nvec) {
+        if (warm()) {
+            // the same sequence of launches every time: replayed as a CUDA graph (as sqeq_coulomb_fixed does)
+            uint64_t key = hash_mix(0x52, ctx->geom_serial);
+            for (uint64_t x : {(uint64_t)(uintptr_t)q, (uint64_t)(uintptr_t)phi, (uint64_t)nvec, (uint64_t)v0}) key = hash_mix(key, x);
+            SQEQ_TRY(graph_run(ctx, 2, key, rest));
+        } else {
+            SQEQ_TRY(rest());
+        }
+    }
+    ctx->last_had_force = false;
+    ctx->last_n = n;
+    ctx->energy_pending = false;
     return SQEQ_OK;
 }
 

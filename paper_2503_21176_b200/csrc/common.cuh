@@ -118,6 +118,7 @@ struct sqeq_ctx {
     double diag_box[3] = {0, 0, 0}, diag_alpha = 0, diag_val = 0;     // ewald_self_diag of the last (box, alpha)
     // stand-in O-O repulsion (md.cu): the oxygens' list positions, cell by cell, for the list with this serial
     DevBuf rep_oslot, rep_ostart;
+    DevBuf batch_q, batch_r;              // sqeq_coulomb_fixed_batch: [4][n] sorted charge vectors / real-space potentials
     const void* rep_nl = nullptr;
     uint64_t rep_serial = 0;
     GeomCache gc;
@@ -303,6 +304,8 @@ int prep_charges(sqeq_ctx* ctx, const sqeq_nlist* nl, const float* q_f, const do
                  cudaStream_t st);
 int realspace_run(sqeq_ctx* ctx, const sqeq_nlist* nl, double rc, double alpha, bool want_force,
                   cudaStream_t st, int geom = GEOM_NEW, bool want_phi = true);
+int realspace_cached_multi(sqeq_ctx* ctx, const sqeq_nlist* nl, int nvec, const float* q, cudaStream_t st);
+int realspace_multi_select(sqeq_ctx* ctx, const sqeq_nlist* nl, int v, cudaStream_t st);
 int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3], int order);
 // nl supplies the cell-major atom runs the shared-memory tiles are built on (NULL: global kernels)
 int pme_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3], bool want_force,

@@ -523,6 +523,128 @@ k_real_cached(const float4* __restrict__ xq, const int* __restrict__ cell_start,
     }   // row batches
 }
 
+// NEXT-1, batched right-hand sides: the same sparse product for NV charge vectors in ONE pass over the cache
+// (phi^v_i = sum_j t_ij q^v_j, v < NV).  The cache stream (6 B per entry) is what bounds k_real_cached; here it is read
+// once for all vectors.  The neighbourhood's charges are staged interleaved (NV floats per slot: one LDS.64 / LDS.128 per
+// entry), qs_sorted = the vectors in the list's sorted order [NV][n], out = [NV][n] in sorted order.
+template <int NV, bool SCALED>
+__global__ void __launch_bounds__(REAL_NT, 3)
+k_real_cached_multi(const float* __restrict__ qs_sorted, int64_t n, const int* __restrict__ cell_start, GroupGeom gg,
+                    const int64_t* __restrict__ row_start, int ngroups, float* __restrict__ out, RealCache rcache)
+{
+    static_assert(NV == 2 || NV == 4, "two or four vectors per pass");
+    extern __shared__ __align__(16) float4 xs[];               // float [pop + 1][NV]
+    __shared__ GroupPiece pieces[GRP_MAXPIECE];
+    __shared__ int s_scratch, s_roff[GRP_G * GRP_G], s_rpre[GRP_G * GRP_G + 1];
+    float* qs = (float*)xs;
+    const int grp = blockIdx.x;
+    const GroupInfo gi = group_layout(gg, cell_start, grp, pieces, &s_scratch);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        int acc = 0;
+        for (int r = 0; r < GRP_G * GRP_G; ++r) {
+            s_rpre[r] = acc;
+            const int ix = r / GRP_G, iy = r % GRP_G;
+            if (ix < gi.ge[0] && iy < gi.ge[1]) {
+                const int colw = ((gi.c0[0] + ix) * gg.nc[1] + gi.c0[1] + iy) * gg.nc[2] + gi.c0[2];
+                const int beg = cell_start[colw];
+                s_roff[r] = beg - acc;
+                acc += cell_start[colw + gi.ge[2]] - beg;
+            } else {
+                s_roff[r] = 0;
+            }
+        }
+        s_rpre[GRP_G * GRP_G] = acc;
+        for (int v = 0; v < NV; ++v) qs[gi.pop * NV + v] = 0.f;    // the slot the row padding points at
+    }
+    const int np = gi.ncol * 3;
+    for (int ip = wid; ip < np; ip += REAL_NT / 32) {
+        const GroupPiece pc = pieces[ip];
+        for (int k = lane; k < pc.len; k += 32)
+#pragma unroll
+            for (int v = 0; v < NV; ++v) qs[(pc.lbase + k) * NV + v] = __ldg(qs_sorted + (int64_t)v * n + pc.gbeg + k);
+    }
+    __syncthreads();
+    const int natoms = s_rpre[GRP_G * GRP_G];
+    const int p1 = s_rpre[1], p2 = s_rpre[2], p3 = s_rpre[3];
+    const unsigned xs_addr = (unsigned)__cvta_generic_to_shared(xs);
+    constexpr int NW = REAL_NT / 32;
+    for (int base = 0; base < natoms; base += NW * 32) {
+        int my_s = 0, my_len = 0;
+        int64_t my_r0 = 0;
+        {
+            const int ia = base + wid + NW * lane;
+            if (ia < natoms) {
+                my_s = ia + s_roff[(ia >= p1) + (ia >= p2) + (ia >= p3)];
+                my_r0 = row_start[my_s];
+                my_len = rcache.len[my_s];
+            }
+        }
+        for (int l = 0; l < 32; ++l) {
+            const int ia = base + wid + NW * l;
+            if (ia >= natoms) break;
+            const int s = __shfl_sync(0xffffffffu, my_s, l);
+            const int len_s = __shfl_sync(0xffffffffu, my_len, l);
+            const int64_t r0 = __shfl_sync(0xffffffffu, my_r0, l) + 4 * lane;
+            const uint2* __restrict__ ri = (const uint2*)(rcache.idx + r0);
+            const float4* __restrict__ rv = (const float4*)(rcache.t + r0);
+            const int padlen = (len_s + 31) & ~31;
+            float acc[NV];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) acc[v] = 0.f;
+            auto term = [&](unsigned e, float t) {                 // e: 16-bit entry (slot, or slot << 4 when SCALED)
+                if (NV == 2) {
+                    float q0, q1;
+                    const unsigned a = xs_addr + (SCALED ? e >> 1 : e << 3);
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(q0), "=f"(q1) : "r"(a));
+                    acc[0] = fmaf(q0, t, acc[0]);
+                    acc[1] = fmaf(q1, t, acc[1]);
+                } else {
+                    const float4 qv = lds128(xs_addr + (SCALED ? e : e << 4));
+                    acc[0] = fmaf(qv.x, t, acc[0]);
+                    acc[1] = fmaf(qv.y, t, acc[1]);
+                    acc[NV - 2] = fmaf(qv.z, t, acc[NV - 2]);
+                    acc[NV - 1] = fmaf(qv.w, t, acc[NV - 1]);
+                }
+            };
+            constexpr int B = 4;                                   // chunks of 128 entries in flight
+            for (int c0 = 0; c0 < padlen; c0 += 128 * B) {
+                uint2 e[B];
+                float4 t[B];
+#pragma unroll
+                for (int k = 0; k < B; ++k) {
+                    e[k] = make_uint2(0u, 0u);
+                    t[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (c0 + 128 * k + 4 * lane < padlen) {
+                        e[k] = __ldg(ri + ((c0 + 128 * k) >> 2));
+                        t[k] = __ldg(rv + ((c0 + 128 * k) >> 2));
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < B; ++k) {
+                    if (c0 + 128 * k < padlen) {
+                        term(e[k].x & 0xffffu, t[k].x);
+                        term(e[k].x >> 16, t[k].y);
+                        term(e[k].y & 0xffffu, t[k].z);
+                        term(e[k].y >> 16, t[k].w);
+                    }
+                }
+            }
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) acc[v] += __shfl_xor_sync(0xffffffffu, acc[v], o);
+            }
+            if (lane < NV) {
+                float r = acc[0];
+#pragma unroll
+                for (int v = 1; v < NV; ++v) r = lane == v ? acc[v] : r;
+                out[(int64_t)lane * n + s] = r;
+            }
+        }
+    }
+}
+
 // The same sparse product with the rows STREAMED BY THE BULK-COPY ENGINE (TMA 1-D, cp.async.bulk + mbarrier): one
 // lane of a warp asks for a whole row -- its compact entries and their t, two contiguous 16-byte-aligned stretches of
 // the cache -- to be copied into the warp's shared-memory buffer, and the copy of the NEXT row is in flight while the
@@ -671,6 +793,57 @@ k_real_cached_tma(const float4* __restrict__ xq, const int* __restrict__ cell_st
             if (lane == 0) out[s] = make_float4(0.f, 0.f, 0.f, a3);
         }
     }
+}
+
+// ---- batched right-hand sides on the geometry cache (NEXT-1) ------------------------------------------------------
+// qs[v][s] = q[v][perm[s]] for v < nvec, zero for nvec <= v < nv (the kernel takes two or four vectors)
+__global__ void k_sort_charges_multi(int64_t n, int nvec, int nv, const float* __restrict__ q, const int* __restrict__ perm,
+                                     float* __restrict__ qs)
+{
+    const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int64_t i = perm[s];
+    for (int v = 0; v < nv; ++v) qs[(int64_t)v * n + s] = v < nvec ? q[(int64_t)v * n + i] : 0.f;
+}
+
+__global__ void k_multi_to_out(int64_t n, const float* __restrict__ r, float4* __restrict__ out)
+{
+    const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s < n) out[s] = make_float4(0.f, 0.f, 0.f, r[s]);
+}
+
+// Real-space potentials of nvec (1..4) charge vectors q[nvec][n] (caller order) in one pass over the geometry cache of
+// `nl` (which must be warm: the caller checks); results in ctx->batch_r [nv][n], sorted order.
+int realspace_cached_multi(sqeq_ctx* ctx, const sqeq_nlist* nl, int nvec, const float* q, cudaStream_t st)
+{
+    const int64_t n = nl->n;
+    const int nv = nvec <= 2 ? 2 : 4;
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->batch_q, sizeof(float) * 4 * (size_t)n));
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->batch_r, sizeof(float) * 4 * (size_t)n));
+    GeomCache& gc = ctx->gc;
+    RealCache rcache = {(uint16_t*)gc.idx.p, (float*)gc.t.p, (int*)gc.len.p};
+    k_sort_charges_multi<<<ceil_div(n, 256), 256, 0, st>>>(n, nvec, nv, q, nl->perm, (float*)ctx->batch_q.p);
+    KERNEL_CHECK(ctx);
+    StageTimer tm(ctx, SQEQ_T_REAL, st);
+    const int ngroups = nl->gg.ng[0] * nl->gg.ng[1] * nl->gg.ng[2];
+    const size_t sm = sizeof(float) * nv * ((size_t)nl->max_pop + 1);
+    auto kern = nv == 2 ? (nl->lshift ? k_real_cached_multi<2, true> : k_real_cached_multi<2, false>)
+                        : (nl->lshift ? k_real_cached_multi<4, true> : k_real_cached_multi<4, false>);
+    CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    kern<<<ngroups, REAL_NT, sm, st>>>((const float*)ctx->batch_q.p, n, nl->cell_start, nl->gg, nl->row_start, ngroups,
+                                       (float*)ctx->batch_r.p, rcache);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
+}
+
+// vector v of the last realspace_cached_multi into the slot the assembly reads
+int realspace_multi_select(sqeq_ctx* ctx, const sqeq_nlist* nl, int v, cudaStream_t st)
+{
+    const int64_t n = nl->n;
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->real_out, sizeof(float4) * n));
+    k_multi_to_out<<<ceil_div(n, 256), 256, 0, st>>>(n, (const float*)ctx->batch_r.p + (int64_t)v * n, (float4*)ctx->real_out.p);
+    KERNEL_CHECK(ctx);
+    return SQEQ_OK;
 }
 
 // geom: GEOM_NEW = plain evaluation; GEOM_BUILD = plain evaluation that also writes the geometry cache (t, and g

@@ -768,6 +768,38 @@ def test_fixed_geometry_cache(ctx, k):
     nl.free()
 
 
+@pytest.mark.parametrize("k", [2, 4])
+def test_fixed_geometry_batched_vectors(ctx, k):
+    """NEXT-1, the batched half: sqeq_coulomb_fixed_batch -- nvec charge vectors, up to four per pass over the
+    geometry cache.  Cold cache (the first vector is evaluated alone and writes it) and warm cache; nvec = 1, 2, 3, 4,
+    7 (a group of four, then three); every vector against the oracle (cfg 2: all atoms; cfg 4: sampled rows) and
+    against the single-vector entry."""
+    c = W.CONFIGS[k]
+    pos, q = inputs(k)
+    n = len(q)
+    rng = np.random.default_rng(60 + k)
+    nl = ctx.nl_build(dev(pos), c.box, c.rc + 1.0)
+    p = W.perturb(pos, 0, 0.02, cfg_index=3)
+    rows = None if k == 2 else np.sort(rng.choice(n, 128, replace=False))
+    sel = slice(None) if rows is None else rows
+    vecs = np.stack([q] + [(rng.normal(size=n) if j % 2 else q * rng.uniform(0.5, 1.5, n)).astype(np.float32) for j in range(6)])
+    want = [oracle.coulomb_pme(p, v, c.box, c.rc, c.alpha, c.grid, c.order, rows=rows)[0] for v in vecs[:4 if k == 4 else 7]]
+    worst = 0.0
+    for nvec, cold in ((7 if k == 2 else 4, True), (1, False), (2, False), (3, True), (4, False)):
+        if cold:
+            ctx.geometry_set(nl, dev(p), c.box, c.rc, c.alpha, c.grid, c.order)
+        phi = ctx.coulomb_fixed_batch(dev(vecs[:nvec])).cpu().numpy()
+        for v in range(nvec):
+            e = relrms(phi[v][sel], want[v])
+            worst = max(worst, e)
+            assert e < TOL, (nvec, cold, v, e)
+    one = torch.empty(n, device="cuda")
+    ctx.coulomb_fixed(dev(vecs[2]), one)
+    assert relrms(phi[2], one.cpu().numpy()) < 1e-6
+    record(f"fixed_geometry_batch_cfg{k}", worst_relrms_phi=worst)
+    nl.free()
+
+
 def test_pme_thread_per_atom_kernels(ctx):
     """The one-thread-per-atom tile kernels (default from two tiles per SM on, i.e. cfg 3 and cfg 4) forced on for the
     small configs too, all three spline orders, atoms that left their window, potential-only mode."""
