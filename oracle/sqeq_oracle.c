@@ -470,6 +470,10 @@ void orc_dft3(double *z, const int K[3], int sign)
 /* |b(m)|^2 = 1 / | sum_{k=0}^{p-2} M_p(k+1) e^{2 pi i m k/K} |^2  (DESIGN.md R-PME) */
 static double orc_bmod2(int m, int K, int p)
 {
+    /* odd p, m = K/2: the sum below is exactly zero (M_p(k+1) is symmetric in k about (p-2)/2 and the signs
+     * alternate), the order-p exponential spline cannot carry the Nyquist frequency.  The paper is silent on odd
+     * orders; reading G19: that plane is left out, |b|^2 := 0, hence G = 0 there. */
+    if ((p & 1) && 2 * m == K) return 0.0;
     double re = 0.0, im = 0.0;
     for (int k = 0; k <= p - 2; ++k) {
         double a = 2.0 * ORC_PI * (double)m * (double)k / (double)K;

@@ -450,3 +450,36 @@ def test_shadow_closed_form_eq22():
     q, lam = oracle.shadow_charges(chi, u, v, 0.25)
     assert abs(q.sum() - 0.25) < 1e-13
     assert np.abs(u * q + lam + chi + v).max() < 1e-13       # rows of Eq. 22
+
+
+def test_pme_odd_spline_orders_converge_between_their_neighbours():
+    """Odd orders (reading G19: for odd p the Nyquist plane m_d = K_d/2, where the order-p
+    exponential spline vanishes identically, is left out of the influence function).  Pinned by what the method must
+    do, not by itself: against the CONVERGED Ewald sum the error of smooth PME falls with every order, 4 > 5 > 6 > 7 > 8,
+    on a coarse and on a fine mesh, and order 5 gains at least 2^4 from a mesh 1.6 times finer; a wrong Nyquist rule
+    (a huge or NaN |b|^2 there) breaks the ordering at once."""
+    box = (13.0, 11.0, 12.0)
+    rng = np.random.default_rng(5)
+    m = 5
+    g = np.stack(np.meshgrid(*[np.arange(m)] * 3, indexing="ij"), -1).reshape(-1, 3)
+    pos = (g + 0.5) / m * np.array(box) + rng.uniform(-0.3, 0.3, (m ** 3, 3))
+    q = np.where(g.sum(1) % 2 == 0, 1.0, -1.0) * rng.uniform(0.6, 1.0, m ** 3)
+    q -= q.mean()
+    alpha, rc = 0.7, 5.4                       # erfc(alpha rc) = 9e-8: the real-space truncation is out of the way
+    p0, F0, _ = oracle.ewald_direct(pos, q, box, alpha)
+    err = {}
+    for grid in ((20, 18, 18), (32, 28, 30)):
+        for order in (4, 5, 6, 7, 8):
+            pp, Fp, _, _ = oracle.coulomb_pme(pos, q, box, rc, alpha, list(grid), order)
+            assert np.isfinite(pp).all() and np.isfinite(Fp).all()
+            err[grid, order] = relrms(Fp, F0)
+        e = [err[grid, o] for o in (4, 5, 6, 7, 8)]
+        assert all(a > 1.8 * b for a, b in zip(e, e[1:])), e
+    assert err[(20, 18, 18), 5] > 10 * err[(32, 28, 30), 5]
+    # the rule itself: G vanishes on the Nyquist planes for odd p and nowhere else but the origin
+    G = oracle.pme_influence(box, [8, 10, 12], 5, alpha)
+    assert np.all(G[4, :, :] == 0) and np.all(G[:, 5, :] == 0) and np.all(G[:, :, 6] == 0)
+    mask = np.ones_like(G, dtype=bool)
+    mask[4, :, :] = mask[:, 5, :] = mask[:, :, 6] = False
+    mask[0, 0, 0] = False
+    assert np.all(G[mask] > 0) and np.all(np.isfinite(G))
