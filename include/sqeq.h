@@ -121,7 +121,8 @@ int  sqeq_nl_free  (sqeq_nlist* nl);
  *           background term is omitted, DESIGN.md R-G11)
  *   rc      real-space cutoff, 0 < rc <= list cutoff
  *   alpha   Ewald splitting parameter (1/Angstrom), > 0
- *   grid    host int[3] PME grid points per axis, each >= order and even; order in {4, 6, 8}
+ *   grid    host int[3] PME grid points per axis, each >= order and even; order in 4..8 (6 is the paper's; for the odd ones
+ *           the Nyquist plane is left out of the influence function, reading G19)
  *   phi     device fp32 [n]    out: phi_i = dE/dq_i (may be NULL)
  *   force   device fp32 [n][3] out: F_i = -dE/dr_i; NULL selects the cheaper potential-only mode
  *   energy  host double* out: E = 1/2 sum q_i phi_i (may be NULL; non-NULL synchronises the stream)

@@ -467,8 +467,8 @@ int validate_coulomb_args(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const 
         return sqeq_fail(ctx, SQEQ_EINVAL, "%s: rc = %g must satisfy 0 < rc <= list cutoff %g", who, rc, nl->cutoff);
     if (!(alpha > 0.0) || !isfinite(alpha))
         return sqeq_fail(ctx, SQEQ_EINVAL, "%s: alpha = %g must be > 0", who, alpha);
-    if (order != 4 && order != 6 && order != 8)
-        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: spline order %d unsupported (4, 6 or 8)", who, order);
+    if (order < 4 || order > 8)
+        return sqeq_fail(ctx, SQEQ_EINVAL, "%s: spline order %d unsupported (4 to 8)", who, order);
     if (!grid) return sqeq_fail(ctx, SQEQ_EINVAL, "%s: grid is NULL", who);
     for (int d = 0; d < 3; ++d)
         if (grid[d] < order || grid[d] > 2048 || (grid[d] & 1))

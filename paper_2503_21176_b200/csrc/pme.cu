@@ -96,7 +96,7 @@ k_spread(int64_t n, const float4* __restrict__ frac, const int4* __restrict__ ba
         int pz = zs - odd;                       // even start of the first pair
 #pragma unroll
         for (int j = 0; j <= P / 2; ++j) {
-            if (j == P / 2 && !odd) break;
+            if (j == P / 2 && !odd && !(P & 1)) break;      // odd P: (P + 1)/2 pairs either way, one zero pad
             const float lo = odd ? ext[2 * j] : ext[2 * j + 1];
             const float hi = odd ? ext[2 * j + 1] : ext[2 * j + 2];
             red_add_v2(rowp + pz, lo, hi);
@@ -1067,7 +1067,9 @@ int pme_setup(sqeq_ctx* ctx, const double box[3], double alpha, const int grid[3
             }
             double mp = (m <= K / 2 ? m : m - K) / box[d];
             s[m] = (float)(mp * mp);
-            Bg[m] = (float)(exp(-M_PI * M_PI * mp * mp / (alpha * alpha)) / (re * re + im * im));
+            // odd order: the sum is exactly zero on the Nyquist plane; that plane is left out (reading G19)
+            const bool nyq_odd = (order & 1) && 2 * m == K;
+            Bg[m] = nyq_odd ? 0.f : (float)(exp(-M_PI * M_PI * mp * mp / (alpha * alpha)) / (re * re + im * im));
         }
         off += 2 * (size_t)K;
     }
@@ -1299,7 +1301,9 @@ int pme_run(sqeq_ctx* ctx, const sqeq_nlist* nl, int64_t n, const double box[3],
 {
     switch (ctx->order) {
         case 4: return pme_run_t<4>(ctx, nl, n, box, want_force, want_energy, st);
+        case 5: return pme_run_t<5>(ctx, nl, n, box, want_force, want_energy, st);
         case 6: return pme_run_t<6>(ctx, nl, n, box, want_force, want_energy, st);
+        case 7: return pme_run_t<7>(ctx, nl, n, box, want_force, want_energy, st);
         case 8: return pme_run_t<8>(ctx, nl, n, box, want_force, want_energy, st);
     }
     return sqeq_fail(ctx, SQEQ_EINVAL, "pme_run: unsupported order %d", ctx->order);

@@ -175,13 +175,13 @@ def test_edge_cases_small_and_shifted(ctx):
     op, oF, oE, _ = oracle.coulomb_pme(one, np.ones(1), box, 3.0, 0.9, [16, 20, 24], 6)
     assert abs(phi.item() - op[0]) < 1e-5 * abs(op[0])
     nl.free()
-    # far-from-origin, unwrapped, non-cubic box, all three orders
+    # far-from-origin, unwrapped, non-cubic box, all five orders (odd ones: DESIGN.md reading G19)
     n = 500
     boxn = np.array([17.0, 19.5, 23.0])
     p = (rng.uniform(0, 1, (n, 3)) * boxn + rng.integers(-3, 4, (n, 3)) * boxn).astype(np.float32)
     qq = rng.normal(size=n).astype(np.float32)
     nl, _ = check_nl_exact(ctx, p, boxn, 8.4)
-    for order, grid in ((4, [32, 36, 40]), (6, [24, 28, 32]), (8, [24, 28, 32])):
+    for order, grid in ((4, [32, 36, 40]), (5, [26, 30, 34]), (6, [24, 28, 32]), (7, [24, 30, 34]), (8, [24, 28, 32])):
         phi, F, E = ctx.coulomb(nl, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
         op, oF, oE, _ = oracle.coulomb_pme(p, qq, boxn, 8.0, 0.4, grid, order)
         assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL
@@ -204,7 +204,7 @@ def test_argument_validation(ctx):
     with pytest.raises(SqeqError):
         ctx.coulomb(nl, pos, q, [10.0] * 3, 3.0, 0.4, 16, 6)        # rc > list cutoff
     with pytest.raises(SqeqError):
-        ctx.coulomb(nl, pos, q, [10.0] * 3, 2.0, 0.4, 16, 5)        # odd order
+        ctx.coulomb(nl, pos, q, [10.0] * 3, 2.0, 0.4, 16, 9)        # order outside 4..8
     with pytest.raises(SqeqError):
         ctx.coulomb(nl, pos, q, [10.0] * 3, 2.0, 0.4, 4, 6)         # grid < order
     nl.free()
@@ -841,7 +841,7 @@ def test_pme_thread_per_atom_kernels(ctx):
         p = (rng.uniform(0, 1, (n, 3)) * boxn).astype(np.float32)
         qq = rng.normal(size=n).astype(np.float32)
         nl = c2.nl_build(dev(p), boxn, 8.4)
-        for order, grid in ((4, [64, 72, 80]), (8, [48, 56, 64])):
+        for order, grid in ((4, [64, 72, 80]), (5, [56, 64, 72]), (7, [48, 56, 64]), (8, [48, 56, 64])):
             phi, F, E = c2.coulomb(nl, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
             op, oF, oE, _ = oracle.coulomb_pme(p, qq, boxn, 8.0, 0.4, grid, order)
             assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL
@@ -871,7 +871,7 @@ def test_own_transforms_every_size(ctx):
         nlr = ref.nl_build(dev(p), boxn, 8.4)
         for i, K0 in enumerate(sizes):
             grid = [K0, sizes[(i + 5) % 14], sizes[(i + 9) % 14]]
-            order = (4, 6, 8)[i % 3]
+            order = (4, 5, 6, 7, 8)[i % 5]
             phi, F, E = ctx.coulomb(nl, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
             phr, Fr, Er = ref.coulomb(nlr, dev(p), dev(qq), boxn, 8.0, 0.4, grid, order)
             e_phi, e_F = relrms(phi.cpu().numpy(), phr.cpu().numpy()), relrms(F.cpu().numpy(), Fr.cpu().numpy())
@@ -953,6 +953,20 @@ def test_pme_tile_window_fallbacks(ctx, monkeypatch):
         phi, F, E = c2.coulomb(nl2, dev(pos), dev(q), c.box, c.rc, c.alpha, c.grid, c.order)
         assert relrms(phi.cpu().numpy()[rows], op) < TOL and relrms(F.cpu().numpy()[rows], oF) < TOL
         nl2.free()
+        # the global kernels at the odd orders (their rows are an odd number of points: one zero pad per row)
+        rng = np.random.default_rng(14)
+        n = 700
+        boxn = np.array([19.0, 21.0, 24.0])
+        pp = (rng.uniform(0, 1, (n, 3)) * boxn).astype(np.float32)
+        qq = rng.normal(size=n).astype(np.float32)
+        nl3 = c2.nl_build(dev(pp), boxn, 8.4)
+        for order, grid in ((5, [26, 30, 34]), (7, [28, 30, 32])):
+            phi, F, E = c2.coulomb(nl3, dev(pp), dev(qq), boxn, 8.0, 0.4, grid, order)
+            op, oF, oE, _ = oracle.coulomb_pme(pp, qq, boxn, 8.0, 0.4, grid, order)
+            assert relrms(phi.cpu().numpy(), op) < TOL and relrms(F.cpu().numpy(), oF) < TOL
+            phi2, _, _ = c2.coulomb(nl3, dev(pp), dev(qq), boxn, 8.0, 0.4, grid, order, want_force=False, want_energy=False)
+            assert relrms(phi2.cpu().numpy(), op) < TOL
+        nl3.free()
     finally:
         c2.close()
 
