@@ -802,7 +802,7 @@ def test_fixed_geometry_batched_vectors(ctx, k):
 
 def test_pme_thread_per_atom_kernels(ctx):
     """The one-thread-per-atom tile kernels (default from two tiles per SM on, i.e. cfg 3 and cfg 4) forced on for the
-    small configs too, all three spline orders, atoms that left their window, potential-only mode."""
+    small configs too, spline orders 4 to 8, atoms that left their window, potential-only mode."""
     from paper_2503_21176_b200 import binding
     c2 = binding.Context(0)
     c2.set_option("pme_atom_threads", 2)
