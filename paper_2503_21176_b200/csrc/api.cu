@@ -216,7 +216,7 @@ int sqeq_destroy(sqeq_ctx* ctx)
     DevBuf* bufs[] = {&ctx->gc.idx, &ctx->gc.t, &ctx->gc.len, &ctx->ew_tab, &ctx->ew_sf, &ctx->xf_tw,
                       &ctx->grid, &ctx->gridQ, &ctx->spec, &ctx->tabs, &ctx->xq, &ctx->frac,
                       &ctx->base, &ctx->real_out, &ctx->rec_out, &ctx->scal, &ctx->kry_V,
-                      &ctx->kry_w, &ctx->kry_h, &ctx->rep_oslot, &ctx->rep_ostart, &ctx->batch_q, &ctx->batch_r};
+                      &ctx->kry_w, &ctx->kry_h, &ctx->rep_oslot, &ctx->rep_ostart, &ctx->batch_q, &ctx->batch_r, &ctx->qeq_vin};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     for (auto& b : ctx->vec_f) if (b.p) cudaFree(b.p);

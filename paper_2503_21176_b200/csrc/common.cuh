@@ -118,6 +118,7 @@ struct sqeq_ctx {
     double diag_box[3] = {0, 0, 0}, diag_alpha = 0, diag_val = 0;     // ewald_self_diag of the last (box, alpha)
     // stand-in O-O repulsion (md.cu): the oxygens' list positions, cell by cell, for the list with this serial
     DevBuf rep_oslot, rep_ostart;
+    DevBuf qeq_vin;                       // qeq.cu: fixed input buffer of the graph-replayed mat-vec
     DevBuf batch_q, batch_r;              // sqeq_coulomb_fixed_batch: [4][n] sorted charge vectors / real-space potentials
     const void* rep_nl = nullptr;
     uint64_t rep_serial = 0;

@@ -577,7 +577,7 @@ struct QeqOp {
     float* phi;   // scratch [n]
 };
 
-static int qeq_apply(const QeqOp& op, const double* v, double* w)
+static int qeq_apply_body(const QeqOp& op, const double* v, double* w)
 {
     sqeq_ctx* ctx = op.ctx;
     cudaStream_t st = ctx->stream;
@@ -590,6 +590,35 @@ static int qeq_apply(const QeqOp& op, const double* v, double* w)
     k_qeq_matvec<<<ceil_div(n, 256), 256, 0, st>>>(n, v, op.J, op.phi, op.ke, w);
     KERNEL_CHECK(ctx);
     return SQEQ_OK;
+}
+
+static int qeq_apply(const QeqOp& op, const double* v, double* w)
+{
+    sqeq_ctx* ctx = op.ctx;
+    cudaStream_t st = ctx->stream;
+    const int64_t n = op.n;
+    const sqeq_nlist* nl = op.nl;
+    // Small systems are launch-bound (648 atoms: a dozen kernels of ~3 us per mat-vec against ~6 us of host time per
+    // launch).  Once the geometry cache is warm every mat-vec is the same sequence of launches: the Krylov vector is
+    // copied into a fixed buffer, so that the arguments never change, and the sequence is replayed as a CUDA graph.
+    const GeomCache& gc = ctx->gc;
+    const bool warm = gc.valid && gc.nl == nl && gc.serial == nl->serial && gc.rc == op.rc && gc.alpha == op.alpha && nl->fmt == 1;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (n > 65536 || !warm || !ctx->graphs || ctx->profiling || st == nullptr || st == cudaStreamLegacy ||
+        cudaStreamIsCapturing(st, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone)
+        return qeq_apply_body(op, v, w);
+    SQEQ_TRY(sqeq_reserve(ctx, ctx->qeq_vin, sizeof(double) * (size_t)(n + 1)));
+    double* vin = (double*)ctx->qeq_vin.p;
+    CUDA_TRY(ctx, cudaMemcpyAsync(vin, v, sizeof(double) * (size_t)(n + 1), cudaMemcpyDeviceToDevice, st));
+    uint64_t key = hash_mix(0x53, nl->serial);
+    double kd[3] = {op.rc, op.alpha, op.ke};
+    uint64_t kb[3];
+    memcpy(kb, kd, sizeof(kb));
+    for (uint64_t x : {(uint64_t)(uintptr_t)nl, (uint64_t)(uintptr_t)vin, (uint64_t)(uintptr_t)w, (uint64_t)(uintptr_t)op.phi,
+                       (uint64_t)(uintptr_t)op.J, (uint64_t)n, kb[0], kb[1], kb[2], (uint64_t)ctx->K[0], (uint64_t)ctx->K[1],
+                       (uint64_t)ctx->K[2], (uint64_t)ctx->order})
+        key = hash_mix(key, x);
+    return graph_run(ctx, 2, key, [&]() { return qeq_apply_body(op, vin, w); });
 }
 
 // A_ii of the Ewald matrix for r_c < L/2 (no image of an atom inside its own cutoff): the reciprocal-space self
