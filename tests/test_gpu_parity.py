@@ -466,7 +466,8 @@ def test_shadow_md_steps_config2_geometry(ctx):
 def test_cuda_graph_replay_matches_plain_launches():
     """On a context with its own stream sqeq_coulomb_fixed replays a cached geometry as a CUDA graph, and
     sqeq_shadow_md_run replays the MD step: same numbers as kernel-by-kernel launches ("graphs" = 0), the launch
-    counter keeps counting, a changed charge pointer or a new geometry re-captures."""
+    counter keeps counting, a changed charge pointer or a new geometry re-captures.  Also replayed: the QEq mat-vec of
+    a small system (two solves with the atoms moved in between) and the batched fixed-geometry entry."""
     from paper_2503_21176_b200 import binding
     c = W.CONFIGS[0]
     pos, q = inputs(0)
@@ -515,6 +516,26 @@ def test_cuda_graph_replay_matches_plain_launches():
                     torch.cuda.synchronize()
             outs.append(phi2.cpu().numpy().copy())
             outs.append(np.array([E2]))
+            # the QEq mat-vec of a small system is a replayed graph once the geometry cache is warm (fixed input buffer):
+            # two solves, the atoms moved in between -- the second must see the new geometry
+            chi, u = W.qeq_params_water_pd(n)
+            its = []
+            for xq_ in (dev(pos), x2):
+                torch.cuda.synchronize()
+                qs_, lam_, it_, rel_, ok_ = cx.qeq_solve(nl, xq_, c.box, c.rc, c.alpha, c.grid, c.order, W.KE_EV_A, dev(chi), dev(u),
+                                                         0.0, tol=1e-6, max_iter=200)
+                assert ok_
+                its.append(it_)
+                extra_q = qs_.cpu().numpy().copy()
+                res.setdefault(("q", graphs), []).append((extra_q, lam_))
+            res[("its", graphs)] = its
+            # and the batched fixed-geometry entry
+            cx.geometry_set(nl, dev(pos), c.box, c.rc, c.alpha, c.grid, c.order)
+            vb = dev(np.stack([q, q[::-1].copy(), (0.5 * q).astype(np.float32)]))
+            for _ in range(3):
+                pb = cx.coulomb_fixed_batch(vb)
+            torch.cuda.synchronize()
+            res[("batch", graphs)] = pb.cpu().numpy().copy()
             res[graphs] = (outs, per_eval, E)
             nl.free()
         finally:
@@ -523,7 +544,13 @@ def test_cuda_graph_replay_matches_plain_launches():
     for a, b in zip(res[1][0], res[0][0]):
         assert relrms(a, b) < 2e-6                              # only the order of atomic tile flushes differs
     assert abs(res[1][2] / res[0][2] - 1) < 1e-6
+    assert res[("its", 1)] == res[("its", 0)]
+    for (qa_, la_), (qb_, lb_) in zip(res[("q", 1)], res[("q", 0)]):
+        assert relrms(qa_, qb_) < 1e-5 and abs(la_ - lb_) < 1e-5 * abs(lb_)
+    assert relrms(res[("q", 1)][0][0], res[("q", 1)][1][0]) > 1e-4          # the moved atoms gave other charges
+    assert relrms(res[("batch", 1)], res[("batch", 0)]) < 2e-6
     op, oF, _, _ = oracle.coulomb_pme(pos, q, c.box, c.rc, c.alpha, c.grid, c.order)
+    assert relrms(res[("batch", 1)][0], op) < TOL and relrms(res[("batch", 1)][2], 0.5 * op) < TOL
     assert relrms(res[1][0][2], op) < TOL and relrms(res[1][0][0], op) < TOL
     assert relrms(res[1][0][-4], op) < TOL and relrms(res[1][0][-3], oF) < TOL         # replayed plain evaluation
     op2, _, oE2, _ = oracle.coulomb_pme(W.perturb(pos, 0, 0.02, 0), q, c.box, c.rc, c.alpha, c.grid, c.order)
