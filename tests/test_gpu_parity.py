@@ -207,6 +207,25 @@ def test_argument_validation(ctx):
         ctx.coulomb(nl, pos, q, [10.0] * 3, 2.0, 0.4, 16, 9)        # order outside 4..8
     with pytest.raises(SqeqError):
         ctx.coulomb(nl, pos, q, [10.0] * 3, 2.0, 0.4, 4, 6)         # grid < order
+    # the fixed-geometry entries refuse to run without a geometry, with another n, or with too many vectors
+    from paper_2503_21176_b200 import binding
+    c2 = binding.Context(0)
+    try:
+        with pytest.raises(SqeqError):
+            c2.coulomb_fixed_batch(torch.zeros((2, 4), device="cuda"))          # no sqeq_geometry_set yet
+        nl2 = c2.nl_build(pos + dev(np.arange(12, dtype=np.float32).reshape(4, 3)), [10.0] * 3, 2.0)
+        c2.geometry_set(nl2, pos, [10.0] * 3, 2.0, 0.4, [16, 16, 16], 6)
+        with pytest.raises(SqeqError):
+            c2.coulomb_fixed_batch(torch.zeros((2, 5), device="cuda"))          # n differs from the geometry
+        with pytest.raises(SqeqError):
+            c2.coulomb_fixed_batch(torch.zeros((65, 4), device="cuda"))         # more than 64 vectors
+        out = c2.coulomb_fixed_batch(torch.zeros((3, 4), device="cuda"))
+        assert float(out.abs().max()) == 0.0                                     # zero charges, zero potentials
+        nl2.free()
+        with pytest.raises(SqeqError):
+            c2.coulomb_fixed_batch(torch.zeros((2, 4), device="cuda"))          # the geometry's list was freed
+    finally:
+        c2.close()
     nl.free()
 
 
